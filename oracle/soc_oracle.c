@@ -1,0 +1,536 @@
+/*
+ * soc_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, fp64, single-threaded CPU statement of the per-frequency photon-package
+ * simulation of SOC (Juvela, arXiv:1812.06632) and of the energy-balance temperature
+ * lookup.  It exists so that the CUDA path can be checked against something that can be
+ * read next to the paper.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may load it.  It shares no code, header, table
+ * or constant generator with paper_1812_06632_b200/csrc.
+ *
+ * What the paper fixes (PAPER.md = /root/reference/PAPER.md):
+ *   - grid: regular Cartesian root grid of cubic cells, octree refinement into "octets",
+ *     one cell vector, root level first then level 2, ...; parent -> first child link,
+ *     one reverse link per octet; every cell change is a partial tree traversal, up to
+ *     the common parent and down to the new leaf            (Sect. 2.1.1)
+ *   - per frequency the kernel sees density, optical depth and an absorption counter;
+ *     host loops over frequencies
+ *   - absorbed energy integrated over frequency -> temperature, separate kernel;
+ *     cells never hit get an ad hoc constant temperature
+ *   - sources: isotropic external background, blackbody point sources, a source may sit
+ *     in a zero-density cell
+ * Everything the paper is silent on (RNG stream, emission sampling, tie-break, free path
+ * in scattering optical depth with continuous absorption, Henyey-Greenstein angle,
+ * termination, quadrature, table form) follows the readings S1-S16 listed in DESIGN.md
+ * (taken from SURVEY.md 8c and BASELINE.json:north_star).
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known answers, slab transmission
+ * exp(-tau), optically thin bath A = 4 pi I kabs rho V, energy conservation 1e-9,
+ * point-source escape fraction by quadrature, HG moments, emission laws / mean number of
+ * cells crossed, brute-force geometric replay on tiny octrees, fully-refined == regular
+ * 2N identity, temperature power law.  No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define SOC_O_PI 3.14159265358979323846
+
+/* ------------------------------------------------------------------ a1: RNG ---------
+ * Philox4x32-10 (Salmon, Moraes, Dror, Shaw 2011), standard multipliers and Weyl
+ * constants.  Block b of package p at frequency index f with a 64-bit seed:
+ *   counter = (b, p & 0xffffffff, p >> 32, f),  key = (seed & 0xffffffff, seed >> 32)
+ * Word -> uniform  u = ((x >> 9) + 0.5) * 2^-23, exactly representable in fp32 and fp64.
+ * (north_star: "counter-based Philox4x32 stream per package keyed by (seed, frequency,
+ * package id)"; layout = reading S2.) */
+void soc_oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+void soc_oracle_stream_block(uint64_t seed, int32_t ifreq, int64_t pkg, uint32_t block, uint32_t out[4])
+{
+    uint32_t ctr[4] = { block, (uint32_t)((uint64_t)pkg & 0xffffffffu), (uint32_t)((uint64_t)pkg >> 32),
+                        (uint32_t)ifreq };
+    uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
+    soc_oracle_philox4x32_10(ctr, key, out);
+}
+
+double soc_oracle_uniform(uint32_t word)
+{
+    return ((double)(word >> 9) + 0.5) * (1.0 / 8388608.0);
+}
+
+/* ------------------------------------------------------------------ a8: scattering --
+ * Henyey-Greenstein polar angle (north_star; the paper itself tabulates scattering
+ * functions).  With mu0 = 2u - 1 the inverse CDF
+ *   cos = (1 + g^2 - ((1 - g^2)/(1 - g + 2 g u))^2) / (2 g)
+ * is rewritten without the 1/g cancellation (reading S6):
+ *   cos = [mu0 + g (3 + mu0^2)/2 + g^2 mu0 + g^3 (mu0^2 - 1)/2] / (1 + g mu0)^2 . */
+double soc_oracle_hg_cos(double g, double u)
+{
+    double mu0 = 2.0 * u - 1.0;
+    double num = mu0 + g * (3.0 + mu0 * mu0) * 0.5 + g * g * mu0 + g * g * g * (mu0 * mu0 - 1.0) * 0.5;
+    double den = (1.0 + g * mu0) * (1.0 + g * mu0);
+    double c = num / den;
+    if (c > 1.0) c = 1.0;
+    if (c < -1.0) c = -1.0;
+    return c;
+}
+
+/* New direction at polar angle acos(cost) and azimuth phi about d (reading: rotation
+ * basis of Duff et al. 2017, no singular direction), then renormalised. */
+void soc_oracle_rotate(const double d[3], double cost, double phi, double out[3])
+{
+    double sint = sqrt(fmax(0.0, 1.0 - cost * cost));
+    double sg = copysign(1.0, d[2]);
+    double a = -1.0 / (sg + d[2]);
+    double b = d[0] * d[1] * a;
+    double t1[3] = { 1.0 + sg * d[0] * d[0] * a, sg * b, -sg * d[0] };
+    double t2[3] = { b, sg + d[1] * d[1] * a, -d[1] };
+    double cp = cos(phi), sp = sin(phi);
+    double n[3];
+    for (int j = 0; j < 3; ++j) n[j] = sint * cp * t1[j] + sint * sp * t2[j] + cost * d[j];
+    double inv = 1.0 / sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+    for (int j = 0; j < 3; ++j) out[j] = n[j] * inv;
+}
+
+/* ------------------------------------------------------------------ grid ------------
+ * Cell vector, level-major.  Level l = 1..n_levels has n_cells[l-1] cells,
+ * global id = level_off[l-1] + c.  Root index c = ix + nx (iy + ny iz).  For l > 1 the
+ * octet is c >> 3 and the slot c & 7 = bx + 2 by + 4 bz.  child[gid] = -1 for a leaf,
+ * else the index (within level l+1, a multiple of 8) of the first cell of its octet.
+ * parent[l-1][c >> 3] = index (within level l-1) of the parent: one reverse link per
+ * octet, as in the paper. */
+typedef struct soc_oracle_grid {
+    int32_t nx, ny, nz, n_levels;
+    int64_t *level_off;   /* [n_levels + 1] */
+    int64_t n_total;
+    float *rho;           /* [n_total], own copy */
+    int32_t *child;       /* [n_total], own copy (all -1 when n_levels == 1) */
+    int32_t **parent;     /* [n_levels]; parent[0] = NULL */
+} soc_oracle_grid;
+
+void soc_oracle_grid_destroy(soc_oracle_grid *G)
+{
+    if (!G) return;
+    if (G->parent) {
+        for (int l = 0; l < G->n_levels; ++l) free(G->parent[l]);
+        free(G->parent);
+    }
+    free(G->level_off); free(G->rho); free(G->child); free(G);
+}
+
+/* Returns NULL on an inconsistent hierarchy. */
+soc_oracle_grid *soc_oracle_grid_create(int32_t nx, int32_t ny, int32_t nz, int32_t n_levels,
+                                        const int64_t *n_cells, const float *rho, const int32_t *child)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || n_levels < 1) return NULL;
+    if (n_cells[0] != (int64_t)nx * ny * nz) return NULL;
+    soc_oracle_grid *G = (soc_oracle_grid *)calloc(1, sizeof(*G));
+    G->nx = nx; G->ny = ny; G->nz = nz; G->n_levels = n_levels;
+    G->level_off = (int64_t *)calloc((size_t)n_levels + 1, sizeof(int64_t));
+    for (int l = 0; l < n_levels; ++l) {
+        if (l > 0 && (n_cells[l] % 8 != 0)) { soc_oracle_grid_destroy(G); return NULL; }
+        G->level_off[l + 1] = G->level_off[l] + n_cells[l];
+    }
+    G->n_total = G->level_off[n_levels];
+    G->rho = (float *)malloc(sizeof(float) * (size_t)G->n_total);
+    G->child = (int32_t *)malloc(sizeof(int32_t) * (size_t)G->n_total);
+    memcpy(G->rho, rho, sizeof(float) * (size_t)G->n_total);
+    if (child) memcpy(G->child, child, sizeof(int32_t) * (size_t)G->n_total);
+    else for (int64_t i = 0; i < G->n_total; ++i) G->child[i] = -1;
+    G->parent = (int32_t **)calloc((size_t)n_levels, sizeof(int32_t *));
+    for (int l = 1; l < n_levels; ++l) {
+        int64_t n_oct = n_cells[l] / 8;
+        G->parent[l] = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_oct > 0 ? n_oct : 1));
+        for (int64_t o = 0; o < n_oct; ++o) G->parent[l][o] = -1;
+    }
+    for (int l = 0; l < n_levels; ++l) {
+        for (int64_t c = 0; c < n_cells[l]; ++c) {
+            int64_t gid = G->level_off[l] + c;
+            int32_t ch = G->child[gid];
+            if (ch < 0) {
+                if (!(G->rho[gid] >= 0.0f) || !isfinite(G->rho[gid])) { soc_oracle_grid_destroy(G); return NULL; }
+                continue;
+            }
+            if (l + 1 >= n_levels || (ch & 7) != 0 || ch + 8 > n_cells[l + 1] ||
+                G->parent[l + 1][ch >> 3] != -1) { soc_oracle_grid_destroy(G); return NULL; }
+            G->parent[l + 1][ch >> 3] = (int32_t)c;
+        }
+    }
+    for (int l = 1; l < n_levels; ++l)
+        for (int64_t o = 0; o < n_cells[l] / 8; ++o)
+            if (G->parent[l][o] < 0) { soc_oracle_grid_destroy(G); return NULL; }
+    return G;
+}
+
+/* ------------------------------------------------------------------ package state --- */
+typedef struct {
+    int32_t level;      /* l = 1..n_levels */
+    int32_t cell;       /* index within the level: authoritative, never re-derived (S4) */
+    double f[3];        /* position inside the cell, in units of the cell edge, [0,1]^3 */
+    double d[3];        /* unit direction */
+} soc_oracle_state;
+
+typedef struct {
+    double bg_intensity;   /* I_nu of the isotropic background, 0 = none */
+    int32_t n_point;
+    const double *ps_pos;  /* [n_point][3] root-grid units, strictly inside the grid */
+    const double *ps_lum;  /* [n_point] */
+    int64_t n_bg;          /* ids [0,n_bg) background, the rest point sources; -1 = default split */
+    const double *beam;    /* test hook: [6] = position, direction; every package is this beam, E0 = 1 */
+} soc_oracle_sources;
+
+typedef struct {
+    double emitted, escaped, absorbed;
+    uint64_t cell_steps, scatterings, terminated;
+} soc_oracle_result;
+
+typedef struct {           /* per-package replay record */
+    uint64_t hash;         /* FNV-style hash of the visited global cell ids */
+    uint32_t steps, scatters;
+    double e_escaped;
+} soc_oracle_replay;
+
+typedef struct {           /* one cell-step, global coordinates in root-cell units */
+    int64_t pkg, gid;
+    int32_t level, kind;   /* kind: 0 cross, 1 scatter, 2 terminated here, 3 cross and escape */
+    double p0[3], p1[3];
+    double ds, tau_sca;    /* path length and scattering optical depth of the step */
+    double tau_drawn;      /* -ln u of the flight segment this step belongs to */
+} soc_oracle_trace;
+
+/* origin (lower corner, root units) of cell (level, c) by following the reverse links */
+static void cell_origin(const soc_oracle_grid *G, int32_t level, int32_t c, double org[3])
+{
+    double h = ldexp(1.0, -(level - 1));
+    double o[3] = { 0.0, 0.0, 0.0 };
+    while (level > 1) {
+        o[0] += h * (double)(c & 1);
+        o[1] += h * (double)((c >> 1) & 1);
+        o[2] += h * (double)((c >> 2) & 1);
+        c = G->parent[level - 1][c >> 3];
+        level -= 1;
+        h *= 2.0;
+    }
+    int32_t ix = c % G->nx, iy = (c / G->nx) % G->ny, iz = c / (G->nx * G->ny);
+    org[0] = o[0] + ix; org[1] = o[1] + iy; org[2] = o[2] + iz;
+}
+
+/* Descend to the leaf that holds the position ("down to the new leaf node").
+ * f >= 0.5 goes to the upper child; 2f and 2f-1 are exact. */
+static void descend(const soc_oracle_grid *G, soc_oracle_state *S)
+{
+    for (;;) {
+        int32_t ch = G->child[G->level_off[S->level - 1] + S->cell];
+        if (ch < 0) return;
+        int32_t slot = 0;
+        for (int j = 0; j < 3; ++j) {
+            if (S->f[j] >= 0.5) { slot |= (1 << j); S->f[j] = 2.0 * S->f[j] - 1.0; }
+            else S->f[j] = 2.0 * S->f[j];
+        }
+        S->cell = ch + slot;
+        S->level += 1;
+    }
+}
+
+/* Move across the face of axis a in direction sg (+1/-1): sibling flip, else up to the
+ * common parent, then down.  Returns 0 if the package left the root grid. */
+static int move_across(const soc_oracle_grid *G, soc_oracle_state *S, int a, int sg)
+{
+    for (;;) {
+        if (S->level == 1) {
+            int32_t n[3] = { G->nx, G->ny, G->nz };
+            int32_t i[3] = { S->cell % G->nx, (S->cell / G->nx) % G->ny, S->cell / (G->nx * G->ny) };
+            i[a] += sg;
+            if (i[a] < 0 || i[a] >= n[a]) return 0;
+            S->cell = i[0] + G->nx * (i[1] + G->ny * i[2]);
+            break;
+        }
+        int bit = (S->cell >> a) & 1;
+        if ((sg > 0 && bit == 0) || (sg < 0 && bit == 1)) { S->cell ^= (1 << a); break; }
+        for (int j = 0; j < 3; ++j) S->f[j] = (S->f[j] + (double)((S->cell >> j) & 1)) * 0.5;
+        S->cell = G->parent[S->level - 1][S->cell >> 3];
+        S->level -= 1;
+    }
+    S->f[a] = (sg > 0) ? 0.0 : 1.0;   /* entry face, in the neighbour's frame */
+    descend(G, S);
+    return 1;
+}
+
+/* ------------------------------------------------------------------ a2, a3: emission - */
+/* Number of background packages and package energies (reading S3). */
+static int64_t split_n_bg(const soc_oracle_sources *src, int64_t n_packages)
+{
+    if (src->n_bg >= 0) return src->n_bg;
+    int has_bg = src->bg_intensity > 0.0, has_ps = src->n_point > 0;
+    if (has_bg && has_ps) return n_packages / 2;
+    return has_bg ? n_packages : 0;
+}
+
+/* Background: face chosen in proportion to its area, uniform point on
+ * the face, cosine-law direction into the volume; E0 = pi I S / n_bg. */
+void soc_oracle_emit_background(int32_t nx, int32_t ny, int32_t nz, const double u[5],
+                                int32_t cell_ijk[3], double f[3], double d[3])
+{
+    double N[3] = { (double)nx, (double)ny, (double)nz };
+    double area[3] = { N[1] * N[2], N[2] * N[0], N[0] * N[1] };   /* faces normal to x, y, z */
+    double S = 2.0 * (area[0] + area[1] + area[2]);
+    double x = u[0] * S, cum = 0.0;
+    int face = 5;
+    for (int k = 0; k < 6; ++k) { cum += area[k / 2]; if (x < cum) { face = k; break; } }
+    int a = face / 2, a1 = (a + 1) % 3, a2 = (a + 2) % 3, high = face & 1;
+    int32_t n_i[3] = { nx, ny, nz };
+    double t1 = u[1] * N[a1], t2 = u[2] * N[a2];
+    int32_t i1 = (int32_t)floor(t1); if (i1 > n_i[a1] - 1) i1 = n_i[a1] - 1;
+    int32_t i2 = (int32_t)floor(t2); if (i2 > n_i[a2] - 1) i2 = n_i[a2] - 1;
+    cell_ijk[a1] = i1; f[a1] = t1 - i1;
+    cell_ijk[a2] = i2; f[a2] = t2 - i2;
+    cell_ijk[a] = high ? n_i[a] - 1 : 0;
+    f[a] = high ? 1.0 : 0.0;
+    double mu = sqrt(u[3]), st = sqrt(1.0 - u[3]), phi = 2.0 * SOC_O_PI * u[4];
+    d[a] = high ? -mu : mu;
+    d[a1] = st * cos(phi);
+    d[a2] = st * sin(phi);
+}
+
+/* Point source: fixed position, isotropic direction. */
+void soc_oracle_emit_point(const double pos[3], const double u[2],
+                           int32_t cell_ijk[3], double f[3], double d[3])
+{
+    for (int j = 0; j < 3; ++j) { cell_ijk[j] = (int32_t)floor(pos[j]); f[j] = pos[j] - cell_ijk[j]; }
+    double mu = 2.0 * u[0] - 1.0, st = sqrt(fmax(0.0, 1.0 - mu * mu)), phi = 2.0 * SOC_O_PI * u[1];
+    d[0] = st * cos(phi); d[1] = st * sin(phi); d[2] = mu;
+}
+
+/* ------------------------------------------------------------------ a4-a9: the walk - */
+#define SOC_O_WMIN 1e-9   /* termination: weight below WMIN * E0, residual deposited (S7) */
+
+/* Simulate package ids [pkg_begin, pkg_begin + pkg_count) of a run of n_packages at
+ * frequency index ifreq.  absorbed[gid] += weight * (energy absorbed in the cell).
+ * replay (may be NULL): pkg_count records.  trace (may be NULL): up to trace_cap steps,
+ * *n_trace receives the number written.  Returns 0, or -1 on a bad argument. */
+int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, double g, int32_t ifreq,
+                        const soc_oracle_sources *src, int64_t n_packages, uint64_t seed, double weight,
+                        int64_t pkg_begin, int64_t pkg_count, double *absorbed,
+                        soc_oracle_result *res, soc_oracle_replay *replay,
+                        soc_oracle_trace *trace, int64_t trace_cap, int64_t *n_trace)
+{
+    if (!G || !src || !absorbed || n_packages < 0 || pkg_begin < 0 || pkg_count < 0 ||
+        pkg_begin + pkg_count > n_packages || !(kabs >= 0.0) || !(ksca >= 0.0) || !(fabs(g) < 1.0))
+        return -1;
+    const int64_t n_bg = src->beam ? 0 : split_n_bg(src, n_packages);
+    if (n_bg > n_packages) return -1;
+    if (!src->beam) {
+        if (n_bg > 0 && !(src->bg_intensity > 0.0)) return -1;
+        if (n_packages - n_bg > 0 && src->n_point <= 0) return -1;
+        for (int k = 0; k < src->n_point; ++k) {
+            const double *p = src->ps_pos + 3 * k;
+            if (!(p[0] > 0.0 && p[0] < G->nx && p[1] > 0.0 && p[1] < G->ny && p[2] > 0.0 && p[2] < G->nz)) return -1;
+        }
+    }
+    const double surf = 2.0 * ((double)G->ny * G->nz + (double)G->nz * G->nx + (double)G->nx * G->ny);
+    soc_oracle_result R; memset(&R, 0, sizeof(R));
+    int64_t nt = 0;
+
+    for (int64_t p = pkg_begin; p < pkg_begin + pkg_count; ++p) {
+        soc_oracle_state S;
+        int32_t ijk[3];
+        double E0;
+        uint32_t w0[4], w1[4];
+        soc_oracle_stream_block(seed, ifreq, p, 0u, w0);
+        soc_oracle_stream_block(seed, ifreq, p, 1u, w1);
+        if (src->beam) {
+            E0 = 1.0;
+            for (int j = 0; j < 3; ++j) {
+                ijk[j] = (int32_t)floor(src->beam[j]);
+                int32_t nj = (j == 0) ? G->nx : (j == 1) ? G->ny : G->nz;
+                if (ijk[j] > nj - 1) ijk[j] = nj - 1;     /* a beam may start on the upper boundary */
+                S.f[j] = src->beam[j] - ijk[j];
+                S.d[j] = src->beam[3 + j];
+            }
+        } else if (p < n_bg) {
+            double u[5] = { soc_oracle_uniform(w0[0]), soc_oracle_uniform(w0[1]), soc_oracle_uniform(w0[2]),
+                            soc_oracle_uniform(w0[3]), soc_oracle_uniform(w1[0]) };
+            soc_oracle_emit_background(G->nx, G->ny, G->nz, u, ijk, S.f, S.d);
+            E0 = SOC_O_PI * src->bg_intensity * surf / (double)n_bg;
+        } else {
+            int64_t q = p - n_bg, n_ps = n_packages - n_bg;
+            int32_t k = (int32_t)(q % src->n_point);
+            /* count_k = number of ids q in [0, n_ps) with q mod n_point == k */
+            int64_t count_k = n_ps / src->n_point + ((n_ps % src->n_point) > k ? 1 : 0);
+            double u[2] = { soc_oracle_uniform(w0[0]), soc_oracle_uniform(w0[1]) };
+            soc_oracle_emit_point(src->ps_pos + 3 * k, u, ijk, S.f, S.d);
+            E0 = src->ps_lum[k] / (double)count_k;
+        }
+        S.level = 1;
+        S.cell = ijk[0] + G->nx * (ijk[1] + G->ny * ijk[2]);
+        descend(G, &S);
+
+        double E = E0;
+        R.emitted += E0;
+        uint32_t seg = 0, steps = 0, scat = 0;
+        uint64_t hash = 0xcbf29ce484222325ull;
+        double e_esc = 0.0;
+        uint32_t ws[4];
+        soc_oracle_stream_block(seed, ifreq, p, 2u + seg, ws);
+        double tau_drawn = -log(soc_oracle_uniform(ws[0]));   /* a4: free path, scattering depth */
+        double tau_rem = tau_drawn;
+
+        for (;;) {
+            const int64_t gid = G->level_off[S.level - 1] + S.cell;
+            const double rho = (double)G->rho[gid];
+            const double h = ldexp(1.0, -(S.level - 1));
+            /* a5/a6: distance (in cell edges) to the face of each axis */
+            double t[3];
+            for (int j = 0; j < 3; ++j) {
+                if (S.d[j] > 0.0) t[j] = (1.0 - S.f[j]) / S.d[j];
+                else if (S.d[j] < 0.0) t[j] = (-S.f[j]) / S.d[j];
+                else t[j] = INFINITY;
+                if (t[j] < 0.0) t[j] = 0.0;
+            }
+            int a = 0;                                    /* lowest axis wins a tie (S4) */
+            if (t[1] < t[a]) a = 1;
+            if (t[2] < t[a]) a = 2;
+            const double tstar = t[a];
+            const double ds = tstar * h;
+            const double ks_rho = rho * ksca;
+            const double dtau = ds * ks_rho;
+            int scatter = 0;
+            double ds_used = ds, t_used = tstar;
+            if (ks_rho > 0.0 && dtau >= tau_rem) {
+                scatter = 1;
+                ds_used = tau_rem / ks_rho;
+                t_used = ds_used / h;
+            }
+            /* a7: path-length estimator, continuous absorption */
+            const double dep = E * (-expm1(-ds_used * rho * kabs));
+            absorbed[gid] += weight * dep;
+            R.absorbed += dep;
+            E -= dep;
+            steps += 1;
+            hash = (hash ^ (uint64_t)gid) * 0x100000001b3ull;
+
+            soc_oracle_trace *T = NULL;
+            if (trace && nt < trace_cap) {
+                T = &trace[nt++];
+                double org[3];
+                cell_origin(G, S.level, S.cell, org);
+                T->pkg = p; T->gid = gid; T->level = S.level; T->kind = scatter ? 1 : 0;
+                for (int j = 0; j < 3; ++j) T->p0[j] = org[j] + h * S.f[j];
+                T->ds = ds_used; T->tau_sca = ds_used * ks_rho; T->tau_drawn = tau_drawn;
+            }
+            /* a9: termination */
+            if (E < SOC_O_WMIN * E0) {
+                absorbed[gid] += weight * E;
+                R.absorbed += E;
+                E = 0.0;
+                R.terminated += 1;
+                if (T) { T->kind = 2; for (int j = 0; j < 3; ++j) T->p1[j] = T->p0[j] + ds_used * S.d[j]; }
+                break;
+            }
+            for (int j = 0; j < 3; ++j) {
+                S.f[j] += t_used * S.d[j];
+                if (S.f[j] < 0.0) S.f[j] = 0.0;
+                if (S.f[j] > 1.0) S.f[j] = 1.0;
+            }
+            if (T) {
+                double org[3];
+                cell_origin(G, S.level, S.cell, org);
+                for (int j = 0; j < 3; ++j) T->p1[j] = org[j] + h * S.f[j];
+            }
+            if (scatter) {
+                /* a8 */
+                double cost = soc_oracle_hg_cos(g, soc_oracle_uniform(ws[1]));
+                double phi = 2.0 * SOC_O_PI * soc_oracle_uniform(ws[2]);
+                double nd[3];
+                soc_oracle_rotate(S.d, cost, phi, nd);
+                S.d[0] = nd[0]; S.d[1] = nd[1]; S.d[2] = nd[2];
+                seg += 1; scat += 1;
+                soc_oracle_stream_block(seed, ifreq, p, 2u + seg, ws);
+                tau_drawn = -log(soc_oracle_uniform(ws[0]));
+                tau_rem = tau_drawn;
+            } else {
+                tau_rem -= dtau;
+                if (!move_across(G, &S, a, S.d[a] > 0.0 ? 1 : -1)) {
+                    e_esc = E;                           /* a9: escape */
+                    R.escaped += E;
+                    if (T) T->kind = 3;
+                    break;
+                }
+            }
+        }
+        R.cell_steps += steps;
+        R.scatterings += scat;
+        if (replay) {
+            soc_oracle_replay *rp = &replay[p - pkg_begin];
+            rp->hash = hash; rp->steps = steps; rp->scatters = scat; rp->e_escaped = e_esc;
+        }
+    }
+    if (res) *res = R;
+    if (n_trace) *n_trace = nt;
+    return 0;
+}
+
+/* ------------------------------------------------------------------ a10 -------------
+ * Trapezoid weights in nu on the given grid (PAPER.md:67 only says the integral over
+ * frequency is gathered during the simulation; quadrature = reading S9). */
+void soc_oracle_trapezoid_weights(const double *freq, int32_t n, double *w)
+{
+    if (n == 1) { w[0] = 1.0; return; }
+    for (int i = 0; i < n; ++i) {
+        double lo = freq[i > 0 ? i - 1 : 0], hi = freq[i < n - 1 ? i + 1 : n - 1];
+        w[i] = 0.5 * fabs(hi - lo);
+    }
+}
+
+/* ------------------------------------------------------------------ a11 -------------
+ * Energy balance by table lookup (table form = reading S10).
+ * E_c = scale * Aint_c / (rho_c h_l^3); table T_k on E_k = E_min (E_max/E_min)^(k/(n-1));
+ * linear interpolation in the table index; E_c <= E_min (also unhit cells) -> T_0;
+ * E_c >= E_max -> T_{n-1}; rho = 0 leaves and parent cells -> 0. */
+void soc_oracle_update_temperatures(const soc_oracle_grid *G, const double *absorbed, double scale,
+                                    const float *table_T, int32_t n_table, double E_min, double E_max,
+                                    float *T_out)
+{
+    const double lmin = log(E_min), lmax = log(E_max);
+    for (int l = 1; l <= G->n_levels; ++l) {
+        const double h = ldexp(1.0, -(l - 1)), vol = h * h * h;
+        for (int64_t gid = G->level_off[l - 1]; gid < G->level_off[l]; ++gid) {
+            const double rho = (double)G->rho[gid];
+            if (G->child[gid] >= 0 || !(rho > 0.0)) { T_out[gid] = 0.0f; continue; }
+            const double Ec = scale * absorbed[gid] / (rho * vol);
+            double T;
+            if (!(Ec > E_min)) T = (double)table_T[0];
+            else if (Ec >= E_max) T = (double)table_T[n_table - 1];
+            else {
+                double x = (log(Ec) - lmin) / (lmax - lmin) * (double)(n_table - 1);
+                int32_t i = (int32_t)floor(x);
+                if (i > n_table - 2) i = n_table - 2;
+                if (i < 0) i = 0;
+                T = (double)table_T[i] + (x - (double)i) * ((double)table_T[i + 1] - (double)table_T[i]);
+            }
+            T_out[gid] = (float)T;
+        }
+    }
+}
+
+int64_t soc_oracle_sizeof_replay(void) { return (int64_t)sizeof(soc_oracle_replay); }
+int64_t soc_oracle_sizeof_trace(void) { return (int64_t)sizeof(soc_oracle_trace); }
+int64_t soc_oracle_grid_n_total(const soc_oracle_grid *G) { return G->n_total; }
+const int32_t *soc_oracle_grid_parent(const soc_oracle_grid *G, int32_t level) { return G->parent[level - 1]; }
