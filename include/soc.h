@@ -1,0 +1,164 @@
+/*
+ * soc.h -- C ABI of libsoc_b200: the per-frequency photon-package simulation of SOC's Monte Carlo
+ * radiative transfer (Juvela, arXiv:1812.06632) and the energy-balance temperature kernel, as
+ * hand-written CUDA for sm_100a.
+ *
+ * Citations are lines of the paper text and readings S1-S17 of DESIGN.md where the paper is
+ * silent.  What the calls compute:
+ *   - the model is a regular Cartesian root grid of cubic cells with octree refinement; all cells form ONE
+ *     vector: root cells first, then level 2, ... (Sect. 2.1.1)
+ *   - one kernel simulates the photon packages of ONE frequency; it sees the densities, the optical depth
+ *     of that frequency and a per-cell absorption counter; the host loops over frequencies
+ *   - packages come from an isotropic external background and from blackbody point sources
+ *
+ *   - the absorbed energy integrated over frequency is turned into dust temperatures by a separate kernel;
+ *     cells that were never hit get a constant temperature
+ *
+ * Conventions
+ *   - every function returns SOC_OK (0) or a negative error code; the text of the last error of the calling
+ *     thread is available from soc_last_error().  No exception or abort crosses the boundary.
+ *   - pointers are HOST memory unless the comment says DEVICE.  Host arrays are borrowed for the duration
+ *     of the call only; the library never frees or keeps caller memory.  DEVICE arrays are caller-owned.
+ *   - lengths are in units of the root-cell edge ("GL").  Cell order of every per-cell array is the paper's
+ *     cell vector: level 1 (root, index = ix + nx*(iy + ny*iz)), then level 2, ...; the 8 cells of an octet
+ *     are consecutive with slot = bx + 2*by + 4*bz (reading S5).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - there is no CPU fallback: without a CUDA device every compute call fails with SOC_ECUDA.
+ */
+#ifndef SOC_B200_H
+#define SOC_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SOC_OK      0
+#define SOC_EINVAL (-1)   /* bad argument or inconsistent hierarchy */
+#define SOC_ENOMEM (-2)   /* host or device allocation failed */
+#define SOC_ECUDA  (-3)   /* CUDA runtime error; text in soc_last_error() */
+
+#define SOC_MAX_POINT_SOURCES 64
+#define SOC_MAX_LEVELS 16
+
+/* flags of the simulate calls */
+#define SOC_GEOM_FP32 0u  /* production: fp32 in-cell positions/directions, fp64 weights and accumulators */
+#define SOC_GEOM_FP64 1u  /* replay: fp64 positions/directions (same decisions as the fp64 oracle up to 1e-16) */
+
+typedef struct soc_grid soc_grid;    /* opaque; owns its device copies of the cloud and the dust tables */
+
+/* Inputs named by the paper: the cloud hierarchy with the density values, the dust cross sections for
+ * absorption and scattering, the scattering function per frequency (here Henyey-Greenstein g,
+ * north_star).  Single dust population. */
+typedef struct {
+    int32_t nx, ny, nz;         /* root grid */
+    int32_t n_levels;           /* n_L >= 1; 1 = regular grid; <= SOC_MAX_LEVELS */
+    const int64_t *n_cells;     /* [n_levels]; n_cells[0] = nx*ny*nz, the others multiples of 8; sum < 2^31 */
+    const float *density;       /* [n_total] level-major; leaves finite and >= 0; parents ignored */
+    const int32_t *child;       /* [n_total]: -1 = leaf, else index WITHIN level l+1 of the first cell of the
+                                   cell's octet (multiple of 8).  NULL when n_levels == 1 */
+    int32_t n_freq;
+    const double *freq_hz;      /* [n_freq] strictly ascending (index 0 = lowest frequency) */
+    const double *kabs, *ksca;  /* [n_freq] optical depth per unit density per GL, >= 0 */
+    const double *g;            /* [n_freq] Henyey-Greenstein asymmetry, |g| < 1 */
+} soc_grid_desc;
+
+/* Radiation sources at one frequency.  Package ids [0, n_bg) are background
+ * packages of energy pi*I*S/n_bg (S = surface of the root grid); id p >= n_bg belongs to point source
+ * (p - n_bg) mod n_point and carries L_k / count_k (reading S3). */
+typedef struct {
+    double bg_intensity;        /* I_nu of the isotropic background; 0 = none */
+    int32_t n_point;            /* <= SOC_MAX_POINT_SOURCES */
+    const double *ps_pos;       /* [n_point][3], GL, strictly inside the root grid; a source may sit in an
+                                   empty cell */
+    const double *ps_lum;       /* [n_point] L_nu in the same energy unit as pi*I*S */
+    int64_t n_bg;               /* -1 = default split: all packages to the only class present, n/2 each if both */
+    const double *beam;         /* test hook, normally NULL: [6] = position, unit direction; every package is
+                                   this beam with energy 1 and no random emission */
+} soc_sources;
+
+typedef struct {
+    double emitted, escaped, absorbed;   /* energies of the simulated packages (not multiplied by `weight`) */
+    uint64_t cell_steps, scatterings, terminated;
+} soc_freq_result;
+
+/* per-package replay record (DEVICE array written by soc_simulate_packages) */
+typedef struct {
+    uint64_t hash;              /* h = 0xcbf29ce484222325; per cell-step h = (h ^ cell id) * 0x100000001b3 */
+    uint32_t steps, scatters;
+    double e_escaped;           /* weight with which the package left the grid (0 if terminated) */
+} soc_replay_record;
+
+/* Copies and validates the model (child indices in range and multiples of 8, every octet has exactly one
+ * parent, leaf densities finite and >= 0, dust tables finite).  On success *out owns device memory until
+ * soc_grid_destroy. */
+int soc_grid_create(const soc_grid_desc *desc, soc_grid **out);
+void soc_grid_destroy(soc_grid *grid);
+int64_t soc_grid_n_total(const soc_grid *grid);
+
+/* Quadrature weights of the frequency integral (trapezoid in nu, reading S9): w[n_freq]. */
+int soc_freq_weights(const soc_grid *grid, double *w);
+
+/* Simulate package ids [0, n_packages) at frequency index ifreq (rows a1-a9 of the scope table):
+ *   absorbed[cell] += weight * (energy absorbed in the cell)     DEVICE, n_total doubles, accumulated into
+ * Philox4x32-10 stream keyed by (seed, ifreq, package id) (north_star; reading S2).  `res` (may be NULL)
+ * receives the totals; when it is non-NULL the call synchronises the stream before returning, otherwise it
+ * only enqueues work. */
+int soc_simulate_frequency(soc_grid *grid, int32_t ifreq, const soc_sources *src, int64_t n_packages,
+                           uint64_t seed, double weight, double *absorbed, soc_freq_result *res,
+                           uint32_t flags, void *cuda_stream);
+
+/* Replay / subset entry: package ids [pkg_begin, pkg_begin + pkg_count) of the same run (package energies
+ * depend on the full n_packages).  `replay` (DEVICE, pkg_count records) may be NULL. */
+int soc_simulate_packages(soc_grid *grid, int32_t ifreq, const soc_sources *src, int64_t n_packages,
+                          uint64_t seed, double weight, int64_t pkg_begin, int64_t pkg_count,
+                          double *absorbed, soc_replay_record *replay, soc_freq_result *res,
+                          uint32_t flags, void *cuda_stream);
+
+/* Frequency loop (row a10): for every frequency f of the grid, packages
+ * [pkg_begin, pkg_begin + pkg_count) of n_packages with sources src[f], accumulated as
+ *   absorbed_int[cell] += w_f * A_f[cell]            (w = soc_freq_weights)
+ * All launches are queued back to back on the stream; results[n_freq] (may be NULL) are fetched once at
+ * the end (the call then synchronises). */
+int soc_simulate_spectrum(soc_grid *grid, const soc_sources *src, int64_t n_packages, uint64_t seed,
+                          int64_t pkg_begin, int64_t pkg_count, double *absorbed_int,
+                          soc_freq_result *results, uint32_t flags, void *cuda_stream);
+
+/* Energy balance by table lookup (row a11; reading S10).  For every leaf with rho > 0:
+ *   E = scale * absorbed[cell] / (rho * h^3),  h = 2^-(level-1)
+ *   T = table_T interpolated linearly in the index x = (ln E - ln E_min)/(ln E_max - ln E_min)*(n_table-1);
+ *   E <= E_min (also cells never hit) -> table_T[0];  E >= E_max -> table_T[n_table-1].
+ * Parent cells and rho = 0 leaves get 0.  table_T: HOST, n_table floats (2 <= n_table <= 8192).
+ * absorbed: DEVICE n_total doubles.  T_out: DEVICE n_total floats. */
+int soc_update_temperatures(soc_grid *grid, const double *absorbed, double scale, const float *table_T,
+                            int32_t n_table, double E_min, double E_max, float *T_out, void *cuda_stream);
+
+/* End-to-end entry with HOST buffers only: uploads the model, zeroes a device accumulator, runs
+ * soc_simulate_spectrum for seeds seed, seed+1, ... seed+n_iter-1 (running mean over iterations, reading
+ * S12), updates the temperatures, and copies absorbed_int (mean over iterations, n_total doubles) and
+ * T (n_total floats) back.  Either output pointer may be NULL.  results: [n_iter][n_freq] or NULL. */
+int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_packages, uint64_t seed,
+                 int32_t n_iter, double t_scale, const float *table_T, int32_t n_table, double E_min,
+                 double E_max, double *absorbed_int_out, float *T_out, soc_freq_result *results,
+                 uint32_t flags);
+
+/* Tuning knobs (all have defaults chosen for B200): "blocks_per_sm", "threads", "refill_threshold".
+ * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
+int soc_set_option(soc_grid *grid, const char *key, int64_t value);
+
+/* Roofline probes: random 4-byte gathers (kind 0), random fp64 red.global.add (kind 1) and
+ * random fp32 red.global.add (kind 2) over a footprint of `footprint_bytes`, n_ops operations in total,
+ * uniform addresses.  *ms receives the CUDA-event time of the probe kernel. */
+int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms);
+
+/* Number of kernel launches issued by this library in the calling process (bench.py's "gpu_launches"). */
+uint64_t soc_launch_count(void);
+
+const char *soc_last_error(void);
+const char *soc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SOC_B200_H */

@@ -169,9 +169,12 @@ class Grid:
             raise ValueError("soc_oracle_grid_create: inconsistent hierarchy")
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().soc_oracle_grid_destroy(self._h)
-            self._h = None
+        try:
+            if getattr(self, "_h", None):
+                lib().soc_oracle_grid_destroy(self._h)
+                self._h = None
+        except Exception:       # interpreter shutdown
+            pass
 
     def parent(self, level):
         """Reverse links of `level` (1-based, > 1): one entry per octet."""

@@ -24,6 +24,16 @@
  * termination, quadrature, table form) follows the readings S1-S16 listed in DESIGN.md
  * (taken from SURVEY.md 8c and BASELINE.json:north_star).
  *
+ * Precision (reading S11; north_star "fp32 positions / fp64 accumulators", "one floating
+ * point number per cell", PAPER.md:367 single precision): the package STATE -- in-cell position,
+ * direction, remaining optical depth of the flight segment -- is held in fp32; every update is
+ * evaluated in fp64 from that state and rounded once to fp32 when stored.  Weights, deposits and
+ * accumulators are fp64.  The walk through a cloud with sharp density contrasts amplifies
+ * perturbations of the state (a lateral shift changes chord lengths in dense cells, hence where the
+ * next scattering falls in a thin one); snapping the state to fp32 after each update keeps two
+ * independent fp64 evaluations on the same trajectory, which is what makes package-by-package replay
+ * against the CUDA path meaningful.
+ *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known answers, slab transmission
  * exp(-tau), optically thin bath A = 4 pi I kabs rho V, energy conservation 1e-9,
  * point-source escape fraction by quadrature, HG moments, emission laws / mean number of
@@ -183,8 +193,8 @@ soc_oracle_grid *soc_oracle_grid_create(int32_t nx, int32_t ny, int32_t nz, int3
 typedef struct {
     int32_t level;      /* l = 1..n_levels */
     int32_t cell;       /* index within the level: authoritative, never re-derived (S4) */
-    double f[3];        /* position inside the cell, in units of the cell edge, [0,1]^3 */
-    double d[3];        /* unit direction */
+    float f[3];         /* position inside the cell, in units of the cell edge, [0,1]^3 (fp32 state, S11) */
+    float d[3];         /* direction, unit length up to fp32 rounding */
 } soc_oracle_state;
 
 typedef struct {
@@ -241,8 +251,8 @@ static void descend(const soc_oracle_grid *G, soc_oracle_state *S)
         if (ch < 0) return;
         int32_t slot = 0;
         for (int j = 0; j < 3; ++j) {
-            if (S->f[j] >= 0.5) { slot |= (1 << j); S->f[j] = 2.0 * S->f[j] - 1.0; }
-            else S->f[j] = 2.0 * S->f[j];
+            if (S->f[j] >= 0.5f) { slot |= (1 << j); S->f[j] = (float)(2.0 * (double)S->f[j] - 1.0); }
+            else S->f[j] = (float)(2.0 * (double)S->f[j]);
         }
         S->cell = ch + slot;
         S->level += 1;
@@ -264,11 +274,11 @@ static int move_across(const soc_oracle_grid *G, soc_oracle_state *S, int a, int
         }
         int bit = (S->cell >> a) & 1;
         if ((sg > 0 && bit == 0) || (sg < 0 && bit == 1)) { S->cell ^= (1 << a); break; }
-        for (int j = 0; j < 3; ++j) S->f[j] = (S->f[j] + (double)((S->cell >> j) & 1)) * 0.5;
+        for (int j = 0; j < 3; ++j) S->f[j] = (float)(((double)S->f[j] + (double)((S->cell >> j) & 1)) * 0.5);
         S->cell = G->parent[S->level - 1][S->cell >> 3];
         S->level -= 1;
     }
-    S->f[a] = (sg > 0) ? 0.0 : 1.0;   /* entry face, in the neighbour's frame */
+    S->f[a] = (sg > 0) ? 0.0f : 1.0f; /* entry face, in the neighbour's frame */
     descend(G, S);
     return 1;
 }
@@ -351,7 +361,7 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
     for (int64_t p = pkg_begin; p < pkg_begin + pkg_count; ++p) {
         soc_oracle_state S;
         int32_t ijk[3];
-        double E0;
+        double E0, f0[3], d0[3];
         uint32_t w0[4], w1[4];
         soc_oracle_stream_block(seed, ifreq, p, 0u, w0);
         soc_oracle_stream_block(seed, ifreq, p, 1u, w1);
@@ -361,13 +371,13 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
                 ijk[j] = (int32_t)floor(src->beam[j]);
                 int32_t nj = (j == 0) ? G->nx : (j == 1) ? G->ny : G->nz;
                 if (ijk[j] > nj - 1) ijk[j] = nj - 1;     /* a beam may start on the upper boundary */
-                S.f[j] = src->beam[j] - ijk[j];
-                S.d[j] = src->beam[3 + j];
+                f0[j] = src->beam[j] - ijk[j];
+                d0[j] = src->beam[3 + j];
             }
         } else if (p < n_bg) {
             double u[5] = { soc_oracle_uniform(w0[0]), soc_oracle_uniform(w0[1]), soc_oracle_uniform(w0[2]),
                             soc_oracle_uniform(w0[3]), soc_oracle_uniform(w1[0]) };
-            soc_oracle_emit_background(G->nx, G->ny, G->nz, u, ijk, S.f, S.d);
+            soc_oracle_emit_background(G->nx, G->ny, G->nz, u, ijk, f0, d0);
             E0 = SOC_O_PI * src->bg_intensity * surf / (double)n_bg;
         } else {
             int64_t q = p - n_bg, n_ps = n_packages - n_bg;
@@ -375,9 +385,10 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
             /* count_k = number of ids q in [0, n_ps) with q mod n_point == k */
             int64_t count_k = n_ps / src->n_point + ((n_ps % src->n_point) > k ? 1 : 0);
             double u[2] = { soc_oracle_uniform(w0[0]), soc_oracle_uniform(w0[1]) };
-            soc_oracle_emit_point(src->ps_pos + 3 * k, u, ijk, S.f, S.d);
+            soc_oracle_emit_point(src->ps_pos + 3 * k, u, ijk, f0, d0);
             E0 = src->ps_lum[k] / (double)count_k;
         }
+        for (int j = 0; j < 3; ++j) { S.f[j] = (float)f0[j]; S.d[j] = (float)d0[j]; }   /* fp32 state */
         S.level = 1;
         S.cell = ijk[0] + G->nx * (ijk[1] + G->ny * ijk[2]);
         descend(G, &S);
@@ -389,8 +400,8 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
         double e_esc = 0.0;
         uint32_t ws[4];
         soc_oracle_stream_block(seed, ifreq, p, 2u + seg, ws);
-        double tau_drawn = -log(soc_oracle_uniform(ws[0]));   /* a4: free path, scattering depth */
-        double tau_rem = tau_drawn;
+        float tau_drawn = (float)(-log(soc_oracle_uniform(ws[0])));   /* a4: free path, scattering depth */
+        float tau_rem = tau_drawn;
 
         for (;;) {
             const int64_t gid = G->level_off[S.level - 1] + S.cell;
@@ -399,8 +410,9 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
             /* a5/a6: distance (in cell edges) to the face of each axis */
             double t[3];
             for (int j = 0; j < 3; ++j) {
-                if (S.d[j] > 0.0) t[j] = (1.0 - S.f[j]) / S.d[j];
-                else if (S.d[j] < 0.0) t[j] = (-S.f[j]) / S.d[j];
+                const double fj = (double)S.f[j], dj = (double)S.d[j];
+                if (dj > 0.0) t[j] = (1.0 - fj) / dj;
+                else if (dj < 0.0) t[j] = (-fj) / dj;
                 else t[j] = INFINITY;
                 if (t[j] < 0.0) t[j] = 0.0;
             }
@@ -413,9 +425,9 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
             const double dtau = ds * ks_rho;
             int scatter = 0;
             double ds_used = ds, t_used = tstar;
-            if (ks_rho > 0.0 && dtau >= tau_rem) {
+            if (ks_rho > 0.0 && dtau >= (double)tau_rem) {
                 scatter = 1;
-                ds_used = tau_rem / ks_rho;
+                ds_used = (double)tau_rem / ks_rho;
                 t_used = ds_used / h;
             }
             /* a7: path-length estimator, continuous absorption */
@@ -432,8 +444,8 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
                 double org[3];
                 cell_origin(G, S.level, S.cell, org);
                 T->pkg = p; T->gid = gid; T->level = S.level; T->kind = scatter ? 1 : 0;
-                for (int j = 0; j < 3; ++j) T->p0[j] = org[j] + h * S.f[j];
-                T->ds = ds_used; T->tau_sca = ds_used * ks_rho; T->tau_drawn = tau_drawn;
+                for (int j = 0; j < 3; ++j) T->p0[j] = org[j] + h * (double)S.f[j];
+                T->ds = ds_used; T->tau_sca = ds_used * ks_rho; T->tau_drawn = (double)tau_drawn;
             }
             /* a9: termination */
             if (E < SOC_O_WMIN * E0) {
@@ -441,33 +453,34 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
                 R.absorbed += E;
                 E = 0.0;
                 R.terminated += 1;
-                if (T) { T->kind = 2; for (int j = 0; j < 3; ++j) T->p1[j] = T->p0[j] + ds_used * S.d[j]; }
+                if (T) { T->kind = 2; for (int j = 0; j < 3; ++j) T->p1[j] = T->p0[j] + ds_used * (double)S.d[j]; }
                 break;
             }
             for (int j = 0; j < 3; ++j) {
-                S.f[j] += t_used * S.d[j];
-                if (S.f[j] < 0.0) S.f[j] = 0.0;
-                if (S.f[j] > 1.0) S.f[j] = 1.0;
+                double fn = (double)S.f[j] + t_used * (double)S.d[j];
+                if (fn < 0.0) fn = 0.0;
+                if (fn > 1.0) fn = 1.0;
+                S.f[j] = (float)fn;
             }
             if (T) {
                 double org[3];
                 cell_origin(G, S.level, S.cell, org);
-                for (int j = 0; j < 3; ++j) T->p1[j] = org[j] + h * S.f[j];
+                for (int j = 0; j < 3; ++j) T->p1[j] = org[j] + h * (double)S.f[j];
             }
             if (scatter) {
                 /* a8 */
                 double cost = soc_oracle_hg_cos(g, soc_oracle_uniform(ws[1]));
                 double phi = 2.0 * SOC_O_PI * soc_oracle_uniform(ws[2]);
-                double nd[3];
-                soc_oracle_rotate(S.d, cost, phi, nd);
-                S.d[0] = nd[0]; S.d[1] = nd[1]; S.d[2] = nd[2];
+                double od[3] = { (double)S.d[0], (double)S.d[1], (double)S.d[2] }, nd[3];
+                soc_oracle_rotate(od, cost, phi, nd);
+                S.d[0] = (float)nd[0]; S.d[1] = (float)nd[1]; S.d[2] = (float)nd[2];
                 seg += 1; scat += 1;
                 soc_oracle_stream_block(seed, ifreq, p, 2u + seg, ws);
-                tau_drawn = -log(soc_oracle_uniform(ws[0]));
+                tau_drawn = (float)(-log(soc_oracle_uniform(ws[0])));
                 tau_rem = tau_drawn;
             } else {
-                tau_rem -= dtau;
-                if (!move_across(G, &S, a, S.d[a] > 0.0 ? 1 : -1)) {
+                tau_rem = (float)((double)tau_rem - dtau);
+                if (!move_across(G, &S, a, S.d[a] > 0.0f ? 1 : -1)) {
                     e_esc = E;                           /* a9: escape */
                     R.escaped += E;
                     if (T) T->kind = 3;

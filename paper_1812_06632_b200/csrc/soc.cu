@@ -1,0 +1,989 @@
+// libsoc_b200 -- photon-package simulation and temperature kernels for sm_100a, plus the C ABI of
+// include/soc.h.  See DESIGN.md for the data layout, the kernels and the rooflines that bound them.
+//
+// No tensor cores here: the path is a random walk with one dependent 4-byte gather and one 8-byte
+// scatter-add per cell-step, not a dense contraction (BASELINE.json:north_star).
+#include "soc.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+// ------------------------------------------------------------------------------------------------
+// host-side bookkeeping
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+thread_local std::string g_last_error;
+unsigned long long g_launches = 0;
+
+int fail(int code, const std::string &msg)
+{
+    g_last_error = msg;
+    return code;
+}
+
+#define SOC_CUDA(call)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return fail(SOC_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));             \
+    } while (0)
+
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kWMin = 1e-9;          // termination threshold relative to the initial weight (reading S7)
+constexpr int kChunk = 64;              // package ids a warp claims from the global counter at a time
+constexpr unsigned kFull = 0xffffffffu;
+
+struct DevResult {                      // one slot per launch, accumulated with atomics
+    double emitted, escaped, absorbed;
+    unsigned long long cell_steps, scatterings, terminated;
+};
+
+struct SimParams {
+    // grid
+    int nx, ny, nz, n_root;
+    const uint32_t *cellw;              // [n_total] leaf: fp32 density bits; parent: 0x80000000 | (first child id - n_root)
+    const int32_t *parent;              // [n_octets] (parent id - n_root) of octet (id - n_root) >> 3
+    // dust at this frequency
+    double kabs, ksca, g;
+    // sources
+    int is_beam, n_point;
+    long long n_bg;
+    double bg_e0, surf;
+    double beam[6];
+    double ps_pos[SOC_MAX_POINT_SOURCES][3];
+    double ps_e0[SOC_MAX_POINT_SOURCES];
+    // run
+    long long pkg_begin, pkg_end;
+    unsigned long long seed;
+    int ifreq;
+    int refill_threshold;
+    double weight;
+    double *absorbed;
+    soc_replay_record *replay;
+    unsigned long long *counter;
+    DevResult *result;
+};
+
+}  // namespace
+
+struct soc_grid {
+    int nx = 0, ny = 0, nz = 0, n_levels = 0, n_freq = 0;
+    long long n_total = 0, n_root = 0, n_octets = 0;
+    long long level_off[SOC_MAX_LEVELS + 1] = {0};
+    std::vector<double> freq, kabs, ksca, g;
+    uint32_t *d_cellw = nullptr;
+    int32_t *d_parent = nullptr;
+    DevResult *d_results = nullptr;           // n_slots
+    unsigned long long *d_counters = nullptr; // n_slots
+    DevResult *h_results = nullptr;           // pinned, n_slots
+    float *d_table = nullptr;
+    int n_slots = 0;
+    int device = 0, n_sm = 0;
+    int opt_blocks_per_sm = 0;                // 0 = from the occupancy calculator
+    int opt_threads = 256;
+    int opt_refill_threshold = 1;
+};
+
+// ------------------------------------------------------------------------------------------------
+// device code
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+// a1: Philox4x32-10 (Salmon et al. 2011), counter (block, pkg_lo, pkg_hi, ifreq), key (seed_lo, seed_hi)
+__device__ __forceinline__ void philox_block(unsigned long long seed, int ifreq, long long pkg, uint32_t block,
+                                             uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3)
+{
+    uint32_t c0 = block, c1 = (uint32_t)((unsigned long long)pkg), c2 = (uint32_t)((unsigned long long)pkg >> 32),
+             c3 = (uint32_t)ifreq;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+}
+
+// word -> ((x >> 9) + 0.5) 2^-23, exact in fp32 and fp64
+template <typename R> __device__ __forceinline__ R uniform01(uint32_t w)
+{
+    return (R)(2u * (w >> 9) + 1u) * (R)(1.0 / 16777216.0);
+}
+
+template <typename R> struct RM;
+template <> struct RM<float> {
+    static __device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
+    static __device__ __forceinline__ float log_(float x) { return logf(x); }
+    static __device__ __forceinline__ void sincospi_(float x, float *s, float *c) { sincospif(x, s, c); }
+    static __device__ __forceinline__ float inf() { return __int_as_float(0x7f800000); }
+    static __device__ __forceinline__ float copysign_(float a, float b) { return copysignf(a, b); }
+};
+template <> struct RM<double> {
+    static __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+    static __device__ __forceinline__ double log_(double x) { return log(x); }
+    static __device__ __forceinline__ void sincospi_(double x, double *s, double *c) { sincospi(x, s, c); }
+    static __device__ __forceinline__ double inf() { return __longlong_as_double(0x7ff0000000000000ll); }
+    static __device__ __forceinline__ double copysign_(double a, double b) { return copysign(a, b); }
+};
+
+// Precision (reading S11): the package state (position in the cell, direction, remaining optical
+// depth) is fp32; A is the type the updates are evaluated in before they are rounded back to fp32:
+//   A = float  : production (SOC_GEOM_FP32)
+//   A = double : replay (SOC_GEOM_FP64) -- the same evaluation as the fp64 oracle up to 1e-16, so the
+//                rounded fp32 state stays bit-identical except within 2^-29 of a rounding boundary.
+template <typename A> __device__ __forceinline__ float clamp01f(A x)
+{
+    return (float)(x < (A)0 ? (A)0 : (x > (A)1 ? (A)1 : x));
+}
+
+// per-lane package state
+template <typename A> struct Pkg {
+    float fx, fy, fz;      // position inside the cell, units of the cell edge, [0,1]
+    float dx, dy, dz;      // direction (unit length up to fp32 rounding)
+    A rx, ry, rz;          // 1 / direction, in the arithmetic type
+    float tau_rem;         // remaining scattering optical depth of the flight segment
+    float h;               // cell edge 2^-(level-1), exact
+    int ix, iy, iz;        // root cell
+    int rel;               // HIER: cell id - n_root (< 0: root cell, level 1); regular grid: cell id
+    uint32_t cw;           // cell word of the current cell (fp32 density bits for a leaf)
+    uint32_t w_hg, w_az;   // words 1, 2 of the current segment's Philox block
+    uint32_t seg, steps, scat;
+    unsigned long long hash;
+    double E, e_min;       // weight and termination threshold 1e-9 E0
+    double pend;           // energy absorbed in the current cell, not yet added to the accumulator
+    long long id;
+};
+
+template <typename A> __device__ __forceinline__ void set_direction(Pkg<A> &p, A dx, A dy, A dz)
+{
+    p.dx = (float)dx; p.dy = (float)dy; p.dz = (float)dz;
+    p.rx = (A)1 / (A)p.dx; p.ry = (A)1 / (A)p.dy; p.rz = (A)1 / (A)p.dz;
+}
+
+// a6: descend to the leaf that holds the position; 2f and 2f-1 are exact in fp32
+template <typename A> __device__ __forceinline__ void descend(const SimParams &P, Pkg<A> &p)
+{
+    uint32_t cw = __ldg(P.cellw + (p.rel + P.n_root));
+    while ((int32_t)cw < 0) {
+        int slot = 0;
+        if (p.fx >= 0.5f) { slot |= 1; p.fx = 2.0f * p.fx - 1.0f; } else p.fx = 2.0f * p.fx;
+        if (p.fy >= 0.5f) { slot |= 2; p.fy = 2.0f * p.fy - 1.0f; } else p.fy = 2.0f * p.fy;
+        if (p.fz >= 0.5f) { slot |= 4; p.fz = 2.0f * p.fz - 1.0f; } else p.fz = 2.0f * p.fz;
+        p.rel = (int)(cw & 0x7fffffffu) + slot;
+        p.h *= 0.5f;
+        cw = __ldg(P.cellw + (p.rel + P.n_root));
+    }
+    p.cw = cw;
+}
+
+// a1-a3: create package `id` (SURVEY.md 8c.3 / DESIGN.md readings S2, S3)
+template <typename A, bool HIER>
+__device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long id)
+{
+    double e0;
+    A dx, dy, dz;
+    p.id = id;
+    if (P.is_beam) {
+        const int n[3] = {P.nx, P.ny, P.nz};
+        int c[3];
+        float f[3];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            int i = (int)floor(P.beam[j]);
+            i = i > n[j] - 1 ? n[j] - 1 : i;
+            c[j] = i;
+            f[j] = (float)(P.beam[j] - (double)i);
+        }
+        p.ix = c[0]; p.iy = c[1]; p.iz = c[2];
+        p.fx = f[0]; p.fy = f[1]; p.fz = f[2];
+        dx = (A)P.beam[3]; dy = (A)P.beam[4]; dz = (A)P.beam[5];
+        e0 = 1.0;
+    } else if (id < P.n_bg) {
+        uint32_t w0, w1, w2, w3, v0, v1, v2, v3;
+        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
+        philox_block(P.seed, P.ifreq, id, 1u, v0, v1, v2, v3);
+        // face in proportion to its area, order x-, x+, y-, y+, z-, z+ (exact in fp64 like the definition)
+        const double ax = (double)P.ny * P.nz, ay = (double)P.nz * P.nx, az = (double)P.nx * P.ny;
+        const double x = uniform01<double>(w0) * P.surf;
+        int face = 5;
+        if (x < ax) face = 0;
+        else if (x < 2 * ax) face = 1;
+        else if (x < 2 * ax + ay) face = 2;
+        else if (x < 2 * ax + 2 * ay) face = 3;
+        else if (x < 2 * ax + 2 * ay + az) face = 4;
+        const int a = face >> 1, high = face & 1;
+        const int n1 = a == 0 ? P.ny : (a == 1 ? P.nz : P.nx);     // extent along a1 = (a+1)%3
+        const int n2 = a == 0 ? P.nz : (a == 1 ? P.nx : P.ny);     // extent along a2 = (a+2)%3
+        const int na = a == 0 ? P.nx : (a == 1 ? P.ny : P.nz);
+        // u*N = (2k+1) N / 2^24: integer cell and fraction, rounded once to fp32 like fl32(u*N - i)
+        const unsigned long long m1 = (unsigned long long)(2u * (w1 >> 9) + 1u) * (unsigned)n1;
+        const unsigned long long m2 = (unsigned long long)(2u * (w2 >> 9) + 1u) * (unsigned)n2;
+        const int i1 = (int)(m1 >> 24), i2 = (int)(m2 >> 24);
+        const float f1 = (float)(uint32_t)(m1 & 0xffffffu) * (float)(1.0 / 16777216.0);
+        const float f2 = (float)(uint32_t)(m2 & 0xffffffu) * (float)(1.0 / 16777216.0);
+        const int ia = high ? na - 1 : 0;
+        const float fa = high ? 1.0f : 0.0f;
+        const A u3 = uniform01<A>(w3);
+        const A mu = RM<A>::sqrt_(u3), st = RM<A>::sqrt_((A)1 - u3);
+        A sp, cp;
+        RM<A>::sincospi_((A)2 * uniform01<A>(v0), &sp, &cp);
+        const A da = high ? -mu : mu, d1 = st * cp, d2 = st * sp;
+        if (a == 0)      { p.ix = ia; p.iy = i1; p.iz = i2; p.fx = fa; p.fy = f1; p.fz = f2; dx = da; dy = d1; dz = d2; }
+        else if (a == 1) { p.iy = ia; p.iz = i1; p.ix = i2; p.fy = fa; p.fz = f1; p.fx = f2; dy = da; dz = d1; dx = d2; }
+        else             { p.iz = ia; p.ix = i1; p.iy = i2; p.fz = fa; p.fx = f1; p.fy = f2; dz = da; dx = d1; dy = d2; }
+        e0 = P.bg_e0;
+    } else {
+        uint32_t w0, w1, w2, w3;
+        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
+        const int k = (int)((id - P.n_bg) % P.n_point);
+        const double px = P.ps_pos[k][0], py = P.ps_pos[k][1], pz = P.ps_pos[k][2];
+        p.ix = (int)floor(px); p.iy = (int)floor(py); p.iz = (int)floor(pz);
+        p.fx = (float)(px - (double)p.ix); p.fy = (float)(py - (double)p.iy); p.fz = (float)(pz - (double)p.iz);
+        const A mu = (A)2 * uniform01<A>(w0) - (A)1;
+        const A st = RM<A>::sqrt_(fmax((A)0, (A)1 - mu * mu));
+        A sp, cp;
+        RM<A>::sincospi_((A)2 * uniform01<A>(w1), &sp, &cp);
+        dx = st * cp; dy = st * sp; dz = mu;
+        e0 = P.ps_e0[k];
+    }
+    set_direction(p, dx, dy, dz);
+    p.h = 1.0f;
+    const int root = p.ix + P.nx * (p.iy + P.ny * p.iz);
+    if (HIER) {
+        p.rel = root - P.n_root;
+        descend(P, p);
+    } else {
+        p.rel = root;
+        p.cw = __ldg(P.cellw + root);
+    }
+    p.seg = 0; p.steps = 0; p.scat = 0;
+    p.hash = 0xcbf29ce484222325ull;
+    p.E = e0;
+    p.e_min = kWMin * e0;
+    p.pend = 0.0;
+    uint32_t s0, s1, s2, s3;
+    philox_block(P.seed, P.ifreq, id, 2u, s0, s1, s2, s3);
+    p.tau_rem = (float)(-RM<A>::log_(uniform01<A>(s0)));          // a4
+    p.w_hg = s1; p.w_az = s2;
+    return e0;
+}
+
+// a8: Henyey-Greenstein polar angle in the cancellation-free form (reading S6), rotation (Duff et al. 2017 basis)
+template <typename A> __device__ __forceinline__ void scatter(const SimParams &P, Pkg<A> &p)
+{
+    const A g = (A)P.g;
+    const A odx = (A)p.dx, ody = (A)p.dy, odz = (A)p.dz;
+    const A mu0 = (A)2 * uniform01<A>(p.w_hg) - (A)1;
+    const A num = mu0 + g * ((A)3 + mu0 * mu0) * (A)0.5 + g * g * mu0 + g * g * g * (mu0 * mu0 - (A)1) * (A)0.5;
+    const A den = ((A)1 + g * mu0) * ((A)1 + g * mu0);
+    A ct = num / den;
+    ct = ct > (A)1 ? (A)1 : (ct < (A)-1 ? (A)-1 : ct);
+    const A st = RM<A>::sqrt_(fmax((A)0, (A)1 - ct * ct));
+    A sp, cp;
+    RM<A>::sincospi_((A)2 * uniform01<A>(p.w_az), &sp, &cp);
+    const A sg = RM<A>::copysign_((A)1, odz);
+    const A a = (A)-1 / (sg + odz);
+    const A b = odx * ody * a;
+    const A t1x = (A)1 + sg * odx * odx * a, t1y = sg * b, t1z = -sg * odx;
+    const A t2x = b, t2y = sg + ody * ody * a, t2z = -ody;
+    const A c1 = st * cp, c2 = st * sp;
+    const A nx = c1 * t1x + c2 * t2x + ct * odx;
+    const A ny = c1 * t1y + c2 * t2y + ct * ody;
+    const A nz = c1 * t1z + c2 * t2z + ct * odz;
+    const A inv = (A)1 / RM<A>::sqrt_(nx * nx + ny * ny + nz * nz);
+    set_direction(p, nx * inv, ny * inv, nz * inv);
+    p.seg += 1; p.scat += 1;
+    uint32_t s0, s1, s2, s3;
+    philox_block(P.seed, P.ifreq, p.id, 2u + p.seg, s0, s1, s2, s3);
+    p.tau_rem = (float)(-RM<A>::log_(uniform01<A>(s0)));
+    p.w_hg = s1; p.w_az = s2;
+}
+
+// a5/a6: move across the face of axis a in direction sg.  Returns false when the package leaves the grid.
+template <typename A, bool HIER>
+__device__ __forceinline__ bool move_across(const SimParams &P, Pkg<A> &p, int a, int sg)
+{
+    if (HIER) {
+        // sibling flip, else up to the common parent; (f + bit)/2 rounds once to fp32
+        while (p.rel >= 0) {
+            const int bit = (p.rel >> a) & 1;
+            if ((sg > 0) != (bit != 0)) { p.rel ^= (1 << a); goto found; }
+            p.fx = (p.fx + (float)(p.rel & 1)) * 0.5f;
+            p.fy = (p.fy + (float)((p.rel >> 1) & 1)) * 0.5f;
+            p.fz = (p.fz + (float)((p.rel >> 2) & 1)) * 0.5f;
+            p.rel = __ldg(P.parent + (p.rel >> 3));
+            p.h *= 2.0f;
+        }
+    }
+    {
+        bool out;
+        if (a == 0)      { p.ix += sg; out = (unsigned)p.ix >= (unsigned)P.nx; }
+        else if (a == 1) { p.iy += sg; out = (unsigned)p.iy >= (unsigned)P.ny; }
+        else             { p.iz += sg; out = (unsigned)p.iz >= (unsigned)P.nz; }
+        if (out) return false;
+        const int root = p.ix + P.nx * (p.iy + P.ny * p.iz);
+        p.rel = HIER ? root - P.n_root : root;
+    }
+found:
+    {
+        const float face = sg > 0 ? 0.0f : 1.0f;      // entry face in the neighbour's frame
+        if (a == 0) p.fx = face; else if (a == 1) p.fy = face; else p.fz = face;
+    }
+    if (HIER) descend(P, p);
+    else p.cw = __ldg(P.cellw + p.rel);
+    return true;
+}
+
+template <typename A, bool HIER, bool REPLAY>
+__global__ void __launch_bounds__(256) photon_kernel(const __grid_constant__ SimParams P)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    double acc_emit = 0.0, acc_esc = 0.0, acc_abs = 0.0;
+    unsigned long long acc_steps = 0;
+    unsigned acc_scat = 0, acc_term = 0;
+    Pkg<A> p;
+    bool active = false;
+    long long pool_next = 0, pool_end = 0;       // warp-uniform id pool
+    bool exhausted = false;
+    const A ksca = (A)P.ksca;
+    const float kabs_f = (float)P.kabs;
+
+    for (;;) {
+        unsigned idle = __ballot_sync(kFull, !active);
+        if (idle && !exhausted && (__popc(idle) >= P.refill_threshold || idle == kFull)) {
+            do {
+                if (pool_next >= pool_end) {
+                    long long base = 0;
+                    if (lane == 0) base = (long long)atomicAdd(P.counter, (unsigned long long)kChunk);
+                    base = __shfl_sync(kFull, base, 0) + P.pkg_begin;
+                    if (base >= P.pkg_end) { exhausted = true; break; }
+                    pool_next = base;
+                    pool_end = base + kChunk < P.pkg_end ? base + kChunk : P.pkg_end;
+                }
+                const long long avail = pool_end - pool_next;
+                const int rank = __popc(idle & lt_mask);
+                if (!active && rank < avail) {
+                    acc_emit += emit<A, HIER>(P, p, pool_next + rank);
+                    active = true;
+                }
+                const int n_idle = __popc(idle);
+                pool_next += n_idle < avail ? n_idle : avail;
+                idle = __ballot_sync(kFull, !active);
+            } while (idle);
+        }
+        if (idle == kFull) break;                // nothing left for this warp
+
+        if (active) {
+            // ---- geometry: distance (in cell edges) to the face of each axis
+            const A inf = RM<A>::inf();
+            const A tx = p.dx == 0.0f ? inf : ((p.dx > 0.0f ? (A)1 : (A)0) - (A)p.fx) * p.rx;
+            const A ty = p.dy == 0.0f ? inf : ((p.dy > 0.0f ? (A)1 : (A)0) - (A)p.fy) * p.ry;
+            const A tz = p.dz == 0.0f ? inf : ((p.dz > 0.0f ? (A)1 : (A)0) - (A)p.fz) * p.rz;
+            int a = 0;
+            A ts = tx;
+            if (ty < ts) { a = 1; ts = ty; }         // lowest axis wins a tie (reading S4)
+            if (tz < ts) { a = 2; ts = tz; }
+            const float rho = __uint_as_float(p.cw);
+            const A ds = HIER ? ts * (A)p.h : ts;
+            const A ksr = (A)rho * ksca;
+            const A dtau = ds * ksr;
+            const bool sc = ksr > (A)0 && dtau >= (A)p.tau_rem;
+            A ds_u = ds, t_u = ts;
+            if (sc) {
+                ds_u = (A)p.tau_rem / ksr;
+                t_u = HIER ? ds_u / (A)p.h : ds_u;
+            }
+            // ---- a7: path-length estimator, continuous absorption
+            const int gid = HIER ? p.rel + P.n_root : p.rel;
+            const float x = (float)ds_u * rho * kabs_f;
+            double frac;
+            if (x > 4.0f) frac = -expm1(-((double)ds_u * (double)rho * P.kabs));   // rare: keep the tail of the weight
+            else frac = (double)(-expm1f(-x));
+            double dep = p.E * frac;
+            double e_new = p.E - dep;
+            const bool term = e_new < p.e_min;      // a9: residual stays in the cell
+            if (term) { dep = p.E; e_new = 0.0; }
+            p.pend += dep;
+            acc_abs += dep;
+            p.E = e_new;
+            p.steps += 1;
+            if (REPLAY) p.hash = (p.hash ^ (unsigned long long)gid) * 0x100000001b3ull;
+            bool done = term;
+            bool flush = term;
+            double e_esc = 0.0;
+            if (term) {
+                acc_term += 1;
+            } else {
+                p.fx = clamp01f<A>((A)p.fx + t_u * (A)p.dx);
+                p.fy = clamp01f<A>((A)p.fy + t_u * (A)p.dy);
+                p.fz = clamp01f<A>((A)p.fz + t_u * (A)p.dz);
+                if (sc) {
+                    scatter(P, p);
+                } else {
+                    flush = true;                    // leaving the cell: hand its energy to the accumulator
+                    p.tau_rem = (float)((A)p.tau_rem - dtau);
+                    const float da = a == 0 ? p.dx : (a == 1 ? p.dy : p.dz);
+                    if (!move_across<A, HIER>(P, p, a, da > 0.0f ? 1 : -1)) {
+                        e_esc = p.E;
+                        acc_esc += p.E;
+                        done = true;
+                    }
+                }
+            }
+            // scatterings inside one cell are summed in a register: one atomic per cell visit, not per
+            // step (the hot-cell contention of PAPER.md:151, 279)
+            if (flush) {
+                if (p.pend > 0.0) atomicAdd(P.absorbed + gid, P.weight * p.pend);
+                p.pend = 0.0;
+            }
+            if (done) {
+                acc_steps += p.steps;
+                acc_scat += p.scat;
+                if (REPLAY) {
+                    soc_replay_record r;
+                    r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = e_esc;
+                    P.replay[p.id - P.pkg_begin] = r;
+                }
+                active = false;
+            }
+        }
+    }
+
+    // ---- per-launch totals: warp shuffle reduction, one set of atomics per warp
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        acc_emit += __shfl_xor_sync(kFull, acc_emit, o);
+        acc_esc += __shfl_xor_sync(kFull, acc_esc, o);
+        acc_abs += __shfl_xor_sync(kFull, acc_abs, o);
+        acc_steps += __shfl_xor_sync(kFull, acc_steps, o);
+        acc_scat += __shfl_xor_sync(kFull, acc_scat, o);
+        acc_term += __shfl_xor_sync(kFull, acc_term, o);
+    }
+    if (lane == 0 && acc_steps != 0) {
+        atomicAdd(&P.result->emitted, acc_emit);
+        atomicAdd(&P.result->escaped, acc_esc);
+        atomicAdd(&P.result->absorbed, acc_abs);
+        atomicAdd(&P.result->cell_steps, acc_steps);
+        atomicAdd(&P.result->scatterings, (unsigned long long)acc_scat);
+        atomicAdd(&P.result->terminated, (unsigned long long)acc_term);
+    }
+}
+
+// a11: energy balance by table lookup, 4 cells per thread, table in shared memory
+struct TempParams {
+    const uint32_t *cellw;
+    const double *absorbed;
+    const float *table;
+    float *T_out;
+    long long n_total;
+    long long level_off[SOC_MAX_LEVELS + 1];
+    int n_levels, n_table;
+    double scale, e_min, e_max, inv_e_min;
+    float x_scale;          // (n_table - 1) / ln(E_max / E_min)
+};
+
+__device__ __forceinline__ float temperature_of(const TempParams &P, const float *tab, uint32_t cw, double a, double inv_vol)
+{
+    if ((int32_t)cw < 0) return 0.0f;                       // parent cell
+    const float rho = __uint_as_float(cw);
+    if (!(rho > 0.0f)) return 0.0f;
+    const double e = P.scale * a / (double)rho * inv_vol;
+    if (!(e > P.e_min)) return tab[0];                      // also cells never hit
+    if (e >= P.e_max) return tab[P.n_table - 1];
+    const float x = logf((float)(e * P.inv_e_min)) * P.x_scale;
+    int i = (int)x;
+    i = i > P.n_table - 2 ? P.n_table - 2 : i;
+    const float t0 = tab[i], t1 = tab[i + 1];
+    return fmaf(x - (float)i, t1 - t0, t0);
+}
+
+__global__ void __launch_bounds__(256) temperature_kernel(const __grid_constant__ TempParams P)
+{
+    extern __shared__ float tab[];
+    for (int i = threadIdx.x; i < P.n_table; i += blockDim.x) tab[i] = P.table[i];
+    __syncthreads();
+    const long long n4 = P.n_total >> 2;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n4 + 1; q += stride) {
+        const long long c0 = q << 2;
+        if (q < n4) {
+            const uint4 cw = __ldg(reinterpret_cast<const uint4 *>(P.cellw) + q);
+            const double2 a01 = __ldg(reinterpret_cast<const double2 *>(P.absorbed) + 2 * q);
+            const double2 a23 = __ldg(reinterpret_cast<const double2 *>(P.absorbed) + 2 * q + 1);
+            // the four cells may straddle a level boundary: find the inverse volume per cell
+            double iv[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                int l = 0;
+                while (l + 1 < P.n_levels && c0 + j >= P.level_off[l + 1]) ++l;
+                iv[j] = (double)(1ull << (3 * l));
+            }
+            float4 t;
+            t.x = temperature_of(P, tab, cw.x, a01.x, iv[0]);
+            t.y = temperature_of(P, tab, cw.y, a01.y, iv[1]);
+            t.z = temperature_of(P, tab, cw.z, a23.x, iv[2]);
+            t.w = temperature_of(P, tab, cw.w, a23.y, iv[3]);
+            reinterpret_cast<float4 *>(P.T_out)[q] = t;
+        } else {
+            for (long long c = c0; c < P.n_total; ++c) {     // ragged tail
+                int l = 0;
+                while (l + 1 < P.n_levels && c >= P.level_off[l + 1]) ++l;
+                P.T_out[c] = temperature_of(P, tab, P.cellw[c], P.absorbed[c], (double)(1ull << (3 * l)));
+            }
+        }
+    }
+}
+
+__global__ void scale_kernel(double *a, long long n, double s)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) a[i] *= s;
+}
+
+// roofline probes: random gathers / random reductions over a footprint
+__device__ __forceinline__ uint32_t mix32(uint32_t x)
+{
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(256) probe_kernel(void *buf, unsigned long long n_elem, long long ops_per_thread, float *sink)
+{
+    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t s = mix32(tid * 2654435761u + 12345u);
+    float acc = 0.f;
+    for (long long i = 0; i < ops_per_thread; ++i) {
+        s = mix32(s + 0x9e3779b9u);
+        const unsigned long long j = ((unsigned long long)s * n_elem) >> 32;
+        if (KIND == 0) acc += __ldg(reinterpret_cast<const float *>(buf) + j);
+        else if (KIND == 1) atomicAdd(reinterpret_cast<double *>(buf) + j, 1.0);
+        else atomicAdd(reinterpret_cast<float *>(buf) + j, 1.0f);
+    }
+    if (KIND == 0 && acc == 123.456f) *sink = acc;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+int ensure_slots(soc_grid *G, int n)
+{
+    if (n <= G->n_slots) return SOC_OK;
+    if (G->d_results) cudaFree(G->d_results);
+    if (G->d_counters) cudaFree(G->d_counters);
+    if (G->h_results) cudaFreeHost(G->h_results);
+    G->d_results = nullptr; G->d_counters = nullptr; G->h_results = nullptr; G->n_slots = 0;
+    SOC_CUDA(cudaMalloc(&G->d_results, sizeof(DevResult) * n));
+    SOC_CUDA(cudaMalloc(&G->d_counters, sizeof(unsigned long long) * n));
+    SOC_CUDA(cudaMallocHost(&G->h_results, sizeof(DevResult) * n));
+    G->n_slots = n;
+    return SOC_OK;
+}
+
+template <typename K> int blocks_for(soc_grid *G, K kernel, int threads, int *blocks)
+{
+    int per_sm = 0;
+    SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0));
+    if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
+    if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
+    *blocks = per_sm * G->n_sm;                 // persistent: a whole number of CTAs per SM
+    return SOC_OK;
+}
+
+template <typename R, bool HIER, bool REPLAY> int launch_photon(soc_grid *G, const SimParams &P, cudaStream_t st)
+{
+    int blocks = 0;
+    const int threads = G->opt_threads;
+    int rc = blocks_for(G, photon_kernel<R, HIER, REPLAY>, threads, &blocks);
+    if (rc != SOC_OK) return rc;
+    // do not launch more lanes than there are packages (rounded up to whole blocks)
+    const long long n_pkg = P.pkg_end - P.pkg_begin;
+    const long long need = (n_pkg + threads - 1) / threads;
+    if (need < blocks) blocks = (int)(need > 0 ? need : 1);
+    photon_kernel<R, HIER, REPLAY><<<blocks, threads, 0, st>>>(P);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    return SOC_OK;
+}
+
+int check_sources(const soc_grid *G, const soc_sources *src, long long n_packages, long long *n_bg_out)
+{
+    if (!src) return fail(SOC_EINVAL, "sources is NULL");
+    if (src->beam) {
+        for (int j = 0; j < 6; ++j)
+            if (!std::isfinite(src->beam[j])) return fail(SOC_EINVAL, "beam is not finite");
+        const int n[3] = {G->nx, G->ny, G->nz};
+        for (int j = 0; j < 3; ++j)
+            if (src->beam[j] < 0.0 || src->beam[j] > n[j]) return fail(SOC_EINVAL, "beam starts outside the grid");
+        *n_bg_out = 0;
+        return SOC_OK;
+    }
+    if (src->n_point < 0 || src->n_point > SOC_MAX_POINT_SOURCES) return fail(SOC_EINVAL, "n_point out of range");
+    if (src->n_point > 0 && (!src->ps_pos || !src->ps_lum)) return fail(SOC_EINVAL, "point source arrays are NULL");
+    const bool has_bg = src->bg_intensity > 0.0, has_ps = src->n_point > 0;
+    long long n_bg = src->n_bg;
+    if (n_bg < 0) n_bg = (has_bg && has_ps) ? n_packages / 2 : (has_bg ? n_packages : 0);
+    if (n_bg > n_packages) return fail(SOC_EINVAL, "n_bg > n_packages");
+    if (n_bg > 0 && !(has_bg && std::isfinite(src->bg_intensity)))
+        return fail(SOC_EINVAL, "background packages requested but bg_intensity <= 0");
+    if (n_packages - n_bg > 0 && !has_ps) return fail(SOC_EINVAL, "point-source packages requested but n_point == 0");
+    for (int k = 0; k < src->n_point; ++k) {
+        const double *q = src->ps_pos + 3 * k;
+        if (!(q[0] > 0.0 && q[0] < G->nx && q[1] > 0.0 && q[1] < G->ny && q[2] > 0.0 && q[2] < G->nz))
+            return fail(SOC_EINVAL, "point source outside the root grid");
+        if (!(src->ps_lum[k] >= 0.0) || !std::isfinite(src->ps_lum[k])) return fail(SOC_EINVAL, "bad point source luminosity");
+    }
+    *n_bg_out = n_bg;
+    return SOC_OK;
+}
+
+// enqueue one frequency into result slot `slot`
+int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long n_packages, unsigned long long seed,
+                      double weight, long long pkg_begin, long long pkg_count, double *absorbed,
+                      soc_replay_record *replay, uint32_t flags, int slot, cudaStream_t st)
+{
+    if (!G) return fail(SOC_EINVAL, "grid is NULL");
+    if (ifreq < 0 || ifreq >= G->n_freq) return fail(SOC_EINVAL, "ifreq out of range");
+    if (n_packages < 0 || pkg_begin < 0 || pkg_count < 0 || pkg_begin + pkg_count > n_packages)
+        return fail(SOC_EINVAL, "bad package range");
+    if (!absorbed) return fail(SOC_EINVAL, "absorbed is NULL");
+    if (!std::isfinite(weight)) return fail(SOC_EINVAL, "weight is not finite");
+    if (flags & ~1u) return fail(SOC_EINVAL, "unknown flags");
+    long long n_bg = 0;
+    int rc = check_sources(G, src, n_packages, &n_bg);
+    if (rc != SOC_OK) return rc;
+
+    SimParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.nx = G->nx; P.ny = G->ny; P.nz = G->nz; P.n_root = (int)G->n_root;
+    P.cellw = G->d_cellw; P.parent = G->d_parent;
+    P.kabs = G->kabs[ifreq]; P.ksca = G->ksca[ifreq]; P.g = G->g[ifreq];
+    P.surf = 2.0 * ((double)G->ny * G->nz + (double)G->nz * G->nx + (double)G->nx * G->ny);
+    P.n_bg = n_bg;
+    if (src->beam) {
+        P.is_beam = 1;
+        for (int j = 0; j < 6; ++j) P.beam[j] = src->beam[j];
+    } else {
+        P.n_point = src->n_point;
+        if (n_bg > 0) P.bg_e0 = kPi * src->bg_intensity * P.surf / (double)n_bg;
+        const long long n_ps = n_packages - n_bg;
+        for (int k = 0; k < src->n_point; ++k) {
+            for (int j = 0; j < 3; ++j) P.ps_pos[k][j] = src->ps_pos[3 * k + j];
+            const long long count_k = n_ps / src->n_point + ((n_ps % src->n_point) > k ? 1 : 0);
+            P.ps_e0[k] = count_k > 0 ? src->ps_lum[k] / (double)count_k : 0.0;
+        }
+    }
+    P.pkg_begin = pkg_begin; P.pkg_end = pkg_begin + pkg_count;
+    P.seed = seed; P.ifreq = ifreq; P.weight = weight;
+    P.refill_threshold = G->opt_refill_threshold;
+    P.absorbed = absorbed; P.replay = replay;
+    P.counter = G->d_counters + slot; P.result = G->d_results + slot;
+
+    SOC_CUDA(cudaMemsetAsync(G->d_counters + slot, 0, sizeof(unsigned long long), st));
+    SOC_CUDA(cudaMemsetAsync(G->d_results + slot, 0, sizeof(DevResult), st));
+    if (pkg_count == 0) return SOC_OK;
+    const bool hier = G->n_levels > 1, f64 = (flags & SOC_GEOM_FP64) != 0, rep = replay != nullptr;
+#define SOC_DISPATCH(R)                                                                             \
+    (hier ? (rep ? launch_photon<R, true, true>(G, P, st) : launch_photon<R, true, false>(G, P, st)) \
+          : (rep ? launch_photon<R, false, true>(G, P, st) : launch_photon<R, false, false>(G, P, st)))
+    return f64 ? SOC_DISPATCH(double) : SOC_DISPATCH(float);
+#undef SOC_DISPATCH
+}
+
+int fetch_results(soc_grid *G, int n, soc_freq_result *out, cudaStream_t st)
+{
+    SOC_CUDA(cudaMemcpyAsync(G->h_results, G->d_results, sizeof(DevResult) * n, cudaMemcpyDeviceToHost, st));
+    SOC_CUDA(cudaStreamSynchronize(st));
+    for (int i = 0; i < n; ++i) {
+        out[i].emitted = G->h_results[i].emitted; out[i].escaped = G->h_results[i].escaped;
+        out[i].absorbed = G->h_results[i].absorbed; out[i].cell_steps = G->h_results[i].cell_steps;
+        out[i].scatterings = G->h_results[i].scatterings; out[i].terminated = G->h_results[i].terminated;
+    }
+    return SOC_OK;
+}
+
+void trapezoid(const std::vector<double> &nu, std::vector<double> &w)
+{
+    const size_t n = nu.size();
+    w.assign(n, 1.0);
+    if (n < 2) return;
+    for (size_t i = 0; i < n; ++i) {
+        const double lo = nu[i > 0 ? i - 1 : 0], hi = nu[i + 1 < n ? i + 1 : n - 1];
+        w[i] = 0.5 * (hi - lo);
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *soc_last_error(void) { return g_last_error.c_str(); }
+const char *soc_version(void) { return "soc_b200 0.1 (sm_100a)"; }
+uint64_t soc_launch_count(void) { return g_launches; }
+
+void soc_grid_destroy(soc_grid *G)
+{
+    if (!G) return;
+    cudaFree(G->d_cellw); cudaFree(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
+    cudaFree(G->d_table);
+    if (G->h_results) cudaFreeHost(G->h_results);
+    delete G;
+}
+
+int64_t soc_grid_n_total(const soc_grid *G) { return G ? G->n_total : 0; }
+
+int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
+{
+    if (!d || !out) return fail(SOC_EINVAL, "NULL argument");
+    *out = nullptr;
+    if (d->nx < 1 || d->ny < 1 || d->nz < 1) return fail(SOC_EINVAL, "root grid dimensions must be >= 1");
+    if (d->n_levels < 1 || d->n_levels > SOC_MAX_LEVELS) return fail(SOC_EINVAL, "n_levels out of range");
+    if (!d->n_cells || !d->density) return fail(SOC_EINVAL, "n_cells / density is NULL");
+    if (d->n_levels > 1 && !d->child) return fail(SOC_EINVAL, "child is NULL for a hierarchical grid");
+    if (d->n_freq < 1 || !d->freq_hz || !d->kabs || !d->ksca || !d->g) return fail(SOC_EINVAL, "dust tables missing");
+    if (d->n_cells[0] != (int64_t)d->nx * d->ny * d->nz) return fail(SOC_EINVAL, "n_cells[0] != nx*ny*nz");
+    soc_grid *G = new (std::nothrow) soc_grid;
+    if (!G) return fail(SOC_ENOMEM, "out of host memory");
+    struct Guard { soc_grid *g; ~Guard() { if (g) soc_grid_destroy(g); } } guard{G};
+    G->nx = d->nx; G->ny = d->ny; G->nz = d->nz; G->n_levels = d->n_levels; G->n_freq = d->n_freq;
+    for (int l = 0; l < d->n_levels; ++l) {
+        if (d->n_cells[l] < 0 || (l > 0 && d->n_cells[l] % 8 != 0)) return fail(SOC_EINVAL, "level sizes must be multiples of 8");
+        G->level_off[l + 1] = G->level_off[l] + d->n_cells[l];
+    }
+    G->n_total = G->level_off[d->n_levels];
+    G->n_root = d->n_cells[0];
+    if (G->n_total >= (1ll << 31)) return fail(SOC_EINVAL, "more than 2^31 cells");
+    G->n_octets = (G->n_total - G->n_root) / 8;
+    for (int f = 0; f < d->n_freq; ++f) {
+        if (!std::isfinite(d->freq_hz[f]) || !(d->freq_hz[f] > 0) || (f > 0 && !(d->freq_hz[f] > d->freq_hz[f - 1])))
+            return fail(SOC_EINVAL, "freq_hz must be positive and strictly ascending");
+        if (!(d->kabs[f] >= 0) || !(d->ksca[f] >= 0) || !std::isfinite(d->kabs[f]) || !std::isfinite(d->ksca[f]))
+            return fail(SOC_EINVAL, "kabs / ksca must be finite and >= 0");
+        if (!(std::fabs(d->g[f]) < 1.0)) return fail(SOC_EINVAL, "|g| must be < 1");
+    }
+    G->freq.assign(d->freq_hz, d->freq_hz + d->n_freq);
+    G->kabs.assign(d->kabs, d->kabs + d->n_freq);
+    G->ksca.assign(d->ksca, d->ksca + d->n_freq);
+    G->g.assign(d->g, d->g + d->n_freq);
+
+    // cell words and reverse links (the link replaces the density of the parent; one reverse
+    // link per octet)
+    std::vector<uint32_t> cellw;
+    std::vector<int32_t> parent;
+    try {
+        cellw.resize((size_t)G->n_total);
+        parent.assign((size_t)(G->n_octets > 0 ? G->n_octets : 1), INT32_MIN);
+    } catch (const std::bad_alloc &) {
+        return fail(SOC_ENOMEM, "out of host memory");
+    }
+    for (int l = 0; l < d->n_levels; ++l) {
+        for (long long c = 0; c < d->n_cells[l]; ++c) {
+            const long long gid = G->level_off[l] + c;
+            const int32_t ch = d->child ? d->child[gid] : -1;
+            if (ch < 0) {
+                const float r = d->density[gid];
+                if (!(r >= 0.0f) || !std::isfinite(r)) return fail(SOC_EINVAL, "leaf density must be finite and >= 0");
+                float rp = r + 0.0f;                         // -0.0 -> +0.0 so that the sign bit means "parent"
+                uint32_t bits;
+                std::memcpy(&bits, &rp, 4);
+                cellw[(size_t)gid] = bits & 0x7fffffffu;
+                continue;
+            }
+            if (l + 1 >= d->n_levels || (ch & 7) != 0 || (long long)ch + 8 > d->n_cells[l + 1])
+                return fail(SOC_EINVAL, "child index out of range or not a multiple of 8");
+            const long long child_rel = G->level_off[l + 1] + ch - G->n_root;
+            if (parent[(size_t)(child_rel >> 3)] != INT32_MIN) return fail(SOC_EINVAL, "octet has two parents");
+            parent[(size_t)(child_rel >> 3)] = (int32_t)(gid - G->n_root);
+            cellw[(size_t)gid] = 0x80000000u | (uint32_t)child_rel;
+        }
+    }
+    for (long long o = 0; o < G->n_octets; ++o)
+        if (parent[(size_t)o] == INT32_MIN) return fail(SOC_EINVAL, "octet without a parent");
+
+    SOC_CUDA(cudaGetDevice(&G->device));
+    SOC_CUDA(cudaDeviceGetAttribute(&G->n_sm, cudaDevAttrMultiProcessorCount, G->device));
+    SOC_CUDA(cudaMalloc(&G->d_cellw, sizeof(uint32_t) * (size_t)G->n_total));
+    SOC_CUDA(cudaMalloc(&G->d_parent, sizeof(int32_t) * parent.size()));
+    SOC_CUDA(cudaMalloc(&G->d_table, sizeof(float) * 8192));
+    SOC_CUDA(cudaMemcpy(G->d_cellw, cellw.data(), sizeof(uint32_t) * (size_t)G->n_total, cudaMemcpyHostToDevice));
+    SOC_CUDA(cudaMemcpy(G->d_parent, parent.data(), sizeof(int32_t) * parent.size(), cudaMemcpyHostToDevice));
+    int rc = ensure_slots(G, d->n_freq > 8 ? d->n_freq : 8);
+    if (rc != SOC_OK) return rc;
+    guard.g = nullptr;
+    *out = G;
+    return SOC_OK;
+}
+
+int soc_freq_weights(const soc_grid *G, double *w)
+{
+    if (!G || !w) return fail(SOC_EINVAL, "NULL argument");
+    std::vector<double> ww;
+    trapezoid(G->freq, ww);
+    for (int f = 0; f < G->n_freq; ++f) w[f] = ww[f];
+    return SOC_OK;
+}
+
+int soc_set_option(soc_grid *G, const char *key, int64_t value)
+{
+    if (!G || !key) return fail(SOC_EINVAL, "NULL argument");
+    const std::string k(key);
+    if (k == "blocks_per_sm" && value >= 0 && value <= 32) G->opt_blocks_per_sm = (int)value;
+    else if (k == "threads" && (value == 64 || value == 128 || value == 256)) G->opt_threads = (int)value;
+    else if (k == "refill_threshold" && value >= 1 && value <= 32) G->opt_refill_threshold = (int)value;
+    else return fail(SOC_EINVAL, "unknown option or value out of range: " + k);
+    return SOC_OK;
+}
+
+int soc_simulate_packages(soc_grid *G, int32_t ifreq, const soc_sources *src, int64_t n_packages, uint64_t seed,
+                          double weight, int64_t pkg_begin, int64_t pkg_count, double *absorbed,
+                          soc_replay_record *replay, soc_freq_result *res, uint32_t flags, void *stream)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = enqueue_frequency(G, ifreq, src, n_packages, seed, weight, pkg_begin, pkg_count, absorbed, replay,
+                               flags, 0, st);
+    if (rc != SOC_OK) return rc;
+    if (res) return fetch_results(G, 1, res, st);
+    return SOC_OK;
+}
+
+int soc_simulate_frequency(soc_grid *G, int32_t ifreq, const soc_sources *src, int64_t n_packages, uint64_t seed,
+                           double weight, double *absorbed, soc_freq_result *res, uint32_t flags, void *stream)
+{
+    return soc_simulate_packages(G, ifreq, src, n_packages, seed, weight, 0, n_packages, absorbed, nullptr, res,
+                                 flags, stream);
+}
+
+int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_packages, uint64_t seed, int64_t pkg_begin,
+                          int64_t pkg_count, double *absorbed_int, soc_freq_result *results, uint32_t flags,
+                          void *stream)
+{
+    if (!G || !src) return fail(SOC_EINVAL, "NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<double> w;
+    trapezoid(G->freq, w);
+    int rc = ensure_slots(G, G->n_freq);
+    if (rc != SOC_OK) return rc;
+    for (int f = 0; f < G->n_freq; ++f) {
+        rc = enqueue_frequency(G, f, src + f, n_packages, seed, w[f], pkg_begin, pkg_count, absorbed_int, nullptr,
+                               flags, f, st);
+        if (rc != SOC_OK) return rc;
+    }
+    if (results) return fetch_results(G, G->n_freq, results, st);
+    return SOC_OK;
+}
+
+int soc_update_temperatures(soc_grid *G, const double *absorbed, double scale, const float *table_T, int32_t n_table,
+                            double E_min, double E_max, float *T_out, void *stream)
+{
+    if (!G || !absorbed || !table_T || !T_out) return fail(SOC_EINVAL, "NULL argument");
+    if (n_table < 2 || n_table > 8192) return fail(SOC_EINVAL, "n_table out of range");
+    if (!(E_min > 0.0) || !(E_max > E_min) || !std::isfinite(E_max) || !std::isfinite(scale))
+        return fail(SOC_EINVAL, "need 0 < E_min < E_max and a finite scale");
+    if ((reinterpret_cast<uintptr_t>(absorbed) & 15) || (reinterpret_cast<uintptr_t>(T_out) & 15))
+        return fail(SOC_EINVAL, "absorbed and T_out must be 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    SOC_CUDA(cudaMemcpyAsync(G->d_table, table_T, sizeof(float) * n_table, cudaMemcpyHostToDevice, st));
+    TempParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.cellw = G->d_cellw; P.absorbed = absorbed; P.table = G->d_table; P.T_out = T_out;
+    P.n_total = G->n_total; P.n_levels = G->n_levels; P.n_table = n_table;
+    for (int l = 0; l <= G->n_levels; ++l) P.level_off[l] = G->level_off[l];
+    P.scale = scale; P.e_min = E_min; P.e_max = E_max; P.inv_e_min = 1.0 / E_min;
+    P.x_scale = (float)((double)(n_table - 1) / std::log(E_max / E_min));
+    const long long n4 = (G->n_total >> 2) + 1;
+    long long blocks = (n4 + 255) / 256;
+    const long long cap = (long long)G->n_sm * 8;       // grid-stride over a whole number of CTAs per SM
+    if (blocks > cap) blocks = cap;
+    temperature_kernel<<<(int)blocks, 256, sizeof(float) * n_table, st>>>(P);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    return SOC_OK;
+}
+
+int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_packages, uint64_t seed, int32_t n_iter,
+                 double t_scale, const float *table_T, int32_t n_table, double E_min, double E_max,
+                 double *absorbed_int_out, float *T_out, soc_freq_result *results, uint32_t flags)
+{
+    if (n_iter < 1) return fail(SOC_EINVAL, "n_iter must be >= 1");
+    soc_grid *G = nullptr;
+    int rc = soc_grid_create(desc, &G);
+    if (rc != SOC_OK) return rc;
+    double *d_abs = nullptr;
+    float *d_T = nullptr;
+    cudaStream_t st = nullptr;
+    auto cleanup = [&]() { cudaFree(d_abs); cudaFree(d_T); soc_grid_destroy(G); };
+    cudaError_t e = cudaMalloc(&d_abs, sizeof(double) * (size_t)G->n_total);
+    if (e == cudaSuccess) e = cudaMalloc(&d_T, sizeof(float) * (size_t)G->n_total);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_abs, 0, sizeof(double) * (size_t)G->n_total, st);
+    if (e != cudaSuccess) { cleanup(); return fail(SOC_ECUDA, cudaGetErrorString(e)); }
+    for (int it = 0; it < n_iter && rc == SOC_OK; ++it)
+        rc = soc_simulate_spectrum(G, src, n_packages, seed + (uint64_t)it, 0, n_packages, d_abs,
+                                   results ? results + (size_t)it * G->n_freq : nullptr, flags, st);
+    if (rc == SOC_OK && n_iter > 1) {                    // running mean over iterations (reading S12)
+        scale_kernel<<<G->n_sm * 4, 256, 0, st>>>(d_abs, G->n_total, 1.0 / n_iter);
+        g_launches += 1;
+    }
+    if (rc == SOC_OK && table_T && T_out)
+        rc = soc_update_temperatures(G, d_abs, t_scale, table_T, n_table, E_min, E_max, d_T, st);
+    if (rc == SOC_OK) {
+        if (absorbed_int_out) e = cudaMemcpyAsync(absorbed_int_out, d_abs, sizeof(double) * (size_t)G->n_total, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && T_out && table_T) e = cudaMemcpyAsync(T_out, d_T, sizeof(float) * (size_t)G->n_total, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) rc = fail(SOC_ECUDA, cudaGetErrorString(e));
+    }
+    cleanup();
+    return rc;
+}
+
+int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms)
+{
+    if (kind < 0 || kind > 2 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
+    const size_t elem = kind == 1 ? 8 : 4;
+    const unsigned long long n_elem = (unsigned long long)footprint_bytes / elem;
+    void *buf = nullptr;
+    float *sink = nullptr;
+    int dev = 0, n_sm = 0;
+    SOC_CUDA(cudaGetDevice(&dev));
+    SOC_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    SOC_CUDA(cudaMalloc(&buf, n_elem * elem));
+    SOC_CUDA(cudaMalloc(&sink, 4));
+    SOC_CUDA(cudaMemset(buf, 0, n_elem * elem));
+    const int blocks = n_sm * 8, threads = 256;
+    const long long per_thread = (n_ops + (long long)blocks * threads - 1) / ((long long)blocks * threads);
+    cudaEvent_t e0, e1;
+    SOC_CUDA(cudaEventCreate(&e0));
+    SOC_CUDA(cudaEventCreate(&e1));
+    for (int rep = 0; rep < 2; ++rep) {                  // first pass warms the caches / TLB
+        SOC_CUDA(cudaEventRecord(e0));
+        if (kind == 0) probe_kernel<0><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else if (kind == 1) probe_kernel<1><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else probe_kernel<2><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        g_launches += 1;
+        SOC_CUDA(cudaEventRecord(e1));
+        SOC_CUDA(cudaEventSynchronize(e1));
+    }
+    SOC_CUDA(cudaEventElapsedTime(ms, e0, e1));
+    // report the time for exactly n_ops operations
+    *ms = (float)((double)*ms * (double)n_ops / ((double)per_thread * blocks * threads));
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf); cudaFree(sink);
+    return SOC_OK;
+}
+
+}  // extern "C"

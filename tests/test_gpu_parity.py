@@ -1,0 +1,337 @@
+"""GPU parity: the CUDA path behind the C ABI against the fp64 CPU oracle, on the same seeded inputs.
+
+Tolerances (BASELINE.json:north_star):
+  replay mode      >= 99.9 % of packages visit identical cell sequences (hash, steps, scatterings);
+                   per-cell absorbed energy relative L1 error <= 1e-4
+  production mode  every cell within 5 sigma of the MC noise estimated from 8 seeds
+  temperatures     within 0.01 K
+  conservation     emitted = absorbed + escaped to 1e-6 (relative)
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle
+from gpu_common import (N_THREADS, gpu_packages, oracle_grid, oracle_packages, rel_l1, replay_match)
+from helpers import random_octree
+from paper_1812_06632_b200 import inputs, soc
+
+REPLAY, PROD = soc.SOC_GEOM_FP64, soc.SOC_GEOM_FP32
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _problem_from_arrays(shape, n_cells, rho, child, kabs, ksca, g, n_packages):
+    nx, ny, nz = shape
+    return inputs.Problem("adhoc", nx, ny, nz, np.asarray(n_cells, dtype=np.int64), np.asarray(rho, dtype=np.float32),
+                          child, np.array([1e14]), np.array([kabs]), np.array([ksca]), np.array([g]), np.array([1.0]),
+                          np.zeros((0, 3)), np.zeros((1, 0)), n_packages)
+
+
+def _check_replay(P, ifreq, src, n_packages, seed, pkg_begin=0, pkg_count=None, min_match=0.999, max_l1=1e-4, weight=1.0):
+    G = soc.Grid.from_problem(P)
+    og = oracle_grid(P)
+    Ao, ro, repo = oracle_packages(og, P, ifreq, src, n_packages, seed, weight, pkg_begin, pkg_count)
+    Ag, rg, repg = gpu_packages(G, P, ifreq, src, n_packages, seed, weight, pkg_begin, pkg_count, flags=REPLAY)
+    G.close()
+    m = replay_match(repg, repo)
+    l1 = rel_l1(Ag, Ao)
+    assert m >= min_match, f"only {m:.5f} of the packages visit identical cell sequences"
+    assert l1 <= max_l1, f"relative L1 error {l1:.2e}"
+    assert abs(rg["emitted"] - rg["absorbed"] - rg["escaped"]) <= 1e-6 * rg["emitted"]
+    assert Ag.sum() == pytest.approx(weight * rg["absorbed"], rel=1e-9)          # nothing lost in the scatter-adds
+    assert rg["emitted"] == pytest.approx(ro.emitted, rel=1e-12)
+    assert rg["escaped"] == pytest.approx(ro.escaped, rel=1e-5)
+    assert abs(rg["cell_steps"] - ro.cell_steps) <= 1e-3 * ro.cell_steps
+    return m, l1, rg, ro
+
+
+# ----------------------------------------------------------------------------------------- closed forms on the GPU
+@pytest.mark.parametrize("flags", [REPLAY, PROD])
+@pytest.mark.parametrize("axis,sign", [(0, 1), (1, -1), (2, 1)])
+def test_gpu_beam_through_pure_absorber(axis, sign, flags):
+    """P2 on the GPU: cell i receives exp(-i tau_c)(1 - exp(-tau_c)), transmission exp(-tau), to 1e-6."""
+    shape = (7, 5, 9)
+    n = shape[axis]
+    P = _problem_from_arrays(shape, [7 * 5 * 9], np.full(7 * 5 * 9, 2.0), None, 0.15, 0.0, 0.0, 1)
+    G = soc.Grid.from_problem(P)
+    pos = np.array([3.25, 2.5, 4.75]); pos[axis] = 0.0 if sign > 0 else n
+    d = np.zeros(3); d[axis] = sign
+    A, res, rep = gpu_packages(G, P, 0, dict(beam=np.concatenate([pos, d])), 1, 1, flags=flags)
+    G.close()
+    A3 = A.reshape(shape[2], shape[1], shape[0])
+    idx = [int(pos[0]), int(pos[1]), int(pos[2])]
+    line = []
+    for i in (range(n) if sign > 0 else range(n - 1, -1, -1)):
+        idx[axis] = i
+        line.append(A3[idx[2], idx[1], idx[0]])
+    expect = np.exp(-0.3 * np.arange(n)) * (1 - np.exp(-0.3))
+    assert np.allclose(line, expect, rtol=1e-6, atol=0)
+    assert res["escaped"] == pytest.approx(math.exp(-0.3 * n), rel=1e-6)
+    assert A.sum() == pytest.approx(sum(line), rel=1e-12)
+    assert rep["steps"][0] == n and res["scatterings"] == 0 and res["cell_steps"] == n
+
+
+def test_gpu_termination_threshold():
+    P = _problem_from_arrays((12, 3, 3), [108], np.ones(108), None, 2.5, 0.0, 0.0, 1)
+    G = soc.Grid.from_problem(P)
+    A, res, rep = gpu_packages(G, P, 0, dict(beam=[0, 1.5, 1.5, 1, 0, 0]), 1, 1, flags=REPLAY)
+    G.close()
+    assert rep["steps"][0] == 9 and res["terminated"] == 1 and res["escaped"] == 0.0
+    assert A.sum() == pytest.approx(1.0, rel=1e-12)
+
+
+# ----------------------------------------------------------------------------------------- configs 1 and 2 in full
+def test_config1_replay_full():
+    P = inputs.make_config("1")
+    m, l1, rg, ro = _check_replay(P, 0, P.sources(0), P.n_packages, P.seed)
+    assert rg["cell_steps"] == ro.cell_steps and rg["scatterings"] == ro.scatterings
+
+
+def test_config2_replay_full():
+    P = inputs.make_config("2")
+    _check_replay(P, 0, P.sources(0), P.n_packages, P.seed)
+
+
+@pytest.mark.parametrize("which,kw", [("1", {}), ("2", dict(n=32, n_packages=200_000))])
+def test_production_mode_within_5_sigma(which, kw):
+    """Seeds 1..8 on both sides; sigma_c = per-cell sample standard deviation of the oracle's 8 runs;
+    |A_gpu(s) - A_orc(s)| <= 5 sigma_c for every cell and seed."""
+    P = inputs.make_config(which, **kw)
+    G = soc.Grid.from_problem(P)
+    og = oracle_grid(P)
+    src = P.sources(0)
+    Ao, Ag = [], []
+    for seed in range(1, 9):
+        Ao.append(oracle_packages(og, P, 0, src, P.n_packages, seed, want_replay=False)[0])
+        a, rg, _ = gpu_packages(G, P, 0, src, P.n_packages, seed, flags=PROD, want_replay=False)
+        assert abs(rg["emitted"] - rg["absorbed"] - rg["escaped"]) <= 1e-6 * rg["emitted"]
+        Ag.append(a)
+    G.close()
+    Ao, Ag = np.array(Ao), np.array(Ag)
+    sigma = Ao.std(axis=0, ddof=1)
+    diff = np.abs(Ag - Ao)
+    ok = diff <= 5 * sigma
+    zero = sigma == 0
+    ok[:, zero] = diff[:, zero] <= 1e-6 * np.abs(Ao[:, zero])
+    assert ok.all(), f"{(~ok).sum()} cell/seed pairs beyond 5 sigma; worst {np.nanmax(diff / np.where(sigma > 0, sigma, np.nan)):.2f} sigma"
+    # production mode is the fp32 evaluation of the same fp32 state: most packages still replay exactly
+    assert rel_l1(Ag[0], Ao[0]) < 1e-2
+
+
+# ----------------------------------------------------------------------------------------- configs 3, 5: full-size grids, id subsets
+@pytest.mark.parametrize("which,n_sub", [("3", 60_000), ("5", 40_000)])
+def test_spectral_configs_subset_replay(which, n_sub):
+    """Full-size grid and full n_packages; package-id subsets straddling the background / point-source
+    boundary at one UV, one visual, one near-IR and one far-IR frequency."""
+    P = inputs.make_config(which)
+    lam = P.notes["lam_um"]
+    picks = [int(np.argmin(np.abs(lam - x))) for x in (0.12, 0.55, 2.2, 100.0)]
+    G = soc.Grid.from_problem(P)
+    og = oracle_grid(P)
+    n = P.n_packages
+    tot_same = tot = 0
+    for ifreq in picks:
+        src = P.sources(ifreq)
+        begin = n // 2 - n_sub // 2
+        Ao, ro, repo = oracle_packages(og, P, ifreq, src, n, P.seed, 1.0, begin, n_sub)
+        Ag, rg, repg = gpu_packages(G, P, ifreq, src, n, P.seed, 1.0, begin, n_sub, flags=REPLAY)
+        m, l1 = replay_match(repg, repo), rel_l1(Ag, Ao)
+        assert m >= 0.999, f"lambda {lam[ifreq]:.3g} um: match {m:.5f}"
+        assert l1 <= 1e-4, f"lambda {lam[ifreq]:.3g} um: L1 {l1:.2e}"
+        assert abs(rg["emitted"] - rg["absorbed"] - rg["escaped"]) <= 1e-6 * rg["emitted"]
+        assert rg["emitted"] == pytest.approx(ro.emitted, rel=1e-12)
+        tot_same += m * n_sub; tot += n_sub
+    G.close()
+    assert tot_same / tot >= 0.999
+
+
+# ----------------------------------------------------------------------------------------- hierarchical grids (config 4)
+@pytest.mark.parametrize("seed", [1, 2])
+def test_random_octree_replay(seed):
+    shape = (5, 4, 6)
+    n_cells, rho, child = random_octree(shape, 4, 0.3, seed=seed, p_empty=0.1)
+    P = _problem_from_arrays(shape, n_cells, rho, child, 0.4, 0.9, 0.5, 50_000)
+    src = dict(bg_intensity=2.0, ps_pos=np.array([[2.3, 1.7, 3.1], [0.5, 3.5, 5.5]]), ps_lum=np.array([30.0, 5.0]))
+    m, l1, rg, ro = _check_replay(P, 0, src, 50_001, 9, weight=0.25)
+    assert rg["scatterings"] == pytest.approx(ro.scatterings, rel=1e-3)
+
+
+@pytest.mark.parametrize("which", ["4", "4p"])
+def test_config4_reduced_replay(which):
+    """Config 4 recipe on a 16^3 root (128^3 field, 4 levels): all 32 frequencies are too many for the
+    oracle in a test, so one UV, one visual and one far-IR frequency, full package count of the reduced case."""
+    P = inputs.make_config(which, n=16, n_packages=100_000)
+    lam = P.notes["lam_um"]
+    for x in (0.15, 0.55, 200.0):
+        ifreq = int(np.argmin(np.abs(lam - x)))
+        _check_replay(P, ifreq, P.sources(ifreq), P.n_packages, P.seed)
+
+
+def test_config4_full_size_subset_replay():
+    """Config 4 as written (root 64^3 from a 512^3 field, theta = 4, ~3.4 M leaves): id subset at 2 frequencies."""
+    P = inputs.make_config("4")
+    assert P.n_levels == 4 and P.n_total > 3_000_000
+    lam = P.notes["lam_um"]
+    G = soc.Grid.from_problem(P)
+    og = oracle_grid(P)
+    for x in (0.55, 100.0):
+        ifreq = int(np.argmin(np.abs(lam - x)))
+        src = P.sources(ifreq)
+        Ao, ro, repo = oracle_packages(og, P, ifreq, src, P.n_packages, P.seed, 1.0, 1000, 30_000)
+        Ag, rg, repg = gpu_packages(G, P, ifreq, src, P.n_packages, P.seed, 1.0, 1000, 30_000, flags=REPLAY)
+        assert replay_match(repg, repo) >= 0.999 and rel_l1(Ag, Ao) <= 1e-4
+        assert abs(rg["emitted"] - rg["absorbed"] - rg["escaped"]) <= 1e-6 * rg["emitted"]
+    G.close()
+
+
+# ----------------------------------------------------------------------------------------- frequency loop + temperatures
+def test_spectrum_and_temperatures_match_oracle():
+    """Config 3 recipe on a 32^3 grid with 12 frequencies: absorbed_int = sum_f w_f A_f and T within 0.01 K."""
+    torch = _torch()
+    P = inputs.make_config("3", n=32, n_packages=60_000, n_freq=12)
+    G = soc.Grid.from_problem(P)
+    og = oracle_grid(P)
+    w = G.freq_weights()
+    assert np.allclose(w, oracle.trapezoid_weights(P.freq_hz), rtol=1e-14)
+    Aint = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+    res = G.simulate_spectrum([P.sources(f) for f in range(P.n_freq)], P.n_packages, P.seed, Aint, flags=REPLAY)
+    Ao = np.zeros(P.n_total)
+    for f in range(P.n_freq):
+        _, ro, _ = oracle.simulate(og, P.kabs[f], P.ksca[f], P.g[f], f, P.sources(f), P.n_packages, P.seed, w[f],
+                                   absorbed=Ao, threads=N_THREADS)[:3]
+        assert res[f].emitted == pytest.approx(ro.emitted, rel=1e-12)
+        assert abs(res[f].emitted - res[f].absorbed - res[f].escaped) <= 1e-6 * res[f].emitted
+    Ag = Aint.cpu().numpy()
+    assert rel_l1(Ag, Ao) <= 1e-4
+    T = torch.empty(P.n_total, dtype=torch.float32, device="cuda")
+    G.update_temperatures(Aint, P.t_scale, P.table_T, P.e_min, P.e_max, T)
+    Tg = T.cpu().numpy()
+    To = oracle.update_temperatures(og, Ao, P.t_scale, P.table_T, P.e_min, P.e_max)
+    assert np.abs(Tg - To).max() <= 0.01
+    # same absorbed field on both sides isolates the lookup kernel itself
+    To2 = oracle.update_temperatures(og, Ag, P.t_scale, P.table_T, P.e_min, P.e_max)
+    assert np.abs(Tg - To2).max() <= 2e-3
+    assert Tg.min() >= 3.0 and 5.0 < np.median(Tg) < 200.0
+    G.close()
+
+
+@pytest.mark.parametrize("shape", [(3, 3, 3), (5, 4, 6)])
+def test_temperature_kernel_edge_cases(shape):
+    """Ragged n_total (not a multiple of 4), parents, empty leaves, unhit cells, clamps at both table ends."""
+    torch = _torch()
+    n_cells, rho, child = random_octree(shape, 3, 0.4, seed=5, p_empty=0.2)
+    P = _problem_from_arrays(shape, n_cells, rho, child, 0.1, 0.1, 0.0, 1)
+    G = soc.Grid.from_problem(P)
+    og = oracle_grid(P)
+    n_t, e_min, e_max = 64, 1e-3, 1e5
+    table = (10.0 * np.geomspace(e_min, e_max, n_t) ** (1 / 6)).astype(np.float32)
+    rng = np.random.default_rng(1)
+    A = 10 ** rng.uniform(-6, 7, P.n_total)
+    A[::7] = 0.0
+    Ad = torch.from_numpy(A).cuda()
+    T = torch.empty(P.n_total, dtype=torch.float32, device="cuda")
+    G.update_temperatures(Ad, 2.5, table, e_min, e_max, T)
+    To = oracle.update_temperatures(og, A, 2.5, table, e_min, e_max)
+    Tg = T.cpu().numpy()
+    assert np.abs(Tg - To).max() <= 1e-3
+    assert (Tg[(child >= 0) | (rho == 0)] == 0).all()
+    G.close()
+
+
+# ----------------------------------------------------------------------------------------- edge cases of the walk
+def test_empty_and_tiny_inputs():
+    torch = _torch()
+    P = inputs.make_config("1", n=4, n_packages=10)
+    G = soc.Grid.from_problem(P)
+    A = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+    r = G.simulate_packages(0, P.sources(0), 10, 1, 1.0, 3, 0, A)            # empty id range
+    assert r.emitted == 0 and r.cell_steps == 0 and float(A.sum()) == 0.0
+    r = G.simulate_frequency(0, P.sources(0), 1, 1, 1.0, A)                  # a single package
+    assert r.cell_steps >= 1 and abs(r.emitted - r.absorbed - r.escaped) < 1e-12 * r.emitted
+    G.close()
+    # zero-density cloud: nothing absorbed, nothing scattered, every package escapes (PAPER.md:117 empty cells)
+    P0 = _problem_from_arrays((6, 5, 4), [120], np.zeros(120), None, 1.0, 1.0, 0.3, 20000)
+    G = soc.Grid.from_problem(P0)
+    A, res, _ = gpu_packages(G, P0, 0, dict(bg_intensity=1.0), 20000, 3, flags=PROD)
+    assert A.sum() == 0.0 and res["scatterings"] == 0 and res["escaped"] == pytest.approx(res["emitted"], rel=1e-12)
+    S = 2 * (5 * 4 + 4 * 6 + 6 * 5)
+    a_int = 3 * 120 - (5 * 4 + 6 * 4 + 6 * 5)
+    assert res["cell_steps"] / 20000 == pytest.approx(1 + 2 * a_int / S, rel=0.02)   # flux argument (pin P7)
+    G.close()
+
+
+def test_point_source_in_empty_cell_and_hot_cell():
+    """All packages start in one cell (the atomic hot spot of PAPER.md:151, 279) which is empty."""
+    rho = np.ones(125, dtype=np.float32); rho[62] = 0.0
+    P = _problem_from_arrays((5, 5, 5), [125], rho, None, 0.3, 0.6, 0.2, 100_000)
+    src = dict(ps_pos=np.array([[2.5, 2.5, 2.5]]), ps_lum=np.array([1.0]))
+    m, l1, rg, ro = _check_replay(P, 0, src, 100_000, 1)
+    G = soc.Grid.from_problem(P)
+    A, _, _ = gpu_packages(G, P, 0, src, 100_000, 1, flags=PROD, want_replay=False)
+    G.close()
+    assert A[62] == 0.0
+
+
+def test_accumulates_with_weight_and_subsets_add_up():
+    torch = _torch()
+    P = inputs.make_config("2", n=16, n_packages=30_000)
+    G = soc.Grid.from_problem(P)
+    src = P.sources(0)
+    A_full, r_full, rep_full = gpu_packages(G, P, 0, src, 30_000, 5, weight=1.0, flags=REPLAY)
+    A = torch.full((P.n_total,), 1.0, dtype=torch.float64, device="cuda")
+    reps = []
+    for b, n in [(0, 10_000), (10_000, 7), (10_007, 19_993)]:
+        _, r, rep = gpu_packages(G, P, 0, src, 30_000, 5, weight=0.5, pkg_begin=b, pkg_count=n, flags=REPLAY, absorbed=A)
+        reps.append(rep)
+    G.close()
+    assert np.array_equal(np.concatenate(reps), rep_full)                    # the stream is keyed by package id
+    assert np.allclose(A.cpu().numpy(), 1.0 + 0.5 * A_full, rtol=1e-11, atol=0)
+
+
+def test_run_host_equals_device_path():
+    """soc_run_host (HOST buffers in and out) against the device-pointer calls."""
+    torch = _torch()
+    P = inputs.make_config("5", n=24, n_packages=20_000, n_freq=6)
+    A_h, T_h, res = soc.run_host(P, n_iter=2, want_results=True)
+    G = soc.Grid.from_problem(P)
+    Aint = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+    for it in range(2):
+        G.simulate_spectrum([P.sources(f) for f in range(P.n_freq)], P.n_packages, P.seed + it, Aint, want_results=False)
+    T = torch.empty(P.n_total, dtype=torch.float32, device="cuda")
+    G.update_temperatures(Aint, P.t_scale / 2, P.table_T, P.e_min, P.e_max, T)
+    G.close()
+    assert np.allclose(A_h, Aint.cpu().numpy() / 2, rtol=1e-9, atol=0)
+    assert np.abs(T_h - T.cpu().numpy()).max() <= 1e-3
+    assert len(res) == 2 * P.n_freq and all(abs(r.emitted - r.absorbed - r.escaped) <= 1e-6 * r.emitted for r in res)
+
+
+def test_bad_arguments_are_rejected():
+    torch = _torch()
+    P = inputs.make_config("1", n=4, n_packages=10)
+    with pytest.raises(soc.SocError):
+        soc.Grid(4, 4, 4, [63], P.rho[:63], None, P.freq_hz, P.kabs, P.ksca, P.g)
+    bad = P.rho.copy(); bad[3] = np.nan
+    with pytest.raises(soc.SocError):
+        soc.Grid(4, 4, 4, [64], bad, None, P.freq_hz, P.kabs, P.ksca, P.g)
+    n_cells, rho, child = random_octree((2, 2, 2), 2, 0.5, seed=1)
+    c2 = child.copy(); c2[np.argmax(child >= 0)] += 4
+    with pytest.raises(soc.SocError):
+        soc.Grid(2, 2, 2, n_cells, rho, c2, P.freq_hz, P.kabs, P.ksca, P.g)
+    G = soc.Grid.from_problem(P)
+    A = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+    with pytest.raises(soc.SocError):
+        G.simulate_frequency(1, P.sources(0), 10, 1, 1.0, A)                # ifreq out of range
+    with pytest.raises(soc.SocError):
+        G.simulate_frequency(0, dict(bg_intensity=0.0), 10, 1, 1.0, A)      # no source at all
+    with pytest.raises(soc.SocError):
+        G.simulate_frequency(0, dict(ps_pos=[[9.0, 1, 1]], ps_lum=[1.0]), 10, 1, 1.0, A)   # source outside
+    with pytest.raises(soc.SocError):
+        G.simulate_packages(0, P.sources(0), 10, 1, 1.0, 5, 6, A)           # range beyond n_packages
+    G.close()

@@ -2,6 +2,10 @@
 
 Every test compares the oracle with something that is not the oracle: published known answers,
 closed forms, conservation laws, quadrature, or an independent geometric check.
+
+The oracle holds the package state (position in the cell, direction, remaining optical depth) in fp32 and
+evaluates every update in fp64 (reading S11), so pins that involve an oblique direction or an
+accumulated optical depth hold to a few fp32 ulps (F32 below), the axis-aligned ones to fp64 rounding.
 """
 import math
 import os
@@ -13,6 +17,7 @@ import oracle
 from helpers import Geometry, fully_refined, random_octree
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
+F32 = 2.0 ** -23      # one fp32 ulp at 1
 
 
 def _rows(name):
@@ -126,8 +131,8 @@ def test_oblique_beam_path_length():
     pos = np.array([0.0, 1.2, 4.4])
     A, res, _, tr = oracle.simulate(g, 0.2, 0.0, 0.0, 0, dict(beam=np.concatenate([pos, d])), 1, 1, trace_cap=100)
     tmax = min(((shape[j] if d[j] > 0 else 0) - pos[j]) / d[j] for j in range(3))
-    assert res.absorbed == pytest.approx(1 - math.exp(-0.2 * 1.5 * tmax), rel=1e-13)
-    assert tr["ds"].sum() == pytest.approx(tmax, rel=1e-13)
+    assert res.absorbed == pytest.approx(1 - math.exp(-0.2 * 1.5 * tmax), rel=4 * F32)
+    assert tr["ds"].sum() == pytest.approx(tmax, rel=4 * F32)
     for s in tr:   # each visited cell is the cell of the segment mid-point
         mid = 0.5 * (s["p0"] + s["p1"])
         ijk = np.floor(mid).astype(int)
@@ -327,7 +332,7 @@ def test_bruteforce_geometric_replay_on_tiny_octree(seed):
         tau_acc = 0.0
         for i, s in enumerate(steps):
             seglen = np.linalg.norm(s["p1"] - s["p0"])
-            assert seglen == pytest.approx(s["ds"], abs=1e-12)
+            assert seglen == pytest.approx(s["ds"], rel=2 * F32, abs=4 * F32)   # fp32 positions, |d| = 1 +- ulp
             if i > 0:                                    # contiguous path
                 assert np.allclose(steps[i - 1]["p1"], s["p0"], atol=1e-12)
             if seglen > 1e-9:                            # the mid-point lies in the leaf that was charged
@@ -338,10 +343,10 @@ def test_bruteforce_geometric_replay_on_tiny_octree(seed):
             assert s["tau_sca"] == pytest.approx(s["ds"] * float(rho[s["gid"]]) * ksca, rel=1e-12, abs=1e-300)
             tau_acc += s["tau_sca"]
             if s["kind"] == 1:                           # free path really has the drawn optical depth
-                assert tau_acc == pytest.approx(s["tau_drawn"], rel=1e-9)
+                assert tau_acc == pytest.approx(s["tau_drawn"], rel=F32 * (4 + len(steps)))
                 tau_acc = 0.0
             else:
-                assert tau_acc < s["tau_drawn"] * (1 + 1e-12)
+                assert tau_acc < s["tau_drawn"] * (1 + F32 * (4 + len(steps)))
         last = steps[-1]
         assert last["kind"] in (2, 3)
         if last["kind"] == 3:                            # escaped: ends on the outer boundary
@@ -373,11 +378,16 @@ def test_fully_refined_hierarchy_equals_regular_grid():
     # the regular grid's length unit is half a root cell: kappa halves, and I/4 keeps the package energy
     Ah, rh, reph, _ = oracle.simulate(gh, kabs, ksca, gg, 2, dict(bg_intensity=I), n, 5, want_replay=True)
     Ar, rr, repr_, _ = oracle.simulate(gr, kabs / 2, ksca / 2, gg, 2, dict(bg_intensity=I / 4), n, 5, want_replay=True)
+    # Only difference: going up one level rounds (f + bit)/2 to fp32, i.e. drops the last bit of the two
+    # non-crossing coordinates; the few packages that pass within an ulp of a cell edge may then take the
+    # corner cell in the other order (measured: 0.03 %).
     same = (reph["steps"] == repr_["steps"]) & (reph["scatters"] == repr_["scatters"])
-    assert same.mean() >= 0.9999
+    assert same.mean() >= 0.999
     assert rh.emitted == pytest.approx(rr.emitted, rel=1e-13)
-    assert rh.escaped == pytest.approx(rr.escaped, rel=1e-9)
-    assert np.allclose(Ah[gid_of.ravel()], Ar, rtol=1e-9, atol=1e-12 * Ar.max())
+    assert rh.escaped == pytest.approx(rr.escaped, rel=1e-4)
+    Ahl = Ah[gid_of.ravel()]
+    assert np.abs(Ahl - Ar).sum() <= 1e-3 * Ar.sum()
+    assert np.median(np.abs(Ahl - Ar) / Ar) < 1e-6                  # the typical leaf agrees to fp32 rounding
     assert Ah[: N ** 3].sum() == 0.0
 
 
@@ -535,23 +545,23 @@ def test_stream_layout_inside_the_walk():
         u = [oracle.uniform(x) for x in b0] + [oracle.uniform(b1[0])]
         ijk, f, d = oracle.emit_background(*shape, u)
         assert np.allclose(s[0]["p0"], ijk + f, atol=1e-14)
-        nz = s[s["ds"] > 1e-9]
-        assert np.allclose((nz[0]["p1"] - nz[0]["p0"]) / nz[0]["ds"], d, atol=1e-9)
+        nz = s[s["ds"] > 1e-3]
+        assert np.allclose((nz[0]["p1"] - nz[0]["p0"]) / nz[0]["ds"], d, atol=1e-4)
         seg = 0
         d_prev = d
         for i, st in enumerate(s):
             blk = oracle.stream_block(seed, ifreq, p, 2 + seg)
-            assert st["tau_drawn"] == pytest.approx(-math.log(oracle.uniform(blk[0])), rel=1e-14)
+            assert st["tau_drawn"] == float(np.float32(-math.log(oracle.uniform(blk[0]))))
             if st["kind"] == 1:
                 later = s[i + 1:]
-                later = later[later["ds"] > 1e-9]
+                later = later[later["ds"] > 1e-3]
                 if len(later):
                     d_new = (later[0]["p1"] - later[0]["p0"]) / later[0]["ds"]
-                    expect = oracle.rotate(d_prev, oracle.hg_cos(gg, oracle.uniform(blk[1])),
+                    expect = oracle.rotate(np.float32(d_prev).astype(np.float64), oracle.hg_cos(gg, oracle.uniform(blk[1])),
                                            2 * math.pi * oracle.uniform(blk[2]))
                     # only compare when no further scattering happened before the next non-zero step
-                    if not (s[i + 1:i + 1 + int(np.argmax(s[i + 1:]["ds"] > 1e-9))]["kind"] == 1).any():
-                        assert np.allclose(d_new, expect, atol=1e-7)
+                    if not (s[i + 1:i + 1 + int(np.argmax(s[i + 1:]["ds"] > 1e-3))]["kind"] == 1).any():
+                        assert np.allclose(d_new, expect, atol=1e-4)     # p0, p1 carry fp32 positions
                         checked += 1
                     d_prev = expect
                 seg += 1
