@@ -1,0 +1,355 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the photon-package hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3|5|4p|4|2|1] [--impl ours|reference]
+
+One STEP = one pass of the whole hot path over one batch of synthetic input: for every frequency of the
+config, emit / walk / deposit / scatter all packages (soc_simulate_spectrum: one persistent photon kernel per
+frequency queued back to back on one stream, rows a1-a10 of DESIGN.md), then the energy-balance temperature
+update (row a11).  Default workload: BASELINE.json configs[2] ("config 3": 128^3 lognormal cloud, 2 point
+sources + background, 64 frequencies, 4e6 packages per frequency, one temperature update) -- the smallest
+config that exercises every row except the octree walk and still reaches steady state; see DESIGN.md
+"Measurement" for why configs[1] (a single ~1 ms launch) is not the default.
+
+Prints ONE JSON line (rank 0).  `value` = cell-steps of all ranks per second of step time (device time, CUDA
+events on the launching stream, max over ranks), inputs resident in HBM.  `e2e` = the same through
+soc_run_host with pinned HOST buffers (model upload, simulation, download of absorbed energy and
+temperatures inside the timed region).  `roofline` / `cpu_baseline` as described in DESIGN.md.
+
+`--impl reference` times the CPU oracle (oracle/, fp64, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import dataclasses
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "photon-package cell-steps/sec per frequency"
+UNIT = "cell-steps/s"
+ALGO_BYTES_PER_STEP = 12.0          # 4 B density gather + 8 B fp64 scatter-add
+WORKLOADS = {
+    "1": "configs[0]: regular 32^3 uniform, tau=1, albedo 0.5, g=0, background, 1e5 packages",
+    "2": "configs[1]: regular 64^3 lognormal, peak tau 10, albedo 0.6, g=0.6, background, 1e6 packages",
+    "3": "configs[2]: regular 128^3 lognormal, 2 point sources + background, 64 frequencies, 4e6 packages/frequency, temperature update",
+    "4": "configs[3] (rule as written, theta=4): octree root 64^3, 4 levels, ~3.4M leaves, background, 32 frequencies, 1e6 packages/frequency",
+    "4p": "configs[3] (size as written, theta=2): octree root 64^3, 4 levels, ~10M leaves, background, 32 frequencies, 1e6 packages/frequency",
+    "5": "configs[4]: regular 256^3 lognormal, 10 point sources + background, 128 frequencies, 1e7 packages/frequency, temperature update (one of the 3 iterations per step)",
+}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU every 100 ms while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.stop_flag = threading.Event()
+        self.sm, self.reasons, self.sm_max, self.err = [], set(), None, None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.sm_max = int(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            names = {
+                getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+                getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+                getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+                getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+                getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+            }
+            get = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+            while not self.stop_flag.is_set():
+                self.sm.append(int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                mask = int(get(h))
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+                self.stop_flag.wait(0.1)
+        except Exception as e:      # noqa: BLE001 -- the sampler must never kill the bench
+            self.err = repr(e)
+
+    def summary(self):
+        d = {"sm_mhz": (float(np.median(self.sm)) if self.sm else None), "sm_max_mhz": self.sm_max,
+             "reasons": sorted(self.reasons), "samples": len(self.sm)}
+        if self.err:
+            d["error"] = self.err
+        return d
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ------------------------------------------------------------------------------------------------ CPU oracle legs
+def oracle_sample(P, target_s, threads):
+    """Time the oracle, as it stands, on a bounded sample of the workload: equal package-id subsets (straddling
+    the background / point-source boundary) at four frequencies spread over the grid.  Returns
+    (cell_steps, seconds, description)."""
+    import oracle
+    og = oracle.Grid(P.nx, P.ny, P.nz, P.n_cells, P.rho, P.child)
+    freqs = sorted({int(round(x)) for x in np.linspace(0, P.n_freq - 1, 4)})
+    n = P.n_packages
+
+    def run(count):
+        steps = 0
+        t0 = time.perf_counter()
+        for f in freqs:
+            begin = max(0, n // 2 - count // 2)
+            cnt = min(count, n - begin)
+            _, res, _, _ = oracle.simulate(og, P.kabs[f], P.ksca[f], P.g[f], f, P.sources(f), n, P.seed, 1.0,
+                                           begin, cnt, threads=threads)
+            steps += res.cell_steps
+        return steps, time.perf_counter() - t0
+
+    probe = min(n, 4000 * threads)
+    s0, t0 = run(probe)
+    rate = s0 / max(t0, 1e-6)
+    count = int(min(n, max(probe, probe * target_s / max(t0, 1e-6))))
+    steps, secs = run(count)
+    desc = (f"package ids [n/2-{count // 2}, n/2+{count - count // 2}) of {n} at frequency indices {freqs} "
+            f"({len(freqs) * count} packages, {steps} cell-steps; calibration run {rate:.3g} steps/s)")
+    return steps, secs, desc
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_1812_06632_b200 import inputs
+    P = inputs.make_config(args.config)
+    threads = max(1, min(32, os.cpu_count() or 1))
+    per_step_target = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(P, per_step_target / 4, threads)
+    tot_steps, tot_s, desc = 0, 0.0, ""
+    for _ in range(args.steps):
+        s, t, desc = oracle_sample(P, per_step_target, threads)
+        tot_steps += s
+        tot_s += t
+    v = tot_steps / tot_s
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / max(1, args.steps), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.config], "sample_per_step": desc},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ CUDA path
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1812_06632_b200 import dist as socdist
+    from paper_1812_06632_b200 import inputs, soc
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    soc.load()
+
+    P = inputs.make_config(args.config)
+    if args.packages:
+        P.n_packages = int(args.packages)
+    shard = socdist.plan("weak", rank, world, P.n_packages, P.seed)
+    G = soc.Grid.from_problem(P)
+    G.set_option("timing", 1)
+    srcs = [P.sources(f) for f in range(P.n_freq)]
+    has_T = P.table_T is not None
+    Aint = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+    T = torch.zeros(P.n_total, dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # 2 x L2 (126 MB)
+    stream = torch.cuda.current_stream()
+
+    def step(want_results=False):
+        Aint.zero_()
+        res = G.simulate_spectrum(srcs, P.n_packages, shard.seed, Aint, shard.pkg_begin, shard.pkg_count,
+                                  want_results=want_results, stream=stream)
+        socdist.combine(Aint, shard)
+        if has_T:
+            G.update_temperatures(Aint, P.t_scale, P.table_T, P.e_min, P.e_max, T, stream=stream)
+        return res
+
+    # ---- warm-up (the first warm-up step also fetches the device counters: the walk is a deterministic
+    # function of (seed, ids), so the counts are those of every later step)
+    res = step(want_results=True)
+    steps_f = np.array([r.cell_steps for r in res], dtype=np.float64)
+    emitted = sum(r.emitted for r in res)
+    cons = max(abs(r.emitted - r.absorbed - r.escaped) / r.emitted for r in res if r.emitted > 0)
+    scat_total = sum(r.scatterings for r in res)
+    for _ in range(max(0, args.warmup - 1)):
+        step()
+    torch.cuda.synchronize()
+
+    # ---- timed region
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    sampler.start()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    launches0 = soc.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern_ms = np.zeros(P.n_freq)
+    t_wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)                    # L2 flush between timed steps (outside the event pair)
+        ev[k][0].record(stream)
+        step()
+        ev[k][1].record(stream)
+        ev[k][1].synchronize()
+        kern_ms += G.timings_ms()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = soc.launch_count() - launches0
+    sampler.stop_flag.set()
+    sampler.join(2.0)
+    step_ms = float(sum(a.elapsed_time(b) for a, b in ev))
+    kern_ms /= max(1, args.steps)
+
+    tot = torch.tensor([step_ms, float(steps_f.sum()), float(launches)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        mx = tot.clone()
+        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        step_ms = float(mx[0])
+    job_steps = float(tot[1])                    # cell-steps of all ranks in one step
+    job_launches = int(tot[2])
+    ms_per_step = step_ms / args.steps
+    value = job_steps / (ms_per_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry (soc_run_host)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()        # noqa: E731
+    Ph = dataclasses.replace(P, rho=pin(P.rho), child=None if P.child is None else pin(P.child), seed=shard.seed)
+    a_out = torch.zeros(P.n_total, dtype=torch.float64).pin_memory().numpy()
+    t_out = torch.zeros(P.n_total, dtype=torch.float32).pin_memory().numpy()
+    h2d = Ph.rho.nbytes + (0 if P.child is None else Ph.child.nbytes) + 4 * 8 * P.n_freq + \
+        (0 if not has_T else 4 * len(P.table_T))
+    d2h = a_out.nbytes + (t_out.nbytes if has_T else 0)
+    n_e2e = max(1, min(args.steps, 2))
+    soc.run_host(Ph, n_iter=1, absorbed_out=a_out, T_out=t_out if has_T else None)                # warm-up
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        soc.run_host(Ph, n_iter=1, absorbed_out=a_out, T_out=t_out if has_T else None)
+    e2e_s = (time.perf_counter() - t0) / n_e2e
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t[0])
+    e2e_value = job_steps / e2e_s
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (photon kernel): algorithmic bytes per launch / mean launch time
+    peak, peak_src = measured_peaks()
+    mean_launch_ms = float(kern_ms.mean())
+    algo_bytes = ALGO_BYTES_PER_STEP * float(steps_f.mean())
+    achieved = algo_bytes / (mean_launch_ms * 1e-3) / 1e9
+    per_f = steps_f / (kern_ms * 1e-3)
+    roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": None, "peak_source": peak_src, "kernel": "photon_kernel",
+            "algorithmic_bytes_per_launch": algo_bytes, "mean_launch_ms": mean_launch_ms,
+            "kernel_share_of_step": float(kern_ms.sum() / ms_per_step)}
+    roof.update(roofline_notes(args.config))
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32 geometry / f64 weights and accumulators", "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.config], "cells": int(P.n_total), "n_freq": int(P.n_freq),
+                       "packages_per_frequency": int(P.n_packages), "parallelism": f"replicas x{world} (seed + rank), "
+                       "one fp64 all-reduce" if world > 1 else "single GPU",
+                       "l2": "flushed between timed steps (256 MB fill)"},
+            "packages_per_s": world * P.n_packages * P.n_freq / (ms_per_step * 1e-3),
+            "cell_steps_per_s_per_frequency": {"median": float(np.median(per_f)), "min": float(per_f.min()),
+                                               "max": float(per_f.max())},
+            "cell_steps_per_step": job_steps, "scatterings_per_step": float(scat_total) * world,
+            "energy_conservation_rel": cons,
+            "clocks": sampler.summary(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "api": "soc_run_host (pinned host buffers)", "s_per_step": e2e_s},
+            "gpu_launches": job_launches,
+            "wall_s_timed_region": t_wall,
+            "roofline": roof}
+
+    if world == 1 and not args.no_cpu_baseline:
+        threads = max(1, min(32, os.cpu_count() or 1))
+        s, t, desc = oracle_sample(P, 15.0, threads)
+        line["cpu_baseline"] = {"value": s / t, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+# DRAM traffic of one photon-kernel launch from the committed `ncu --set full` capture of this command
+# (dram__bytes_read.sum + dram__bytes_write.sum, mean over the captured launches); None = not captured yet.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+
+
+def roofline_notes(config):
+    """Static facts about the dominant kernel that go with the roofline object."""
+    d = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(str(config))
+    return dict(d) if d else {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", choices=sorted(WORKLOADS), default="3")
+    ap.add_argument("--packages", type=int, default=0, help="override packages per frequency (debugging only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        raise SystemExit("need --steps >= 1 and --warmup >= 0")
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(args.warmup, 1)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

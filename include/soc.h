@@ -143,9 +143,15 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
                  double E_max, double *absorbed_int_out, float *T_out, soc_freq_result *results,
                  uint32_t flags);
 
-/* Tuning knobs (all have defaults chosen for B200): "blocks_per_sm", "threads", "refill_threshold".
+/* Tuning knobs (all have defaults chosen for B200): "blocks_per_sm", "threads", "refill_threshold"; and
+ * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
  * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
 int soc_set_option(soc_grid *grid, const char *key, int64_t value);
+
+/* With option "timing" = 1: ms[i] = device time of the photon kernel last launched into result slot i
+ * (slot = frequency index for soc_simulate_spectrum, 0 for the single-frequency calls); -1 where no launch
+ * was recorded.  Waits for those launches to finish.  ms: HOST, n floats. */
+int soc_get_timings(soc_grid *grid, int32_t n, float *ms);
 
 /* Roofline probes: random 4-byte gathers (kind 0), random fp64 red.global.add (kind 1) and
  * random fp32 red.global.add (kind 2) over a footprint of `footprint_bytes`, n_ops operations in total,

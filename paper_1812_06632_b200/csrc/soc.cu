@@ -90,6 +90,9 @@ struct soc_grid {
     int opt_blocks_per_sm = 0;                // 0 = from the occupancy calculator
     int opt_threads = 256;
     int opt_refill_threshold = 1;
+    int opt_timing = 0;                       // record a CUDA-event pair around every photon launch
+    std::vector<cudaEvent_t> ev0, ev1;        // n_slots each (created on demand)
+    std::vector<char> ev_set;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -596,6 +599,17 @@ int ensure_slots(soc_grid *G, int n)
     return SOC_OK;
 }
 
+int ensure_events(soc_grid *G, int n)
+{
+    while ((int)G->ev0.size() < n) {
+        cudaEvent_t a, b;
+        SOC_CUDA(cudaEventCreate(&a));
+        SOC_CUDA(cudaEventCreate(&b));
+        G->ev0.push_back(a); G->ev1.push_back(b); G->ev_set.push_back(0);
+    }
+    return SOC_OK;
+}
+
 template <typename K> int blocks_for(soc_grid *G, K kernel, int threads, int *blocks)
 {
     int per_sm = 0;
@@ -699,11 +713,21 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
     SOC_CUDA(cudaMemsetAsync(G->d_results + slot, 0, sizeof(DevResult), st));
     if (pkg_count == 0) return SOC_OK;
     const bool hier = G->n_levels > 1, f64 = (flags & SOC_GEOM_FP64) != 0, rep = replay != nullptr;
+    if (G->opt_timing) {
+        rc = ensure_events(G, slot + 1);
+        if (rc != SOC_OK) return rc;
+        SOC_CUDA(cudaEventRecord(G->ev0[slot], st));
+    }
 #define SOC_DISPATCH(R)                                                                             \
     (hier ? (rep ? launch_photon<R, true, true>(G, P, st) : launch_photon<R, true, false>(G, P, st)) \
           : (rep ? launch_photon<R, false, true>(G, P, st) : launch_photon<R, false, false>(G, P, st)))
-    return f64 ? SOC_DISPATCH(double) : SOC_DISPATCH(float);
+    rc = f64 ? SOC_DISPATCH(double) : SOC_DISPATCH(float);
 #undef SOC_DISPATCH
+    if (rc == SOC_OK && G->opt_timing) {
+        SOC_CUDA(cudaEventRecord(G->ev1[slot], st));
+        G->ev_set[slot] = 1;
+    }
+    return rc;
 }
 
 int fetch_results(soc_grid *G, int n, soc_freq_result *out, cudaStream_t st)
@@ -743,6 +767,8 @@ void soc_grid_destroy(soc_grid *G)
     cudaFree(G->d_cellw); cudaFree(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
     cudaFree(G->d_table);
     if (G->h_results) cudaFreeHost(G->h_results);
+    for (cudaEvent_t e : G->ev0) cudaEventDestroy(e);
+    for (cudaEvent_t e : G->ev1) cudaEventDestroy(e);
     delete G;
 }
 
@@ -846,7 +872,21 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     if (k == "blocks_per_sm" && value >= 0 && value <= 32) G->opt_blocks_per_sm = (int)value;
     else if (k == "threads" && (value == 64 || value == 128 || value == 256)) G->opt_threads = (int)value;
     else if (k == "refill_threshold" && value >= 1 && value <= 32) G->opt_refill_threshold = (int)value;
+    else if (k == "timing" && (value == 0 || value == 1)) G->opt_timing = (int)value;
     else return fail(SOC_EINVAL, "unknown option or value out of range: " + k);
+    return SOC_OK;
+}
+
+int soc_get_timings(soc_grid *G, int32_t n, float *ms)
+{
+    if (!G || !ms || n < 0) return fail(SOC_EINVAL, "bad argument");
+    for (int i = 0; i < n; ++i) {
+        ms[i] = -1.0f;
+        if (i < (int)G->ev_set.size() && G->ev_set[i]) {
+            SOC_CUDA(cudaEventSynchronize(G->ev1[i]));
+            SOC_CUDA(cudaEventElapsedTime(&ms[i], G->ev0[i], G->ev1[i]));
+        }
+    }
     return SOC_OK;
 }
 

@@ -20,7 +20,7 @@ MAX_POINT_SOURCES = 64
 
 EXPORTS = ["soc_grid_create", "soc_grid_destroy", "soc_grid_n_total", "soc_freq_weights", "soc_simulate_frequency",
            "soc_simulate_packages", "soc_simulate_spectrum", "soc_update_temperatures", "soc_run_host",
-           "soc_set_option", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version"]
+           "soc_set_option", "soc_get_timings", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version"]
 
 
 class SocError(RuntimeError):
@@ -76,6 +76,7 @@ def load():
     L.soc_run_host.argtypes = [C.POINTER(GridDesc), C.POINTER(Sources), i64, u64, i32, dbl, vp, i32, dbl, dbl, vp, vp,
                                C.POINTER(FreqResult), u32]
     L.soc_set_option.argtypes = [vp, C.c_char_p, i64]
+    L.soc_get_timings.argtypes = [vp, i32, vp]
     L.soc_probe_throughput.argtypes = [i32, i64, i64, C.POINTER(C.c_float)]
     L.soc_launch_count.restype = u64
     L.soc_last_error.restype = C.c_char_p
@@ -178,6 +179,12 @@ class Grid:
 
     def set_option(self, key, value):
         _check(load().soc_set_option(self._h, key.encode(), int(value)))
+
+    def timings_ms(self, n=None):
+        """Per-slot photon-kernel device times (needs set_option("timing", 1) before the launches)."""
+        ms = np.zeros(self.n_freq if n is None else int(n), dtype=np.float32)
+        _check(load().soc_get_timings(self._h, len(ms), _ptr(ms)))
+        return ms
 
     def freq_weights(self):
         w = np.zeros(self.n_freq)
