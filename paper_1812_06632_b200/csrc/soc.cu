@@ -85,14 +85,24 @@ struct soc_grid {
     unsigned long long *d_counters = nullptr; // n_slots
     DevResult *h_results = nullptr;           // pinned, n_slots
     float *d_table = nullptr;
+    // internal layout of the production kernel: root grid with one ghost layer, then the octet levels
+    int nbx = 0, nby = 0, nbz = 0, nrp = 0;
+    long long n_int = 0;
+    uint32_t *d_cellw_int = nullptr;
+    int32_t *d_parent_int = nullptr;
+    double *d_acc = nullptr;                  // [n_int], zero between calls
     int n_slots = 0;
     int device = 0, n_sm = 0;
     int opt_blocks_per_sm = 0;                // 0 = from the occupancy calculator
     int opt_threads = 256;
     int opt_refill_threshold = 1;
+    int opt_service_threshold = 8;
+    int opt_debug = 0;
+    int opt_hot_cache = 1;
     int opt_timing = 0;                       // record a CUDA-event pair around every photon launch
     std::vector<cudaEvent_t> ev0, ev1;        // n_slots each (created on demand)
     std::vector<char> ev_set;
+    cudaEvent_t ev_after_photon = nullptr;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -484,6 +494,464 @@ __global__ void __launch_bounds__(256) photon_kernel(const __grid_constant__ Sim
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// production kernel (SOC_GEOM_FP32)
+//
+// Same method, arranged for the machine:
+//   * internal cell layout: the root grid, surrounded by ghost cells, is stored as 2x2x2 bricks of 8
+//     consecutive cells (slot = bx + 2 by + 4 bz, exactly like an octet of the hierarchy), so that a brick of
+//     fp32 cell words is one 32-byte sector.  Half of all face crossings stay inside the brick (`id ^= 1 << a`,
+//     the same sector: an L1 hit instead of an L2 request), the other half add a brick stride.  Leaving the
+//     grid is "the loaded cell word is the sentinel": no coordinates are carried and no bounds are tested.
+//     The accumulator lives in the same layout and is folded into the caller's array by unpad_add_kernel
+//   * the rare, long code (new package: 2-3 Philox blocks + emission; scattering: HG + rotation + Philox +
+//     log + 3 reciprocals) is NOT executed where it arises: the lane parks, and the warp services all parked
+//     lanes together once `service_threshold` of them wait (or nothing else can run), so that code runs with
+//     many lanes active instead of one or two
+//   * package weight is carried relative to the initial energy in fp32 (w in [1e-9, 1]); every deposit is
+//     w - w_new, so emitted = absorbed + escaped holds per package to fp32 rounding (~1e-7, unbiased), and the
+//     scatter-add is (double)(sum of deposits in the cell visit) * E0 into the fp64 accumulator
+// ------------------------------------------------------------------------------------------------
+constexpr uint32_t kSentinel = 0xffffffffu;       // cell word of a ghost cell
+enum : int { RUN = 0, SCAT = 1, DONE = 2, EMPTY = 3, NEWID = 4, DEAD = 5 };
+
+struct FastParams {
+    int nx, ny, nz;                     // root grid
+    int nbx, nby;                       // bricks along x, y of the padded root grid (cell ix sits at X = ix + 2)
+    int bsy, bsz;                       // id strides between bricks along y, z (along x: 8): 8 nbx, 8 nbx nby
+    int nrp;                            // number of padded root cells = 8 nbx nby nbz
+    int n_root;                         // nx*ny*nz
+    const uint32_t *cellw;              // [n_int] leaf: fp32 density bits; parent: 0x80000000 | internal id of first child
+    const int32_t *parent;              // [n_octets] internal id of the parent of octet (id - nrp) >> 3
+    float kabs, ksca, kratio, g;        // kratio = kabs / ksca
+    int is_beam, n_point;
+    long long n_bg;
+    double bg_e0, surf;
+    double beam[6];
+    double ps_pos[SOC_MAX_POINT_SOURCES][3];
+    double ps_e0[SOC_MAX_POINT_SOURCES];
+    long long pkg_begin, pkg_end;
+    unsigned long long seed;
+    int ifreq;
+    int service_threshold;
+    int debug;                          // bit 0: skip the scatter-adds (measurement only)
+    int hot_r;                          // half-width R of the cached cube around every point source, -1 = no cache
+    double *acc;                        // [n_int] internal accumulator (unweighted energies)
+    soc_replay_record *replay;
+    unsigned long long *counter;
+    DevResult *result;
+};
+
+struct FPkg {
+    float fx, fy, fz;       // position inside the cell, [0,1]
+    float dx, dy, dz;       // direction
+    float rx, ry, rz;       // 1/d (+-inf where d == 0)
+    float tau_rem, h;
+    float w, pend, absrel;  // weight / E0; deposits of this cell visit; deposits of this package
+    int rel;                // internal cell id
+    uint32_t cw;
+    uint32_t steps, scat;   // scat is also the index of the current flight segment
+    int src;                // point source index, -1 = background or beam
+    int disp;               // hot-cell tracking: packed (dx + R) | (dy + R) << 8 | (dz + R) << 16 relative to the
+                            // source cell while the package is inside the cached cube, else -1
+    long long id;
+    unsigned long long hash;
+};
+
+// Distance to the exit face along axis a, in cell edges:  t_a = (d_a > 0 ? 1 - f_a : -f_a) / d_a
+//   = fma(-f_a, r_a, max(r_a, 0)).   d_a == 0 gives r_a = +-inf and t_a = +inf or NaN; fminf skips a NaN and the
+// equality test that picks the axis is false for it, so such an axis is never crossed (as in the definition).
+__device__ __forceinline__ float exit_time(float f, float r) { return fmaf(-f, r, fmaxf(r, 0.0f)); }
+
+__device__ __forceinline__ void fast_set_direction(FPkg &p, float dx, float dy, float dz)
+{
+    p.dx = dx; p.dy = dy; p.dz = dz;
+    p.rx = 1.0f / dx; p.ry = 1.0f / dy; p.rz = 1.0f / dz;
+}
+
+__device__ __forceinline__ double package_e0(const FastParams &P, int src)
+{
+    return src >= 0 ? P.ps_e0[src] : (P.is_beam ? 1.0 : P.bg_e0);
+}
+
+// a6: descend to the leaf.  Returns false on the sentinel (outside the root grid).
+__device__ __forceinline__ bool fast_descend(const FastParams &P, FPkg &p)
+{
+    uint32_t cw = __ldg(P.cellw + p.rel);
+    if (cw == kSentinel) { p.cw = cw; return false; }
+    while ((int32_t)cw < 0) {
+        int slot = 0;
+        if (p.fx >= 0.5f) { slot |= 1; p.fx = 2.0f * p.fx - 1.0f; } else p.fx = 2.0f * p.fx;
+        if (p.fy >= 0.5f) { slot |= 2; p.fy = 2.0f * p.fy - 1.0f; } else p.fy = 2.0f * p.fy;
+        if (p.fz >= 0.5f) { slot |= 4; p.fz = 2.0f * p.fz - 1.0f; } else p.fz = 2.0f * p.fz;
+        p.rel = (int)(cw & 0x7fffffffu) + slot;
+        p.h *= 0.5f;
+        cw = __ldg(P.cellw + p.rel);
+    }
+    p.cw = cw;
+    return true;
+}
+
+// internal id of root cell (ix, iy, iz): brick (X>>1, Y>>1, Z>>1), slot (X&1) + 2 (Y&1) + 4 (Z&1), X = ix + 2
+__device__ __forceinline__ int root_id(const FastParams &P, int ix, int iy, int iz)
+{
+    const int X = ix + 2, Y = iy + 2, Z = iz + 2;
+    return 8 * ((X >> 1) + P.nbx * ((Y >> 1) + P.nby * (Z >> 1))) + (X & 1) + 2 * (Y & 1) + 4 * (Z & 1);
+}
+
+// global id (ABI cell vector) of an internal id -- only the replay records need it
+__device__ __forceinline__ long long global_id(const FastParams &P, int rel)
+{
+    if (rel >= P.nrp) return (long long)(rel - P.nrp) + P.n_root;
+    const int B = rel >> 3, bz = B / (P.nbx * P.nby), r = B - bz * (P.nbx * P.nby), by = r / P.nbx, bx = r - by * P.nbx;
+    const int ix = 2 * bx + (rel & 1) - 2, iy = 2 * by + ((rel >> 1) & 1) - 2, iz = 2 * bz + ((rel >> 2) & 1) - 2;
+    return ix + (long long)P.nx * (iy + (long long)P.ny * iz);
+}
+
+// a1-a3: position, cell, direction and energy of package `id`; the direction is returned, not installed
+template <bool HIER>
+__device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, long long id, float &dx, float &dy, float &dz)
+{
+    int ix, iy, iz;
+    p.id = id;
+    if (P.is_beam) {
+        const int n[3] = {P.nx, P.ny, P.nz};
+        int c[3];
+        float f[3];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            int i = (int)floor(P.beam[j]);
+            i = i > n[j] - 1 ? n[j] - 1 : i;
+            c[j] = i;
+            f[j] = (float)(P.beam[j] - (double)i);
+        }
+        ix = c[0]; iy = c[1]; iz = c[2];
+        p.fx = f[0]; p.fy = f[1]; p.fz = f[2];
+        dx = (float)P.beam[3]; dy = (float)P.beam[4]; dz = (float)P.beam[5];
+        p.src = -1;
+    } else if (id < P.n_bg) {
+        uint32_t w0, w1, w2, w3, v0, v1, v2, v3;
+        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
+        philox_block(P.seed, P.ifreq, id, 1u, v0, v1, v2, v3);
+        const double ax = (double)P.ny * P.nz, ay = (double)P.nz * P.nx, az = (double)P.nx * P.ny;
+        const double x = uniform01<double>(w0) * P.surf;
+        int face = 5;
+        if (x < ax) face = 0;
+        else if (x < 2 * ax) face = 1;
+        else if (x < 2 * ax + ay) face = 2;
+        else if (x < 2 * ax + 2 * ay) face = 3;
+        else if (x < 2 * ax + 2 * ay + az) face = 4;
+        const int a = face >> 1, high = face & 1;
+        const int n1 = a == 0 ? P.ny : (a == 1 ? P.nz : P.nx);
+        const int n2 = a == 0 ? P.nz : (a == 1 ? P.nx : P.ny);
+        const int na = a == 0 ? P.nx : (a == 1 ? P.ny : P.nz);
+        const unsigned long long m1 = (unsigned long long)(2u * (w1 >> 9) + 1u) * (unsigned)n1;
+        const unsigned long long m2 = (unsigned long long)(2u * (w2 >> 9) + 1u) * (unsigned)n2;
+        const int i1 = (int)(m1 >> 24), i2 = (int)(m2 >> 24);
+        const float f1 = (float)(uint32_t)(m1 & 0xffffffu) * (float)(1.0 / 16777216.0);
+        const float f2 = (float)(uint32_t)(m2 & 0xffffffu) * (float)(1.0 / 16777216.0);
+        const int ia = high ? na - 1 : 0;
+        const float fa = high ? 1.0f : 0.0f;
+        const float u3 = uniform01<float>(w3);
+        const float mu = sqrtf(u3), st = sqrtf(1.0f - u3);
+        float sp, cp;
+        sincospif(2.0f * uniform01<float>(v0), &sp, &cp);
+        const float da = high ? -mu : mu, d1 = st * cp, d2 = st * sp;
+        if (a == 0)      { ix = ia; iy = i1; iz = i2; p.fx = fa; p.fy = f1; p.fz = f2; dx = da; dy = d1; dz = d2; }
+        else if (a == 1) { iy = ia; iz = i1; ix = i2; p.fy = fa; p.fz = f1; p.fx = f2; dy = da; dz = d1; dx = d2; }
+        else             { iz = ia; ix = i1; iy = i2; p.fz = fa; p.fx = f1; p.fy = f2; dz = da; dx = d1; dy = d2; }
+        p.src = -1;
+    } else {
+        uint32_t w0, w1, w2, w3;
+        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
+        const int k = (int)((id - P.n_bg) % P.n_point);
+        const double px = P.ps_pos[k][0], py = P.ps_pos[k][1], pz = P.ps_pos[k][2];
+        ix = (int)floor(px); iy = (int)floor(py); iz = (int)floor(pz);
+        p.fx = (float)(px - (double)ix); p.fy = (float)(py - (double)iy); p.fz = (float)(pz - (double)iz);
+        const float mu = 2.0f * uniform01<float>(w0) - 1.0f;
+        const float st = sqrtf(fmaxf(0.0f, 1.0f - mu * mu));
+        float sp, cp;
+        sincospif(2.0f * uniform01<float>(w1), &sp, &cp);
+        dx = st * cp; dy = st * sp; dz = mu;
+        p.src = k;
+    }
+    p.h = 1.0f;
+    p.rel = root_id(P, ix, iy, iz);
+    if (HIER) fast_descend(P, p);
+    else p.cw = __ldg(P.cellw + p.rel);
+    // hot-cell tracking starts at the centre of the cube of the package's own source (regular grids only)
+    p.disp = (!HIER && p.src >= 0 && P.hot_r >= 0) ? P.hot_r * 0x010101 : -1;
+    p.steps = 0; p.scat = 0;
+    p.hash = 0xcbf29ce484222325ull;
+    p.w = 1.0f; p.pend = 0.0f; p.absrel = 0.0f;
+}
+
+// 1 - exp(-x) and exp(-x) for x >= 0
+__device__ __forceinline__ void absorb(float w, float x, float &w_new, float &dep)
+{
+    const float e = expf(-x);
+    // x - x^2/2 + x^3/6 - x^4/24 + x^5/120, relative error < 5e-8 for x < 1/8
+    const float small = x * fmaf(x, fmaf(x, fmaf(x, fmaf(x, 1.0f / 120.0f, -1.0f / 24.0f), 1.0f / 6.0f), -0.5f), 1.0f);
+    w_new = x < 0.125f ? w - w * small : w * e;
+    dep = w - w_new;
+}
+
+template <bool HIER, bool REPLAY>
+__global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_constant__ FastParams P)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    double acc_emit = 0.0, acc_esc = 0.0, acc_abs = 0.0;
+    unsigned long long acc_steps = 0;
+    unsigned acc_scat = 0, acc_term = 0;
+    FPkg p;
+    p.src = -1; p.disp = -1; p.w = 0.0f; p.absrel = 0.0f; p.steps = 0; p.scat = 0; p.cw = 0; p.rel = 0; p.h = 1.0f;
+    int need = EMPTY;
+    // hot-cell cache (atomics to the cells around a point source serialise): fp32 partial sums
+    // of the deposits (in units of the source's package energy) into the (2R+1)^3 root cells around each source
+    extern __shared__ float s_hot[];
+    const int hot_side = 2 * P.hot_r + 1;
+    const int hot_cells = P.hot_r >= 0 ? hot_side * hot_side * hot_side : 0;
+    for (int i = threadIdx.x; i < hot_cells * P.n_point; i += blockDim.x) s_hot[i] = 0.0f;
+    __syncthreads();
+    long long pool_next = 0, pool_end = 0;       // warp-uniform id pool
+    bool exhausted = false;
+    const int T = P.service_threshold;
+
+    for (;;) {
+        const unsigned m_park = __ballot_sync(kFull, (unsigned)(need - SCAT) <= (unsigned)(EMPTY - SCAT));
+        const unsigned m_run = __ballot_sync(kFull, need == RUN);
+        if (m_park && (__popc(m_park) >= T || m_run == 0u)) {
+            // ---------------------------------------------------------------- service, all parked lanes together
+            if (need == DONE) {                  // retire the finished package
+                const double e0 = package_e0(P, p.src);
+                acc_esc += (double)p.w * e0;
+                acc_abs += (double)p.absrel * e0;
+                acc_steps += p.steps;
+                acc_scat += p.scat;
+                if (REPLAY) {
+                    soc_replay_record r;
+                    r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = (double)p.w * e0;
+                    P.replay[p.id - P.pkg_begin] = r;
+                }
+                need = EMPTY;
+            }
+            unsigned want = __ballot_sync(kFull, need == EMPTY);
+            if (want && !exhausted) {
+                do {
+                    if (pool_next >= pool_end) {
+                        long long base = 0;
+                        if (lane == 0) base = (long long)atomicAdd(P.counter, (unsigned long long)kChunk);
+                        base = __shfl_sync(kFull, base, 0) + P.pkg_begin;
+                        if (base >= P.pkg_end) { exhausted = true; break; }
+                        pool_next = base;
+                        pool_end = base + kChunk < P.pkg_end ? base + kChunk : P.pkg_end;
+                    }
+                    const long long avail = pool_end - pool_next;
+                    const int rank = __popc(want & lt_mask);
+                    if (need == EMPTY && rank < avail) { p.id = pool_next + rank; need = NEWID; }
+                    const int n_want = __popc(want);
+                    pool_next += n_want < avail ? n_want : avail;
+                    want = __ballot_sync(kFull, need == EMPTY);
+                } while (want);
+            }
+            if (need == EMPTY && exhausted) need = DEAD;
+            float ndx = 0.0f, ndy = 0.0f, ndz = 1.0f;
+            if (need == NEWID) {
+                fast_emit<HIER>(P, p, p.id, ndx, ndy, ndz);
+                acc_emit += package_e0(P, p.src);
+            } else if (need == SCAT) {
+                // finish the flight segment: advance to the scattering point (a4), then a8
+                const float rho = __uint_as_float(p.cw);
+                float t_u = p.tau_rem / (rho * P.ksca);
+                if (HIER) t_u /= p.h;
+                p.fx = __saturatef(fmaf(t_u, p.dx, p.fx));
+                p.fy = __saturatef(fmaf(t_u, p.dy, p.fy));
+                p.fz = __saturatef(fmaf(t_u, p.dz, p.fz));
+                const float g = P.g;
+                uint32_t s0, w_hg, w_az, s3;     // words 1, 2 of the block of the segment that ends here
+                philox_block(P.seed, P.ifreq, p.id, 2u + p.scat, s0, w_hg, w_az, s3);
+                const float mu0 = 2.0f * uniform01<float>(w_hg) - 1.0f;
+                const float num = mu0 + g * (3.0f + mu0 * mu0) * 0.5f + g * g * mu0 + g * g * g * (mu0 * mu0 - 1.0f) * 0.5f;
+                const float den = (1.0f + g * mu0) * (1.0f + g * mu0);
+                float ct = num / den;
+                ct = fminf(1.0f, fmaxf(-1.0f, ct));
+                const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
+                float sp, cp;
+                sincospif(2.0f * uniform01<float>(w_az), &sp, &cp);
+                const float sg = copysignf(1.0f, p.dz);
+                const float a = -1.0f / (sg + p.dz);
+                const float b = p.dx * p.dy * a;
+                const float t1x = 1.0f + sg * p.dx * p.dx * a, t1y = sg * b, t1z = -sg * p.dx;
+                const float t2x = b, t2y = sg + p.dy * p.dy * a, t2z = -p.dy;
+                const float c1 = st * cp, c2 = st * sp;
+                const float qx = c1 * t1x + c2 * t2x + ct * p.dx;
+                const float qy = c1 * t1y + c2 * t2y + ct * p.dy;
+                const float qz = c1 * t1z + c2 * t2z + ct * p.dz;
+                const float inv = rsqrtf(qx * qx + qy * qy + qz * qz);
+                ndx = qx * inv; ndy = qy * inv; ndz = qz * inv;
+                p.scat += 1;
+            }
+            if (need == NEWID || need == SCAT) {
+                fast_set_direction(p, ndx, ndy, ndz);
+                uint32_t s0, s1, s2, s3;
+                philox_block(P.seed, P.ifreq, p.id, 2u + p.scat, s0, s1, s2, s3);
+                p.tau_rem = -__logf(uniform01<float>(s0));                    // a4
+                need = RUN;
+                if (HIER && p.cw == kSentinel) need = DONE;                   // cannot happen for valid sources
+            }
+            continue;
+        }
+        if (m_run == 0u) break;                  // nothing parked that can be serviced, nothing running
+
+        if (need == RUN) {
+            // ---------------------------------------------------------------- one cell-step (a5-a7, a9)
+            const float rho = __uint_as_float(p.cw);
+            const float tx = exit_time(p.fx, p.rx);
+            const float ty = exit_time(p.fy, p.ry);
+            const float tz = exit_time(p.fz, p.rz);
+            const float ts = fminf(fminf(tx, ty), tz);
+            const bool ax0 = tx == ts, ax1 = !ax0 && ty == ts;       // lowest axis wins a tie (reading S4)
+            const float da = ax0 ? p.dx : (ax1 ? p.dy : p.dz);
+            const bool fwd = da > 0.0f;
+            const int bstride = ax0 ? 8 : (ax1 ? P.bsy : P.bsz);      // to the same slot of the next brick
+            const int abit = ax0 ? 1 : (ax1 ? 2 : 4);
+            const float tsh = HIER ? ts * p.h : ts;
+            const float ksr = rho * P.ksca;
+            const float dtau = tsh * ksr;
+            const bool sc = dtau >= p.tau_rem && ksr > 0.0f;
+            const float x = sc ? p.tau_rem * P.kratio : tsh * (rho * P.kabs);
+            float w_new, dep;
+            absorb(p.w, x, w_new, dep);
+            const bool term = w_new < (float)kWMin;                  // a9: residual stays in the cell
+            if (term) { dep = p.w; w_new = 0.0f; }
+            p.pend += dep;
+            p.absrel += dep;
+            p.w = w_new;
+            p.steps += 1;
+            if (REPLAY)                          // the record hashes cell ids of the ABI's cell vector
+                p.hash = (p.hash ^ (unsigned long long)global_id(P, p.rel)) * 0x100000001b3ull;
+            if (term || !sc) {
+                // the package leaves the cell (or ends in it): hand the cell visit's energy to the accumulator --
+                // to the block's shared partial sums while the cell is in the cached cube around the package's
+                // source, with one fp64 reduction to L2 otherwise
+                if (p.disp >= 0) {
+                    const int j = (p.disp & 255) + hot_side * (((p.disp >> 8) & 255) + hot_side * (p.disp >> 16));
+                    atomicAdd(s_hot + p.src * hot_cells + j, p.pend);
+                } else if (p.pend > 0.0f && !(P.debug & 1)) {
+                    atomicAdd(P.acc + p.rel, (double)p.pend * package_e0(P, p.src));
+                }
+                p.pend = 0.0f;
+            }
+            if (term) {
+                acc_term += 1;
+                need = DONE;
+            } else if (sc) {
+                need = SCAT;                     // the segment is finished in the service block
+            } else {
+                p.tau_rem -= dtau;
+                if (!HIER && p.disp >= 0) {      // follow the package through the cached cube
+                    const int sh = ax0 ? 0 : (ax1 ? 8 : 16);
+                    const int nd = p.disp + ((fwd ? 1 : -1) << sh);
+                    p.disp = ((nd >> sh) & 255) < hot_side ? nd : -1;
+                }
+                p.fx = __saturatef(fmaf(ts, p.dx, p.fx));
+                p.fy = __saturatef(fmaf(ts, p.dy, p.fy));
+                p.fz = __saturatef(fmaf(ts, p.dz, p.fz));
+                const float face = fwd ? 0.0f : 1.0f;    // entry face in the neighbour's frame
+                // neighbour inside the brick / octet: flip the slot bit.  Otherwise, for an octet, go up to the
+                // common parent; for a root brick, the same slot bit flips and the brick changes.
+                int rel = p.rel;
+                bool inside = fwd == ((rel & abit) == 0);
+                if (HIER) {
+                    while (!inside && rel >= P.nrp) {
+                        p.fx = (p.fx + (float)(rel & 1)) * 0.5f;
+                        p.fy = (p.fy + (float)((rel >> 1) & 1)) * 0.5f;
+                        p.fz = (p.fz + (float)((rel >> 2) & 1)) * 0.5f;
+                        rel = __ldg(P.parent + ((rel - P.nrp) >> 3));
+                        p.h *= 2.0f;
+                        inside = fwd == ((rel & abit) == 0);
+                    }
+                }
+                rel ^= abit;
+                if (!inside) rel += fwd ? bstride : -bstride;
+                p.rel = rel;
+                if (ax0) p.fx = face; else if (ax1) p.fy = face; else p.fz = face;
+                if (HIER) {
+                    if (!fast_descend(P, p)) need = DONE;            // a9: escaped
+                } else {
+                    p.cw = __ldg(P.cellw + rel);
+                    if (p.cw == kSentinel) need = DONE;              // a9: escaped
+                }
+            }
+        }
+    }
+
+    // ---- the block's hot-cell partial sums go to the accumulator: one fp64 reduction per touched cell and block
+    if (hot_cells > 0) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < hot_cells * P.n_point; i += blockDim.x) {
+            const float v = s_hot[i];
+            if (v != 0.0f) {
+                const int k = i / hot_cells, j = i - k * hot_cells;
+                const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
+                const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
+                          iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
+                atomicAdd(P.acc + root_id(P, ix, iy, iz), (double)v * P.ps_e0[k]);
+            }
+        }
+    }
+
+    // ---- per-launch totals: warp shuffle reduction, one set of atomics per warp
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        acc_emit += __shfl_xor_sync(kFull, acc_emit, o);
+        acc_esc += __shfl_xor_sync(kFull, acc_esc, o);
+        acc_abs += __shfl_xor_sync(kFull, acc_abs, o);
+        acc_steps += __shfl_xor_sync(kFull, acc_steps, o);
+        acc_scat += __shfl_xor_sync(kFull, acc_scat, o);
+        acc_term += __shfl_xor_sync(kFull, acc_term, o);
+    }
+    if (lane == 0 && acc_steps != 0) {
+        atomicAdd(&P.result->emitted, acc_emit);
+        atomicAdd(&P.result->escaped, acc_esc);
+        atomicAdd(&P.result->absorbed, acc_abs);
+        atomicAdd(&P.result->cell_steps, acc_steps);
+        atomicAdd(&P.result->scatterings, (unsigned long long)acc_scat);
+        atomicAdd(&P.result->terminated, (unsigned long long)acc_term);
+    }
+}
+
+// internal accumulator -> caller's array: out[gid] += weight * acc[internal(gid)], acc reset to zero
+struct UnpadParams {
+    double *out, *acc;
+    double weight;
+    int nx, ny, nbx, nby, nrp;
+    long long n_root, n_total;
+};
+
+__global__ void __launch_bounds__(256) unpad_add_kernel(const __grid_constant__ UnpadParams U)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x; gid < U.n_total; gid += stride) {
+        long long j;
+        if (gid < U.n_root) {
+            const int g = (int)gid;
+            const int ix = g % U.nx, r = g / U.nx, iy = r % U.ny, iz = r / U.ny;
+            const int X = ix + 2, Y = iy + 2, Z = iz + 2;
+            j = 8ll * ((X >> 1) + U.nbx * ((Y >> 1) + (long long)U.nby * (Z >> 1))) + (X & 1) + 2 * (Y & 1) + 4 * (Z & 1);
+        } else {
+            j = U.nrp + (gid - U.n_root);
+        }
+        const double v = U.acc[j];
+        if (v != 0.0) {
+            U.out[gid] += U.weight * v;
+            U.acc[j] = 0.0;
+        }
+    }
+}
+
 // a11: energy balance by table lookup, 4 cells per thread, table in shared memory
 struct TempParams {
     const uint32_t *cellw;
@@ -573,9 +1041,19 @@ __global__ void __launch_bounds__(256) probe_kernel(void *buf, unsigned long lon
         const unsigned long long j = ((unsigned long long)s * n_elem) >> 32;
         if (KIND == 0) acc += __ldg(reinterpret_cast<const float *>(buf) + j);
         else if (KIND == 1) atomicAdd(reinterpret_cast<double *>(buf) + j, 1.0);
-        else atomicAdd(reinterpret_cast<float *>(buf) + j, 1.0f);
+        else if (KIND == 2) atomicAdd(reinterpret_cast<float *>(buf) + j, 1.0f);
+        else if (KIND == 3) {                    // 32-byte gather (one sector: a 2x2x2 brick of fp32 cells)
+            float a0, a1, a2, a3, a4, a5, a6, a7;
+            asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                         : "=f"(a0), "=f"(a1), "=f"(a2), "=f"(a3), "=f"(a4), "=f"(a5), "=f"(a6), "=f"(a7)
+                         : "l"(reinterpret_cast<const float *>(buf) + 8 * j));
+            acc += a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+        } else {                                 // 16-byte vector reduction (4 fp32 cells)
+            asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(reinterpret_cast<float *>(buf) + 4 * j),
+                         "f"(1.0f), "f"(1.0f), "f"(1.0f), "f"(1.0f) : "memory");
+        }
     }
-    if (KIND == 0 && acc == 123.456f) *sink = acc;
+    if ((KIND == 0 || KIND == 3) && acc == 123.456f) *sink = acc;
 }
 
 }  // namespace
@@ -631,6 +1109,40 @@ template <typename R, bool HIER, bool REPLAY> int launch_photon(soc_grid *G, con
     const long long need = (n_pkg + threads - 1) / threads;
     if (need < blocks) blocks = (int)(need > 0 ? need : 1);
     photon_kernel<R, HIER, REPLAY><<<blocks, threads, 0, st>>>(P);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    return SOC_OK;
+}
+
+template <bool HIER, bool REPLAY> int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
+{
+    int blocks = 0;
+    const int threads = G->opt_threads;
+    const int side = 2 * P.hot_r + 1;
+    const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
+    int per_sm = 0;
+    SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY>, threads, smem));
+    if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
+    if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
+    blocks = per_sm * G->n_sm;                   // persistent: a whole number of CTAs per SM
+    const long long n_pkg = P.pkg_end - P.pkg_begin;
+    const long long need = (n_pkg + threads - 1) / threads;
+    if (need < blocks) blocks = (int)(need > 0 ? need : 1);
+    photon_fast_kernel<HIER, REPLAY><<<blocks, threads, smem, st>>>(P);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    if (G->ev_after_photon) {                    // "timing": the pair brackets the photon kernel alone
+        SOC_CUDA(cudaEventRecord(G->ev_after_photon, st));
+        G->ev_after_photon = nullptr;
+    }
+    UnpadParams U;
+    U.out = absorbed; U.acc = G->d_acc; U.weight = weight;
+    U.nx = G->nx; U.ny = G->ny; U.nbx = G->nbx; U.nby = G->nby; U.nrp = G->nrp;
+    U.n_root = G->n_root; U.n_total = G->n_total;
+    long long ub = (G->n_total + 255) / 256;
+    const long long cap = (long long)G->n_sm * 8;
+    if (ub > cap) ub = cap;
+    unpad_add_kernel<<<(int)ub, 256, 0, st>>>(U);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     return SOC_OK;
@@ -717,16 +1229,39 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         rc = ensure_events(G, slot + 1);
         if (rc != SOC_OK) return rc;
         SOC_CUDA(cudaEventRecord(G->ev0[slot], st));
+        G->ev_after_photon = G->ev1[slot];
     }
-#define SOC_DISPATCH(R)                                                                             \
-    (hier ? (rep ? launch_photon<R, true, true>(G, P, st) : launch_photon<R, true, false>(G, P, st)) \
-          : (rep ? launch_photon<R, false, true>(G, P, st) : launch_photon<R, false, false>(G, P, st)))
-    rc = f64 ? SOC_DISPATCH(double) : SOC_DISPATCH(float);
-#undef SOC_DISPATCH
+    if (f64) {
+        rc = hier ? (rep ? launch_photon<double, true, true>(G, P, st) : launch_photon<double, true, false>(G, P, st))
+                  : (rep ? launch_photon<double, false, true>(G, P, st) : launch_photon<double, false, false>(G, P, st));
+    } else {
+        FastParams F;
+        std::memset(&F, 0, sizeof(F));
+        F.nx = G->nx; F.ny = G->ny; F.nz = G->nz; F.nbx = G->nbx; F.nby = G->nby;
+        F.bsy = 8 * G->nbx; F.bsz = 8 * G->nbx * G->nby; F.nrp = G->nrp; F.n_root = (int)G->n_root;
+        F.cellw = G->d_cellw_int; F.parent = G->d_parent_int;
+        F.kabs = (float)P.kabs; F.ksca = (float)P.ksca; F.g = (float)P.g;
+        F.kratio = P.ksca > 0.0 ? (float)(P.kabs / P.ksca) : 0.0f;
+        F.is_beam = P.is_beam; F.n_point = P.n_point; F.n_bg = P.n_bg; F.bg_e0 = P.bg_e0; F.surf = P.surf;
+        std::memcpy(F.beam, P.beam, sizeof(F.beam));
+        std::memcpy(F.ps_pos, P.ps_pos, sizeof(F.ps_pos));
+        std::memcpy(F.ps_e0, P.ps_e0, sizeof(F.ps_e0));
+        F.pkg_begin = P.pkg_begin; F.pkg_end = P.pkg_end; F.seed = P.seed; F.ifreq = P.ifreq;
+        F.service_threshold = G->opt_service_threshold;
+        F.debug = G->opt_debug;
+        // hot-cell cache: R = 3 (343 cells per source) while it fits in 40 KB per block, else R = 2; regular grids
+        F.hot_r = -1;
+        if (!hier && P.n_point > 0 && !P.is_beam && G->opt_hot_cache)
+            F.hot_r = (size_t)P.n_point * 343 * sizeof(float) <= 40 * 1024 ? 3 : 2;
+        F.acc = G->d_acc; F.replay = P.replay; F.counter = P.counter; F.result = P.result;
+        rc = hier ? (rep ? launch_fast<true, true>(G, F, weight, absorbed, st) : launch_fast<true, false>(G, F, weight, absorbed, st))
+                  : (rep ? launch_fast<false, true>(G, F, weight, absorbed, st) : launch_fast<false, false>(G, F, weight, absorbed, st));
+    }
     if (rc == SOC_OK && G->opt_timing) {
-        SOC_CUDA(cudaEventRecord(G->ev1[slot], st));
+        if (G->ev_after_photon) SOC_CUDA(cudaEventRecord(G->ev1[slot], st));
         G->ev_set[slot] = 1;
     }
+    G->ev_after_photon = nullptr;
     return rc;
 }
 
@@ -765,7 +1300,7 @@ void soc_grid_destroy(soc_grid *G)
 {
     if (!G) return;
     cudaFree(G->d_cellw); cudaFree(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
-    cudaFree(G->d_table);
+    cudaFree(G->d_table); cudaFree(G->d_cellw_int); cudaFree(G->d_parent_int); cudaFree(G->d_acc);
     if (G->h_results) cudaFreeHost(G->h_results);
     for (cudaEvent_t e : G->ev0) cudaEventDestroy(e);
     for (cudaEvent_t e : G->ev1) cudaEventDestroy(e);
@@ -849,6 +1384,41 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     SOC_CUDA(cudaMalloc(&G->d_table, sizeof(float) * 8192));
     SOC_CUDA(cudaMemcpy(G->d_cellw, cellw.data(), sizeof(uint32_t) * (size_t)G->n_total, cudaMemcpyHostToDevice));
     SOC_CUDA(cudaMemcpy(G->d_parent, parent.data(), sizeof(int32_t) * parent.size(), cudaMemcpyHostToDevice));
+    // internal layout: root grid in 2x2x2 bricks with ghost cells around it (they hold the sentinel; cell ix
+    // sits at X = ix + 2, so the low side has a whole ghost brick and the high side at least one ghost cell),
+    // octet levels shifted behind it
+    {
+        const long long nbx = ((long long)G->nx + 4) / 2, nby = ((long long)G->ny + 4) / 2, nbz = ((long long)G->nz + 4) / 2;
+        const long long nrp = 8 * nbx * nby * nbz;
+        const long long n_int = nrp + (G->n_total - G->n_root);
+        if (n_int >= (1ll << 31)) return fail(SOC_EINVAL, "more than 2^31 cells in the padded layout");
+        G->nbx = (int)nbx; G->nby = (int)nby; G->nbz = (int)nbz; G->nrp = (int)nrp; G->n_int = n_int;
+        std::vector<uint32_t> ci;
+        std::vector<int32_t> pi;
+        try {
+            ci.assign((size_t)n_int, kSentinel);
+            pi.assign(parent.size(), 0);
+        } catch (const std::bad_alloc &) {
+            return fail(SOC_ENOMEM, "out of host memory");
+        }
+        auto internal = [&](long long gid) -> long long {
+            if (gid >= G->n_root) return nrp + (gid - G->n_root);
+            const long long ix = gid % G->nx, r = gid / G->nx, iy = r % G->ny, iz = r / G->ny;
+            const long long X = ix + 2, Y = iy + 2, Z = iz + 2;
+            return 8 * ((X >> 1) + nbx * ((Y >> 1) + nby * (Z >> 1))) + (X & 1) + 2 * (Y & 1) + 4 * (Z & 1);
+        };
+        for (long long gid = 0; gid < G->n_total; ++gid) {
+            const uint32_t cw = cellw[(size_t)gid];
+            ci[(size_t)internal(gid)] = (int32_t)cw < 0 ? (0x80000000u | (uint32_t)(nrp + (cw & 0x7fffffffu))) : cw;
+        }
+        for (long long o = 0; o < G->n_octets; ++o) pi[(size_t)o] = (int32_t)internal((long long)parent[(size_t)o] + G->n_root);
+        SOC_CUDA(cudaMalloc(&G->d_cellw_int, sizeof(uint32_t) * (size_t)n_int));
+        SOC_CUDA(cudaMalloc(&G->d_parent_int, sizeof(int32_t) * pi.size()));
+        SOC_CUDA(cudaMalloc(&G->d_acc, sizeof(double) * (size_t)n_int));
+        SOC_CUDA(cudaMemcpy(G->d_cellw_int, ci.data(), sizeof(uint32_t) * (size_t)n_int, cudaMemcpyHostToDevice));
+        SOC_CUDA(cudaMemcpy(G->d_parent_int, pi.data(), sizeof(int32_t) * pi.size(), cudaMemcpyHostToDevice));
+        SOC_CUDA(cudaMemset(G->d_acc, 0, sizeof(double) * (size_t)n_int));
+    }
     int rc = ensure_slots(G, d->n_freq > 8 ? d->n_freq : 8);
     if (rc != SOC_OK) return rc;
     guard.g = nullptr;
@@ -872,7 +1442,10 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     if (k == "blocks_per_sm" && value >= 0 && value <= 32) G->opt_blocks_per_sm = (int)value;
     else if (k == "threads" && (value == 64 || value == 128 || value == 256)) G->opt_threads = (int)value;
     else if (k == "refill_threshold" && value >= 1 && value <= 32) G->opt_refill_threshold = (int)value;
+    else if (k == "service_threshold" && value >= 1 && value <= 32) G->opt_service_threshold = (int)value;
     else if (k == "timing" && (value == 0 || value == 1)) G->opt_timing = (int)value;
+    else if (k == "debug" && value >= 0 && value <= 255) G->opt_debug = (int)value;
+    else if (k == "hot_cache" && (value == 0 || value == 1)) G->opt_hot_cache = (int)value;
     else return fail(SOC_EINVAL, "unknown option or value out of range: " + k);
     return SOC_OK;
 }
@@ -993,8 +1566,8 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
 
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms)
 {
-    if (kind < 0 || kind > 2 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
-    const size_t elem = kind == 1 ? 8 : 4;
+    if (kind < 0 || kind > 4 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
+    const size_t elem = kind == 1 ? 8 : (kind == 3 ? 32 : (kind == 4 ? 16 : 4));
     const unsigned long long n_elem = (unsigned long long)footprint_bytes / elem;
     void *buf = nullptr;
     float *sink = nullptr;
@@ -1013,7 +1586,9 @@ int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, f
         SOC_CUDA(cudaEventRecord(e0));
         if (kind == 0) probe_kernel<0><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else if (kind == 1) probe_kernel<1><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
-        else probe_kernel<2><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else if (kind == 2) probe_kernel<2><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else if (kind == 3) probe_kernel<3><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else probe_kernel<4><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         g_launches += 1;
         SOC_CUDA(cudaEventRecord(e1));
         SOC_CUDA(cudaEventSynchronize(e1));

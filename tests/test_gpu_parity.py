@@ -99,18 +99,22 @@ def test_config2_replay_full():
     _check_replay(P, 0, P.sources(0), P.n_packages, P.seed)
 
 
-@pytest.mark.parametrize("which,kw", [("1", {}), ("2", dict(n=32, n_packages=200_000))])
+@pytest.mark.parametrize("which,kw", [("1", {}), ("2", dict(n=32, n_packages=200_000)),
+                                      ("3", dict(n=32, n_packages=200_000, n_freq=8))])
 def test_production_mode_within_5_sigma(which, kw):
     """Seeds 1..8 on both sides; sigma_c = per-cell sample standard deviation of the oracle's 8 runs;
-    |A_gpu(s) - A_orc(s)| <= 5 sigma_c for every cell and seed."""
+    |A_gpu(s) - A_orc(s)| <= 5 sigma_c for every cell and seed.  The config-3 case (visual
+    frequency) has two point sources: half of the packages start in two cells, whose surroundings go through
+    the per-block shared partial sums of the production kernel."""
     P = inputs.make_config(which, **kw)
     G = soc.Grid.from_problem(P)
     og = oracle_grid(P)
-    src = P.sources(0)
+    f = 0 if P.n_freq == 1 else int(np.argmin(np.abs(P.notes["lam_um"] - 0.55)))
+    src = P.sources(f)
     Ao, Ag = [], []
     for seed in range(1, 9):
-        Ao.append(oracle_packages(og, P, 0, src, P.n_packages, seed, want_replay=False)[0])
-        a, rg, _ = gpu_packages(G, P, 0, src, P.n_packages, seed, flags=PROD, want_replay=False)
+        Ao.append(oracle_packages(og, P, f, src, P.n_packages, seed, want_replay=False)[0])
+        a, rg, _ = gpu_packages(G, P, f, src, P.n_packages, seed, flags=PROD, want_replay=False)
         assert abs(rg["emitted"] - rg["absorbed"] - rg["escaped"]) <= 1e-6 * rg["emitted"]
         Ag.append(a)
     G.close()
@@ -254,7 +258,9 @@ def test_empty_and_tiny_inputs():
     r = G.simulate_packages(0, P.sources(0), 10, 1, 1.0, 3, 0, A)            # empty id range
     assert r.emitted == 0 and r.cell_steps == 0 and float(A.sum()) == 0.0
     r = G.simulate_frequency(0, P.sources(0), 1, 1, 1.0, A)                  # a single package
-    assert r.cell_steps >= 1 and abs(r.emitted - r.absorbed - r.escaped) < 1e-12 * r.emitted
+    # production mode carries the package weight in fp32: conservation per package to fp32 rounding, inside the
+    # 1e-6 of BASELINE.json:north_star
+    assert r.cell_steps >= 1 and abs(r.emitted - r.absorbed - r.escaped) < 1e-6 * r.emitted
     G.close()
     # zero-density cloud: nothing absorbed, nothing scattered, every package escapes (PAPER.md:117 empty cells)
     P0 = _problem_from_arrays((6, 5, 4), [120], np.zeros(120), None, 1.0, 1.0, 0.3, 20000)
@@ -274,9 +280,14 @@ def test_point_source_in_empty_cell_and_hot_cell():
     src = dict(ps_pos=np.array([[2.5, 2.5, 2.5]]), ps_lum=np.array([1.0]))
     m, l1, rg, ro = _check_replay(P, 0, src, 100_000, 1)
     G = soc.Grid.from_problem(P)
-    A, _, _ = gpu_packages(G, P, 0, src, 100_000, 1, flags=PROD, want_replay=False)
+    A, rp, _ = gpu_packages(G, P, 0, src, 100_000, 1, flags=PROD, want_replay=False)
     G.close()
     assert A[62] == 0.0
+    # production mode: every cell of this grid lies in the cached cube around the source (shared fp32 partial sums)
+    Ao, _, _ = oracle_packages(oracle_grid(P), P, 0, src, 100_000, 1, want_replay=False)
+    assert rel_l1(A, Ao) < 2e-3
+    assert A.sum() == pytest.approx(rp["absorbed"], rel=1e-6)
+    assert abs(rp["emitted"] - rp["absorbed"] - rp["escaped"]) <= 1e-6 * rp["emitted"]
 
 
 def test_accumulates_with_weight_and_subsets_add_up():
@@ -307,7 +318,9 @@ def test_run_host_equals_device_path():
     T = torch.empty(P.n_total, dtype=torch.float32, device="cuda")
     G.update_temperatures(Aint, P.t_scale / 2, P.table_T, P.e_min, P.e_max, T)
     G.close()
-    assert np.allclose(A_h, Aint.cpu().numpy() / 2, rtol=1e-9, atol=0)
+    # the two runs differ only in the order of the scatter-adds: fp64 for the L2 reductions, fp32 for the
+    # per-block partial sums of the cells around the point sources
+    assert np.allclose(A_h, Aint.cpu().numpy() / 2, rtol=2e-5, atol=0)
     assert np.abs(T_h - T.cpu().numpy()).max() <= 1e-3
     assert len(res) == 2 * P.n_freq and all(abs(r.emitted - r.absorbed - r.escaped) <= 1e-6 * r.emitted for r in res)
 
