@@ -189,6 +189,9 @@ def run_ours(args):
     shard = socdist.plan("weak", rank, world, P.n_packages, P.seed)
     G = soc.Grid.from_problem(P)
     G.set_option("timing", 1)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        G.set_option(k, int(v))
     srcs = [P.sources(f) for f in range(P.n_freq)]
     has_T = P.table_T is not None
     Aint = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
@@ -342,6 +345,7 @@ def main():
     ap.add_argument("--config", choices=sorted(WORKLOADS), default="3")
     ap.add_argument("--packages", type=int, default=0, help="override packages per frequency (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], help="library tuning knob key=value (soc_set_option)")
     args = ap.parse_args()
     if args.steps < 1 or args.warmup < 0:
         raise SystemExit("need --steps >= 1 and --warmup >= 0")

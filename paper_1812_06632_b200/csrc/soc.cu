@@ -91,6 +91,8 @@ struct soc_grid {
     uint32_t *d_cellw_int = nullptr;
     int32_t *d_parent_int = nullptr;
     double *d_acc = nullptr;                  // [n_int], zero between calls
+    float *d_acc32 = nullptr;                 // [n_int], zero between calls (fp32 internal accumulator)
+    int opt_acc32 = 1;
     int n_slots = 0;
     int device = 0, n_sm = 0;
     int opt_blocks_per_sm = 0;                // 0 = from the occupancy calculator
@@ -537,7 +539,10 @@ struct FastParams {
     int service_threshold;
     int debug;                          // bit 0: skip the scatter-adds (measurement only)
     int hot_r;                          // half-width R of the cached cube around every point source, -1 = no cache
-    double *acc;                        // [n_int] internal accumulator (unweighted energies)
+    double *acc;                        // [n_int] internal accumulator (unweighted energies), ACC32 = false
+    float *acc32;                       // [n_int] internal accumulator in units of e_ref, ACC32 = true
+    float bg_rel, beam_rel;             // package energy / e_ref of a background / beam package
+    float ps_rel[SOC_MAX_POINT_SOURCES];  // ... of a package of point source k
     soc_replay_record *replay;
     unsigned long long *counter;
     DevResult *result;
@@ -573,6 +578,11 @@ __device__ __forceinline__ void fast_set_direction(FPkg &p, float dx, float dy, 
 __device__ __forceinline__ double package_e0(const FastParams &P, int src)
 {
     return src >= 0 ? P.ps_e0[src] : (P.is_beam ? 1.0 : P.bg_e0);
+}
+
+__device__ __forceinline__ float package_rel(const FastParams &P, int src)
+{
+    return src >= 0 ? P.ps_rel[src] : (P.is_beam ? P.beam_rel : P.bg_rel);
 }
 
 // a6: descend to the leaf.  Returns false on the sentinel (outside the root grid).
@@ -697,7 +707,7 @@ __device__ __forceinline__ void absorb(float w, float x, float &w_new, float &de
     dep = w - w_new;
 }
 
-template <bool HIER, bool REPLAY>
+template <bool HIER, bool REPLAY, bool ACC32>
 __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_constant__ FastParams P)
 {
     const int lane = threadIdx.x & 31;
@@ -840,7 +850,8 @@ __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_consta
                     const int j = (p.disp & 255) + hot_side * (((p.disp >> 8) & 255) + hot_side * (p.disp >> 16));
                     atomicAdd(s_hot + p.src * hot_cells + j, p.pend);
                 } else if (p.pend > 0.0f && !(P.debug & 1)) {
-                    atomicAdd(P.acc + p.rel, (double)p.pend * package_e0(P, p.src));
+                    if (ACC32) atomicAdd(P.acc32 + p.rel, p.pend * package_rel(P, p.src));
+                    else atomicAdd(P.acc + p.rel, (double)p.pend * package_e0(P, p.src));
                 }
                 p.pend = 0.0f;
             }
@@ -898,7 +909,8 @@ __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_consta
                 const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
                 const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
                           iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
-                atomicAdd(P.acc + root_id(P, ix, iy, iz), (double)v * P.ps_e0[k]);
+                if (ACC32) atomicAdd(P.acc32 + root_id(P, ix, iy, iz), v * P.ps_rel[k]);
+                else atomicAdd(P.acc + root_id(P, ix, iy, iz), (double)v * P.ps_e0[k]);
             }
         }
     }
@@ -926,11 +938,13 @@ __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_consta
 // internal accumulator -> caller's array: out[gid] += weight * acc[internal(gid)], acc reset to zero
 struct UnpadParams {
     double *out, *acc;
-    double weight;
+    float *acc32;
+    double weight;                      // ACC32: weight * e_ref
     int nx, ny, nbx, nby, nrp;
     long long n_root, n_total;
 };
 
+template <bool ACC32>
 __global__ void __launch_bounds__(256) unpad_add_kernel(const __grid_constant__ UnpadParams U)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
@@ -944,10 +958,18 @@ __global__ void __launch_bounds__(256) unpad_add_kernel(const __grid_constant__ 
         } else {
             j = U.nrp + (gid - U.n_root);
         }
-        const double v = U.acc[j];
-        if (v != 0.0) {
-            U.out[gid] += U.weight * v;
-            U.acc[j] = 0.0;
+        if (ACC32) {
+            const float v = U.acc32[j];
+            if (v != 0.0f) {
+                U.out[gid] += U.weight * (double)v;
+                U.acc32[j] = 0.0f;
+            }
+        } else {
+            const double v = U.acc[j];
+            if (v != 0.0) {
+                U.out[gid] += U.weight * v;
+                U.acc[j] = 0.0;
+            }
         }
     }
 }
@@ -1114,21 +1136,22 @@ template <typename R, bool HIER, bool REPLAY> int launch_photon(soc_grid *G, con
     return SOC_OK;
 }
 
-template <bool HIER, bool REPLAY> int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
+template <bool HIER, bool REPLAY, bool ACC32>
+int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
 {
     int blocks = 0;
     const int threads = G->opt_threads;
     const int side = 2 * P.hot_r + 1;
     const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
     int per_sm = 0;
-    SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY>, threads, smem));
+    SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY, ACC32>, threads, smem));
     if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
     if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
     blocks = per_sm * G->n_sm;                   // persistent: a whole number of CTAs per SM
     const long long n_pkg = P.pkg_end - P.pkg_begin;
     const long long need = (n_pkg + threads - 1) / threads;
     if (need < blocks) blocks = (int)(need > 0 ? need : 1);
-    photon_fast_kernel<HIER, REPLAY><<<blocks, threads, smem, st>>>(P);
+    photon_fast_kernel<HIER, REPLAY, ACC32><<<blocks, threads, smem, st>>>(P);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     if (G->ev_after_photon) {                    // "timing": the pair brackets the photon kernel alone
@@ -1136,13 +1159,13 @@ template <bool HIER, bool REPLAY> int launch_fast(soc_grid *G, const FastParams 
         G->ev_after_photon = nullptr;
     }
     UnpadParams U;
-    U.out = absorbed; U.acc = G->d_acc; U.weight = weight;
+    U.out = absorbed; U.acc = G->d_acc; U.acc32 = G->d_acc32; U.weight = weight;
     U.nx = G->nx; U.ny = G->ny; U.nbx = G->nbx; U.nby = G->nby; U.nrp = G->nrp;
     U.n_root = G->n_root; U.n_total = G->n_total;
     long long ub = (G->n_total + 255) / 256;
     const long long cap = (long long)G->n_sm * 8;
     if (ub > cap) ub = cap;
-    unpad_add_kernel<<<(int)ub, 256, 0, st>>>(U);
+    unpad_add_kernel<ACC32><<<(int)ub, 256, 0, st>>>(U);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     return SOC_OK;
@@ -1254,8 +1277,33 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         if (!hier && P.n_point > 0 && !P.is_beam && G->opt_hot_cache)
             F.hot_r = (size_t)P.n_point * 343 * sizeof(float) <= 40 * 1024 ? 3 : 2;
         F.acc = G->d_acc; F.replay = P.replay; F.counter = P.counter; F.result = P.result;
-        rc = hier ? (rep ? launch_fast<true, true>(G, F, weight, absorbed, st) : launch_fast<true, false>(G, F, weight, absorbed, st))
-                  : (rep ? launch_fast<false, true>(G, F, weight, absorbed, st) : launch_fast<false, false>(G, F, weight, absorbed, st));
+        // fp32 internal accumulator: deposits in units of the largest package energy of
+        // this launch; falls back to the fp64 accumulator when a source class would underflow in those units
+        double e_ref = P.is_beam ? 1.0 : P.bg_e0;
+        for (int k = 0; k < P.n_point; ++k) e_ref = std::fmax(e_ref, P.ps_e0[k]);
+        bool acc32 = G->opt_acc32 != 0 && e_ref > 0.0 && std::isfinite(e_ref);
+        if (acc32) {
+            F.beam_rel = (float)(1.0 / e_ref);
+            F.bg_rel = (float)(P.bg_e0 / e_ref);
+            if (!P.is_beam && P.n_bg > 0 && P.bg_e0 > 0.0 && F.bg_rel < 1e-20f) acc32 = false;
+            for (int k = 0; k < P.n_point; ++k) {
+                F.ps_rel[k] = (float)(P.ps_e0[k] / e_ref);
+                if (P.ps_e0[k] > 0.0 && F.ps_rel[k] < 1e-20f) acc32 = false;
+            }
+        }
+        F.acc32 = G->d_acc32;
+        const double w_eff = acc32 ? weight * e_ref : weight;
+        const int sel = (hier ? 4 : 0) | (rep ? 2 : 0) | (acc32 ? 1 : 0);
+        switch (sel) {
+        case 0: rc = launch_fast<false, false, false>(G, F, w_eff, absorbed, st); break;
+        case 1: rc = launch_fast<false, false, true>(G, F, w_eff, absorbed, st); break;
+        case 2: rc = launch_fast<false, true, false>(G, F, w_eff, absorbed, st); break;
+        case 3: rc = launch_fast<false, true, true>(G, F, w_eff, absorbed, st); break;
+        case 4: rc = launch_fast<true, false, false>(G, F, w_eff, absorbed, st); break;
+        case 5: rc = launch_fast<true, false, true>(G, F, w_eff, absorbed, st); break;
+        case 6: rc = launch_fast<true, true, false>(G, F, w_eff, absorbed, st); break;
+        default: rc = launch_fast<true, true, true>(G, F, w_eff, absorbed, st); break;
+        }
     }
     if (rc == SOC_OK && G->opt_timing) {
         if (G->ev_after_photon) SOC_CUDA(cudaEventRecord(G->ev1[slot], st));
@@ -1300,7 +1348,7 @@ void soc_grid_destroy(soc_grid *G)
 {
     if (!G) return;
     cudaFree(G->d_cellw); cudaFree(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
-    cudaFree(G->d_table); cudaFree(G->d_cellw_int); cudaFree(G->d_parent_int); cudaFree(G->d_acc);
+    cudaFree(G->d_table); cudaFree(G->d_cellw_int); cudaFree(G->d_parent_int); cudaFree(G->d_acc); cudaFree(G->d_acc32);
     if (G->h_results) cudaFreeHost(G->h_results);
     for (cudaEvent_t e : G->ev0) cudaEventDestroy(e);
     for (cudaEvent_t e : G->ev1) cudaEventDestroy(e);
@@ -1418,6 +1466,8 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
         SOC_CUDA(cudaMemcpy(G->d_cellw_int, ci.data(), sizeof(uint32_t) * (size_t)n_int, cudaMemcpyHostToDevice));
         SOC_CUDA(cudaMemcpy(G->d_parent_int, pi.data(), sizeof(int32_t) * pi.size(), cudaMemcpyHostToDevice));
         SOC_CUDA(cudaMemset(G->d_acc, 0, sizeof(double) * (size_t)n_int));
+        SOC_CUDA(cudaMalloc(&G->d_acc32, sizeof(float) * (size_t)n_int));
+        SOC_CUDA(cudaMemset(G->d_acc32, 0, sizeof(float) * (size_t)n_int));
     }
     int rc = ensure_slots(G, d->n_freq > 8 ? d->n_freq : 8);
     if (rc != SOC_OK) return rc;
@@ -1446,6 +1496,7 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     else if (k == "timing" && (value == 0 || value == 1)) G->opt_timing = (int)value;
     else if (k == "debug" && value >= 0 && value <= 255) G->opt_debug = (int)value;
     else if (k == "hot_cache" && (value == 0 || value == 1)) G->opt_hot_cache = (int)value;
+    else if (k == "acc32" && (value == 0 || value == 1)) G->opt_acc32 = (int)value;
     else return fail(SOC_EINVAL, "unknown option or value out of range: " + k);
     return SOC_OK;
 }
