@@ -342,7 +342,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--config", choices=sorted(WORKLOADS), default="3")
+    ap.add_argument("--config", choices=sorted(WORKLOADS), default="5")
     ap.add_argument("--packages", type=int, default=0, help="override packages per frequency (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--opt", action="append", default=[], help="library tuning knob key=value (soc_set_option)")
