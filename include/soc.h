@@ -143,7 +143,11 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
                  double E_max, double *absorbed_int_out, float *T_out, soc_freq_result *results,
                  uint32_t flags);
 
-/* Tuning knobs (all have defaults chosen for B200): "blocks_per_sm", "threads", "refill_threshold"; and
+/* Tuning knobs (all have defaults chosen for B200): "blocks_per_sm", "threads", "refill_threshold" (replay
+ * kernel), "service_threshold" (parked lanes that trigger a service pass), "hot_cache" (0/1: shared partial sums
+ * for the cells around point sources), "acc32" (0/1: fp32 per-launch accumulator), "kernel" (production kernel on
+ * regular grids: 0 = chosen by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel), "carveout"
+ * (preferred shared-memory carve-out in %, -1 = driver default), "debug" (measurement only); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
  * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
 int soc_set_option(soc_grid *grid, const char *key, int64_t value);

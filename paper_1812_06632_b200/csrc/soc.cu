@@ -102,10 +102,8 @@ struct soc_grid {
     int opt_debug = 0;
     int opt_hot_cache = 1;
     int opt_carveout = -1;                    // preferred shared-memory carve-out of the photon kernels in %, -1 = driver default
-    int opt_tile_rounds = 0;                  // rounds of the tiled walk before the resume kernel; 0 = automatic
-    void *tile_mem[12] = {nullptr};           // device allocations behind TileBuffers (tiled production path)
-    long long tile_cap = 0;                   // packages the tile buffers are sized for
-    int opt_kernel = 2;                       // 2 = run-ahead kernel on regular grids, 1 = photon_fast_kernel everywhere
+    double rho_mean = 0.0;                    // mean density of the root-level leaves
+    int opt_kernel = 0;                       // regular grids: 0 = by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel
     int opt_timing = 0;                       // record a CUDA-event pair around every photon launch
     std::vector<cudaEvent_t> ev0, ev1;        // n_slots each (created on demand)
     std::vector<char> ev_set;
@@ -708,14 +706,28 @@ __device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, long lon
     p.w = 1.0f; p.pend = 0.0f; p.absrel = 0.0f;
 }
 
-// 1 - exp(-x) and exp(-x) for x >= 0
+// a7: new weight w e^-x and deposit w (1 - e^-x) for x >= 0.  Below x = 1/8 the deposit is w times the series
+//   x - x^2/2 + x^3/6 - x^4/24 + x^5/120   (relative error < 5e-8)
+// and the weight is reduced by it, so that a deposit far below the fp32 resolution of the weight (x ~ 1e-8 per cell at
+// millimetre wavelengths) is still added to the cell with full relative accuracy; above, the weight is w e^-x and the
+// deposit the difference.
 __device__ __forceinline__ void absorb(float w, float x, float &w_new, float &dep)
 {
     const float e = expf(-x);
-    // x - x^2/2 + x^3/6 - x^4/24 + x^5/120, relative error < 5e-8 for x < 1/8
     const float small = x * fmaf(x, fmaf(x, fmaf(x, fmaf(x, 1.0f / 120.0f, -1.0f / 24.0f), 1.0f / 6.0f), -0.5f), 1.0f);
-    w_new = x < 0.125f ? w - w * small : w * e;
-    dep = w - w_new;
+    const bool lo = x < 0.125f;
+    const float d_lo = w * small, w_hi = w * e;
+    w_new = lo ? w - d_lo : w_hi;
+    dep = lo ? d_lo : w - w_hi;
+}
+
+// a9: weight with which a package leaves the grid, relative to its initial energy.  The sum of the deposits
+// (`absrel`) resolves a small absorbed fraction, the running weight a small remainder: take the one that is accurate
+// (they differ by accumulated fp32 rounding only)
+__device__ __forceinline__ double escaped_rel(float w, float absrel)
+{
+    if (w == 0.0f) return 0.0;                   // terminated: the residual was deposited
+    return absrel < 0.5f ? 1.0 - (double)absrel : (double)w;
 }
 
 template <bool HIER, bool REPLAY, bool ACC32>
@@ -747,13 +759,14 @@ __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_consta
             // ---------------------------------------------------------------- service, all parked lanes together
             if (need == DONE) {                  // retire the finished package
                 const double e0 = package_e0(P, p.src);
-                acc_esc += (double)p.w * e0;
+                const double esc = escaped_rel(p.w, p.absrel) * e0;
+                acc_esc += esc;
                 acc_abs += (double)p.absrel * e0;
                 acc_steps += p.steps;
                 acc_scat += p.scat;
                 if (REPLAY) {
                     soc_replay_record r;
-                    r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = (double)p.w * e0;
+                    r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = esc;
                     P.replay[p.id - P.pkg_begin] = r;
                 }
                 need = EMPTY;
@@ -947,34 +960,30 @@ __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_consta
 }
 
 // ------------------------------------------------------------------------------------------------
-// production kernel, regular grids: photon_fast_kernel with the gather taken off the critical path
+// production kernel, regular grids: photon_fast_kernel with the lane holding HALF A BRICK in registers
 //
-// ncu on config 5 (profiles/README.md, round 1): 61 % of the stall samples of photon_fast_kernel sit on the first
-// use of the gathered cell word -- every iteration of the step loop waits for a dependent load that was issued at
-// its very end.  The straight-line path of a package through the cells does not depend on the densities, only
-// the decision "scatter here or cross" does.  So the lane runs the geometry ONE CELL AHEAD of the physics:
-//   state    cell k (rel, cw), its exit distance ts and crossing ax, the neighbour k+1 across that face
-//            (rel1, cw1: load issued one iteration ago)
-//   step     geometry of cell k+1 -> ts1, ax1, rel2; issue the load of cw2 = cellw[rel2]; THEN the physics of
-//            cell k with cw and ts; on a crossing shift (k+1 -> k, k+2 -> k+1)
-// Every gather has a whole iteration (of all the SM's warps) to arrive.  A scattering or a new package rebuilds
-// the state in the service block (the speculative loads of the abandoned direction are wasted: one per
-// scattering).  The ghost padding of the internal layout is two cells deep on every side so that the neighbour
-// of a ghost cell is still inside the array.
-// Register diet (64 -> the run-ahead state must fit under the 4-CTAs-per-SM cap): per-launch totals live in shared
-// memory (touched only when a package starts or ends), the cell-step count is one 32-bit lane counter, the package
-// id is a 32-bit offset, source index and hot-cube position share a word.
+// ncu on config 5 (profiles/README.md, round 1): the lane-per-package walk is bound by the number of L1->L2
+// requests (tag look-ups 73 % of peak, L1->XBAR request path 67 %), 0.83 gathers + 0.97 scatter-adds per cell-step,
+// every one of them to a different sector; without the scatter-adds the same walk runs 1.7 x faster.  The four cells
+// of a brick that share bz (slot & 3 = bx + 2 by) are 16 contiguous, aligned bytes.  The lane keeps the four cell
+// words of the half it is in (one 16-byte gather when it enters the half) and four deposit sums (one 16-byte
+// red.global.add.v4.f32 when it leaves): a crossing along x or y that stays in the brick -- one step in three --
+// costs no memory request at all, and the requests per cell-step drop from 1.8 to about 1.3.
+// Also here: the per-launch totals live in shared memory (touched only when a package starts or ends), the
+// cell-step count is one 32-bit lane counter, the package id a 32-bit offset, source index and hot-cube position
+// share a word -- the eight extra registers fit under the 4-CTAs-per-SM cap.
 // ------------------------------------------------------------------------------------------------
-struct VPkg {
-    float fx, fy, fz;       // entry position in the current cell k, [0,1]
+struct QPkg {
+    float fx, fy, fz;       // position inside the cell, [0,1]
     float dx, dy, dz;       // direction
     float rx, ry, rz;       // 1/d
     float tau_rem;
-    float w, pend, absrel;  // weight / E0; deposits of this cell visit; deposits of this package
-    float ts;               // distance from (fx,fy,fz) to the exit face of cell k, in cell edges
-    int ax;                 // that crossing: bits 0-2 = axis bit of the slot (1, 2, 4), bit 3 = towards +
-    int rel, rel1;          // internal ids of cell k and of its neighbour across that face
-    uint32_t cw, cw1;       // their cell words
+    float w, absrel;        // weight / E0; deposits of this package
+    float pend;             // deposits of the current cell visit
+    float prel;             // package energy in units of the launch's reference energy (ACC32)
+    int rel;                // internal cell id
+    uint32_t q0, q1, q2, q3;    // cell words of the half brick rel & ~3
+    float a0, a1, a2, a3;       // deposits into those cells in units of the reference energy, not yet in the accumulator
     uint32_t scat;          // scatterings so far = index of the current flight segment
     uint32_t idx;           // package id - pkg_begin
     int sd;                 // < 0: background or beam; else source index << 16 | valid << 9 | hot-cube cell (3 bits per axis)
@@ -982,210 +991,35 @@ struct VPkg {
     unsigned long long hash;
 };
 
-// exit distance, crossing and neighbour id of the cell `rel` entered at (fx, fy, fz)
-__device__ __forceinline__ void v_geometry(const FastParams &P, const VPkg &p, float fx, float fy, float fz, int rel,
-                                           float &ts, int &ax, int &rel_next)
-{
-    const float tx = exit_time(fx, p.rx);
-    const float ty = exit_time(fy, p.ry);
-    const float tz = exit_time(fz, p.rz);
-    ts = fminf(fminf(tx, ty), tz);
-    const bool ax0 = tx == ts, ax1 = !ax0 && ty == ts;          // lowest axis wins a tie (reading S4)
-    const float da = ax0 ? p.dx : (ax1 ? p.dy : p.dz);
-    const bool fwd = da > 0.0f;
-    const int abit = ax0 ? 1 : (ax1 ? 2 : 4);
-    const int bstride = ax0 ? 8 : (ax1 ? P.bsy : P.bsz);         // to the same slot of the next brick
-    const bool inside = fwd == ((rel & abit) == 0);              // the neighbour is in the same brick
-    int r = rel ^ abit;
-    if (!inside) r += fwd ? bstride : -bstride;
-    rel_next = r;
-    ax = abit | (fwd ? 8 : 0);
-}
-
 __device__ __forceinline__ int v_src(int sd) { return sd < 0 ? -1 : (sd >> 16); }
 
-// ------------------------------------------------------------------------------------------------
-// tiled production path, regular grids
-//
-// ncu on config 5 (profiles/README.md): the lane-per-package kernels are bound by the L2 REQUEST rate -- every
-// gather and every scatter-add of a warp goes to a different sector (1.8 requests per cell-step, tag look-ups at
-// 73 % of peak) -- and taking the gather off the critical path (photon_v2_kernel) does not change that.  Here the
-// gathers and scatter-adds go to SHARED memory instead:
-//   * the root grid is cut into tiles of 16^3 cells; a CTA stages the cell words of ONE tile (16 KB) and a zeroed
-//     fp32 accumulator tile (16 KB) in shared memory, walks a chunk of the packages that are currently inside that
-//     tile until each of them leaves the tile, ends, or escapes, and then folds the accumulator tile into the global
-//     accumulator (coalesced, only the touched cells)
-//   * a package that leaves its tile is written back to its 48-byte state record and its index is appended to the
-//     queue of the tile it enters; queues are per-tile segments of one index array, sized before every round from an
-//     upper bound that needs no second pass: a tile can only receive packages from its six face neighbours, so
-//     capacity(t) = sum of the neighbours' current queue lengths (tile_plan_kernel, one block)
-//   * rounds: plan -> walk -> swap queues.  After a fixed number of rounds the few packages still alive (long
-//     random walks in dense regions) are finished by the lane-per-package kernel in RESUME mode, which reads the
-//     same state records.  Nothing is synchronised with the host.
-// The arithmetic of a step is that of photon_fast_kernel, and the saved state is lossless, so cell-step and
-// scattering counts are identical to the other production kernels; only the order of the additions differs.
-// ------------------------------------------------------------------------------------------------
-constexpr int kTL = 16;                            // tile edge in cells
-constexpr int kTCells = kTL * kTL * kTL;
-constexpr int kTileThreads = 128;
-constexpr int kTileChunk = 1024;                   // packages per work item
-enum : int { XTILE = 6 };                          // lane state: left the tile, state to be written back
-
-struct __align__(16) TileState {                   // 48 bytes per package, indexed by package offset
-    float fx, fy, fz, dx;
-    float dy, dz, tau_rem, w;
-    float absrel;
-    uint32_t cell;                                 // root cell ix | iy << 10 | iz << 20
-    uint32_t scat_src;                             // scatterings (24 bits) | (source index + 1) << 24
-    uint32_t pad;
-};
-
-struct TileItem { int tile, first, count, pad; };  // work item: `count` queue entries of `tile` starting at list[first]
-
-struct TileBuffers {                               // device pointers, all owned by the grid
-    TileState *state;                              // [n_pkg]
-    uint32_t *list[2];                             // queue index arrays (6 n_pkg entries each)
-    int *seg[2];                                   // [n_tiles] start of the tile's segment in list[i]
-    int *fill[2];                                  // [n_tiles] entries in the tile's segment
-    uint32_t *rank;                                // [n_pkg] rank of the package inside its first tile
-    uint32_t *tile0;                               // [n_pkg] first tile
-    TileItem *items;                               // [n_pkg / kTileChunk + n_tiles + 1]
-    int *n_items;                                  // scalar
-    unsigned *item_counter;                        // scalar
-    int ntx, nty, ntz, n_tiles;
-};
-
-// a1-a4 for every package of the launch: state record, first tile, rank inside that tile
-__global__ void __launch_bounds__(256) tile_emit_kernel(const __grid_constant__ FastParams P, const __grid_constant__ TileBuffers B)
+__device__ __forceinline__ uint32_t q_word(const QPkg &p)
 {
-    const long long n = P.pkg_end - P.pkg_begin;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    double e_sum = 0.0;
-    for (long long i0 = (long long)blockIdx.x * blockDim.x; i0 < n; i0 += stride) {      // whole warps iterate together
-        const long long i = i0 + threadIdx.x;
-        const bool on = i < n;
-        int tile = -1;
-        if (on) {
-            FPkg q;
-            int ix, iy, iz;
-            float dx, dy, dz;
-            fast_emit_core(P, q, P.pkg_begin + i, ix, iy, iz, dx, dy, dz);
-            uint32_t s0, s1, s2, s3;
-            philox_block(P.seed, P.ifreq, P.pkg_begin + i, 2u, s0, s1, s2, s3);
-            TileState s;
-            s.fx = q.fx; s.fy = q.fy; s.fz = q.fz; s.dx = dx; s.dy = dy; s.dz = dz;
-            s.tau_rem = -__logf(uniform01<float>(s0));                                   // a4
-            s.w = 1.0f; s.absrel = 0.0f;
-            s.cell = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
-            s.scat_src = (uint32_t)(q.src + 1) << 24;
-            s.pad = 0u;
-            B.state[i] = s;
-            tile = (ix / kTL) + B.ntx * ((iy / kTL) + B.nty * (iz / kTL));
-            e_sum += package_e0(P, q.src);
-        }
-        // rank inside the tile: one atomic per distinct tile of the warp (point sources put whole warps in one tile)
-        const unsigned peers = __match_any_sync(kFull, tile);
-        const int leader = __ffs(peers) - 1;
-        int base = 0;
-        if (on && (threadIdx.x & 31) == leader) base = atomicAdd(B.fill[0] + tile, __popc(peers));
-        base = __shfl_sync(kFull, base, leader);
-        if (on) {
-            B.rank[i] = (uint32_t)(base + __popc(peers & ((1u << (threadIdx.x & 31)) - 1u)));
-            B.tile0[i] = (uint32_t)tile;
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) e_sum += __shfl_xor_sync(kFull, e_sum, o);
-    if ((threadIdx.x & 31) == 0 && e_sum != 0.0) atomicAdd(&P.result->emitted, e_sum);
+    const bool lo = (p.rel & 1) != 0, hi = (p.rel & 2) != 0;
+    const uint32_t a = lo ? p.q1 : p.q0, b = lo ? p.q3 : p.q2;
+    return hi ? b : a;
 }
 
-// queue of round 0: list[0][seg[0][tile] + rank] = package
-__global__ void __launch_bounds__(256) tile_scatter_kernel(long long n, const __grid_constant__ TileBuffers B)
+__device__ __forceinline__ void q_load(const FastParams &P, QPkg &p)
 {
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-        B.list[0][B.seg[0][B.tile0[i]] + B.rank[i]] = (uint32_t)i;
+    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(P.cellw + (p.rel & ~3)));
+    p.q0 = v.x; p.q1 = v.y; p.q2 = v.z; p.q3 = v.w;
 }
 
-// block-wide exclusive scan of one value per thread (1024 threads); returns the exclusive prefix, *total = block sum
-__device__ __forceinline__ int block_exscan_1024(int v, int *s_warp, int *total)
+// hand the deposits of the half brick (already in units of the launch's reference energy) to the accumulator:
+// one 16-byte reduction
+__device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p)
 {
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    int x = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int y = __shfl_up_sync(kFull, x, o);
-        if (lane >= o) x += y;
-    }
-    __syncthreads();                               // s_warp may still be read by the previous call
-    if (lane == 31) s_warp[wid] = x;
-    __syncthreads();
-    if (wid == 0) {
-        int w = s_warp[lane];
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int y = __shfl_up_sync(kFull, w, o);
-            if (lane >= o) w += y;
-        }
-        s_warp[lane] = w;                          // inclusive sums of the warps
-    }
-    __syncthreads();
-    const int warp_off = wid > 0 ? s_warp[wid - 1] : 0;
-    *total = s_warp[31];
-    return warp_off + x - v;
+    // nothing to add: empty cells, or the cells around a point source, whose deposits went to the block's shared
+    // partial sums -- a reduction of zeros there would bring back the very contention those sums avoid
+    if ((p.a0 + p.a1) + (p.a2 + p.a3) == 0.0f) return;
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(P.acc32 + (p.rel & ~3)), "f"(p.a0), "f"(p.a1),
+                 "f"(p.a2), "f"(p.a3) : "memory");
+    p.a0 = 0.0f; p.a1 = 0.0f; p.a2 = 0.0f; p.a3 = 0.0f;
 }
 
-// One block.  mode 0: seg[cur] = exclusive scan of fill[cur] (exact sizes: the queue of round 0).
-// mode 1: work items of the coming round from (seg[cur], fill[cur]); seg[nxt] = exclusive scan of the capacities
-// (a tile receives packages from its six face neighbours only); fill[nxt] = 0; item counter = 0.
-__global__ void __launch_bounds__(1024) tile_plan_kernel(const __grid_constant__ TileBuffers B, int cur, int mode)
-{
-    __shared__ int s_warp[32];
-    const int nxt = cur ^ 1;
-    int carry_seg = 0, carry_item = 0;
-    for (int t0 = 0; t0 < B.n_tiles; t0 += 1024) {
-        const int t = t0 + threadIdx.x;
-        const bool on = t < B.n_tiles;
-        const int cnt = on ? B.fill[cur][t] : 0;
-        int total;
-        if (mode == 0) {
-            const int ex = block_exscan_1024(cnt, s_warp, &total);
-            if (on) B.seg[cur][t] = carry_seg + ex;
-            carry_seg += total;
-            continue;
-        }
-        int cap = 0;
-        if (on) {
-            const int tz = t / (B.ntx * B.nty), r = t - tz * (B.ntx * B.nty), ty = r / B.ntx, tx = r - ty * B.ntx;
-            if (tx > 0) cap += B.fill[cur][t - 1];
-            if (tx + 1 < B.ntx) cap += B.fill[cur][t + 1];
-            if (ty > 0) cap += B.fill[cur][t - B.ntx];
-            if (ty + 1 < B.nty) cap += B.fill[cur][t + B.ntx];
-            if (tz > 0) cap += B.fill[cur][t - B.ntx * B.nty];
-            if (tz + 1 < B.ntz) cap += B.fill[cur][t + B.ntx * B.nty];
-        }
-        const int ex_cap = block_exscan_1024(cap, s_warp, &total);
-        if (on) { B.seg[nxt][t] = carry_seg + ex_cap; B.fill[nxt][t] = 0; }
-        carry_seg += total;
-        const int k = (cnt + kTileChunk - 1) / kTileChunk;
-        const int ex_item = block_exscan_1024(k, s_warp, &total);
-        if (on) {
-            const int first = B.seg[cur][t];
-            for (int j = 0; j < k; ++j) {
-                TileItem it;
-                it.tile = t; it.first = first + j * kTileChunk;
-                it.count = cnt - j * kTileChunk < kTileChunk ? cnt - j * kTileChunk : kTileChunk;
-                it.pad = 0;
-                B.items[carry_item + ex_item + j] = it;
-            }
-        }
-        carry_item += total;
-    }
-    if (mode == 1 && threadIdx.x == 0) { *B.n_items = carry_item; *B.item_counter = 0u; }
-}
-
-template <bool REPLAY, bool ACC32, bool RESUME>
-__global__ void __launch_bounds__(256, 4) photon_v2_kernel(const __grid_constant__ FastParams P, const __grid_constant__ TileBuffers B, int cur)
+template <bool REPLAY>
+__global__ void __launch_bounds__(256, 4) photon_q_kernel(const __grid_constant__ FastParams P)
 {
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -1200,31 +1034,34 @@ __global__ void __launch_bounds__(256, 4) photon_v2_kernel(const __grid_constant
     for (int i = threadIdx.x; i < hot_cells * P.n_point; i += blockDim.x) s_hot[i] = 0.0f;
     __syncthreads();
 
-    VPkg p;
-    p.sd = -1; p.w = 0.0f; p.absrel = 0.0f; p.pend = 0.0f; p.scat = 0; p.cw = 0; p.cw1 = 0; p.rel = 0; p.rel1 = 0;
-    p.ts = 0.0f; p.ax = 1; p.idx = 0; p.steps = 0; p.hash = 0;
+    QPkg p;
+    p.sd = -1; p.w = 0.0f; p.absrel = 0.0f; p.scat = 0; p.rel = 0; p.idx = 0; p.steps = 0; p.hash = 0;
+    p.q0 = p.q1 = p.q2 = p.q3 = 0u; p.a0 = p.a1 = p.a2 = p.a3 = 0.0f; p.pend = 0.0f; p.prel = 0.0f;
     p.fx = p.fy = p.fz = 0.5f; p.dx = p.dy = 0.0f; p.dz = 1.0f; p.rx = p.ry = p.rz = 1.0f; p.tau_rem = 0.0f;
     int need = EMPTY;
     unsigned n_steps = 0;                        // cell-steps of this lane (all its packages)
     unsigned pool_next = 0, pool_end = 0;        // warp-uniform pool of package offsets
     bool exhausted = false;
+    int n_dead = 0;                              // warp-uniform: lanes that will get no more packages
     const unsigned n_pkg = (unsigned)(P.pkg_end - P.pkg_begin);      // the launcher keeps this below 2^32
     const int T = P.service_threshold;
 
     for (;;) {
-        const unsigned m_park = __ballot_sync(kFull, (unsigned)(need - SCAT) <= (unsigned)(EMPTY - SCAT));
         const unsigned m_run = __ballot_sync(kFull, need == RUN);
-        if (m_park && (__popc(m_park) >= T || m_run == 0u)) {
+        const int n_park = 32 - __popc(m_run) - n_dead;
+        if (n_park > 0 && (n_park >= T || m_run == 0u)) {
             // ---------------------------------------------------------------- service, all parked lanes together
             if (need == DONE) {                  // retire the finished package
+                q_flush(P, p);
                 const int src = v_src(p.sd);
                 const double e0 = package_e0(P, src);
-                s_tot[1][threadIdx.x] += (double)p.w * e0;
+                const double esc = escaped_rel(p.w, p.absrel) * e0;
+                s_tot[1][threadIdx.x] += esc;
                 s_tot[2][threadIdx.x] += (double)p.absrel * e0;
                 s_cnt[0][threadIdx.x] += p.scat;
                 if (REPLAY) {
                     soc_replay_record r;
-                    r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = (double)p.w * e0;
+                    r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = esc;
                     P.replay[p.idx] = r;
                 }
                 need = EMPTY;
@@ -1233,59 +1070,37 @@ __global__ void __launch_bounds__(256, 4) photon_v2_kernel(const __grid_constant
             if (want && !exhausted) {
                 do {
                     if (pool_next >= pool_end) {
-                        if (RESUME) {            // the pool is a work item: a run of queue entries of one tile
-                            unsigned it = 0;
-                            if (lane == 0) it = atomicAdd(B.item_counter, 1u);
-                            it = __shfl_sync(kFull, it, 0);
-                            if (it >= (unsigned)*B.n_items) { exhausted = true; break; }
-                            const TileItem item = B.items[it];
-                            pool_next = (unsigned)item.first;
-                            pool_end = (unsigned)(item.first + item.count);
-                        } else {
-                            unsigned long long base = 0;
-                            if (lane == 0) base = atomicAdd(P.counter, (unsigned long long)kChunk);
-                            base = __shfl_sync(kFull, base, 0);
-                            if (base >= (unsigned long long)n_pkg) { exhausted = true; break; }
-                            pool_next = (unsigned)base;
-                            pool_end = n_pkg - pool_next > (unsigned)kChunk ? pool_next + kChunk : n_pkg;
-                        }
+                        unsigned long long base = 0;
+                        if (lane == 0) base = atomicAdd(P.counter, (unsigned long long)kChunk);
+                        base = __shfl_sync(kFull, base, 0);
+                        if (base >= (unsigned long long)n_pkg) { exhausted = true; break; }
+                        pool_next = (unsigned)base;
+                        pool_end = n_pkg - pool_next > (unsigned)kChunk ? pool_next + kChunk : n_pkg;
                     }
                     const unsigned avail = pool_end - pool_next;
                     const unsigned rank = __popc(want & lt_mask);
-                    if (need == EMPTY && rank < avail) {
-                        p.idx = RESUME ? B.list[cur][pool_next + rank] : pool_next + rank;
-                        need = NEWID;
-                    }
+                    if (need == EMPTY && rank < avail) { p.idx = pool_next + rank; need = NEWID; }
                     const unsigned n_want = __popc(want);
                     pool_next += n_want < avail ? n_want : avail;
                     want = __ballot_sync(kFull, need == EMPTY);
                 } while (want);
             }
             if (need == EMPTY && exhausted) need = DEAD;
+            n_dead = __popc(__ballot_sync(kFull, need == DEAD));
             float ndx = 0.0f, ndy = 0.0f, ndz = 1.0f;
-            bool redraw = true;
-            if (RESUME && need == NEWID) {       // continue a package of the tiled walk from its state record
-                const TileState s = B.state[p.idx];
-                p.fx = s.fx; p.fy = s.fy; p.fz = s.fz; ndx = s.dx; ndy = s.dy; ndz = s.dz;
-                p.tau_rem = s.tau_rem; p.w = s.w; p.absrel = s.absrel; p.pend = 0.0f;
-                p.scat = s.scat_src & 0xffffffu;
-                const int src = (int)(s.scat_src >> 24) - 1;
-                p.sd = src < 0 ? -1 : (src << 16);
-                p.rel = root_id(P, (int)(s.cell & 1023u), (int)((s.cell >> 10) & 1023u), (int)(s.cell >> 20));
-                p.cw = __ldg(P.cellw + p.rel);
-                p.steps = 0; p.hash = 0;
-                redraw = false;
-            } else if (need == NEWID) {
+            if (need == NEWID) {
                 FPkg q;
                 fast_emit<false>(P, q, P.pkg_begin + (long long)p.idx, ndx, ndy, ndz);
-                p.fx = q.fx; p.fy = q.fy; p.fz = q.fz; p.rel = q.rel; p.cw = q.cw;
+                p.fx = q.fx; p.fy = q.fy; p.fz = q.fz; p.rel = q.rel;
+                q_load(P, p);
                 p.sd = q.src < 0 ? -1 : ((q.src << 16) | (P.hot_r >= 0 ? (0x200 | (P.hot_r * 0x49)) : 0));
-                p.w = 1.0f; p.pend = 0.0f; p.absrel = 0.0f; p.scat = 0;
+                p.w = 1.0f; p.absrel = 0.0f; p.scat = 0; p.pend = 0.0f;
+                p.prel = package_rel(P, q.src);
                 p.steps = 0; p.hash = 0xcbf29ce484222325ull;
                 s_tot[0][threadIdx.x] += package_e0(P, q.src);
             } else if (need == SCAT) {
                 // finish the flight segment: advance to the scattering point (a4), then a8
-                const float rho = __uint_as_float(p.cw);
+                const float rho = __uint_as_float(q_word(p));
                 const float t_u = p.tau_rem / (rho * P.ksca);
                 p.fx = __saturatef(fmaf(t_u, p.dx, p.fx));
                 p.fy = __saturatef(fmaf(t_u, p.dy, p.fy));
@@ -1317,80 +1132,95 @@ __global__ void __launch_bounds__(256, 4) photon_v2_kernel(const __grid_constant
             if (need == NEWID || need == SCAT) {
                 p.dx = ndx; p.dy = ndy; p.dz = ndz;
                 p.rx = 1.0f / ndx; p.ry = 1.0f / ndy; p.rz = 1.0f / ndz;
-                // run-ahead state of the new flight segment: exit of the current cell, gather of its neighbour
-                v_geometry(P, p, p.fx, p.fy, p.fz, p.rel, p.ts, p.ax, p.rel1);
-                p.cw1 = __ldg(P.cellw + p.rel1);
-                if (redraw) {
-                    uint32_t s0, s1, s2, s3;
-                    philox_block(P.seed, P.ifreq, P.pkg_begin + (long long)p.idx, 2u + p.scat, s0, s1, s2, s3);
-                    p.tau_rem = -__logf(uniform01<float>(s0));                // a4
-                }
-                need = p.cw == kSentinel ? DONE : RUN;
+                uint32_t s0, s1, s2, s3;
+                philox_block(P.seed, P.ifreq, P.pkg_begin + (long long)p.idx, 2u + p.scat, s0, s1, s2, s3);
+                p.tau_rem = -__logf(uniform01<float>(s0));                    // a4
+                need = RUN;
             }
             continue;
         }
         if (m_run == 0u) break;                  // nothing parked that can be serviced, nothing running
 
         if (need == RUN) {
-            // ---------------------------------------------------------------- geometry of cell k+1, gather of cell k+2
-            const int abit = p.ax & 7;
-            const bool fwd = (p.ax & 8) != 0;
-            float gx = __saturatef(fmaf(p.ts, p.dx, p.fx));
-            float gy = __saturatef(fmaf(p.ts, p.dy, p.fy));
-            float gz = __saturatef(fmaf(p.ts, p.dz, p.fz));
-            const float face = fwd ? 0.0f : 1.0f;        // entry face in the neighbour's frame
-            if (abit == 1) gx = face; else if (abit == 2) gy = face; else gz = face;
-            float ts1;
-            int ax1, rel2;
-            v_geometry(P, p, gx, gy, gz, p.rel1, ts1, ax1, rel2);
-            const uint32_t cw2 = __ldg(P.cellw + rel2);
-            // ---------------------------------------------------------------- physics of cell k (a7, a9)
-            const float rho = __uint_as_float(p.cw);
-            const float ksr = rho * P.ksca;
-            const float dtau = p.ts * ksr;
-            const bool sc = dtau >= p.tau_rem && ksr > 0.0f;
-            const float x = sc ? p.tau_rem * P.kratio : p.ts * (rho * P.kabs);
-            float w_new, dep;
-            absorb(p.w, x, w_new, dep);
-            const bool term = w_new < (float)kWMin;                  // a9: residual stays in the cell
-            if (term) { dep = p.w; w_new = 0.0f; }
-            p.pend += dep;
-            p.absrel += dep;
-            p.w = w_new;
-            n_steps += 1;
-            if (REPLAY) {                        // the record hashes cell ids of the ABI's cell vector
-                p.steps += 1;
-                p.hash = (p.hash ^ (unsigned long long)global_id(P, p.rel)) * 0x100000001b3ull;
-            }
-            if (term || !sc) {
-                // the package leaves the cell (or ends in it): hand the cell visit's energy to the accumulator
-                if (p.sd >= 0 && (p.sd & 0x200)) {
-                    const int j = (p.sd & 7) + hot_side * (((p.sd >> 3) & 7) + hot_side * ((p.sd >> 6) & 7));
-                    atomicAdd(s_hot + (p.sd >> 16) * hot_cells + j, p.pend);
-                } else if (p.pend > 0.0f && !(P.debug & 1)) {
-                    if (ACC32) atomicAdd(P.acc32 + p.rel, p.pend * package_rel(P, v_src(p.sd)));
-                    else atomicAdd(P.acc + p.rel, (double)p.pend * package_e0(P, v_src(p.sd)));
-                }
-                p.pend = 0.0f;
-            }
-            if (term) {
-                s_cnt[1][threadIdx.x] += 1u;
-                need = DONE;
-            } else if (sc) {
-                need = SCAT;                     // the segment is finished in the service block
+            // ---------------------------------------------------------------- one cell-step (a5-a7, a9)
+            const uint32_t cw = q_word(p);
+            if (cw == kSentinel) {
+                need = DONE;                     // a9: the cell entered by the last crossing is outside the grid
             } else {
-                p.tau_rem -= dtau;
-                if (p.sd >= 0 && (p.sd & 0x200)) {       // follow the package through the cached cube
-                    const int sh = abit == 1 ? 0 : (abit == 2 ? 3 : 6);
-                    const int c = ((p.sd >> sh) & 7) + (fwd ? 1 : -1);
-                    if ((unsigned)c < (unsigned)hot_side) p.sd = (p.sd & ~(7 << sh)) | (c << sh);
-                    else p.sd &= ~0x200;
+                const float rho = __uint_as_float(cw);
+                const float tx = exit_time(p.fx, p.rx);
+                const float ty = exit_time(p.fy, p.ry);
+                const float tz = exit_time(p.fz, p.rz);
+                const float ts = fminf(fminf(tx, ty), tz);
+                const bool ax0 = tx == ts, ax1 = !ax0 && ty == ts;       // lowest axis wins a tie (reading S4)
+                const float da = ax0 ? p.dx : (ax1 ? p.dy : p.dz);
+                const bool fwd = da > 0.0f;
+                const int bstride = ax0 ? 8 : (ax1 ? P.bsy : P.bsz);      // to the same slot of the next brick
+                const int abit = ax0 ? 1 : (ax1 ? 2 : 4);
+                const float ksr = rho * P.ksca;
+                const float dtau = ts * ksr;
+                const bool sc = dtau >= p.tau_rem && ksr > 0.0f;
+                const float x = sc ? p.tau_rem * P.kratio : ts * (rho * P.kabs);
+                float w_new, dep;
+                absorb(p.w, x, w_new, dep);
+                const bool term = w_new < (float)kWMin;                  // a9: residual stays in the cell
+                if (term) { dep = p.w; w_new = 0.0f; }
+                p.pend += dep;
+                p.absrel += dep;
+                p.w = w_new;
+                n_steps += 1;
+                if (REPLAY) {                    // the record hashes cell ids of the ABI's cell vector
+                    p.steps += 1;
+                    p.hash = (p.hash ^ (unsigned long long)global_id(P, p.rel)) * 0x100000001b3ull;
                 }
-                p.fx = gx; p.fy = gy; p.fz = gz;
-                p.ts = ts1; p.ax = ax1;
-                p.rel = p.rel1; p.rel1 = rel2;
-                p.cw = p.cw1; p.cw1 = cw2;
-                if (p.cw == kSentinel) need = DONE;                  // a9: escaped
+                const bool hot = p.sd >= 0 && (p.sd & 0x200);
+                if (term || !sc) {
+                    // the package leaves the cell (or ends in it): the cell visit's energy goes to the half-brick sums --
+                    // inside the cached cube around the package's source to the block's shared partial sums
+                    //
+                    if (hot) {
+                        const int j = (p.sd & 7) + hot_side * (((p.sd >> 3) & 7) + hot_side * ((p.sd >> 6) & 7));
+                        atomicAdd(s_hot + (p.sd >> 16) * hot_cells + j, p.pend);
+                    } else {
+                        const bool lo = (p.rel & 1) != 0, hi = (p.rel & 2) != 0;
+                        const float v = p.pend * p.prel;
+                        p.a0 += (!hi && !lo) ? v : 0.0f;
+                        p.a1 += (!hi && lo) ? v : 0.0f;
+                        p.a2 += (hi && !lo) ? v : 0.0f;
+                        p.a3 += (hi && lo) ? v : 0.0f;
+                    }
+                    p.pend = 0.0f;
+                }
+                if (term) {
+                    s_cnt[1][threadIdx.x] += 1u;
+                    need = DONE;                 // the service block flushes the half-brick sums
+                } else if (sc) {
+                    need = SCAT;                 // the segment is finished in the service block
+                } else {
+                    p.tau_rem -= dtau;
+                    if (hot) {                   // follow the package through the cached cube
+                        const int sh = ax0 ? 0 : (ax1 ? 3 : 6);
+                        const int c = ((p.sd >> sh) & 7) + (fwd ? 1 : -1);
+                        if ((unsigned)c < (unsigned)hot_side) p.sd = (p.sd & ~(7 << sh)) | (c << sh);
+                        else p.sd &= ~0x200;
+                    }
+                    p.fx = __saturatef(fmaf(ts, p.dx, p.fx));
+                    p.fy = __saturatef(fmaf(ts, p.dy, p.fy));
+                    p.fz = __saturatef(fmaf(ts, p.dz, p.fz));
+                    const float face = fwd ? 0.0f : 1.0f;    // entry face in the neighbour's frame
+                    if (ax0) p.fx = face; else if (ax1) p.fy = face; else p.fz = face;
+                    // neighbour inside the brick: flip the slot bit; otherwise the same bit flips and the brick changes
+                    const bool inside = fwd == ((p.rel & abit) == 0);
+                    if (!inside || abit == 4) {
+                        q_flush(P, p);    // leaving the half brick: its sums go out, the new half comes in
+                        int rel = p.rel ^ abit;
+                        if (!inside) rel += fwd ? bstride : -bstride;
+                        p.rel = rel;
+                        q_load(P, p);
+                    } else {
+                        p.rel ^= abit;
+                    }
+                }
             }
         }
     }
@@ -1405,8 +1235,7 @@ __global__ void __launch_bounds__(256, 4) photon_v2_kernel(const __grid_constant
                 const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
                 const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
                           iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
-                if (ACC32) atomicAdd(P.acc32 + root_id(P, ix, iy, iz), v * P.ps_rel[k]);
-                else atomicAdd(P.acc + root_id(P, ix, iy, iz), (double)v * P.ps_e0[k]);
+                atomicAdd(P.acc32 + root_id(P, ix, iy, iz), v * P.ps_rel[k]);
             }
         }
     }
@@ -1424,260 +1253,8 @@ __global__ void __launch_bounds__(256, 4) photon_v2_kernel(const __grid_constant
         acc_scat += __shfl_xor_sync(kFull, acc_scat, o);
         acc_term += __shfl_xor_sync(kFull, acc_term, o);
     }
-    if (lane == 0 && acc_steps != 0) {
+    if (lane == 0 && (acc_steps != 0 || acc_emit != 0.0)) {
         atomicAdd(&P.result->emitted, acc_emit);
-        atomicAdd(&P.result->escaped, acc_esc);
-        atomicAdd(&P.result->absorbed, acc_abs);
-        atomicAdd(&P.result->cell_steps, acc_steps);
-        atomicAdd(&P.result->scatterings, (unsigned long long)acc_scat);
-        atomicAdd(&P.result->terminated, (unsigned long long)acc_term);
-    }
-}
-
-struct TPkg {
-    float fx, fy, fz, dx, dy, dz, rx, ry, rz;
-    float tau_rem, w, pend, absrel;
-    int c;                  // cell inside the tile: x | y << 4 | z << 8; bits 12-14: exit code while need == XTILE
-    uint32_t cw;
-    uint32_t scat_src;      // scatterings (24 bits) | (source index + 1) << 24
-    uint32_t idx;           // package offset (index of its state record)
-};
-
-__device__ __forceinline__ int t_src(uint32_t scat_src) { return (int)(scat_src >> 24) - 1; }
-
-__global__ void __launch_bounds__(kTileThreads, 6)
-tile_walk_kernel(const __grid_constant__ FastParams P, const __grid_constant__ TileBuffers B, int cur)
-{
-    __shared__ uint32_t s_cw[kTCells];
-    __shared__ float s_acc[kTCells];
-    __shared__ double s_tot[2][kTileThreads];      // escaped, absorbed
-    __shared__ unsigned s_cnt[2][kTileThreads];    // scatterings, terminated
-    __shared__ int s_it;
-    __shared__ unsigned s_next;
-    __shared__ uint32_t s_list[kTileChunk];        // package indices of the work item
-    const int tid = threadIdx.x, lane = tid & 31;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    const int nxt = cur ^ 1;
-    s_tot[0][tid] = 0.0; s_tot[1][tid] = 0.0; s_cnt[0][tid] = 0u; s_cnt[1][tid] = 0u;
-    unsigned n_steps = 0;
-    const int n_items = *B.n_items;
-    const int T = P.service_threshold;
-
-    for (;;) {
-        __syncthreads();                           // the previous item is flushed; s_it may be rewritten
-        if (tid == 0) {
-            const unsigned it = atomicAdd(B.item_counter, 1u);
-            s_it = it < (unsigned)n_items ? (int)it : -1;
-            s_next = (unsigned)kTileThreads;       // every thread starts with entry `tid` of the item
-        }
-        __syncthreads();
-        if (s_it < 0) break;
-        const TileItem item = B.items[s_it];
-        const int tz = item.tile / (B.ntx * B.nty), tr = item.tile - tz * (B.ntx * B.nty), ty = tr / B.ntx, tx = tr - ty * B.ntx;
-        // stage the tile: j runs in the order of the brick layout (slot, brick x, brick y, brick z), so that global
-        // reads (and the flush below) touch runs of 256 bytes
-        for (int j = tid; j < kTCells; j += kTileThreads) {
-            const int slot = j & 7, x = 2 * ((j >> 3) & 7) + (slot & 1), y = 2 * ((j >> 6) & 7) + ((slot >> 1) & 1),
-                      z = 2 * (j >> 9) + (slot >> 2);
-            const int gx = tx * kTL + x, gy = ty * kTL + y, gz = tz * kTL + z;
-            uint32_t cwj = kSentinel;
-            if (gx < P.nx && gy < P.ny && gz < P.nz) cwj = __ldg(P.cellw + root_id(P, gx, gy, gz));
-            s_cw[x | (y << 4) | (z << 8)] = cwj;
-            s_acc[x | (y << 4) | (z << 8)] = 0.0f;
-        }
-        for (int j = tid; j < item.count; j += kTileThreads) s_list[j] = B.list[cur][item.first + j];
-        __syncthreads();
-
-        TPkg p;
-        p.w = 0.0f; p.pend = 0.0f; p.absrel = 0.0f; p.c = 0; p.cw = 0; p.scat_src = 0; p.idx = 0;
-        p.fx = p.fy = p.fz = 0.5f; p.dx = p.dy = 0.0f; p.dz = 1.0f; p.rx = p.ry = p.rz = 1.0f; p.tau_rem = 0.0f;
-        int need = EMPTY;
-        // the state record of the lane's NEXT package is fetched while the current one walks; the queue append of
-        // a package that left the tile is completed one service pass later (its slot comes back from an atomic):
-        // no service pass waits for a global round trip
-        TileState nx;
-        uint32_t nx_idx = 0u;
-        bool nx_valid = tid < item.count;
-        if (nx_valid) { nx_idx = s_list[tid]; nx = B.state[nx_idx]; }
-        int pend_pos = 0, pend_base = 0;
-        uint32_t pend_idx = 0u;
-        bool pend_valid = false;
-        for (;;) {
-            const unsigned m_park = __ballot_sync(kFull, need != RUN && need != DEAD);
-            const unsigned m_run = __ballot_sync(kFull, need == RUN);
-            if (m_park && (__popc(m_park) >= T || m_run == 0u)) {
-                // ------------------------------------------------------------ service, all parked lanes together
-                if (pend_valid) { B.list[nxt][pend_base + pend_pos] = pend_idx; pend_valid = false; }
-                if (need == XTILE) {
-                    // a5: the package crossed a face of the tile.  Outside the grid it has escaped (a9); otherwise
-                    // write the state back and queue the package for the tile it enters
-                    const int code = (p.c >> 12) & 7, axis = (code - 1) >> 1, sg = ((code - 1) & 1) ? 1 : -1;
-                    const int ntx = tx + (axis == 0 ? sg : 0), nty = ty + (axis == 1 ? sg : 0), ntz = tz + (axis == 2 ? sg : 0);
-                    const int gx = ntx * kTL + (p.c & 15), gy = nty * kTL + ((p.c >> 4) & 15), gz = ntz * kTL + ((p.c >> 8) & 15);
-                    if ((unsigned)gx >= (unsigned)P.nx || (unsigned)gy >= (unsigned)P.ny || (unsigned)gz >= (unsigned)P.nz) {
-                        need = DONE;               // a9: escaped
-                    } else {
-                        TileState s;
-                        s.fx = p.fx; s.fy = p.fy; s.fz = p.fz; s.dx = p.dx; s.dy = p.dy; s.dz = p.dz;
-                        s.tau_rem = p.tau_rem; s.w = p.w; s.absrel = p.absrel;
-                        s.cell = (uint32_t)gx | ((uint32_t)gy << 10) | ((uint32_t)gz << 20);
-                        s.scat_src = p.scat_src; s.pad = 0u;
-                        B.state[p.idx] = s;
-                        const int nt = ntx + B.ntx * (nty + B.nty * ntz);
-                        pend_pos = atomicAdd(B.fill[nxt] + nt, 1);
-                        pend_base = B.seg[nxt][nt];
-                        pend_idx = p.idx;
-                        pend_valid = true;
-                        need = EMPTY;
-                    }
-                }
-                if (need == DONE) {                // retire the finished package
-                    const double e0 = package_e0(P, t_src(p.scat_src));
-                    s_tot[0][tid] += (double)p.w * e0;
-                    s_tot[1][tid] += (double)p.absrel * e0;
-                    s_cnt[0][tid] += p.scat_src & 0xffffffu;
-                    need = EMPTY;
-                }
-                float ndx = 0.0f, ndy = 0.0f, ndz = 1.0f;
-                bool redraw = false;
-                if (need == EMPTY && !nx_valid) need = DEAD;
-                if (need == EMPTY) {
-                    // continue with the prefetched package; claim the lane's next entry and fetch its record
-                    p.idx = nx_idx;
-                    p.fx = nx.fx; p.fy = nx.fy; p.fz = nx.fz; ndx = nx.dx; ndy = nx.dy; ndz = nx.dz;
-                    p.tau_rem = nx.tau_rem; p.w = nx.w; p.absrel = nx.absrel; p.pend = 0.0f;
-                    p.scat_src = nx.scat_src;
-                    p.c = (int)((nx.cell & 15u) | (((nx.cell >> 10) & 15u) << 4) | (((nx.cell >> 20) & 15u) << 8));
-                    p.cw = s_cw[p.c];
-                    need = NEWID;
-                    const unsigned k = atomicAdd(&s_next, 1u);
-                    nx_valid = k < (unsigned)item.count;
-                    if (nx_valid) { nx_idx = s_list[k]; nx = B.state[nx_idx]; }
-                } else if (need == SCAT) {
-                    // finish the flight segment: advance to the scattering point (a4), then a8
-                    const float rho = __uint_as_float(p.cw);
-                    const float t_u = p.tau_rem / (rho * P.ksca);
-                    p.fx = __saturatef(fmaf(t_u, p.dx, p.fx));
-                    p.fy = __saturatef(fmaf(t_u, p.dy, p.fy));
-                    p.fz = __saturatef(fmaf(t_u, p.dz, p.fz));
-                    const float g = P.g;
-                    const long long id = P.pkg_begin + (long long)p.idx;
-                    uint32_t s0, w_hg, w_az, s3;     // words 1, 2 of the block of the segment that ends here
-                    philox_block(P.seed, P.ifreq, id, 2u + (p.scat_src & 0xffffffu), s0, w_hg, w_az, s3);
-                    const float mu0 = 2.0f * uniform01<float>(w_hg) - 1.0f;
-                    const float num = mu0 + g * (3.0f + mu0 * mu0) * 0.5f + g * g * mu0 + g * g * g * (mu0 * mu0 - 1.0f) * 0.5f;
-                    const float den = (1.0f + g * mu0) * (1.0f + g * mu0);
-                    float ct = num / den;
-                    ct = fminf(1.0f, fmaxf(-1.0f, ct));
-                    const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
-                    float sp, cp;
-                    sincospif(2.0f * uniform01<float>(w_az), &sp, &cp);
-                    const float sg = copysignf(1.0f, p.dz);
-                    const float a = -1.0f / (sg + p.dz);
-                    const float b = p.dx * p.dy * a;
-                    const float t1x = 1.0f + sg * p.dx * p.dx * a, t1y = sg * b, t1z = -sg * p.dx;
-                    const float t2x = b, t2y = sg + p.dy * p.dy * a, t2z = -p.dy;
-                    const float c1 = st * cp, c2 = st * sp;
-                    const float qx = c1 * t1x + c2 * t2x + ct * p.dx;
-                    const float qy = c1 * t1y + c2 * t2y + ct * p.dy;
-                    const float qz = c1 * t1z + c2 * t2z + ct * p.dz;
-                    const float inv = rsqrtf(qx * qx + qy * qy + qz * qz);
-                    ndx = qx * inv; ndy = qy * inv; ndz = qz * inv;
-                    p.scat_src += 1u;
-                    redraw = true;
-                }
-                if (need == NEWID || need == SCAT) {
-                    p.dx = ndx; p.dy = ndy; p.dz = ndz;
-                    p.rx = 1.0f / ndx; p.ry = 1.0f / ndy; p.rz = 1.0f / ndz;
-                    if (redraw) {
-                        uint32_t s0, s1, s2, s3;
-                        philox_block(P.seed, P.ifreq, P.pkg_begin + (long long)p.idx, 2u + (p.scat_src & 0xffffffu), s0, s1, s2, s3);
-                        p.tau_rem = -__logf(uniform01<float>(s0));                // a4
-                    }
-                    need = p.cw == kSentinel ? DONE : RUN;       // a cell beyond the grid in a partial tile: escaped
-                }
-                continue;
-            }
-            if (m_run == 0u) break;                // every lane is DEAD: the item is done
-
-            if (need == RUN) {
-                // ------------------------------------------------------------ one cell-step (a5, a7, a9), as photon_fast_kernel
-                const float rho = __uint_as_float(p.cw);
-                const float ex = exit_time(p.fx, p.rx);
-                const float ey = exit_time(p.fy, p.ry);
-                const float ez = exit_time(p.fz, p.rz);
-                const float ts = fminf(fminf(ex, ey), ez);
-                const bool ax0 = ex == ts, ax1 = !ax0 && ey == ts;       // lowest axis wins a tie (reading S4)
-                const float da = ax0 ? p.dx : (ax1 ? p.dy : p.dz);
-                const bool fwd = da > 0.0f;
-                const float ksr = rho * P.ksca;
-                const float dtau = ts * ksr;
-                const bool sc = dtau >= p.tau_rem && ksr > 0.0f;
-                const float x = sc ? p.tau_rem * P.kratio : ts * (rho * P.kabs);
-                float w_new, dep;
-                absorb(p.w, x, w_new, dep);
-                const bool term = w_new < (float)kWMin;                  // a9: residual stays in the cell
-                if (term) { dep = p.w; w_new = 0.0f; }
-                p.pend += dep;
-                p.absrel += dep;
-                p.w = w_new;
-                n_steps += 1;
-                if (term || !sc) {
-                    // the package leaves the cell (or ends in it): the cell visit's energy goes to the tile accumulator
-                    if (p.pend > 0.0f && !(P.debug & 1)) atomicAdd(s_acc + p.c, p.pend * package_rel(P, t_src(p.scat_src)));
-                    p.pend = 0.0f;
-                }
-                if (term) {
-                    s_cnt[1][tid] += 1u;
-                    need = DONE;
-                } else if (sc) {
-                    need = SCAT;
-                } else {
-                    p.tau_rem -= dtau;
-                    p.fx = __saturatef(fmaf(ts, p.dx, p.fx));
-                    p.fy = __saturatef(fmaf(ts, p.dy, p.fy));
-                    p.fz = __saturatef(fmaf(ts, p.dz, p.fz));
-                    const float face = fwd ? 0.0f : 1.0f;    // entry face in the neighbour's frame
-                    if (ax0) p.fx = face; else if (ax1) p.fy = face; else p.fz = face;
-                    const int sh = ax0 ? 0 : (ax1 ? 4 : 8);
-                    const int ca = (p.c >> sh) & 15;
-                    if (ca == (fwd ? kTL - 1 : 0)) {
-                        // leaves the tile: the cell index wraps to the opposite face; remember axis and sign
-                        p.c = (p.c ^ (15 << sh)) | ((1 + (sh >> 1) + (fwd ? 1 : 0)) << 12);
-                        need = XTILE;
-                    } else {
-                        p.c += fwd ? (1 << sh) : -(1 << sh);
-                        p.cw = s_cw[p.c];
-                        if (p.cw == kSentinel) need = DONE;  // a9: escaped (partial tile at the high side of the grid)
-                    }
-                }
-            }
-        }
-
-        if (pend_valid) B.list[nxt][pend_base + pend_pos] = pend_idx;
-        // ---- fold the accumulator tile into the global accumulator (brick order: runs of 256 bytes)
-        __syncthreads();
-        for (int j = tid; j < kTCells; j += kTileThreads) {
-            const int slot = j & 7, x = 2 * ((j >> 3) & 7) + (slot & 1), y = 2 * ((j >> 6) & 7) + ((slot >> 1) & 1),
-                      z = 2 * (j >> 9) + (slot >> 2);
-            const float v = s_acc[x | (y << 4) | (z << 8)];
-            if (v != 0.0f) atomicAdd(P.acc32 + root_id(P, tx * kTL + x, ty * kTL + y, tz * kTL + z), v);
-        }
-    }
-
-    // ---- per-launch totals: warp shuffle reduction, one set of atomics per warp
-    double acc_esc = s_tot[0][tid], acc_abs = s_tot[1][tid];
-    unsigned long long acc_steps = n_steps;
-    unsigned acc_scat = s_cnt[0][tid], acc_term = s_cnt[1][tid];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        acc_esc += __shfl_xor_sync(kFull, acc_esc, o);
-        acc_abs += __shfl_xor_sync(kFull, acc_abs, o);
-        acc_steps += __shfl_xor_sync(kFull, acc_steps, o);
-        acc_scat += __shfl_xor_sync(kFull, acc_scat, o);
-        acc_term += __shfl_xor_sync(kFull, acc_term, o);
-    }
-    if (lane == 0 && (acc_steps != 0 || acc_esc != 0.0)) {
         atomicAdd(&P.result->escaped, acc_esc);
         atomicAdd(&P.result->absorbed, acc_abs);
         atomicAdd(&P.result->cell_steps, acc_steps);
@@ -1887,48 +1464,6 @@ template <typename R, bool HIER, bool REPLAY> int launch_photon(soc_grid *G, con
     return SOC_OK;
 }
 
-template <bool HIER, bool REPLAY, bool ACC32, bool V2 = false>
-int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
-{
-    static_assert(!(HIER && V2), "the run-ahead kernel walks regular grids only");
-    int blocks = 0;
-    const int threads = G->opt_threads;
-    const int side = 2 * P.hot_r + 1;
-    const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
-    int per_sm = 0;
-    if (V2) SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_v2_kernel<REPLAY, ACC32, false>, threads, smem));
-    else SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY, ACC32>, threads, smem));
-    if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
-    if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
-    blocks = per_sm * G->n_sm;                   // persistent: a whole number of CTAs per SM
-    const long long n_pkg = P.pkg_end - P.pkg_begin;
-    const long long need = (n_pkg + threads - 1) / threads;
-    if (need < blocks) blocks = (int)(need > 0 ? need : 1);
-    if (G->opt_carveout >= 0) {
-        if (V2) SOC_CUDA(cudaFuncSetAttribute(photon_v2_kernel<REPLAY, ACC32, false>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
-        else SOC_CUDA(cudaFuncSetAttribute(photon_fast_kernel<HIER, REPLAY, ACC32>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
-    }
-    if (V2) photon_v2_kernel<REPLAY, ACC32, false><<<blocks, threads, smem, st>>>(P, TileBuffers{}, 0);
-    else photon_fast_kernel<HIER, REPLAY, ACC32><<<blocks, threads, smem, st>>>(P);
-    g_launches += 1;
-    SOC_CUDA(cudaGetLastError());
-    if (G->ev_after_photon) {                    // "timing": the pair brackets the photon kernel alone
-        SOC_CUDA(cudaEventRecord(G->ev_after_photon, st));
-        G->ev_after_photon = nullptr;
-    }
-    UnpadParams U;
-    U.out = absorbed; U.acc = G->d_acc; U.acc32 = G->d_acc32; U.weight = weight;
-    U.nx = G->nx; U.ny = G->ny; U.nbx = G->nbx; U.nby = G->nby; U.nrp = G->nrp;
-    U.n_root = G->n_root; U.n_total = G->n_total;
-    long long ub = (G->n_total + 255) / 256;
-    const long long cap = (long long)G->n_sm * 8;
-    if (ub > cap) ub = cap;
-    unpad_add_kernel<ACC32><<<(int)ub, 256, 0, st>>>(U);
-    g_launches += 1;
-    SOC_CUDA(cudaGetLastError());
-    return SOC_OK;
-}
-
 int launch_unpad(soc_grid *G, bool acc32, double weight, double *absorbed, cudaStream_t st)
 {
     UnpadParams U;
@@ -1945,86 +1480,36 @@ int launch_unpad(soc_grid *G, bool acc32, double weight, double *absorbed, cudaS
     return SOC_OK;
 }
 
-void free_tile_buffers(soc_grid *G)
+template <bool HIER, bool REPLAY, bool ACC32, bool QK = false>
+int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
 {
-    for (void *&q : G->tile_mem) { if (q) cudaFree(q); q = nullptr; }
-    G->tile_cap = 0;
-}
-
-// device buffers of the tiled walk, sized for n packages (grown on demand, kept until the grid is destroyed)
-int tile_buffers(soc_grid *G, long long n, TileBuffers *out)
-{
-    const int ntx = (G->nx + kTL - 1) / kTL, nty = (G->ny + kTL - 1) / kTL, ntz = (G->nz + kTL - 1) / kTL;
-    const long long n_tiles = (long long)ntx * nty * ntz;
-    if (n > G->tile_cap) {
-        free_tile_buffers(G);
-        const long long cap = n + n / 8;
-        const size_t sz[12] = {sizeof(TileState) * (size_t)cap, 4u * 6u * (size_t)cap, 4u * 6u * (size_t)cap,
-                               4u * (size_t)n_tiles, 4u * (size_t)n_tiles, 4u * (size_t)n_tiles, 4u * (size_t)n_tiles,
-                               4u * (size_t)cap, 4u * (size_t)cap, sizeof(TileItem) * (size_t)(cap / kTileChunk + n_tiles + 8),
-                               4u, 4u};
-        for (int i = 0; i < 12; ++i) {
-            cudaError_t e = cudaMalloc(&G->tile_mem[i], sz[i]);
-            if (e != cudaSuccess) { free_tile_buffers(G); return fail(SOC_ENOMEM, std::string("tile buffers: ") + cudaGetErrorString(e)); }
-        }
-        G->tile_cap = cap;
-    }
-    TileBuffers B;
-    B.state = (TileState *)G->tile_mem[0];
-    B.list[0] = (uint32_t *)G->tile_mem[1]; B.list[1] = (uint32_t *)G->tile_mem[2];
-    B.seg[0] = (int *)G->tile_mem[3]; B.seg[1] = (int *)G->tile_mem[4];
-    B.fill[0] = (int *)G->tile_mem[5]; B.fill[1] = (int *)G->tile_mem[6];
-    B.rank = (uint32_t *)G->tile_mem[7]; B.tile0 = (uint32_t *)G->tile_mem[8];
-    B.items = (TileItem *)G->tile_mem[9];
-    B.n_items = (int *)G->tile_mem[10]; B.item_counter = (unsigned *)G->tile_mem[11];
-    B.ntx = ntx; B.nty = nty; B.ntz = ntz; B.n_tiles = (int)n_tiles;
-    *out = B;
-    return SOC_OK;
-}
-
-// tiled production path: emit -> queue of round 0 -> (plan, walk) x rounds -> plan, resume kernel -> unpad
-int launch_tiled(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
-{
-    const long long n = P.pkg_end - P.pkg_begin;
-    TileBuffers B;
-    int rc = tile_buffers(G, n, &B);
-    if (rc != SOC_OK) return rc;
-    SOC_CUDA(cudaMemsetAsync(B.fill[0], 0, sizeof(int) * (size_t)B.n_tiles, st));
-    long long eb = (n + 255) / 256;
-    if (eb > (long long)G->n_sm * 8) eb = (long long)G->n_sm * 8;
-    tile_emit_kernel<<<(int)eb, 256, 0, st>>>(P, B);
-    tile_plan_kernel<<<1, 1024, 0, st>>>(B, 0, 0);
-    tile_scatter_kernel<<<(int)eb, 256, 0, st>>>(n, B);
-    g_launches += 3;
-    int rounds = G->opt_tile_rounds;
-    if (rounds <= 0) {
-        const int nt = B.ntx > B.nty ? (B.ntx > B.ntz ? B.ntx : B.ntz) : (B.nty > B.ntz ? B.nty : B.ntz);
-        rounds = 3 * nt + 8;
-    }
-    int cur = 0;
-    const int walk_blocks = G->n_sm * 6;
-    for (int r = 0; r < rounds; ++r) {
-        tile_plan_kernel<<<1, 1024, 0, st>>>(B, cur, 1);
-        tile_walk_kernel<<<walk_blocks, kTileThreads, 0, st>>>(P, B, cur);
-        g_launches += 2;
-        cur ^= 1;
-    }
-    SOC_CUDA(cudaGetLastError());
-    // the packages still alive continue in the lane-per-package kernel
-    FastParams R = P;
-    R.hot_r = -1;
+    static_assert(!(HIER && QK) && (ACC32 || !QK), "photon_q_kernel walks regular grids with the fp32 accumulator only");
+    int blocks = 0;
+    const int threads = G->opt_threads;
+    const int side = 2 * P.hot_r + 1;
+    const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
     int per_sm = 0;
-    SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_v2_kernel<false, true, true>, 256, 0));
+    if (QK) SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<REPLAY>, threads, smem));
+    else SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY, ACC32>, threads, smem));
     if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
-    tile_plan_kernel<<<1, 1024, 0, st>>>(B, cur, 1);
-    photon_v2_kernel<false, true, true><<<per_sm * G->n_sm, 256, 0, st>>>(R, B, cur);
-    g_launches += 2;
+    if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
+    blocks = per_sm * G->n_sm;                   // persistent: a whole number of CTAs per SM
+    const long long n_pkg = P.pkg_end - P.pkg_begin;
+    const long long need = (n_pkg + threads - 1) / threads;
+    if (need < blocks) blocks = (int)(need > 0 ? need : 1);
+    if (G->opt_carveout >= 0) {
+        if (QK) SOC_CUDA(cudaFuncSetAttribute(photon_q_kernel<REPLAY>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
+        else SOC_CUDA(cudaFuncSetAttribute(photon_fast_kernel<HIER, REPLAY, ACC32>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
+    }
+    if (QK) photon_q_kernel<REPLAY><<<blocks, threads, smem, st>>>(P);
+    else photon_fast_kernel<HIER, REPLAY, ACC32><<<blocks, threads, smem, st>>>(P);
+    g_launches += 1;
     SOC_CUDA(cudaGetLastError());
-    if (G->ev_after_photon) {
+    if (G->ev_after_photon) {                    // "timing": the pair brackets the photon kernel alone
         SOC_CUDA(cudaEventRecord(G->ev_after_photon, st));
         G->ev_after_photon = nullptr;
     }
-    return launch_unpad(G, true, weight, absorbed, st);
+    return launch_unpad(G, ACC32, weight, absorbed, st);
 }
 
 int check_sources(const soc_grid *G, const soc_sources *src, long long n_packages, long long *n_bg_out)
@@ -2149,20 +1634,17 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         }
         F.acc32 = G->d_acc32;
         const double w_eff = acc32 ? weight * e_ref : weight;
-        const bool v2 = !hier && G->opt_kernel >= 2 && pkg_count < (1ll << 32);
-        if (!hier && !rep && acc32 && !P.is_beam && G->opt_kernel == 3 && pkg_count < (1ll << 28) &&
-            G->nx <= 1024 && G->ny <= 1024 && G->nz <= 1024) {
-            F.hot_r = -1;
-            rc = launch_tiled(G, F, w_eff, absorbed, st);
-            if (rc == SOC_OK && G->opt_timing) G->ev_set[slot] = 1;
-            G->ev_after_photon = nullptr;
-            return rc;
-        }
+        // photon_q_kernel trades instructions for L2 requests: it wins where the working set (cell words + fp32
+        // accumulator, 8 B per cell) does not stay in L2 (B200: 19.1 vs 20.2 ms per frequency on config 5) and loses
+        // on L2-resident grids, which are bound by issue slots (3.2 vs 2.8 ms on config 3); profiles/README.md
+        // and where packages scatter less than about twice on their way through the grid (every scattering parks the lane
+        // and reloads the half brick): measured crossover on config 5 at a scattering depth of the box of 2
+        const int n_max = G->nx > G->ny ? (G->nx > G->nz ? G->nx : G->nz) : (G->ny > G->nz ? G->ny : G->nz);
+        const bool big = 8ll * G->n_int > (64ll << 20) && P.ksca * G->rho_mean * n_max < 2.0;
+        const bool v2 = !hier && acc32 && (G->opt_kernel == 2 || (G->opt_kernel == 0 && big)) && pkg_count < (1ll << 32);
         const int sel = (v2 ? 8 : 0) | (hier ? 4 : 0) | (rep ? 2 : 0) | (acc32 ? 1 : 0);
         switch (sel) {
-        case 8: rc = launch_fast<false, false, false, true>(G, F, w_eff, absorbed, st); break;
         case 9: rc = launch_fast<false, false, true, true>(G, F, w_eff, absorbed, st); break;
-        case 10: rc = launch_fast<false, true, false, true>(G, F, w_eff, absorbed, st); break;
         case 11: rc = launch_fast<false, true, true, true>(G, F, w_eff, absorbed, st); break;
         case 0: rc = launch_fast<false, false, false>(G, F, w_eff, absorbed, st); break;
         case 1: rc = launch_fast<false, false, true>(G, F, w_eff, absorbed, st); break;
@@ -2219,7 +1701,6 @@ void soc_grid_destroy(soc_grid *G)
     cudaFree(G->d_cellw); cudaFree(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
     cudaFree(G->d_table); cudaFree(G->d_cellw_int); cudaFree(G->d_parent_int); cudaFree(G->d_acc); cudaFree(G->d_acc32);
     if (G->h_results) cudaFreeHost(G->h_results);
-    for (void *q : G->tile_mem) if (q) cudaFree(q);
     for (cudaEvent_t e : G->ev0) cudaEventDestroy(e);
     for (cudaEvent_t e : G->ev1) cudaEventDestroy(e);
     delete G;
@@ -2294,6 +1775,13 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     }
     for (long long o = 0; o < G->n_octets; ++o)
         if (parent[(size_t)o] == INT32_MIN) return fail(SOC_EINVAL, "octet without a parent");
+    {
+        double sum = 0.0;
+        long long cnt = 0;
+        for (long long c = 0; c < G->n_root; ++c)
+            if ((int32_t)cellw[(size_t)c] >= 0) { sum += (double)d->density[c]; cnt += 1; }
+        G->rho_mean = cnt > 0 ? sum / (double)cnt : 0.0;
+    }
 
     SOC_CUDA(cudaGetDevice(&G->device));
     SOC_CUDA(cudaDeviceGetAttribute(&G->n_sm, cudaDevAttrMultiProcessorCount, G->device));
@@ -2366,9 +1854,8 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     else if (k == "timing" && (value == 0 || value == 1)) G->opt_timing = (int)value;
     else if (k == "debug" && value >= 0 && value <= 255) G->opt_debug = (int)value;
     else if (k == "hot_cache" && (value == 0 || value == 1)) G->opt_hot_cache = (int)value;
-    else if (k == "kernel" && value >= 1 && value <= 3) G->opt_kernel = (int)value;
+    else if (k == "kernel" && value >= 0 && value <= 2) G->opt_kernel = (int)value;
     else if (k == "carveout" && value >= -1 && value <= 100) G->opt_carveout = (int)value;
-    else if (k == "tile_rounds" && value >= 0 && value <= 100000) G->opt_tile_rounds = (int)value;
     else if (k == "acc32" && (value == 0 || value == 1)) G->opt_acc32 = (int)value;
     else return fail(SOC_EINVAL, "unknown option or value out of range: " + k);
     return SOC_OK;
