@@ -291,14 +291,16 @@ def run_ours(args):
     achieved = algo_bytes / (mean_launch_ms * 1e-3) / 1e9
     per_f = steps_f / (kern_ms * 1e-3)
     roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": None, "peak_source": peak_src, "kernel": "photon_kernel",
+            "traffic": None, "peak_source": peak_src,
+            "kernel": "photon_q_kernel / photon_fast_kernel (production photon kernel, chosen per frequency)",
             "algorithmic_bytes_per_launch": algo_bytes, "mean_launch_ms": mean_launch_ms,
             "kernel_share_of_step": float(kern_ms.sum() / ms_per_step)}
     roof.update(roofline_notes(args.config))
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32 geometry / f64 weights and accumulators", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "dtype_note": "fp32 package state, weights and per-launch accumulator; fp64 frequency integral and totals",
             "config": {"workload": WORKLOADS[args.config], "cells": int(P.n_total), "n_freq": int(P.n_freq),
                        "packages_per_frequency": int(P.n_packages), "parallelism": f"replicas x{world} (seed + rank), "
                        "one fp64 all-reduce" if world > 1 else "single GPU",
@@ -327,7 +329,13 @@ def run_ours(args):
 
 # DRAM traffic of one photon-kernel launch from the committed `ncu --set full` capture of this command
 # (dram__bytes_read.sum + dram__bytes_write.sum, mean over the captured launches); None = not captured yet.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {
+    "5": {"traffic": 54.66e9,
+          "traffic_source": "profiles/r01b_ncu_full_photon_q_config5.txt: dram__bytes_read.sum 40.41 GB + "
+                            "dram__bytes_write.sum 14.25 GB, mean of launches 65-67 (frequency indices 64-66)",
+          "binding_unit": "L1->L2 request rate and issue slots, not bytes: lts__t_tag_requests 54 %, l1tex2xbar 48 %, "
+                          "issue slots 66 %, DRAM 35 % busy (same capture); see DESIGN.md 6.1"},
+}
 
 
 def roofline_notes(config):

@@ -1791,10 +1791,10 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     SOC_CUDA(cudaMemcpy(G->d_cellw, cellw.data(), sizeof(uint32_t) * (size_t)G->n_total, cudaMemcpyHostToDevice));
     SOC_CUDA(cudaMemcpy(G->d_parent, parent.data(), sizeof(int32_t) * parent.size(), cudaMemcpyHostToDevice));
     // internal layout: root grid in 2x2x2 bricks with ghost cells around it (they hold the sentinel; cell ix
-    // sits at X = ix + 2, so the low side has a whole ghost brick and the high side at least two ghost cells:
-    // the run-ahead kernel gathers the neighbour of the first ghost cell it meets), octet levels shifted behind it
+    // sits at X = ix + 2, so the low side has a whole ghost brick and the high side at least one ghost cell),
+    // octet levels shifted behind it
     {
-        const long long nbx = ((long long)G->nx + 5) / 2, nby = ((long long)G->ny + 5) / 2, nbz = ((long long)G->nz + 5) / 2;
+        const long long nbx = ((long long)G->nx + 4) / 2, nby = ((long long)G->ny + 4) / 2, nbz = ((long long)G->nz + 4) / 2;
         const long long nrp = 8 * nbx * nby * nbz;
         const long long n_int = nrp + (G->n_total - G->n_root);
         if (n_int >= (1ll << 31)) return fail(SOC_EINVAL, "more than 2^31 cells in the padded layout");
