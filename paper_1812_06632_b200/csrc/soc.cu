@@ -839,7 +839,9 @@ __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_consta
         }
         if (m_run == 0u) break;                  // nothing parked that can be serviced, nothing running
 
-        if (need == RUN) {
+        // two cell-steps per look at the warp's state: the ballots and the loop overhead are paid once; a lane
+        // that parks in the first step sits out the second
+        auto cell_step = [&]() {
             // ---------------------------------------------------------------- one cell-step (a5-a7, a9)
             const float rho = __uint_as_float(p.cw);
             const float tx = exit_time(p.fx, p.rx);
@@ -920,7 +922,9 @@ __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_consta
                     if (p.cw == kSentinel) need = DONE;              // a9: escaped
                 }
             }
-        }
+        };
+        if (need == RUN) cell_step();
+        if (need == RUN) cell_step();
     }
 
     // ---- the block's hot-cell partial sums go to the accumulator: one fp64 reduction per touched cell and block
@@ -1141,7 +1145,9 @@ __global__ void __launch_bounds__(256, 4) photon_q_kernel(const __grid_constant_
         }
         if (m_run == 0u) break;                  // nothing parked that can be serviced, nothing running
 
-        if (need == RUN) {
+        // two cell-steps per look at the warp's state: the ballots and the loop overhead are paid once; a lane
+        // that parks in the first step sits out the second
+        auto cell_step = [&]() {
             // ---------------------------------------------------------------- one cell-step (a5-a7, a9)
             const uint32_t cw = q_word(p);
             if (cw == kSentinel) {
@@ -1222,7 +1228,9 @@ __global__ void __launch_bounds__(256, 4) photon_q_kernel(const __grid_constant_
                     }
                 }
             }
-        }
+        };
+        if (need == RUN) cell_step();
+        if (need == RUN) cell_step();
     }
 
     // ---- the block's hot-cell partial sums go to the accumulator: one reduction per touched cell and block
