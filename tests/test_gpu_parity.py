@@ -102,7 +102,8 @@ def test_config2_replay_full():
 
 
 @pytest.mark.parametrize("which,kw", [("1", {}), ("2", dict(n=32, n_packages=200_000)),
-                                      ("3", dict(n=32, n_packages=200_000, n_freq=8))])
+                                      ("3", dict(n=32, n_packages=200_000, n_freq=8)),
+                                      ("4p", dict(n=16, n_packages=150_000, n_freq=8))])
 def test_production_mode_within_5_sigma(which, kw):
     """Seeds 1..8 on both sides; sigma_c = per-cell sample standard deviation of the oracle's 8 runs;
     |A_gpu(s) - A_orc(s)| <= 5 sigma_c for every cell and seed.  The config-3 case (visual
