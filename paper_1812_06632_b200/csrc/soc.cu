@@ -13,6 +13,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <thread>
 #include <vector>
 
 // ------------------------------------------------------------------------------------------------
@@ -1194,12 +1195,12 @@ __global__ void __launch_bounds__(256, 4) photon_q_kernel(const __grid_constant_
                         const int j = (p.sd & 7) + hot_side * (((p.sd >> 3) & 7) + hot_side * ((p.sd >> 6) & 7));
                         atomicAdd(s_hot + (p.sd >> 16) * hot_cells + j, p.pend);
                     } else {
-                        const bool lo = (p.rel & 1) != 0, hi = (p.rel & 2) != 0;
+                        const int s2 = p.rel & 3;
                         const float v = p.pend * p.prel;
-                        p.a0 += (!hi && !lo) ? v : 0.0f;
-                        p.a1 += (!hi && lo) ? v : 0.0f;
-                        p.a2 += (hi && !lo) ? v : 0.0f;
-                        p.a3 += (hi && lo) ? v : 0.0f;
+                        p.a0 += s2 == 0 ? v : 0.0f;
+                        p.a1 += s2 == 1 ? v : 0.0f;
+                        p.a2 += s2 == 2 ? v : 0.0f;
+                        p.a3 += s2 == 3 ? v : 0.0f;
                     }
                     p.pend = 0.0f;
                 }
@@ -1378,6 +1379,30 @@ __global__ void __launch_bounds__(256) temperature_kernel(const __grid_constant_
                 P.T_out[c] = temperature_of(P, tab, P.cellw[c], P.absorbed[c], (double)(1ull << (3 * l)));
             }
         }
+    }
+}
+
+// ABI-order cell words -> internal layout (ghost-padded 2x2x2 bricks of the root grid, then the octet levels with
+// their links shifted behind the padded root grid); runs once per soc_grid_create
+__global__ void __launch_bounds__(256) repad_kernel(const uint32_t *cellw, uint32_t *ci, int nx, int ny, int nz, int nbx,
+                                                    int nby, long long nrp, long long n_root, long long n_int)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < n_int; j += stride) {
+        uint32_t cw = kSentinel;
+        bool real = true;
+        if (j < nrp) {
+            const long long B = j >> 3;
+            const int slot = (int)(j & 7);
+            const int bx = (int)(B % nbx), by = (int)((B / nbx) % nby), bz = (int)(B / ((long long)nbx * nby));
+            const int ix = 2 * bx + (slot & 1) - 2, iy = 2 * by + ((slot >> 1) & 1) - 2, iz = 2 * bz + (slot >> 2) - 2;
+            real = (unsigned)ix < (unsigned)nx && (unsigned)iy < (unsigned)ny && (unsigned)iz < (unsigned)nz;
+            if (real) cw = cellw[ix + (long long)nx * (iy + (long long)ny * iz)];
+        } else {
+            cw = cellw[n_root + (j - nrp)];
+        }
+        if (real && (int32_t)cw < 0) cw = 0x80000000u | (uint32_t)(nrp + (cw & 0x7fffffffu));
+        ci[j] = cw;
     }
 }
 
@@ -1772,7 +1797,38 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     } catch (const std::bad_alloc &) {
         return fail(SOC_ENOMEM, "out of host memory");
     }
-    for (int l = 0; l < d->n_levels; ++l) {
+    bool words_done = false;
+    if (!d->child && G->n_total >= (1ll << 20)) {
+        // regular grid: every cell is a leaf, the words are independent -- validate and convert on all host cores
+        const unsigned hw = std::thread::hardware_concurrency();
+        const int nt = (int)(hw < 1 ? 1 : (hw > 32 ? 32 : hw));
+        std::vector<int> bad((size_t)nt, 0);
+        std::vector<double> sums((size_t)nt, 0.0);
+        std::vector<std::thread> pool;
+        for (int t = 0; t < nt; ++t)
+            pool.emplace_back([&, t]() {
+                const long long b = G->n_total * t / nt, e = G->n_total * (t + 1) / nt;
+                double sum = 0.0;
+                for (long long gid = b; gid < e; ++gid) {
+                    const float r = d->density[gid];
+                    if (!(r >= 0.0f) || !std::isfinite(r)) { bad[(size_t)t] = 1; return; }
+                    float rp = r + 0.0f;
+                    uint32_t bits;
+                    std::memcpy(&bits, &rp, 4);
+                    cellw[(size_t)gid] = bits & 0x7fffffffu;
+                    sum += (double)r;
+                }
+                sums[(size_t)t] = sum;
+            });
+        for (std::thread &th : pool) th.join();
+        for (int t = 0; t < nt; ++t)
+            if (bad[(size_t)t]) return fail(SOC_EINVAL, "leaf density must be finite and >= 0");
+        double sum = 0.0;
+        for (double v : sums) sum += v;
+        G->rho_mean = sum / (double)G->n_total;
+        words_done = true;
+    }
+    for (int l = 0; l < d->n_levels && !words_done; ++l) {
         for (long long c = 0; c < d->n_cells[l]; ++c) {
             const long long gid = G->level_off[l] + c;
             const int32_t ch = d->child ? d->child[gid] : -1;
@@ -1795,7 +1851,7 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     }
     for (long long o = 0; o < G->n_octets; ++o)
         if (parent[(size_t)o] == INT32_MIN) return fail(SOC_EINVAL, "octet without a parent");
-    {
+    if (!words_done) {
         double sum = 0.0;
         long long cnt = 0;
         for (long long c = 0; c < G->n_root; ++c)
@@ -1819,10 +1875,8 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
         const long long n_int = nrp + (G->n_total - G->n_root);
         if (n_int >= (1ll << 31)) return fail(SOC_EINVAL, "more than 2^31 cells in the padded layout");
         G->nbx = (int)nbx; G->nby = (int)nby; G->nbz = (int)nbz; G->nrp = (int)nrp; G->n_int = n_int;
-        std::vector<uint32_t> ci;
         std::vector<int32_t> pi;
         try {
-            ci.assign((size_t)n_int, kSentinel);
             pi.assign(parent.size(), 0);
         } catch (const std::bad_alloc &) {
             return fail(SOC_ENOMEM, "out of host memory");
@@ -1833,15 +1887,13 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
             const long long X = ix + 2, Y = iy + 2, Z = iz + 2;
             return 8 * ((X >> 1) + nbx * ((Y >> 1) + nby * (Z >> 1))) + (X & 1) + 2 * (Y & 1) + 4 * (Z & 1);
         };
-        for (long long gid = 0; gid < G->n_total; ++gid) {
-            const uint32_t cw = cellw[(size_t)gid];
-            ci[(size_t)internal(gid)] = (int32_t)cw < 0 ? (0x80000000u | (uint32_t)(nrp + (cw & 0x7fffffffu))) : cw;
-        }
         for (long long o = 0; o < G->n_octets; ++o) pi[(size_t)o] = (int32_t)internal((long long)parent[(size_t)o] + G->n_root);
         SOC_CUDA(cudaMalloc(&G->d_cellw_int, sizeof(uint32_t) * (size_t)n_int));
         SOC_CUDA(cudaMalloc(&G->d_parent_int, sizeof(int32_t) * pi.size()));
         SOC_CUDA(cudaMalloc(&G->d_acc, sizeof(double) * (size_t)n_int));
-        SOC_CUDA(cudaMemcpy(G->d_cellw_int, ci.data(), sizeof(uint32_t) * (size_t)n_int, cudaMemcpyHostToDevice));
+        repad_kernel<<<G->n_sm * 8, 256>>>(G->d_cellw, G->d_cellw_int, G->nx, G->ny, G->nz, (int)nbx, (int)nby, nrp, G->n_root, n_int);
+        g_launches += 1;
+        SOC_CUDA(cudaGetLastError());
         SOC_CUDA(cudaMemcpy(G->d_parent_int, pi.data(), sizeof(int32_t) * pi.size(), cudaMemcpyHostToDevice));
         SOC_CUDA(cudaMemset(G->d_acc, 0, sizeof(double) * (size_t)n_int));
         SOC_CUDA(cudaMalloc(&G->d_acc32, sizeof(float) * (size_t)n_int));
