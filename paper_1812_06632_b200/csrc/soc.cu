@@ -736,7 +736,7 @@ __device__ __forceinline__ double escaped_rel(float w, float absrel)
 }
 
 template <bool HIER, bool REPLAY, bool ACC32>
-__global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_constant__ FastParams P)
+__global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __grid_constant__ FastParams P)
 {
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -932,6 +932,8 @@ __global__ void __launch_bounds__(256, 4) photon_fast_kernel(const __grid_consta
         };
         if (need == RUN) cell_step();
         if (need == RUN) cell_step();
+        if (need == RUN) cell_step();
+        if (need == RUN) cell_step();
     }
 
     // ---- the block's hot-cell partial sums go to the accumulator: one fp64 reduction per touched cell and block
@@ -1030,7 +1032,7 @@ __device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p)
 }
 
 template <bool REPLAY>
-__global__ void __launch_bounds__(256, 4) photon_q_kernel(const __grid_constant__ FastParams P)
+__global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant__ FastParams P)
 {
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -1236,6 +1238,8 @@ __global__ void __launch_bounds__(256, 4) photon_q_kernel(const __grid_constant_
                 }
             }
         };
+        if (need == RUN) cell_step();
+        if (need == RUN) cell_step();
         if (need == RUN) cell_step();
         if (need == RUN) cell_step();
     }
