@@ -1924,7 +1924,7 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     if (!G || !key) return fail(SOC_EINVAL, "NULL argument");
     const std::string k(key);
     if (k == "blocks_per_sm" && value >= 0 && value <= 32) G->opt_blocks_per_sm = (int)value;
-    else if (k == "threads" && (value == 64 || value == 128 || value == 256)) G->opt_threads = (int)value;
+    else if (k == "threads" && (value == 64 || value == 128 || value == 192 || value == 256)) G->opt_threads = (int)value;
     else if (k == "refill_threshold" && value >= 1 && value <= 32) G->opt_refill_threshold = (int)value;
     else if (k == "service_threshold" && value >= 0 && value <= 32) G->opt_service_threshold = (int)value;
     else if (k == "timing" && (value == 0 || value == 1)) G->opt_timing = (int)value;

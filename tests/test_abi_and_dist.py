@@ -164,3 +164,24 @@ def test_world_size_2_gloo_all_reduce(mode, tmp_path):
         assert np.allclose(a0, sim(3), rtol=1e-12, atol=0)
     else:                     # seeds 3 and 4: the mean of two realisations
         assert np.allclose(a0, 0.5 * (sim(3) + sim(4)), rtol=1e-12, atol=0)
+
+
+def test_bench_reference_arm_prints_the_contract_line():
+    """bench.py --impl reference runs the oracle on the host cores and prints ONE JSON line with the keys the
+    driver reads (no GPU involved)."""
+    import json
+    import subprocess
+    import sys
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1",
+                          "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for key in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert key in d, key
+    assert d["impl"] == "reference" and d["value"] > 0 and d["unit"] == "cell-steps/s" and d["vs_baseline"] is None
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+    assert "workload" in d["config"]
