@@ -1661,6 +1661,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
             F.service_threshold = G->opt_service_threshold > 0 ? G->opt_service_threshold
                                                                : (P.ksca * G->rho_mean * nm >= 4.0 ? 16 : 8);
         }
+        const int auto_threshold = G->opt_service_threshold > 0 ? G->opt_service_threshold : 8;     // photon_q_kernel: 8 throughout
         F.debug = G->opt_debug;
         // hot-cell cache: R = 3 (343 cells per source) while it fits in 40 KB per block, else R = 2; regular grids
         F.hot_r = -1;
@@ -1686,11 +1687,12 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         // photon_q_kernel trades instructions for L2 requests: it wins where the working set (cell words + fp32
         // accumulator, 8 B per cell) does not stay in L2 (B200: 19.1 vs 20.2 ms per frequency on config 5) and loses
         // on L2-resident grids, which are bound by issue slots (3.2 vs 2.8 ms on config 3); profiles/README.md
-        // and where packages scatter less than about twice on their way through the grid (every scattering parks the lane
-        // and reloads the half brick): measured crossover on config 5 at a scattering depth of the box of 2
+        // and where packages do not scatter very often (every scattering parks the lane and reloads the half brick):
+        // measured crossover on config 5, both kernels at their best occupancy, at a scattering depth of the box of 12-16
         const int n_max = G->nx > G->ny ? (G->nx > G->nz ? G->nx : G->nz) : (G->ny > G->nz ? G->ny : G->nz);
-        const bool big = 8ll * G->n_int > (64ll << 20) && P.ksca * G->rho_mean * n_max < 2.0;
+        const bool big = 8ll * G->n_int > (64ll << 20) && P.ksca * G->rho_mean * n_max < 12.0;
         const bool v2 = !hier && acc32 && (G->opt_kernel == 2 || (G->opt_kernel == 0 && big)) && pkg_count < (1ll << 32);
+        if (v2) F.service_threshold = auto_threshold;
         const int sel = (v2 ? 8 : 0) | (hier ? 4 : 0) | (rep ? 2 : 0) | (acc32 ? 1 : 0);
         switch (sel) {
         case 9: rc = launch_fast<false, false, true, true>(G, F, w_eff, absorbed, st); break;
