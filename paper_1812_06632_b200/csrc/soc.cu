@@ -1158,20 +1158,25 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
         // that parks in the first step sits out the second
         auto cell_step = [&]() {
             // ---------------------------------------------------------------- one cell-step (a5-a7, a9)
+            // the geometry of the step does not need the cell word: it goes first, so that the gather issued by the last
+            // crossing has that much longer to arrive
+            const float tx = exit_time(p.fx, p.rx);
+            const float ty = exit_time(p.fy, p.ry);
+            const float tz = exit_time(p.fz, p.rz);
+            const float ts = fminf(fminf(tx, ty), tz);
+            const bool ax0 = tx == ts, ax1 = !ax0 && ty == ts;           // lowest axis wins a tie (reading S4)
+            const float da = ax0 ? p.dx : (ax1 ? p.dy : p.dz);
+            const bool fwd = da > 0.0f;
+            const int bstride = ax0 ? 8 : (ax1 ? P.bsy : P.bsz);          // to the same slot of the next brick
+            const int abit = ax0 ? 1 : (ax1 ? 2 : 4);
+            const float gx = __saturatef(fmaf(ts, p.dx, p.fx));           // position after a crossing
+            const float gy = __saturatef(fmaf(ts, p.dy, p.fy));
+            const float gz = __saturatef(fmaf(ts, p.dz, p.fz));
             const uint32_t cw = q_word(p);
             if (cw == kSentinel) {
                 need = DONE;                     // a9: the cell entered by the last crossing is outside the grid
             } else {
                 const float rho = __uint_as_float(cw);
-                const float tx = exit_time(p.fx, p.rx);
-                const float ty = exit_time(p.fy, p.ry);
-                const float tz = exit_time(p.fz, p.rz);
-                const float ts = fminf(fminf(tx, ty), tz);
-                const bool ax0 = tx == ts, ax1 = !ax0 && ty == ts;       // lowest axis wins a tie (reading S4)
-                const float da = ax0 ? p.dx : (ax1 ? p.dy : p.dz);
-                const bool fwd = da > 0.0f;
-                const int bstride = ax0 ? 8 : (ax1 ? P.bsy : P.bsz);      // to the same slot of the next brick
-                const int abit = ax0 ? 1 : (ax1 ? 2 : 4);
                 const float ksr = rho * P.ksca;
                 const float dtau = ts * ksr;
                 const bool sc = dtau >= p.tau_rem && ksr > 0.0f;
@@ -1219,9 +1224,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                         if ((unsigned)c < (unsigned)hot_side) p.sd = (p.sd & ~(7 << sh)) | (c << sh);
                         else p.sd &= ~0x200;
                     }
-                    p.fx = __saturatef(fmaf(ts, p.dx, p.fx));
-                    p.fy = __saturatef(fmaf(ts, p.dy, p.fy));
-                    p.fz = __saturatef(fmaf(ts, p.dz, p.fz));
+                    p.fx = gx; p.fy = gy; p.fz = gz;
                     const float face = fwd ? 0.0f : 1.0f;    // entry face in the neighbour's frame
                     if (ax0) p.fx = face; else if (ax1) p.fy = face; else p.fz = face;
                     // neighbour inside the brick: flip the slot bit; otherwise the same bit flips and the brick changes
