@@ -296,6 +296,19 @@ def run_ours(args):
             "algorithmic_bytes_per_launch": algo_bytes, "mean_launch_ms": mean_launch_ms,
             "kernel_share_of_step": float(kern_ms.sum() / ms_per_step)}
     roof.update(roofline_notes(args.config))
+    if world == 1 and not args.no_probes:
+        # ceilings of the memory system for this footprint, measured in the same run:
+        # independent random accesses with no arithmetic, over 8 B per cell (cell words + fp32 accumulator)
+        fp = 8 * int(P.n_total)
+        n_ops = 1 << 31
+        rate = lambda kind: n_ops / (soc.probe_throughput(kind, fp, n_ops) * 1e-3)          # noqa: E731
+        g4, r4, cs = rate(0), rate(2), rate(5)
+        per_launch = float(steps_f.mean()) / (mean_launch_ms * 1e-3)
+        roof["probes"] = {"footprint_bytes": fp, "random_gather_4B_per_s": g4, "random_red_f32_per_s": r4,
+                          "gather_plus_red_per_s": cs, "cell_steps_per_s_mean_launch": per_launch,
+                          "frac_of_gather_plus_red": per_launch / cs,
+                          "note": "gather_plus_red = one 4-byte gather and one fp32 red.global.add per random cell: the memory "
+                                  "side of a cell-step with every access independent and no arithmetic"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -353,6 +366,7 @@ def main():
     ap.add_argument("--config", choices=sorted(WORKLOADS), default="5")
     ap.add_argument("--packages", type=int, default=0, help="override packages per frequency (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-probes", action="store_true", help="skip the random gather / scatter-add ceiling probes")
     ap.add_argument("--opt", action="append", default=[], help="library tuning knob key=value (soc_set_option)")
     args = ap.parse_args()
     if args.steps < 1 or args.warmup < 0:

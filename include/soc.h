@@ -158,9 +158,11 @@ int soc_set_option(soc_grid *grid, const char *key, int64_t value);
 int soc_get_timings(soc_grid *grid, int32_t n, float *ms);
 
 /* Roofline probes: random 4-byte gathers (kind 0), random fp64 red.global.add (kind 1),
- * random fp32 red.global.add (kind 2), random 32-byte gathers (kind 3: one sector = a 2x2x2 brick of fp32 cells)
- * and random 16-byte red.global.add.v4.f32 (kind 4) over a footprint of `footprint_bytes`, n_ops operations in
- * total, uniform addresses.  *ms receives the CUDA-event time of the probe kernel. */
+ * random fp32 red.global.add (kind 2), random 32-byte gathers (kind 3: one sector = a 2x2x2 brick of fp32 cells),
+ * random 16-byte red.global.add.v4.f32 (kind 4), and the memory side of one cell-step (kind 5: a 4-byte gather from
+ * the first half of the footprint and an fp32 red.global.add at the same random cell of the second half) over a
+ * footprint of `footprint_bytes`, n_ops operations in total, uniform addresses, no arithmetic, every access
+ * independent of the others.  *ms receives the CUDA-event time of the probe kernel. */
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms);
 
 /* Number of kernel launches issued by this library in the calling process (bench.py's "gpu_launches"). */

@@ -1431,25 +1431,31 @@ __global__ void __launch_bounds__(256) probe_kernel(void *buf, unsigned long lon
 {
     const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t s = mix32(tid * 2654435761u + 12345u);
-    float acc = 0.f;
-    for (long long i = 0; i < ops_per_thread; ++i) {
-        s = mix32(s + 0x9e3779b9u);
-        const unsigned long long j = ((unsigned long long)s * n_elem) >> 32;
-        if (KIND == 0) acc += __ldg(reinterpret_cast<const float *>(buf) + j);
-        else if (KIND == 1) atomicAdd(reinterpret_cast<double *>(buf) + j, 1.0);
-        else if (KIND == 2) atomicAdd(reinterpret_cast<float *>(buf) + j, 1.0f);
-        else if (KIND == 3) {                    // 32-byte gather (one sector: a 2x2x2 brick of fp32 cells)
-            float a0, a1, a2, a3, a4, a5, a6, a7;
-            asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                         : "=f"(a0), "=f"(a1), "=f"(a2), "=f"(a3), "=f"(a4), "=f"(a5), "=f"(a6), "=f"(a7)
-                         : "l"(reinterpret_cast<const float *>(buf) + 8 * j));
-            acc += a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-        } else {                                 // 16-byte vector reduction (4 fp32 cells)
-            asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(reinterpret_cast<float *>(buf) + 4 * j),
-                         "f"(1.0f), "f"(1.0f), "f"(1.0f), "f"(1.0f) : "memory");
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};          // four independent chains: four gathers in flight per thread
+    for (long long i = 0; i < ops_per_thread; i += 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            s = mix32(s + 0x9e3779b9u);
+            const unsigned long long j = ((unsigned long long)s * n_elem) >> 32;
+            if (KIND == 0) acc[u] += __ldg(reinterpret_cast<const float *>(buf) + j);
+            else if (KIND == 1) atomicAdd(reinterpret_cast<double *>(buf) + j, 1.0);
+            else if (KIND == 2) atomicAdd(reinterpret_cast<float *>(buf) + j, 1.0f);
+            else if (KIND == 3) {                // 32-byte gather (one sector: a 2x2x2 brick of fp32 cells)
+                float a0, a1, a2, a3, a4, a5, a6, a7;
+                asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                             : "=f"(a0), "=f"(a1), "=f"(a2), "=f"(a3), "=f"(a4), "=f"(a5), "=f"(a6), "=f"(a7)
+                             : "l"(reinterpret_cast<const float *>(buf) + 8 * j));
+                acc[u] += a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+            } else if (KIND == 4) {              // 16-byte vector reduction (4 fp32 cells)
+                asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(reinterpret_cast<float *>(buf) + 4 * j),
+                             "f"(1.0f), "f"(1.0f), "f"(1.0f), "f"(1.0f) : "memory");
+            } else {                             // the memory side of one cell-step: gather rho[cell], add to acc[cell]
+                acc[u] += __ldg(reinterpret_cast<const float *>(buf) + j);
+                atomicAdd(reinterpret_cast<float *>(buf) + n_elem + j, 1.0f);
+            }
         }
     }
-    if ((KIND == 0 || KIND == 3) && acc == 123.456f) *sink = acc;
+    if ((KIND == 0 || KIND == 3 || KIND == 5) && acc[0] + acc[1] + acc[2] + acc[3] == 123.456f) *sink = acc[0];
 }
 
 }  // namespace
@@ -2058,8 +2064,8 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
 
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms)
 {
-    if (kind < 0 || kind > 4 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
-    const size_t elem = kind == 1 ? 8 : (kind == 3 ? 32 : (kind == 4 ? 16 : 4));
+    if (kind < 0 || kind > 5 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
+    const size_t elem = (kind == 1 || kind == 5) ? 8 : (kind == 3 ? 32 : (kind == 4 ? 16 : 4));   // kind 5: 4 B rho + 4 B acc per cell
     const unsigned long long n_elem = (unsigned long long)footprint_bytes / elem;
     void *buf = nullptr;
     float *sink = nullptr;
@@ -2070,7 +2076,8 @@ int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, f
     SOC_CUDA(cudaMalloc(&sink, 4));
     SOC_CUDA(cudaMemset(buf, 0, n_elem * elem));
     const int blocks = n_sm * 8, threads = 256;
-    const long long per_thread = (n_ops + (long long)blocks * threads - 1) / ((long long)blocks * threads);
+    long long per_thread = (n_ops + (long long)blocks * threads - 1) / ((long long)blocks * threads);
+    per_thread = (per_thread + 3) / 4 * 4;           // the probe loop is unrolled by four
     cudaEvent_t e0, e1;
     SOC_CUDA(cudaEventCreate(&e0));
     SOC_CUDA(cudaEventCreate(&e1));
@@ -2080,7 +2087,8 @@ int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, f
         else if (kind == 1) probe_kernel<1><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else if (kind == 2) probe_kernel<2><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else if (kind == 3) probe_kernel<3><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
-        else probe_kernel<4><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else if (kind == 4) probe_kernel<4><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else probe_kernel<5><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         g_launches += 1;
         SOC_CUDA(cudaEventRecord(e1));
         SOC_CUDA(cudaEventSynchronize(e1));
