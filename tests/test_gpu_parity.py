@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 
 import oracle
 from gpu_common import (N_THREADS, gpu_packages, oracle_grid, oracle_packages, rel_l1, replay_match)
-from helpers import random_octree
+from helpers import fully_refined, random_octree
 from paper_1812_06632_b200 import inputs, soc
 
 REPLAY, PROD = soc.SOC_GEOM_FP64, soc.SOC_GEOM_FP32
@@ -292,6 +292,55 @@ def test_full_size_launch_properties():
     assert abs(r.emitted - r.absorbed - r.escaped) <= 1e-6 * r.emitted
     assert float(A.sum()) == pytest.approx(r.absorbed, rel=5e-6)
     G.close()
+
+
+# ----------------------------------------------------------------------------------------- octree walk against the regular walk
+@pytest.mark.parametrize("flags", [REPLAY, PROD])
+def test_gpu_fully_refined_hierarchy_equals_regular_grid(flags):
+    """Pin P9 on the GPU: a hierarchy in which every root cell is refined once, with the densities of a regular 2N
+    grid, against the regular-grid kernels on that grid (kappa halved, I / 4: the regular grid's length unit is half a
+    root cell).  Row a6 against row a5 with no oracle in between."""
+    N = 12
+    rng = np.random.default_rng(7)
+    rho2n = rng.lognormal(0, 0.8, (2 * N, 2 * N, 2 * N)).astype(np.float32)
+    n_cells, rho, child, gid_of = fully_refined(rho2n)
+    # (a scattering depth of a few: with many scatterings per package the dropped bits are amplified and the fp64
+    # oracle itself matches only 98.4 % of the packages between the two grids at ksca = 0.8)
+    n, kabs, ksca, gg, I = 200_000, 0.35, 0.2, 0.45, 3.0
+    Ph = _problem_from_arrays((N, N, N), n_cells, rho, child, kabs, ksca, gg, n)
+    Pr = _problem_from_arrays((2 * N, 2 * N, 2 * N), [8 * N ** 3], rho2n.ravel(), None, kabs / 2, ksca / 2, gg, n)
+    Gh, Gr = soc.Grid.from_problem(Ph), soc.Grid.from_problem(Pr)
+    Ah, rh, reph = gpu_packages(Gh, Ph, 0, dict(bg_intensity=I), n, 5, flags=flags)
+    Ar, rr, repr_ = gpu_packages(Gr, Pr, 0, dict(bg_intensity=I / 4), n, 5, flags=flags)
+    Gh.close(); Gr.close()
+    same = (reph["steps"] == repr_["steps"]) & (reph["scatters"] == repr_["scatters"])
+    assert same.mean() >= 0.999                  # the climb rounds (f + bit)/2 to fp32: near-ties may flip
+    assert rh["emitted"] == pytest.approx(rr["emitted"], rel=1e-12)
+    assert rh["escaped"] == pytest.approx(rr["escaped"], rel=1e-4)
+    Ahl = Ah[gid_of.ravel()]
+    assert np.abs(Ahl - Ar).sum() <= 1e-3 * Ar.sum()
+    assert Ah[: N ** 3].sum() == 0.0             # parents receive nothing
+
+
+def test_octree_full_size_mean_cells_crossed():
+    """Pin P7 at full size on the production octree kernel (config 4', 1e6 packages, far infrared, where nothing
+    scatters or terminates): a package of the isotropic background crosses 1 + 2 A_int / S leaf cells on average,
+    A_int = total interior leaf-interface area = (sum over leaves of 6 h^2 - S) / 2."""
+    torch = _torch()
+    P = inputs.make_config("4p")
+    leaf = P.child < 0
+    level = np.repeat(np.arange(P.n_levels), P.n_cells)
+    S = 6.0 * 64 ** 2
+    a_int = (np.sum(6.0 * 4.0 ** (-level[leaf].astype(np.float64))) - S) / 2
+    G = soc.Grid.from_problem(P)
+    A = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+    r = G.simulate_frequency(0, P.sources(0), P.n_packages, P.seed, 1.0, A)
+    G.close()
+    assert r.scatterings < 1e-3 * P.n_packages and r.terminated == 0
+    assert r.cell_steps / P.n_packages == pytest.approx(1 + 2 * a_int / S, rel=3e-3)
+    assert abs(r.emitted - r.absorbed - r.escaped) <= 1e-6 * r.emitted
+    assert float(A.sum()) == pytest.approx(r.absorbed, rel=2e-6)
+    assert float(A[torch.from_numpy(~leaf).cuda()].sum()) == 0.0
 
 
 # ----------------------------------------------------------------------------------------- frequency loop + temperatures
