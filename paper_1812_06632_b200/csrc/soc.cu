@@ -562,8 +562,9 @@ struct FPkg {
     uint32_t cw;
     uint32_t steps, scat;   // scat is also the index of the current flight segment
     int src;                // point source index, -1 = background or beam
-    int anc1, anc2, anc3;   // hierarchy: ids of the ancestors of the current cell on levels 1-3 (the package's own path,
-                            // kept so that climbing to the common parent needs no reverse-link loads while level <= 4)
+    int anc1, anc2, anc3;   // hierarchy: ids of the parent, grandparent and great-grandparent of the current cell (the
+                            // package's own path down, shifted on every descent / climb; -1 = not known), so that
+                            // climbing to the common parent loads no reverse links for the last three levels descended
     int disp;               // hot-cell tracking: packed (dx + R) | (dy + R) << 8 | (dz + R) << 16 relative to the
                             // source cell while the package is inside the cached cube, else -1
     long long id;
@@ -601,8 +602,7 @@ __device__ __forceinline__ bool fast_descend(const FastParams &P, FPkg &p)
         if (p.fx >= 0.5f) { slot |= 1; p.fx = 2.0f * p.fx - 1.0f; } else p.fx = 2.0f * p.fx;
         if (p.fy >= 0.5f) { slot |= 2; p.fy = 2.0f * p.fy - 1.0f; } else p.fy = 2.0f * p.fy;
         if (p.fz >= 0.5f) { slot |= 4; p.fz = 2.0f * p.fz - 1.0f; } else p.fz = 2.0f * p.fz;
-        const int lev = 128 - (__float_as_int(p.h) >> 23);      // level of the cell being left: h = 2^-(lev-1)
-        if (lev == 1) p.anc1 = p.rel; else if (lev == 2) p.anc2 = p.rel; else if (lev == 3) p.anc3 = p.rel;
+        p.anc3 = p.anc2; p.anc2 = p.anc1; p.anc1 = p.rel;       // the cell being left becomes the parent
         p.rel = (int)(cw & 0x7fffffffu) + slot;
         p.h *= 0.5f;
         cw = __ldg(P.cellw + p.rel);
@@ -702,7 +702,7 @@ __device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, long lon
     fast_emit_core(P, p, id, ix, iy, iz, dx, dy, dz);
     p.h = 1.0f;
     p.rel = root_id(P, ix, iy, iz);
-    if (HIER) fast_descend(P, p);
+    if (HIER) { p.anc1 = p.anc2 = p.anc3 = -1; fast_descend(P, p); }
     else p.cw = __ldg(P.cellw + p.rel);
     // hot-cell tracking starts at the centre of the cube of the package's own source (regular grids only)
     p.disp = (!HIER && p.src >= 0 && P.hot_r >= 0) ? P.hot_r * 0x010101 : -1;
@@ -745,7 +745,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
     unsigned acc_scat = 0, acc_term = 0;
     FPkg p;
     p.src = -1; p.disp = -1; p.w = 0.0f; p.absrel = 0.0f; p.steps = 0; p.scat = 0; p.cw = 0; p.rel = 0; p.h = 1.0f;
-    p.anc1 = p.anc2 = p.anc3 = 0;
+    p.anc1 = p.anc2 = p.anc3 = -1;
     int need = EMPTY;
     // hot-cell cache (atomics to the cells around a point source serialise): fp32 partial sums
     // of the deposits (in units of the source's package energy) into the (2R+1)^3 root cells around each source
@@ -912,8 +912,8 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                         p.fx = (p.fx + (float)(rel & 1)) * 0.5f;
                         p.fy = (p.fy + (float)((rel >> 1) & 1)) * 0.5f;
                         p.fz = (p.fz + (float)((rel >> 2) & 1)) * 0.5f;
-                        const int lev = 128 - (__float_as_int(p.h) >> 23);
-                        rel = lev == 2 ? p.anc1 : (lev == 3 ? p.anc2 : (lev == 4 ? p.anc3 : __ldg(P.parent + ((rel - P.nrp) >> 3))));
+                        rel = p.anc1 >= 0 ? p.anc1 : __ldg(P.parent + ((rel - P.nrp) >> 3));
+                        p.anc1 = p.anc2; p.anc2 = p.anc3; p.anc3 = -1;
                         p.h *= 2.0f;
                         inside = fwd == ((rel & abit) == 0);
                     }
