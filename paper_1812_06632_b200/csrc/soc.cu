@@ -13,7 +13,6 @@
 #include <cstring>
 #include <new>
 #include <string>
-#include <thread>
 #include <vector>
 
 // ------------------------------------------------------------------------------------------------
@@ -1389,6 +1388,30 @@ __global__ void __launch_bounds__(256) temperature_kernel(const __grid_constant_
     }
 }
 
+// regular grid, every cell a leaf: density -> cell word in place (-0 -> +0, sign bit clear), validity flag and sum of
+// the densities (soc_grid_create of large regular grids; small and hierarchical grids are converted on the host)
+__global__ void __launch_bounds__(256) leafwords_kernel(uint32_t *cellw, long long n, double *sum_out, int *bad_out)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double sum = 0.0;
+    int bad = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const float r = __uint_as_float(cellw[i]);
+        if (!(r >= 0.0f) || isinf(r)) bad = 1;
+        cellw[i] = __float_as_uint(r + 0.0f) & 0x7fffffffu;
+        sum += (double)r;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sum += __shfl_xor_sync(kFull, sum, o);
+        bad |= __shfl_xor_sync(kFull, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(sum_out, sum);
+        if (bad) atomicOr(bad_out, 1);
+    }
+}
+
 // ABI-order cell words -> internal layout (ghost-padded 2x2x2 bricks of the root grid, then the octet levels with
 // their links shifted behind the padded root grid); runs once per soc_grid_create
 __global__ void __launch_bounds__(256) repad_kernel(const uint32_t *cellw, uint32_t *ci, int nx, int ny, int nz, int nbx,
@@ -1807,42 +1830,13 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     std::vector<uint32_t> cellw;
     std::vector<int32_t> parent;
     try {
-        cellw.resize((size_t)G->n_total);
+        if (d->child || G->n_total < (1ll << 20)) cellw.resize((size_t)G->n_total);
         parent.assign((size_t)(G->n_octets > 0 ? G->n_octets : 1), INT32_MIN);
     } catch (const std::bad_alloc &) {
         return fail(SOC_ENOMEM, "out of host memory");
     }
-    bool words_done = false;
-    if (!d->child && G->n_total >= (1ll << 20)) {
-        // regular grid: every cell is a leaf, the words are independent -- validate and convert on all host cores
-        const unsigned hw = std::thread::hardware_concurrency();
-        const int nt = (int)(hw < 1 ? 1 : (hw > 32 ? 32 : hw));
-        std::vector<int> bad((size_t)nt, 0);
-        std::vector<double> sums((size_t)nt, 0.0);
-        std::vector<std::thread> pool;
-        for (int t = 0; t < nt; ++t)
-            pool.emplace_back([&, t]() {
-                const long long b = G->n_total * t / nt, e = G->n_total * (t + 1) / nt;
-                double sum = 0.0;
-                for (long long gid = b; gid < e; ++gid) {
-                    const float r = d->density[gid];
-                    if (!(r >= 0.0f) || !std::isfinite(r)) { bad[(size_t)t] = 1; return; }
-                    float rp = r + 0.0f;
-                    uint32_t bits;
-                    std::memcpy(&bits, &rp, 4);
-                    cellw[(size_t)gid] = bits & 0x7fffffffu;
-                    sum += (double)r;
-                }
-                sums[(size_t)t] = sum;
-            });
-        for (std::thread &th : pool) th.join();
-        for (int t = 0; t < nt; ++t)
-            if (bad[(size_t)t]) return fail(SOC_EINVAL, "leaf density must be finite and >= 0");
-        double sum = 0.0;
-        for (double v : sums) sum += v;
-        G->rho_mean = sum / (double)G->n_total;
-        words_done = true;
-    }
+    // large regular grids: every cell is a leaf, the words are converted and validated on the GPU (leafwords_kernel)
+    const bool words_done = !d->child && G->n_total >= (1ll << 20);
     for (int l = 0; l < d->n_levels && !words_done; ++l) {
         for (long long c = 0; c < d->n_cells[l]; ++c) {
             const long long gid = G->level_off[l] + c;
@@ -1879,7 +1873,24 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     SOC_CUDA(cudaMalloc(&G->d_cellw, sizeof(uint32_t) * (size_t)G->n_total));
     SOC_CUDA(cudaMalloc(&G->d_parent, sizeof(int32_t) * parent.size()));
     SOC_CUDA(cudaMalloc(&G->d_table, sizeof(float) * 8192));
-    SOC_CUDA(cudaMemcpy(G->d_cellw, cellw.data(), sizeof(uint32_t) * (size_t)G->n_total, cudaMemcpyHostToDevice));
+    if (words_done) {
+        double *d_sum = nullptr;
+        SOC_CUDA(cudaMalloc(&d_sum, 16));
+        SOC_CUDA(cudaMemset(d_sum, 0, 16));
+        SOC_CUDA(cudaMemcpy(G->d_cellw, d->density, sizeof(float) * (size_t)G->n_total, cudaMemcpyHostToDevice));
+        leafwords_kernel<<<G->n_sm * 8, 256>>>(G->d_cellw, G->n_total, d_sum, reinterpret_cast<int *>(d_sum + 1));
+        g_launches += 1;
+        double h_sum[2] = {0.0, 0.0};
+        cudaError_t e = cudaMemcpy(h_sum, d_sum, 16, cudaMemcpyDeviceToHost);
+        cudaFree(d_sum);
+        if (e != cudaSuccess) return fail(SOC_ECUDA, std::string("leafwords_kernel: ") + cudaGetErrorString(e));
+        int bad = 0;
+        std::memcpy(&bad, &h_sum[1], sizeof(int));
+        if (bad) return fail(SOC_EINVAL, "leaf density must be finite and >= 0");
+        G->rho_mean = h_sum[0] / (double)G->n_total;
+    } else {
+        SOC_CUDA(cudaMemcpy(G->d_cellw, cellw.data(), sizeof(uint32_t) * (size_t)G->n_total, cudaMemcpyHostToDevice));
+    }
     SOC_CUDA(cudaMemcpy(G->d_parent, parent.data(), sizeof(int32_t) * parent.size(), cudaMemcpyHostToDevice));
     // internal layout: root grid in 2x2x2 bricks with ghost cells around it (they hold the sentinel; cell ix
     // sits at X = ix + 2, so the low side has a whole ghost brick and the high side at least one ghost cell),

@@ -481,6 +481,12 @@ def test_bad_arguments_are_rejected():
     bad = P.rho.copy(); bad[3] = np.nan
     with pytest.raises(soc.SocError):
         soc.Grid(4, 4, 4, [64], bad, None, P.freq_hz, P.kabs, P.ksca, P.g)
+    big = np.ones(104 ** 3, dtype=np.float32); big[777_777] = -1.0        # large regular grids are validated on the GPU
+    with pytest.raises(soc.SocError, match="density"):
+        soc.Grid(104, 104, 104, [104 ** 3], big, None, P.freq_hz, P.kabs, P.ksca, P.g)
+    big[777_777] = np.inf
+    with pytest.raises(soc.SocError, match="density"):
+        soc.Grid(104, 104, 104, [104 ** 3], big, None, P.freq_hz, P.kabs, P.ksca, P.g)
     n_cells, rho, child = random_octree((2, 2, 2), 2, 0.5, seed=1)
     c2 = child.copy(); c2[np.argmax(child >= 0)] += 4
     with pytest.raises(soc.SocError):
