@@ -223,6 +223,50 @@ def test_production_optically_thin_deposits(kernel):
     assert abs(r["emitted"] - r["absorbed"] - r["escaped"]) <= 1e-6 * r["emitted"]
 
 
+# ----------------------------------------------------------------------------------------- closed forms, production kernels
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_gpu_point_source_in_uniform_absorber(kernel):
+    """Pin P5 on the GPU in production mode: escape fraction = <exp(-kappa rho d(Omega))> over directions (direct
+    quadrature of the distance to the cube surface); energy absorbed inside radius R = 1 - exp(-kappa rho R).
+    All packages start in one cell: the shared partial sums of the hot-cell cache carry the inner cells."""
+    N, kr, n = 21, 0.1, 400_000
+    P = _problem_from_arrays((N, N, N), [N ** 3], np.ones(N ** 3), None, kr, 0.0, 0.0, n)
+    src = dict(ps_pos=np.array([[N / 2, N / 2, N / 2]]), ps_lum=np.array([1.0]))
+    G = soc.Grid.from_problem(P)
+    G.set_option("kernel", kernel)
+    A, res, _ = gpu_packages(G, P, 0, src, n, 2, flags=PROD, want_replay=False)
+    G.close()
+    mu = (np.arange(2000) + 0.5) / 2000 * 2 - 1
+    ph = (np.arange(4000) + 0.5) / 4000 * 2 * np.pi
+    st = np.sqrt(1 - mu ** 2)[:, None]
+    comp = np.stack([st * np.cos(ph)[None, :], st * np.sin(ph)[None, :], np.broadcast_to(mu[:, None], (2000, 4000))])
+    w = np.exp(-kr * (N / 2) / np.abs(comp).max(axis=0))
+    assert res["escaped"] == pytest.approx(w.mean(), abs=5 * w.std() / n ** 0.5)
+    c = np.arange(N) + 0.5 - N / 2
+    zz, yy, xx = np.meshgrid(c, c, c, indexing="ij")
+    rmin = np.sqrt(np.maximum(np.abs(xx) - 0.5, 0) ** 2 + np.maximum(np.abs(yy) - 0.5, 0) ** 2 + np.maximum(np.abs(zz) - 0.5, 0) ** 2)
+    rmax = np.sqrt((np.abs(xx) + 0.5) ** 2 + (np.abs(yy) + 0.5) ** 2 + (np.abs(zz) + 0.5) ** 2)
+    A3 = A.reshape(N, N, N)
+    for R in (2.0, 4.0, 8.0):
+        exact = 1 - math.exp(-kr * R)
+        assert A3[rmax <= R].sum() <= exact * 1.002 and A3[rmin < R].sum() >= exact * 0.998
+    assert abs(res["emitted"] - res["absorbed"] - res["escaped"]) <= 1e-6 * res["emitted"]
+
+
+def test_gpu_noise_scales_as_inverse_sqrt_n():
+    """PAPER.md:125 on the GPU: the rms difference between two seeds falls as n^-1/2."""
+    P = inputs.make_config("2", n=16, n_packages=1)
+    G = soc.Grid.from_problem(P)
+    src = P.sources(0)
+
+    def rms(n):
+        a = [gpu_packages(G, P, 0, src, n, s, flags=PROD, want_replay=False)[0] for s in (1, 2)]
+        return np.sqrt(np.mean((a[0] - a[1]) ** 2))
+    r1, r2 = rms(20_000), rms(320_000)
+    G.close()
+    assert r1 / r2 == pytest.approx(4.0, rel=0.15)
+
+
 # ----------------------------------------------------------------------------------------- production kernels at full size
 def test_production_kernels_walk_the_same_paths():
     """photon_fast_kernel and photon_q_kernel evaluate the same fp32 arithmetic: identical cell-step, scattering and
