@@ -145,7 +145,7 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
 
 /* Tuning knobs (all have defaults chosen for B200): "blocks_per_sm", "threads", "refill_threshold" (replay
  * kernel), "service_threshold" (parked lanes that trigger a service pass), "hot_cache" (0/1: shared partial sums
- * for the cells around point sources), "acc32" (0/1: fp32 per-launch accumulator), "kernel" (production kernel on
+ * for the cells around point sources), "acc32" (0/1: fp32 per-launch accumulator), "overlap" (0/1: soc_simulate_spectrum overlaps consecutive frequencies on two streams), "kernel" (production kernel on
  * regular grids: 0 = chosen by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel), "carveout"
  * (preferred shared-memory carve-out in %, -1 = driver default), "debug" (measurement only); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
@@ -154,7 +154,9 @@ int soc_set_option(soc_grid *grid, const char *key, int64_t value);
 
 /* With option "timing" = 1: ms[i] = device time of the photon kernel last launched into result slot i
  * (slot = frequency index for soc_simulate_spectrum, 0 for the single-frequency calls); -1 where no launch
- * was recorded.  Waits for those launches to finish.  ms: HOST, n floats. */
+ * was recorded.  soc_simulate_spectrum overlaps consecutive frequencies on two streams (option "overlap", default 1):
+ * there ms[i], i > 0, is the advance of the completion front, end of launch i - end of launch i-1, so that the sum
+ * is the span from the first start to the last end.  Waits for those launches to finish.  ms: HOST, n floats. */
 int soc_get_timings(soc_grid *grid, int32_t n, float *ms);
 
 /* Roofline probes: random 4-byte gathers (kind 0), random fp64 red.global.add (kind 1),

@@ -92,6 +92,15 @@ struct soc_grid {
     int32_t *d_parent_int = nullptr;
     double *d_acc = nullptr;                  // [n_int], zero between calls
     float *d_acc32 = nullptr;                 // [n_int], zero between calls (fp32 internal accumulator)
+    // soc_simulate_spectrum overlaps consecutive frequencies on two streams (the tail of one launch, where lanes run
+    // out of packages, is filled by the next): a second set of accumulators and the stream / events that order them
+    float *d_acc32_b = nullptr;
+    double *d_acc_b = nullptr;
+    int acc_sel = 0;                          // accumulator set the next launch uses
+    int overlap_active = 0, last_overlap = 0, opt_overlap = 1;
+    cudaStream_t aux = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_unpad[2] = {nullptr, nullptr};
+    cudaEvent_t unpad_wait = nullptr;         // the next fold into the caller's array waits for this one
     int opt_acc32 = 1;
     int n_slots = 0;
     int device = 0, n_sm = 0;
@@ -1542,7 +1551,8 @@ template <typename R, bool HIER, bool REPLAY> int launch_photon(soc_grid *G, con
 int launch_unpad(soc_grid *G, bool acc32, double weight, double *absorbed, cudaStream_t st)
 {
     UnpadParams U;
-    U.out = absorbed; U.acc = G->d_acc; U.acc32 = G->d_acc32; U.weight = weight;
+    U.out = absorbed; U.acc = G->acc_sel ? G->d_acc_b : G->d_acc; U.acc32 = G->acc_sel ? G->d_acc32_b : G->d_acc32; U.weight = weight;
+    if (G->unpad_wait) SOC_CUDA(cudaStreamWaitEvent(st, G->unpad_wait, 0));     // folds into the caller's array one at a time
     U.nx = G->nx; U.ny = G->ny; U.nbx = G->nbx; U.nby = G->nby; U.nrp = G->nrp;
     U.n_root = G->n_root; U.n_total = G->n_total;
     long long ub = (G->n_total + 255) / 256;
@@ -1552,6 +1562,10 @@ int launch_unpad(soc_grid *G, bool acc32, double weight, double *absorbed, cudaS
     else unpad_add_kernel<false><<<(int)ub, 256, 0, st>>>(U);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
+    if (G->overlap_active) {
+        SOC_CUDA(cudaEventRecord(G->ev_unpad[G->acc_sel], st));
+        G->unpad_wait = G->ev_unpad[G->acc_sel];
+    }
     return SOC_OK;
 }
 
@@ -1699,7 +1713,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         F.hot_r = -1;
         if (!hier && P.n_point > 0 && !P.is_beam && G->opt_hot_cache)
             F.hot_r = (size_t)P.n_point * 343 * sizeof(float) <= 40 * 1024 ? 3 : 2;
-        F.acc = G->d_acc; F.replay = P.replay; F.counter = P.counter; F.result = P.result;
+        F.acc = G->acc_sel ? G->d_acc_b : G->d_acc; F.replay = P.replay; F.counter = P.counter; F.result = P.result;
         // fp32 internal accumulator: deposits in units of the largest package energy of
         // this launch; falls back to the fp64 accumulator when a source class would underflow in those units
         double e_ref = P.is_beam ? 1.0 : P.bg_e0;
@@ -1714,7 +1728,12 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
                 if (P.ps_e0[k] > 0.0 && F.ps_rel[k] < 1e-20f) acc32 = false;
             }
         }
-        F.acc32 = G->d_acc32;
+        F.acc32 = G->acc_sel ? G->d_acc32_b : G->d_acc32;
+        if (!acc32 && G->acc_sel && !G->d_acc_b) {           // fp64 fallback on the second stream: its own accumulator
+            SOC_CUDA(cudaMalloc(&G->d_acc_b, sizeof(double) * (size_t)G->n_int));
+            SOC_CUDA(cudaMemset(G->d_acc_b, 0, sizeof(double) * (size_t)G->n_int));
+            F.acc = G->d_acc_b;
+        }
         const double w_eff = acc32 ? weight * e_ref : weight;
         // photon_q_kernel trades instructions for L2 requests: it wins where the working set (cell words + fp32
         // accumulator, 8 B per cell) does not stay in L2 (B200: 19.1 vs 20.2 ms per frequency on config 5) and loses
@@ -1784,6 +1803,12 @@ void soc_grid_destroy(soc_grid *G)
     cudaFree(G->d_cellw); cudaFree(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
     cudaFree(G->d_table); cudaFree(G->d_cellw_int); cudaFree(G->d_parent_int); cudaFree(G->d_acc); cudaFree(G->d_acc32);
     if (G->h_results) cudaFreeHost(G->h_results);
+    cudaFree(G->d_acc32_b); cudaFree(G->d_acc_b);
+    if (G->aux) cudaStreamDestroy(G->aux);
+    if (G->ev_fork) cudaEventDestroy(G->ev_fork);
+    if (G->ev_join) cudaEventDestroy(G->ev_join);
+    if (G->ev_unpad[0]) cudaEventDestroy(G->ev_unpad[0]);
+    if (G->ev_unpad[1]) cudaEventDestroy(G->ev_unpad[1]);
     for (cudaEvent_t e : G->ev0) cudaEventDestroy(e);
     for (cudaEvent_t e : G->ev1) cudaEventDestroy(e);
     delete G;
@@ -1953,6 +1978,7 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     else if (k == "debug" && value >= 0 && value <= 255) G->opt_debug = (int)value;
     else if (k == "hot_cache" && (value == 0 || value == 1)) G->opt_hot_cache = (int)value;
     else if (k == "kernel" && value >= 0 && value <= 2) G->opt_kernel = (int)value;
+    else if (k == "overlap" && (value == 0 || value == 1)) G->opt_overlap = (int)value;
     else if (k == "carveout" && value >= -1 && value <= 100) G->opt_carveout = (int)value;
     else if (k == "acc32" && (value == 0 || value == 1)) G->opt_acc32 = (int)value;
     else return fail(SOC_EINVAL, "unknown option or value out of range: " + k);
@@ -1966,7 +1992,14 @@ int soc_get_timings(soc_grid *G, int32_t n, float *ms)
         ms[i] = -1.0f;
         if (i < (int)G->ev_set.size() && G->ev_set[i]) {
             SOC_CUDA(cudaEventSynchronize(G->ev1[i]));
-            SOC_CUDA(cudaEventElapsedTime(&ms[i], G->ev0[i], G->ev1[i]));
+            if (G->last_overlap && i > 0 && G->ev_set[i - 1]) {
+                // overlapped launches: the time attributed to launch i is the advance of the completion front, so that the
+                // sum over the launches is the span from the first start to the last end
+                SOC_CUDA(cudaEventElapsedTime(&ms[i], G->ev1[i - 1], G->ev1[i]));
+                if (ms[i] < 0.0f) ms[i] = 0.0f;
+            } else {
+                SOC_CUDA(cudaEventElapsedTime(&ms[i], G->ev0[i], G->ev1[i]));
+            }
         }
     }
     return SOC_OK;
@@ -1977,6 +2010,7 @@ int soc_simulate_packages(soc_grid *G, int32_t ifreq, const soc_sources *src, in
                           soc_replay_record *replay, soc_freq_result *res, uint32_t flags, void *stream)
 {
     cudaStream_t st = (cudaStream_t)stream;
+    if (G) G->last_overlap = 0;
     int rc = enqueue_frequency(G, ifreq, src, n_packages, seed, weight, pkg_begin, pkg_count, absorbed, replay,
                                flags, 0, st);
     if (rc != SOC_OK) return rc;
@@ -2001,11 +2035,37 @@ int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_package
     trapezoid(G->freq, w);
     int rc = ensure_slots(G, G->n_freq);
     if (rc != SOC_OK) return rc;
-    for (int f = 0; f < G->n_freq; ++f) {
-        rc = enqueue_frequency(G, f, src + f, n_packages, seed, w[f], pkg_begin, pkg_count, absorbed_int, nullptr,
-                               flags, f, st);
-        if (rc != SOC_OK) return rc;
+    // production mode: odd frequencies go to a second stream with their own accumulators, so that the tail of one launch
+    // (lanes that have run out of packages) is filled by the blocks of the next; the folds into absorbed_int stay ordered
+    const bool overlap = G->opt_overlap && G->n_freq > 1 && !(flags & SOC_GEOM_FP64);
+    if (overlap) {
+        if (!G->aux) {
+            SOC_CUDA(cudaStreamCreateWithFlags(&G->aux, cudaStreamNonBlocking));
+            SOC_CUDA(cudaEventCreateWithFlags(&G->ev_fork, cudaEventDisableTiming));
+            SOC_CUDA(cudaEventCreateWithFlags(&G->ev_join, cudaEventDisableTiming));
+            SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[0], cudaEventDisableTiming));
+            SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[1], cudaEventDisableTiming));
+            SOC_CUDA(cudaMalloc(&G->d_acc32_b, sizeof(float) * (size_t)G->n_int));
+            SOC_CUDA(cudaMemset(G->d_acc32_b, 0, sizeof(float) * (size_t)G->n_int));
+        }
+        SOC_CUDA(cudaEventRecord(G->ev_fork, st));
+        SOC_CUDA(cudaStreamWaitEvent(G->aux, G->ev_fork, 0));
+        G->unpad_wait = nullptr;
+        G->overlap_active = 1;
     }
+    for (int f = 0; f < G->n_freq && rc == SOC_OK; ++f) {
+        G->acc_sel = overlap ? (f & 1) : 0;
+        rc = enqueue_frequency(G, f, src + f, n_packages, seed, w[f], pkg_begin, pkg_count, absorbed_int, nullptr,
+                               flags, f, G->acc_sel ? G->aux : st);
+    }
+    G->acc_sel = 0; G->overlap_active = 0; G->unpad_wait = nullptr;
+    G->last_overlap = overlap ? 1 : 0;
+    if (overlap) {
+        cudaError_t e = cudaEventRecord(G->ev_join, G->aux);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, G->ev_join, 0);
+        if (e != cudaSuccess && rc == SOC_OK) rc = fail(SOC_ECUDA, cudaGetErrorString(e));
+    }
+    if (rc != SOC_OK) return rc;
     if (results) return fetch_results(G, G->n_freq, results, st);
     return SOC_OK;
 }
