@@ -418,6 +418,27 @@ def test_spectrum_and_temperatures_match_oracle():
     G.close()
 
 
+@pytest.mark.parametrize("which,kw", [("3", dict(n=32, n_packages=60_000, n_freq=9)), ("4p", dict(n=8, n_packages=40_000, n_freq=5))])
+def test_spectrum_overlap_equals_serial(which, kw):
+    """soc_simulate_spectrum overlaps consecutive frequencies on two streams with two internal accumulators: same
+    per-frequency counters as the serial order, same frequency integral up to the order of the additions."""
+    torch = _torch()
+    P = inputs.make_config(which, **kw)
+    G = soc.Grid.from_problem(P)
+    srcs = [P.sources(f) for f in range(P.n_freq)]
+    out = []
+    for overlap in (1, 0, 1):
+        G.set_option("overlap", overlap)
+        A = torch.full((P.n_total,), 0.5, dtype=torch.float64, device="cuda")
+        res = G.simulate_spectrum(srcs, P.n_packages, P.seed, A)
+        out.append((A.cpu().numpy(), res))
+    G.close()
+    for A, res in out[1:]:
+        assert [(r.cell_steps, r.scatterings, r.terminated) for r in res] == [(r.cell_steps, r.scatterings, r.terminated) for r in out[0][1]]
+        assert np.allclose(A, out[0][0], rtol=2e-5, atol=0)
+    assert all(abs(r.emitted - r.absorbed - r.escaped) <= 1e-6 * r.emitted for r in out[0][1])
+
+
 @pytest.mark.parametrize("shape", [(3, 3, 3), (5, 4, 6)])
 def test_temperature_kernel_edge_cases(shape):
     """Ragged n_total (not a multiple of 4), parents, empty leaves, unhit cells, clamps at both table ends."""
