@@ -344,7 +344,7 @@ def run_ours(args):
 # (dram__bytes_read.sum + dram__bytes_write.sum, mean over the captured launches); None = not captured yet.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     "5": {"traffic": 54.81e9,
-          "traffic_source": "profiles/r01d_ncu_full_photon_q_config5.txt: dram__bytes_read.sum 40.46 GB + "
+          "traffic_source": "profiles/r01e_ncu_full_photon_q_config5.txt: dram__bytes_read.sum 40.46 GB + "
                             "dram__bytes_write.sum 14.36 GB, mean of launches 65-67 (frequency indices 64-66)",
           "binding_unit": "latency of dependent gathers at 62 % occupancy, not bytes: lts__t_tag_requests 60 %, l1tex2xbar 54 %, "
                           "issue slots 64 %, DRAM 38 % busy (same capture); see DESIGN.md 6.1"},
