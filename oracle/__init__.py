@@ -70,6 +70,8 @@ def lib():
                                           C.c_int64, C.c_int64, C.c_void_p, C.POINTER(_Result),
                                           C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         L.soc_oracle_simulate.restype = C.c_int
+        L.soc_oracle_simulate_f32state.argtypes = L.soc_oracle_simulate.argtypes
+        L.soc_oracle_simulate_f32state.restype = C.c_int
         L.soc_oracle_trapezoid_weights.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
         L.soc_oracle_update_temperatures.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p,
                                                      C.c_int32, C.c_double, C.c_double, C.c_void_p]
@@ -204,12 +206,16 @@ def _sources_struct(src, keep):
 
 
 def simulate(grid: Grid, kabs, ksca, g, ifreq, sources: dict, n_packages, seed, weight=1.0,
-             pkg_begin=0, pkg_count=None, absorbed=None, want_replay=False, trace_cap=0, threads=1):
+             pkg_begin=0, pkg_count=None, absorbed=None, want_replay=False, trace_cap=0, threads=1,
+             f32state=False):
     """Run packages [pkg_begin, pkg_begin+pkg_count).  Returns (absorbed, Result, replay, trace).
 
     sources: dict(bg_intensity=, ps_pos=, ps_lum=, n_bg=, beam=).  `absorbed` is accumulated into.
+    f32state=False: soc_oracle_simulate, THE oracle (fp64 throughout).  f32state=True: the named variant
+    soc_oracle_simulate_f32state (state snapped to fp32 at every store; replay-parity tests only).
     """
     L = lib()
+    entry = L.soc_oracle_simulate_f32state if f32state else L.soc_oracle_simulate
     if pkg_count is None:
         pkg_count = n_packages - pkg_begin
     if absorbed is None:
@@ -223,9 +229,9 @@ def simulate(grid: Grid, kabs, ksca, g, ifreq, sources: dict, n_packages, seed, 
     def run(b, n, acc, rep, trc):
         r = _Result()
         nt = C.c_int64(0)
-        rc = L.soc_oracle_simulate(grid._h, float(kabs), float(ksca), float(g), int(ifreq), C.byref(s),
-                                   int(n_packages), int(seed), float(weight), int(b), int(n), _p(acc),
-                                   C.byref(r), _p(rep), _p(trc), 0 if trc is None else len(trc), C.byref(nt))
+        rc = entry(grid._h, float(kabs), float(ksca), float(g), int(ifreq), C.byref(s),
+                   int(n_packages), int(seed), float(weight), int(b), int(n), _p(acc),
+                   C.byref(r), _p(rep), _p(trc), 0 if trc is None else len(trc), C.byref(nt))
         if rc != 0:
             raise ValueError("soc_oracle_simulate: bad argument")
         return r, nt.value

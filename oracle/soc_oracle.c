@@ -24,15 +24,21 @@
  * termination, quadrature, table form) follows the readings S1-S16 listed in DESIGN.md
  * (taken from SURVEY.md 8c and BASELINE.json:north_star).
  *
- * Precision (reading S11; north_star "fp32 positions / fp64 accumulators", "one floating
- * point number per cell", PAPER.md:367 single precision): the package STATE -- in-cell position,
- * direction, remaining optical depth of the flight segment -- is held in fp32; every update is
- * evaluated in fp64 from that state and rounded once to fp32 when stored.  Weights, deposits and
- * accumulators are fp64.  The walk through a cloud with sharp density contrasts amplifies
- * perturbations of the state (a lateral shift changes chord lengths in dense cells, hence where the
- * next scattering falls in a thin one); snapping the state to fp32 after each update keeps two
- * independent fp64 evaluations on the same trajectory, which is what makes package-by-package replay
- * against the CUDA path meaningful.
+ * Precision (reading S11; north_star "a plain, slow fp64 CPU implementation", SURVEY.md 8c S11 "oracle
+ * fp64 throughout"): soc_oracle_simulate -- THE oracle -- holds and evaluates everything in fp64.
+ *
+ * soc_oracle_simulate_f32state is a second, named entry over the same walk (the same lines of code; the
+ * only difference is keep() below): in-cell position, direction and remaining optical depth are rounded
+ * to fp32 each time they are stored, every update still being evaluated in fp64.  Why it exists: the walk
+ * through a cloud with sharp density contrasts is a chaotic map where packages scatter many times (a
+ * lateral shift changes the chord lengths in dense cells, hence where the next scattering falls), so two
+ * correct fp64 evaluations that differ in the last bit of a log or a sincos part ways on some packages;
+ * on a state snapped to the fp32 lattice they stay together, which is what package-by-package replay of
+ * the CUDA path needs at the UV frequencies of configs 3 and 5.  Its licence: tests/test_oracle_pins.py
+ * pins it to the fp64 oracle (identical records on non-scattering paths, >= 99 % identical records on
+ * config-1/2-like runs, per-cell agreement within 5 sigma of the MC noise over 8 seeds, the same closed
+ * forms), and tests/test_gpu_parity.py measures the fp64-state replay match it replaces.  Only the
+ * replay-parity tests use it.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known answers, slab transmission
  * exp(-tau), optically thin bath A = 4 pi I kabs rho V, energy conservation 1e-9,
@@ -193,9 +199,14 @@ soc_oracle_grid *soc_oracle_grid_create(int32_t nx, int32_t ny, int32_t nz, int3
 typedef struct {
     int32_t level;      /* l = 1..n_levels */
     int32_t cell;       /* index within the level: authoritative, never re-derived (S4) */
-    float f[3];         /* position inside the cell, in units of the cell edge, [0,1]^3 (fp32 state, S11) */
-    float d[3];         /* direction, unit length up to fp32 rounding */
+    double f[3];        /* position inside the cell, in units of the cell edge, [0,1]^3 */
+    double d[3];        /* unit direction */
+    int32_t f32state;   /* 0: the oracle (fp64 throughout); 1: soc_oracle_simulate_f32state, see keep() */
 } soc_oracle_state;
+
+/* The value of x as the package state stores it: x itself in the oracle; rounded to fp32 in the
+ * f32state variant (header, "Precision").  Everything else is common to both. */
+static double keep(double x, int32_t f32state) { return f32state ? (double)(float)x : x; }
 
 typedef struct {
     double bg_intensity;   /* I_nu of the isotropic background, 0 = none */
@@ -251,8 +262,8 @@ static void descend(const soc_oracle_grid *G, soc_oracle_state *S)
         if (ch < 0) return;
         int32_t slot = 0;
         for (int j = 0; j < 3; ++j) {
-            if (S->f[j] >= 0.5f) { slot |= (1 << j); S->f[j] = (float)(2.0 * (double)S->f[j] - 1.0); }
-            else S->f[j] = (float)(2.0 * (double)S->f[j]);
+            if (S->f[j] >= 0.5) { slot |= (1 << j); S->f[j] = 2.0 * S->f[j] - 1.0; }   /* exact, also in fp32 */
+            else S->f[j] = 2.0 * S->f[j];
         }
         S->cell = ch + slot;
         S->level += 1;
@@ -274,11 +285,11 @@ static int move_across(const soc_oracle_grid *G, soc_oracle_state *S, int a, int
         }
         int bit = (S->cell >> a) & 1;
         if ((sg > 0 && bit == 0) || (sg < 0 && bit == 1)) { S->cell ^= (1 << a); break; }
-        for (int j = 0; j < 3; ++j) S->f[j] = (float)(((double)S->f[j] + (double)((S->cell >> j) & 1)) * 0.5);
+        for (int j = 0; j < 3; ++j) S->f[j] = keep((S->f[j] + (double)((S->cell >> j) & 1)) * 0.5, S->f32state);
         S->cell = G->parent[S->level - 1][S->cell >> 3];
         S->level -= 1;
     }
-    S->f[a] = (sg > 0) ? 0.0f : 1.0f; /* entry face, in the neighbour's frame */
+    S->f[a] = (sg > 0) ? 0.0 : 1.0;   /* entry face, in the neighbour's frame */
     descend(G, S);
     return 1;
 }
@@ -335,11 +346,11 @@ void soc_oracle_emit_point(const double pos[3], const double u[2],
  * frequency index ifreq.  absorbed[gid] += weight * (energy absorbed in the cell).
  * replay (may be NULL): pkg_count records.  trace (may be NULL): up to trace_cap steps,
  * *n_trace receives the number written.  Returns 0, or -1 on a bad argument. */
-int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, double g, int32_t ifreq,
-                        const soc_oracle_sources *src, int64_t n_packages, uint64_t seed, double weight,
-                        int64_t pkg_begin, int64_t pkg_count, double *absorbed,
-                        soc_oracle_result *res, soc_oracle_replay *replay,
-                        soc_oracle_trace *trace, int64_t trace_cap, int64_t *n_trace)
+static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g, int32_t ifreq,
+                    const soc_oracle_sources *src, int64_t n_packages, uint64_t seed, double weight,
+                    int64_t pkg_begin, int64_t pkg_count, double *absorbed,
+                    soc_oracle_result *res, soc_oracle_replay *replay,
+                    soc_oracle_trace *trace, int64_t trace_cap, int64_t *n_trace, int32_t f32state)
 {
     if (!G || !src || !absorbed || n_packages < 0 || pkg_begin < 0 || pkg_count < 0 ||
         pkg_begin + pkg_count > n_packages || !(kabs >= 0.0) || !(ksca >= 0.0) || !(fabs(g) < 1.0))
@@ -388,7 +399,8 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
             soc_oracle_emit_point(src->ps_pos + 3 * k, u, ijk, f0, d0);
             E0 = src->ps_lum[k] / (double)count_k;
         }
-        for (int j = 0; j < 3; ++j) { S.f[j] = (float)f0[j]; S.d[j] = (float)d0[j]; }   /* fp32 state */
+        S.f32state = f32state;
+        for (int j = 0; j < 3; ++j) { S.f[j] = keep(f0[j], f32state); S.d[j] = keep(d0[j], f32state); }
         S.level = 1;
         S.cell = ijk[0] + G->nx * (ijk[1] + G->ny * ijk[2]);
         descend(G, &S);
@@ -400,8 +412,8 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
         double e_esc = 0.0;
         uint32_t ws[4];
         soc_oracle_stream_block(seed, ifreq, p, 2u + seg, ws);
-        float tau_drawn = (float)(-log(soc_oracle_uniform(ws[0])));   /* a4: free path, scattering depth */
-        float tau_rem = tau_drawn;
+        double tau_drawn = keep(-log(soc_oracle_uniform(ws[0])), f32state);   /* a4: free path, scattering depth */
+        double tau_rem = tau_drawn;
 
         for (;;) {
             const int64_t gid = G->level_off[S.level - 1] + S.cell;
@@ -410,7 +422,7 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
             /* a5/a6: distance (in cell edges) to the face of each axis */
             double t[3];
             for (int j = 0; j < 3; ++j) {
-                const double fj = (double)S.f[j], dj = (double)S.d[j];
+                const double fj = S.f[j], dj = S.d[j];
                 if (dj > 0.0) t[j] = (1.0 - fj) / dj;
                 else if (dj < 0.0) t[j] = (-fj) / dj;
                 else t[j] = INFINITY;
@@ -425,9 +437,9 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
             const double dtau = ds * ks_rho;
             int scatter = 0;
             double ds_used = ds, t_used = tstar;
-            if (ks_rho > 0.0 && dtau >= (double)tau_rem) {
+            if (ks_rho > 0.0 && dtau >= tau_rem) {
                 scatter = 1;
-                ds_used = (double)tau_rem / ks_rho;
+                ds_used = tau_rem / ks_rho;
                 t_used = ds_used / h;
             }
             /* a7: path-length estimator, continuous absorption */
@@ -444,8 +456,8 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
                 double org[3];
                 cell_origin(G, S.level, S.cell, org);
                 T->pkg = p; T->gid = gid; T->level = S.level; T->kind = scatter ? 1 : 0;
-                for (int j = 0; j < 3; ++j) T->p0[j] = org[j] + h * (double)S.f[j];
-                T->ds = ds_used; T->tau_sca = ds_used * ks_rho; T->tau_drawn = (double)tau_drawn;
+                for (int j = 0; j < 3; ++j) T->p0[j] = org[j] + h * S.f[j];
+                T->ds = ds_used; T->tau_sca = ds_used * ks_rho; T->tau_drawn = tau_drawn;
             }
             /* a9: termination */
             if (E < SOC_O_WMIN * E0) {
@@ -453,34 +465,34 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
                 R.absorbed += E;
                 E = 0.0;
                 R.terminated += 1;
-                if (T) { T->kind = 2; for (int j = 0; j < 3; ++j) T->p1[j] = T->p0[j] + ds_used * (double)S.d[j]; }
+                if (T) { T->kind = 2; for (int j = 0; j < 3; ++j) T->p1[j] = T->p0[j] + ds_used * S.d[j]; }
                 break;
             }
             for (int j = 0; j < 3; ++j) {
-                double fn = (double)S.f[j] + t_used * (double)S.d[j];
+                double fn = S.f[j] + t_used * S.d[j];
                 if (fn < 0.0) fn = 0.0;
                 if (fn > 1.0) fn = 1.0;
-                S.f[j] = (float)fn;
+                S.f[j] = keep(fn, f32state);
             }
             if (T) {
                 double org[3];
                 cell_origin(G, S.level, S.cell, org);
-                for (int j = 0; j < 3; ++j) T->p1[j] = org[j] + h * (double)S.f[j];
+                for (int j = 0; j < 3; ++j) T->p1[j] = org[j] + h * S.f[j];
             }
             if (scatter) {
                 /* a8 */
                 double cost = soc_oracle_hg_cos(g, soc_oracle_uniform(ws[1]));
                 double phi = 2.0 * SOC_O_PI * soc_oracle_uniform(ws[2]);
-                double od[3] = { (double)S.d[0], (double)S.d[1], (double)S.d[2] }, nd[3];
-                soc_oracle_rotate(od, cost, phi, nd);
-                S.d[0] = (float)nd[0]; S.d[1] = (float)nd[1]; S.d[2] = (float)nd[2];
+                double nd[3];
+                soc_oracle_rotate(S.d, cost, phi, nd);
+                for (int j = 0; j < 3; ++j) S.d[j] = keep(nd[j], f32state);
                 seg += 1; scat += 1;
                 soc_oracle_stream_block(seed, ifreq, p, 2u + seg, ws);
-                tau_drawn = (float)(-log(soc_oracle_uniform(ws[0])));
+                tau_drawn = keep(-log(soc_oracle_uniform(ws[0])), f32state);
                 tau_rem = tau_drawn;
             } else {
-                tau_rem = (float)((double)tau_rem - dtau);
-                if (!move_across(G, &S, a, S.d[a] > 0.0f ? 1 : -1)) {
+                tau_rem = keep(tau_rem - dtau, f32state);
+                if (!move_across(G, &S, a, S.d[a] > 0.0 ? 1 : -1)) {
                     e_esc = E;                           /* a9: escape */
                     R.escaped += E;
                     if (T) T->kind = 3;
@@ -498,6 +510,29 @@ int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, doub
     if (res) *res = R;
     if (n_trace) *n_trace = nt;
     return 0;
+}
+
+/* THE oracle: fp64 throughout (north_star). */
+int soc_oracle_simulate(const soc_oracle_grid *G, double kabs, double ksca, double g, int32_t ifreq,
+                        const soc_oracle_sources *src, int64_t n_packages, uint64_t seed, double weight,
+                        int64_t pkg_begin, int64_t pkg_count, double *absorbed,
+                        soc_oracle_result *res, soc_oracle_replay *replay,
+                        soc_oracle_trace *trace, int64_t trace_cap, int64_t *n_trace)
+{
+    return simulate(G, kabs, ksca, g, ifreq, src, n_packages, seed, weight, pkg_begin, pkg_count, absorbed, res,
+                    replay, trace, trace_cap, n_trace, 0);
+}
+
+/* The same walk with the package state snapped to fp32 at every store (header, "Precision"): used by the
+ * replay-parity tests only, pinned to soc_oracle_simulate by tests/test_oracle_pins.py. */
+int soc_oracle_simulate_f32state(const soc_oracle_grid *G, double kabs, double ksca, double g, int32_t ifreq,
+                                 const soc_oracle_sources *src, int64_t n_packages, uint64_t seed, double weight,
+                                 int64_t pkg_begin, int64_t pkg_count, double *absorbed,
+                                 soc_oracle_result *res, soc_oracle_replay *replay,
+                                 soc_oracle_trace *trace, int64_t trace_cap, int64_t *n_trace)
+{
+    return simulate(G, kabs, ksca, g, ifreq, src, n_packages, seed, weight, pkg_begin, pkg_count, absorbed, res,
+                    replay, trace, trace_cap, n_trace, 1);
 }
 
 /* ------------------------------------------------------------------ a10 -------------

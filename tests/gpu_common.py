@@ -33,9 +33,12 @@ def gpu_packages(G, P, ifreq, sources, n_packages, seed, weight=1.0, pkg_begin=0
 
 
 def oracle_packages(og, P, ifreq, sources, n_packages, seed, weight=1.0, pkg_begin=0, pkg_count=None, want_replay=True,
-                    threads=N_THREADS):
+                    threads=N_THREADS, f32state=False):
+    """f32state=False: THE oracle (fp64 throughout) -- production-mode, closed-form and temperature comparisons.
+    f32state=True: the named variant with the package state snapped to fp32 (oracle/soc_oracle.c header), pinned to
+    the fp64 oracle by tests/test_oracle_pins.py -- package-by-package replay parity only."""
     A, res, rep, _ = oracle.simulate(og, P.kabs[ifreq], P.ksca[ifreq], P.g[ifreq], ifreq, sources, n_packages, seed, weight,
-                                     pkg_begin, pkg_count, want_replay=want_replay, threads=threads)
+                                     pkg_begin, pkg_count, want_replay=want_replay, threads=threads, f32state=f32state)
     return A, res, rep
 
 

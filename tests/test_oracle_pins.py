@@ -3,9 +3,10 @@
 Every test compares the oracle with something that is not the oracle: published known answers,
 closed forms, conservation laws, quadrature, or an independent geometric check.
 
-The oracle holds the package state (position in the cell, direction, remaining optical depth) in fp32 and
-evaluates every update in fp64 (reading S11), so pins that involve an oblique direction or an
-accumulated optical depth hold to a few fp32 ulps (F32 below), the axis-aligned ones to fp64 rounding.
+`oracle.simulate` is THE oracle: fp64 throughout (north_star), pinned here at fp64 tolerances.
+`oracle.simulate(..., f32state=True)` is the named variant whose package state is snapped to fp32 at every
+store (oracle/soc_oracle.c header, "Precision"); the tests at the end of this file pin it to the fp64 oracle,
+which is its only licence (F32 below = one fp32 ulp at 1).
 """
 import math
 import os
@@ -131,8 +132,8 @@ def test_oblique_beam_path_length():
     pos = np.array([0.0, 1.2, 4.4])
     A, res, _, tr = oracle.simulate(g, 0.2, 0.0, 0.0, 0, dict(beam=np.concatenate([pos, d])), 1, 1, trace_cap=100)
     tmax = min(((shape[j] if d[j] > 0 else 0) - pos[j]) / d[j] for j in range(3))
-    assert res.absorbed == pytest.approx(1 - math.exp(-0.2 * 1.5 * tmax), rel=4 * F32)
-    assert tr["ds"].sum() == pytest.approx(tmax, rel=4 * F32)
+    assert res.absorbed == pytest.approx(1 - math.exp(-0.2 * 1.5 * tmax), rel=1e-13)
+    assert tr["ds"].sum() == pytest.approx(tmax, rel=1e-13)
     for s in tr:   # each visited cell is the cell of the segment mid-point
         mid = 0.5 * (s["p0"] + s["p1"])
         ijk = np.floor(mid).astype(int)
@@ -332,7 +333,7 @@ def test_bruteforce_geometric_replay_on_tiny_octree(seed):
         tau_acc = 0.0
         for i, s in enumerate(steps):
             seglen = np.linalg.norm(s["p1"] - s["p0"])
-            assert seglen == pytest.approx(s["ds"], rel=2 * F32, abs=4 * F32)   # fp32 positions, |d| = 1 +- ulp
+            assert seglen == pytest.approx(s["ds"], abs=1e-12)
             if i > 0:                                    # contiguous path
                 assert np.allclose(steps[i - 1]["p1"], s["p0"], atol=1e-12)
             if seglen > 1e-9:                            # the mid-point lies in the leaf that was charged
@@ -343,10 +344,10 @@ def test_bruteforce_geometric_replay_on_tiny_octree(seed):
             assert s["tau_sca"] == pytest.approx(s["ds"] * float(rho[s["gid"]]) * ksca, rel=1e-12, abs=1e-300)
             tau_acc += s["tau_sca"]
             if s["kind"] == 1:                           # free path really has the drawn optical depth
-                assert tau_acc == pytest.approx(s["tau_drawn"], rel=F32 * (4 + len(steps)))
+                assert tau_acc == pytest.approx(s["tau_drawn"], rel=1e-9)
                 tau_acc = 0.0
             else:
-                assert tau_acc < s["tau_drawn"] * (1 + F32 * (4 + len(steps)))
+                assert tau_acc < s["tau_drawn"] * (1 + 1e-12)
         last = steps[-1]
         assert last["kind"] in (2, 3)
         if last["kind"] == 3:                            # escaped: ends on the outer boundary
@@ -378,16 +379,11 @@ def test_fully_refined_hierarchy_equals_regular_grid():
     # the regular grid's length unit is half a root cell: kappa halves, and I/4 keeps the package energy
     Ah, rh, reph, _ = oracle.simulate(gh, kabs, ksca, gg, 2, dict(bg_intensity=I), n, 5, want_replay=True)
     Ar, rr, repr_, _ = oracle.simulate(gr, kabs / 2, ksca / 2, gg, 2, dict(bg_intensity=I / 4), n, 5, want_replay=True)
-    # Only difference: going up one level rounds (f + bit)/2 to fp32, i.e. drops the last bit of the two
-    # non-crossing coordinates; the few packages that pass within an ulp of a cell edge may then take the
-    # corner cell in the other order (measured: 0.03 %).
     same = (reph["steps"] == repr_["steps"]) & (reph["scatters"] == repr_["scatters"])
-    assert same.mean() >= 0.999
+    assert same.mean() >= 0.9999
     assert rh.emitted == pytest.approx(rr.emitted, rel=1e-13)
-    assert rh.escaped == pytest.approx(rr.escaped, rel=1e-4)
-    Ahl = Ah[gid_of.ravel()]
-    assert np.abs(Ahl - Ar).sum() <= 1e-3 * Ar.sum()
-    assert np.median(np.abs(Ahl - Ar) / Ar) < 1e-6                  # the typical leaf agrees to fp32 rounding
+    assert rh.escaped == pytest.approx(rr.escaped, rel=1e-9)
+    assert np.allclose(Ah[gid_of.ravel()], Ar, rtol=1e-9, atol=1e-12 * Ar.max())
     assert Ah[: N ** 3].sum() == 0.0
 
 
@@ -545,24 +541,118 @@ def test_stream_layout_inside_the_walk():
         u = [oracle.uniform(x) for x in b0] + [oracle.uniform(b1[0])]
         ijk, f, d = oracle.emit_background(*shape, u)
         assert np.allclose(s[0]["p0"], ijk + f, atol=1e-14)
-        nz = s[s["ds"] > 1e-3]
-        assert np.allclose((nz[0]["p1"] - nz[0]["p0"]) / nz[0]["ds"], d, atol=1e-4)
+        nz = s[s["ds"] > 1e-9]
+        assert np.allclose((nz[0]["p1"] - nz[0]["p0"]) / nz[0]["ds"], d, atol=1e-9)
         seg = 0
         d_prev = d
         for i, st in enumerate(s):
             blk = oracle.stream_block(seed, ifreq, p, 2 + seg)
-            assert st["tau_drawn"] == float(np.float32(-math.log(oracle.uniform(blk[0]))))
+            assert st["tau_drawn"] == pytest.approx(-math.log(oracle.uniform(blk[0])), rel=1e-14)
             if st["kind"] == 1:
                 later = s[i + 1:]
-                later = later[later["ds"] > 1e-3]
+                later = later[later["ds"] > 1e-9]
                 if len(later):
                     d_new = (later[0]["p1"] - later[0]["p0"]) / later[0]["ds"]
-                    expect = oracle.rotate(np.float32(d_prev).astype(np.float64), oracle.hg_cos(gg, oracle.uniform(blk[1])),
+                    expect = oracle.rotate(d_prev, oracle.hg_cos(gg, oracle.uniform(blk[1])),
                                            2 * math.pi * oracle.uniform(blk[2]))
                     # only compare when no further scattering happened before the next non-zero step
-                    if not (s[i + 1:i + 1 + int(np.argmax(s[i + 1:]["ds"] > 1e-3))]["kind"] == 1).any():
-                        assert np.allclose(d_new, expect, atol=1e-4)     # p0, p1 carry fp32 positions
+                    if not (s[i + 1:i + 1 + int(np.argmax(s[i + 1:]["ds"] > 1e-9))]["kind"] == 1).any():
+                        assert np.allclose(d_new, expect, atol=1e-7)
                         checked += 1
                     d_prev = expect
                 seg += 1
     assert checked > 100
+
+
+# ------------------------------------------------------------------------------ the f32state variant
+# soc_oracle_simulate_f32state (package state snapped to fp32 at every store) is licensed only by these pins
+# against THE oracle (fp64 throughout) and by the closed forms it must still reach at fp32 tolerance.
+def _records_equal(a, b):
+    return (a["hash"] == b["hash"]) & (a["steps"] == b["steps"]) & (a["scatters"] == b["scatters"])
+
+
+def test_f32state_identical_on_non_scattering_paths():
+    # straight paths (ksca = 0): snapping moves a position by <= 6e-8 of a cell, which changes the visited
+    # cells only for a path within that distance of a cell edge -- none among these 30k packages
+    rng = np.random.default_rng(17)
+    g = oracle.Grid(8, 8, 8, [512], rng.lognormal(0, 1, 512).astype(np.float32))
+    src = dict(bg_intensity=1.0, ps_pos=np.array([[3.3, 4.6, 2.2]]), ps_lum=np.array([40.0]))
+    A, r, rep, _ = oracle.simulate(g, 0.3, 0.0, 0.0, 0, src, 30000, 3, want_replay=True)
+    B, q, rq, _ = oracle.simulate(g, 0.3, 0.0, 0.0, 0, src, 30000, 3, want_replay=True, f32state=True)
+    assert _records_equal(rep, rq).all()
+    assert q.emitted == r.emitted and q.cell_steps == r.cell_steps
+    # a path of ~10 cells moves by <= 1e-6 of a cell; e^-tau with kabs rho up to ~10 per cell follows it
+    assert np.allclose(rq["e_escaped"], rep["e_escaped"], rtol=1e-4, atol=0)
+    assert np.abs(B - A).sum() <= 1e-6 * A.sum()
+    n_cells, rho, child = random_octree((4, 4, 4), 3, 0.3, seed=5)
+    gh = oracle.Grid(4, 4, 4, n_cells, rho, child)
+    _, _, rep, _ = oracle.simulate(gh, 0.3, 0.0, 0.0, 0, dict(bg_intensity=1.0), 20000, 3, want_replay=True)
+    _, _, rq, _ = oracle.simulate(gh, 0.3, 0.0, 0.0, 0, dict(bg_intensity=1.0), 20000, 3, want_replay=True, f32state=True)
+    assert _records_equal(rep, rq).all()
+
+
+@pytest.mark.parametrize("which", ["1", "2"])
+def test_f32state_follows_the_fp64_oracle_on_config_1_2_like_runs(which):
+    from paper_1812_06632_b200 import inputs
+    P = inputs.make_config("1", n_packages=40000) if which == "1" else inputs.make_config("2", n=32, n_packages=40000)
+    g = oracle.Grid(P.nx, P.ny, P.nz, P.n_cells, P.rho, P.child)
+    src = P.sources(0)
+    A, r, rep, _ = oracle.simulate(g, P.kabs[0], P.ksca[0], P.g[0], 0, src, P.n_packages, 1, want_replay=True, threads=4)
+    B, q, rq, _ = oracle.simulate(g, P.kabs[0], P.ksca[0], P.g[0], 0, src, P.n_packages, 1, want_replay=True, threads=4,
+                                  f32state=True)
+    same = _records_equal(rep, rq).mean()
+    assert same >= 0.99, same                       # the few that part ways scatter several times (chaotic map)
+    assert np.abs(B - A).sum() <= 0.02 * A.sum()
+    assert q.absorbed == pytest.approx(r.absorbed, rel=2e-3) and q.escaped == pytest.approx(r.escaped, rel=2e-3)
+    assert abs(q.emitted - q.absorbed - q.escaped) <= 1e-9 * q.emitted      # weights and deposits stay fp64
+
+
+def test_f32state_within_5_sigma_of_the_fp64_oracle_over_8_seeds():
+    rng = np.random.default_rng(23)
+    g = oracle.Grid(8, 8, 8, [512], rng.lognormal(0, 1, 512).astype(np.float32))
+    src = dict(bg_intensity=1.0, ps_pos=np.array([[4.5, 3.5, 4.5]]), ps_lum=np.array([60.0]))
+    runs, runs32 = [], []
+    for seed in range(1, 9):
+        runs.append(oracle.simulate(g, 0.2, 0.8, 0.6, 0, src, 20000, seed, threads=4)[0])
+        runs32.append(oracle.simulate(g, 0.2, 0.8, 0.6, 0, src, 20000, seed, threads=4, f32state=True)[0])
+    runs, runs32 = np.array(runs), np.array(runs32)
+    sigma = runs.std(axis=0, ddof=1)
+    assert (sigma > 0).all()
+    assert (np.abs(runs32 - runs) <= 5 * sigma[None, :]).all()
+    # and the 8-seed means agree far inside the noise of the mean
+    assert np.abs(runs32.mean(0) - runs.mean(0)).max() <= 1.0 * (sigma / 8 ** 0.5).max()
+
+
+def test_f32state_reaches_the_same_closed_forms():
+    # slab: transmission exp(-tau) and per-cell deposits (axis-aligned: nothing to round)
+    g = _uniform_grid((7, 5, 9), rho=2.0)
+    beam = np.array([0.0, 2.5, 4.75, 1.0, 0.0, 0.0])
+    A, res, _, _ = oracle.simulate(g, 0.15, 0.0, 0.0, 0, dict(beam=beam), 1, 1, f32state=True)
+    assert res.escaped == pytest.approx(math.exp(-7 * 0.3), rel=1e-13)
+    # oblique chord: to a few fp32 ulps
+    shape = (6, 4, 5)
+    g = _uniform_grid(shape, 1.5)
+    d = np.array([0.6, 0.3, -0.5]); d /= np.linalg.norm(d)
+    pos = np.array([0.0, 1.2, 4.4])
+    _, res, _, tr = oracle.simulate(g, 0.2, 0.0, 0.0, 0, dict(beam=np.concatenate([pos, d])), 1, 1, trace_cap=100,
+                                    f32state=True)
+    tmax = min(((shape[j] if d[j] > 0 else 0) - pos[j]) / d[j] for j in range(3))
+    assert tr["ds"].sum() == pytest.approx(tmax, rel=4 * F32)
+    assert res.absorbed == pytest.approx(1 - math.exp(-0.2 * 1.5 * tmax), rel=4 * F32)
+    # optically thin bath with scattering: A_c = 4 pi I kabs rho_c V_c
+    rng = np.random.default_rng(2)
+    g = oracle.Grid(6, 6, 6, [216], rng.lognormal(0, 1, 216).astype(np.float32))
+    A, res, _, _ = oracle.simulate(g, 1e-6, 0.6, 0.6, 0, dict(bg_intensity=1.7), 150000, 21, threads=4, f32state=True)
+    expect = 4 * math.pi * 1.7 * 1e-6 * g.rho.astype(np.float64)
+    assert A.sum() / expect.sum() == pytest.approx(1.0, abs=0.006)
+    # fully refined hierarchy = regular 2N grid: the ascent rounds (f + bit)/2 to fp32, so a package within an
+    # ulp of a cell edge may take the corner cell in the other order
+    N = 4
+    rho2 = rng.lognormal(0, 0.8, (2 * N, 2 * N, 2 * N)).astype(np.float32)
+    n_cells, rho, child, gid_of = fully_refined(rho2)
+    gh = oracle.Grid(N, N, N, n_cells, rho, child)
+    gr = oracle.Grid(2 * N, 2 * N, 2 * N, [8 * N ** 3], rho2.ravel())
+    Ah, rh, reph, _ = oracle.simulate(gh, 0.3, 0.7, 0.4, 2, dict(bg_intensity=1.0), 20000, 5, want_replay=True, f32state=True)
+    Ar, rr, repr_, _ = oracle.simulate(gr, 0.15, 0.35, 0.4, 2, dict(bg_intensity=0.25), 20000, 5, want_replay=True, f32state=True)
+    assert ((reph["steps"] == repr_["steps"]) & (reph["scatters"] == repr_["scatters"])).mean() >= 0.999
+    assert np.abs(Ah[gid_of.ravel()] - Ar).sum() <= 1e-3 * Ar.sum()
