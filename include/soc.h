@@ -43,10 +43,19 @@ extern "C" {
 #define SOC_MAX_LEVELS 16
 
 /* flags of the simulate calls */
-#define SOC_GEOM_FP32 0u  /* production: fp32 in-cell positions/directions, fp64 weights and accumulators */
-#define SOC_GEOM_FP64 1u  /* replay: fp64 positions/directions (same decisions as the fp64 oracle up to 1e-16) */
+#define SOC_GEOM_FP32 0u  /* production: fp32 package state (in-cell position, direction, remaining optical depth) evaluated
+                             in fp32; fp32 package weight relative to the initial energy; deposits summed per launch in an
+                             internal fp32 accumulator (fp64 with option "acc32" = 0) that is folded into the caller's fp64
+                             array after every frequency */
+#define SOC_GEOM_FP64 1u  /* replay: the same fp32 package state, every update evaluated in fp64 and rounded once; fp64
+                             weight; fp64 atomic adds straight into the caller's array; per-package records.
+                             Same decisions as the oracle's fp32-state variant except within 2^-29 of a rounding boundary */
 
-typedef struct soc_grid soc_grid;    /* opaque; owns its device copies of the cloud and the dust tables */
+/* opaque; owns its device copies of the cloud and the dust tables, its internal accumulators and result slots.
+ * A grid serves ONE stream and ONE host thread at a time: calls on the same grid must be issued in stream order from one
+ * thread (the internal accumulators, result slots and the staged temperature table are per grid, not per call).  Use one
+ * grid per stream for concurrent work.  soc_grid_create returns with the grid complete (device synchronised). */
+typedef struct soc_grid soc_grid;
 
 /* Inputs named by the paper: the cloud hierarchy with the density values, the dust cross sections for
  * absorption and scattering, the scattering function per frequency (here Henyey-Greenstein g,
@@ -81,6 +90,11 @@ typedef struct {
 typedef struct {
     double emitted, escaped, absorbed;   /* energies of the simulated packages (not multiplied by `weight`) */
     uint64_t cell_steps, scatterings, terminated;
+    double weight_drift;                 /* production mode: max over the escaped packages of |w - (1 - sum of deposits)|,
+                                            the fp32 running weight against the deposits actually made, both relative to
+                                            the package's initial energy (escaped is taken from the deposits while less than
+                                            half was absorbed, so emitted = absorbed + escaped does not see this drift);
+                                            replay mode: 0 (fp64 weight, deposit = weight difference) */
 } soc_freq_result;
 
 /* per-package replay record (DEVICE array written by soc_simulate_packages) */
@@ -147,7 +161,7 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
  * kernel), "service_threshold" (parked lanes that trigger a service pass), "hot_cache" (0/1: shared partial sums
  * for the cells around point sources), "acc32" (0/1: fp32 per-launch accumulator), "overlap" (0/1: soc_simulate_spectrum overlaps consecutive frequencies on two streams), "kernel" (production kernel on
  * regular grids: 0 = chosen by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel), "carveout"
- * (preferred shared-memory carve-out in %, -1 = driver default), "debug" (measurement only); and
+ * (preferred shared-memory carve-out in %, -1 = driver default); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
  * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
 int soc_set_option(soc_grid *grid, const char *key, int64_t value);

@@ -44,6 +44,7 @@ constexpr unsigned kFull = 0xffffffffu;
 struct DevResult {                      // one slot per launch, accumulated with atomics
     double emitted, escaped, absorbed;
     unsigned long long cell_steps, scatterings, terminated;
+    unsigned int drift_bits, pad_;      // fp32 bits of max |w - (1 - sum of deposits)| over the packages that escaped
 };
 
 struct SimParams {
@@ -85,6 +86,8 @@ struct soc_grid {
     unsigned long long *d_counters = nullptr; // n_slots
     DevResult *h_results = nullptr;           // pinned, n_slots
     float *d_table = nullptr;
+    float *h_table = nullptr;                 // pinned staging copy of the caller's table (borrowed for the call only)
+    cudaEvent_t ev_table = nullptr;           // the staging copy has been read
     // internal layout of the production kernel: root grid with one ghost layer, then the octet levels
     int nbx = 0, nby = 0, nbz = 0, nrp = 0;
     long long n_int = 0;
@@ -108,7 +111,6 @@ struct soc_grid {
     int opt_threads = 256;
     int opt_refill_threshold = 1;
     int opt_service_threshold = 0;            // parked lanes that trigger a service pass; 0 = by scattering depth (8 or 16)
-    int opt_debug = 0;
     int opt_hot_cache = 1;
     int opt_carveout = -1;                    // preferred shared-memory carve-out of the photon kernels in %, -1 = driver default
     double rho_mean = 0.0;                    // mean density of the root-level leaves
@@ -155,6 +157,7 @@ template <> struct RM<float> {
     static __device__ __forceinline__ void sincospi_(float x, float *s, float *c) { sincospif(x, s, c); }
     static __device__ __forceinline__ float inf() { return __int_as_float(0x7f800000); }
     static __device__ __forceinline__ float copysign_(float a, float b) { return copysignf(a, b); }
+    static __device__ __forceinline__ float rsqrt_(float x) { return rsqrtf(x); }
 };
 template <> struct RM<double> {
     static __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
@@ -162,6 +165,7 @@ template <> struct RM<double> {
     static __device__ __forceinline__ void sincospi_(double x, double *s, double *c) { sincospi(x, s, c); }
     static __device__ __forceinline__ double inf() { return __longlong_as_double(0x7ff0000000000000ll); }
     static __device__ __forceinline__ double copysign_(double a, double b) { return copysign(a, b); }
+    static __device__ __forceinline__ double rsqrt_(double x) { return 1.0 / sqrt(x); }
 };
 
 // Precision (reading S11): the package state (position in the cell, direction, remaining optical
@@ -214,13 +218,14 @@ template <typename A> __device__ __forceinline__ void descend(const SimParams &P
     p.cw = cw;
 }
 
-// a1-a3: create package `id` (SURVEY.md 8c.3 / DESIGN.md readings S2, S3)
-template <typename A, bool HIER>
-__device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long id)
+// a1-a3: position, root cell, direction and source of package `id` (SURVEY.md 8c.3 / DESIGN.md readings S2, S3).
+// One definition for both kernels families: A = double in the replay kernel, float in the production kernels; PARAMS
+// is SimParams or FastParams (same field names).  src = point source index, -1 = background or beam.
+template <typename A, typename PARAMS>
+__device__ __forceinline__ void emit_core(const PARAMS &P, long long id, int &ix, int &iy, int &iz, float &fx, float &fy,
+                                          float &fz, A &dx, A &dy, A &dz, int &src)
 {
-    double e0;
-    A dx, dy, dz;
-    p.id = id;
+    src = -1;
     if (P.is_beam) {
         const int n[3] = {P.nx, P.ny, P.nz};
         int c[3];
@@ -232,10 +237,9 @@ __device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long 
             c[j] = i;
             f[j] = (float)(P.beam[j] - (double)i);
         }
-        p.ix = c[0]; p.iy = c[1]; p.iz = c[2];
-        p.fx = f[0]; p.fy = f[1]; p.fz = f[2];
+        ix = c[0]; iy = c[1]; iz = c[2];
+        fx = f[0]; fy = f[1]; fz = f[2];
         dx = (A)P.beam[3]; dy = (A)P.beam[4]; dz = (A)P.beam[5];
-        e0 = 1.0;
     } else if (id < P.n_bg) {
         uint32_t w0, w1, w2, w3, v0, v1, v2, v3;
         philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
@@ -266,24 +270,60 @@ __device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long 
         A sp, cp;
         RM<A>::sincospi_((A)2 * uniform01<A>(v0), &sp, &cp);
         const A da = high ? -mu : mu, d1 = st * cp, d2 = st * sp;
-        if (a == 0)      { p.ix = ia; p.iy = i1; p.iz = i2; p.fx = fa; p.fy = f1; p.fz = f2; dx = da; dy = d1; dz = d2; }
-        else if (a == 1) { p.iy = ia; p.iz = i1; p.ix = i2; p.fy = fa; p.fz = f1; p.fx = f2; dy = da; dz = d1; dx = d2; }
-        else             { p.iz = ia; p.ix = i1; p.iy = i2; p.fz = fa; p.fx = f1; p.fy = f2; dz = da; dx = d1; dy = d2; }
-        e0 = P.bg_e0;
+        if (a == 0)      { ix = ia; iy = i1; iz = i2; fx = fa; fy = f1; fz = f2; dx = da; dy = d1; dz = d2; }
+        else if (a == 1) { iy = ia; iz = i1; ix = i2; fy = fa; fz = f1; fx = f2; dy = da; dz = d1; dx = d2; }
+        else             { iz = ia; ix = i1; iy = i2; fz = fa; fx = f1; fy = f2; dz = da; dx = d1; dy = d2; }
     } else {
         uint32_t w0, w1, w2, w3;
         philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
         const int k = (int)((id - P.n_bg) % P.n_point);
         const double px = P.ps_pos[k][0], py = P.ps_pos[k][1], pz = P.ps_pos[k][2];
-        p.ix = (int)floor(px); p.iy = (int)floor(py); p.iz = (int)floor(pz);
-        p.fx = (float)(px - (double)p.ix); p.fy = (float)(py - (double)p.iy); p.fz = (float)(pz - (double)p.iz);
+        ix = (int)floor(px); iy = (int)floor(py); iz = (int)floor(pz);
+        fx = (float)(px - (double)ix); fy = (float)(py - (double)iy); fz = (float)(pz - (double)iz);
         const A mu = (A)2 * uniform01<A>(w0) - (A)1;
         const A st = RM<A>::sqrt_(fmax((A)0, (A)1 - mu * mu));
         A sp, cp;
         RM<A>::sincospi_((A)2 * uniform01<A>(w1), &sp, &cp);
         dx = st * cp; dy = st * sp; dz = mu;
-        e0 = P.ps_e0[k];
+        src = k;
     }
+}
+
+// a8: new direction after a scattering: Henyey-Greenstein polar angle in the cancellation-free form (reading S6) from
+// word w_hg, azimuth from word w_az, rotation in the basis of Duff et al. 2017 (reading in SURVEY.md 8c.7), renormalised.
+template <typename A>
+__device__ __forceinline__ void scatter_direction(A g, uint32_t w_hg, uint32_t w_az, A odx, A ody, A odz, A &ndx, A &ndy, A &ndz)
+{
+    const A mu0 = (A)2 * uniform01<A>(w_hg) - (A)1;
+    const A num = mu0 + g * ((A)3 + mu0 * mu0) * (A)0.5 + g * g * mu0 + g * g * g * (mu0 * mu0 - (A)1) * (A)0.5;
+    const A den = ((A)1 + g * mu0) * ((A)1 + g * mu0);
+    A ct = num / den;
+    ct = ct > (A)1 ? (A)1 : (ct < (A)-1 ? (A)-1 : ct);
+    const A st = RM<A>::sqrt_(fmax((A)0, (A)1 - ct * ct));
+    A sp, cp;
+    RM<A>::sincospi_((A)2 * uniform01<A>(w_az), &sp, &cp);
+    const A sg = RM<A>::copysign_((A)1, odz);
+    const A a = (A)-1 / (sg + odz);
+    const A b = odx * ody * a;
+    const A t1x = (A)1 + sg * odx * odx * a, t1y = sg * b, t1z = -sg * odx;
+    const A t2x = b, t2y = sg + ody * ody * a, t2z = -ody;
+    const A c1 = st * cp, c2 = st * sp;
+    const A nx = c1 * t1x + c2 * t2x + ct * odx;
+    const A ny = c1 * t1y + c2 * t2y + ct * ody;
+    const A nz = c1 * t1z + c2 * t2z + ct * odz;
+    const A inv = RM<A>::rsqrt_(nx * nx + ny * ny + nz * nz);
+    ndx = nx * inv; ndy = ny * inv; ndz = nz * inv;
+}
+
+// a1-a4: create package `id` in the replay kernel's state
+template <typename A, bool HIER>
+__device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long id)
+{
+    A dx, dy, dz;
+    int src;
+    p.id = id;
+    emit_core<A>(P, id, p.ix, p.iy, p.iz, p.fx, p.fy, p.fz, dx, dy, dz, src);
+    const double e0 = P.is_beam ? 1.0 : (src >= 0 ? P.ps_e0[src] : P.bg_e0);
     set_direction(p, dx, dy, dz);
     p.h = 1.0f;
     const int root = p.ix + P.nx * (p.iy + P.ny * p.iz);
@@ -306,30 +346,12 @@ __device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long 
     return e0;
 }
 
-// a8: Henyey-Greenstein polar angle in the cancellation-free form (reading S6), rotation (Duff et al. 2017 basis)
+// a8 in the replay kernel: evaluated in A from the fp32 state, rounded once
 template <typename A> __device__ __forceinline__ void scatter(const SimParams &P, Pkg<A> &p)
 {
-    const A g = (A)P.g;
-    const A odx = (A)p.dx, ody = (A)p.dy, odz = (A)p.dz;
-    const A mu0 = (A)2 * uniform01<A>(p.w_hg) - (A)1;
-    const A num = mu0 + g * ((A)3 + mu0 * mu0) * (A)0.5 + g * g * mu0 + g * g * g * (mu0 * mu0 - (A)1) * (A)0.5;
-    const A den = ((A)1 + g * mu0) * ((A)1 + g * mu0);
-    A ct = num / den;
-    ct = ct > (A)1 ? (A)1 : (ct < (A)-1 ? (A)-1 : ct);
-    const A st = RM<A>::sqrt_(fmax((A)0, (A)1 - ct * ct));
-    A sp, cp;
-    RM<A>::sincospi_((A)2 * uniform01<A>(p.w_az), &sp, &cp);
-    const A sg = RM<A>::copysign_((A)1, odz);
-    const A a = (A)-1 / (sg + odz);
-    const A b = odx * ody * a;
-    const A t1x = (A)1 + sg * odx * odx * a, t1y = sg * b, t1z = -sg * odx;
-    const A t2x = b, t2y = sg + ody * ody * a, t2z = -ody;
-    const A c1 = st * cp, c2 = st * sp;
-    const A nx = c1 * t1x + c2 * t2x + ct * odx;
-    const A ny = c1 * t1y + c2 * t2y + ct * ody;
-    const A nz = c1 * t1z + c2 * t2z + ct * odz;
-    const A inv = (A)1 / RM<A>::sqrt_(nx * nx + ny * ny + nz * nz);
-    set_direction(p, nx * inv, ny * inv, nz * inv);
+    A nx, ny, nz;
+    scatter_direction<A>((A)P.g, p.w_hg, p.w_az, (A)p.dx, (A)p.dy, (A)p.dz, nx, ny, nz);
+    set_direction(p, nx, ny, nz);
     p.seg += 1; p.scat += 1;
     uint32_t s0, s1, s2, s3;
     philox_block(P.seed, P.ifreq, p.id, 2u + p.seg, s0, s1, s2, s3);
@@ -549,7 +571,6 @@ struct FastParams {
     unsigned long long seed;
     int ifreq;
     int service_threshold;
-    int debug;                          // bit 0: skip the scatter-adds (measurement only)
     int hot_r;                          // half-width R of the cached cube around every point source, -1 = no cache
     double *acc;                        // [n_int] internal accumulator (unweighted energies), ACC32 = false
     float *acc32;                       // [n_int] internal accumulator in units of e_ref, ACC32 = true
@@ -635,72 +656,12 @@ __device__ __forceinline__ long long global_id(const FastParams &P, int rel)
     return ix + (long long)P.nx * (iy + (long long)P.ny * iz);
 }
 
-// a1-a3: position, cell, direction and energy of package `id`; the direction is returned, not installed
+// a1-a3 in the production kernels: the direction is returned, not installed
 __device__ __forceinline__ void fast_emit_core(const FastParams &P, FPkg &p, long long id, int &ix, int &iy, int &iz,
                                                float &dx, float &dy, float &dz)
 {
     p.id = id;
-    if (P.is_beam) {
-        const int n[3] = {P.nx, P.ny, P.nz};
-        int c[3];
-        float f[3];
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            int i = (int)floor(P.beam[j]);
-            i = i > n[j] - 1 ? n[j] - 1 : i;
-            c[j] = i;
-            f[j] = (float)(P.beam[j] - (double)i);
-        }
-        ix = c[0]; iy = c[1]; iz = c[2];
-        p.fx = f[0]; p.fy = f[1]; p.fz = f[2];
-        dx = (float)P.beam[3]; dy = (float)P.beam[4]; dz = (float)P.beam[5];
-        p.src = -1;
-    } else if (id < P.n_bg) {
-        uint32_t w0, w1, w2, w3, v0, v1, v2, v3;
-        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
-        philox_block(P.seed, P.ifreq, id, 1u, v0, v1, v2, v3);
-        const double ax = (double)P.ny * P.nz, ay = (double)P.nz * P.nx, az = (double)P.nx * P.ny;
-        const double x = uniform01<double>(w0) * P.surf;
-        int face = 5;
-        if (x < ax) face = 0;
-        else if (x < 2 * ax) face = 1;
-        else if (x < 2 * ax + ay) face = 2;
-        else if (x < 2 * ax + 2 * ay) face = 3;
-        else if (x < 2 * ax + 2 * ay + az) face = 4;
-        const int a = face >> 1, high = face & 1;
-        const int n1 = a == 0 ? P.ny : (a == 1 ? P.nz : P.nx);
-        const int n2 = a == 0 ? P.nz : (a == 1 ? P.nx : P.ny);
-        const int na = a == 0 ? P.nx : (a == 1 ? P.ny : P.nz);
-        const unsigned long long m1 = (unsigned long long)(2u * (w1 >> 9) + 1u) * (unsigned)n1;
-        const unsigned long long m2 = (unsigned long long)(2u * (w2 >> 9) + 1u) * (unsigned)n2;
-        const int i1 = (int)(m1 >> 24), i2 = (int)(m2 >> 24);
-        const float f1 = (float)(uint32_t)(m1 & 0xffffffu) * (float)(1.0 / 16777216.0);
-        const float f2 = (float)(uint32_t)(m2 & 0xffffffu) * (float)(1.0 / 16777216.0);
-        const int ia = high ? na - 1 : 0;
-        const float fa = high ? 1.0f : 0.0f;
-        const float u3 = uniform01<float>(w3);
-        const float mu = sqrtf(u3), st = sqrtf(1.0f - u3);
-        float sp, cp;
-        sincospif(2.0f * uniform01<float>(v0), &sp, &cp);
-        const float da = high ? -mu : mu, d1 = st * cp, d2 = st * sp;
-        if (a == 0)      { ix = ia; iy = i1; iz = i2; p.fx = fa; p.fy = f1; p.fz = f2; dx = da; dy = d1; dz = d2; }
-        else if (a == 1) { iy = ia; iz = i1; ix = i2; p.fy = fa; p.fz = f1; p.fx = f2; dy = da; dz = d1; dx = d2; }
-        else             { iz = ia; ix = i1; iy = i2; p.fz = fa; p.fx = f1; p.fy = f2; dz = da; dx = d1; dy = d2; }
-        p.src = -1;
-    } else {
-        uint32_t w0, w1, w2, w3;
-        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
-        const int k = (int)((id - P.n_bg) % P.n_point);
-        const double px = P.ps_pos[k][0], py = P.ps_pos[k][1], pz = P.ps_pos[k][2];
-        ix = (int)floor(px); iy = (int)floor(py); iz = (int)floor(pz);
-        p.fx = (float)(px - (double)ix); p.fy = (float)(py - (double)iy); p.fz = (float)(pz - (double)iz);
-        const float mu = 2.0f * uniform01<float>(w0) - 1.0f;
-        const float st = sqrtf(fmaxf(0.0f, 1.0f - mu * mu));
-        float sp, cp;
-        sincospif(2.0f * uniform01<float>(w1), &sp, &cp);
-        dx = st * cp; dy = st * sp; dz = mu;
-        p.src = k;
-    }
+    emit_core<float>(P, id, ix, iy, iz, p.fx, p.fy, p.fz, dx, dy, dz, p.src);
 }
 
 template <bool HIER>
@@ -751,6 +712,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
     double acc_emit = 0.0, acc_esc = 0.0, acc_abs = 0.0;
     unsigned long long acc_steps = 0;
     unsigned acc_scat = 0, acc_term = 0;
+    float acc_drift = 0.0f;                      // max |w - (1 - absrel)|: the running weight against the sum of the deposits
     FPkg p;
     p.src = -1; p.disp = -1; p.w = 0.0f; p.absrel = 0.0f; p.steps = 0; p.scat = 0; p.cw = 0; p.rel = 0; p.h = 1.0f;
     p.anc1 = p.anc2 = p.anc3 = -1;
@@ -774,6 +736,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
             if (need == DONE) {                  // retire the finished package
                 const double e0 = package_e0(P, p.src);
                 const double esc = escaped_rel(p.w, p.absrel) * e0;
+                if (p.w != 0.0f) acc_drift = fmaxf(acc_drift, fabsf(p.w - (1.0f - p.absrel)));
                 acc_esc += esc;
                 acc_abs += (double)p.absrel * e0;
                 acc_steps += p.steps;
@@ -817,28 +780,9 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 p.fx = __saturatef(fmaf(t_u, p.dx, p.fx));
                 p.fy = __saturatef(fmaf(t_u, p.dy, p.fy));
                 p.fz = __saturatef(fmaf(t_u, p.dz, p.fz));
-                const float g = P.g;
                 uint32_t s0, w_hg, w_az, s3;     // words 1, 2 of the block of the segment that ends here
                 philox_block(P.seed, P.ifreq, p.id, 2u + p.scat, s0, w_hg, w_az, s3);
-                const float mu0 = 2.0f * uniform01<float>(w_hg) - 1.0f;
-                const float num = mu0 + g * (3.0f + mu0 * mu0) * 0.5f + g * g * mu0 + g * g * g * (mu0 * mu0 - 1.0f) * 0.5f;
-                const float den = (1.0f + g * mu0) * (1.0f + g * mu0);
-                float ct = num / den;
-                ct = fminf(1.0f, fmaxf(-1.0f, ct));
-                const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
-                float sp, cp;
-                sincospif(2.0f * uniform01<float>(w_az), &sp, &cp);
-                const float sg = copysignf(1.0f, p.dz);
-                const float a = -1.0f / (sg + p.dz);
-                const float b = p.dx * p.dy * a;
-                const float t1x = 1.0f + sg * p.dx * p.dx * a, t1y = sg * b, t1z = -sg * p.dx;
-                const float t2x = b, t2y = sg + p.dy * p.dy * a, t2z = -p.dy;
-                const float c1 = st * cp, c2 = st * sp;
-                const float qx = c1 * t1x + c2 * t2x + ct * p.dx;
-                const float qy = c1 * t1y + c2 * t2y + ct * p.dy;
-                const float qz = c1 * t1z + c2 * t2z + ct * p.dz;
-                const float inv = rsqrtf(qx * qx + qy * qy + qz * qz);
-                ndx = qx * inv; ndy = qy * inv; ndz = qz * inv;
+                scatter_direction<float>(P.g, w_hg, w_az, p.dx, p.dy, p.dz, ndx, ndy, ndz);
                 p.scat += 1;
             }
             if (need == NEWID || need == SCAT) {
@@ -889,7 +833,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 if (p.disp >= 0) {
                     const int j = (p.disp & 255) + hot_side * (((p.disp >> 8) & 255) + hot_side * (p.disp >> 16));
                     atomicAdd(s_hot + p.src * hot_cells + j, p.pend);
-                } else if (p.pend > 0.0f && !(P.debug & 1)) {
+                } else if (p.pend > 0.0f) {
                     if (ACC32) atomicAdd(P.acc32 + p.rel, p.pend * package_rel(P, p.src));
                     else atomicAdd(P.acc + p.rel, (double)p.pend * package_e0(P, p.src));
                 }
@@ -969,6 +913,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
         acc_steps += __shfl_xor_sync(kFull, acc_steps, o);
         acc_scat += __shfl_xor_sync(kFull, acc_scat, o);
         acc_term += __shfl_xor_sync(kFull, acc_term, o);
+        acc_drift = fmaxf(acc_drift, __shfl_xor_sync(kFull, acc_drift, o));
     }
     if (lane == 0 && acc_steps != 0) {
         atomicAdd(&P.result->emitted, acc_emit);
@@ -977,6 +922,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
         atomicAdd(&P.result->cell_steps, acc_steps);
         atomicAdd(&P.result->scatterings, (unsigned long long)acc_scat);
         atomicAdd(&P.result->terminated, (unsigned long long)acc_term);
+        atomicMax(&P.result->drift_bits, __float_as_uint(acc_drift));     // >= 0: fp32 order = integer order
     }
 }
 
@@ -1047,6 +993,8 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
     // per-launch totals of this thread (touched only in the service block)
     __shared__ double s_tot[3][256];             // emitted, escaped, absorbed
     __shared__ unsigned s_cnt[2][256];           // scatterings, terminated
+    __shared__ float s_drift[256];               // max |w - (1 - absrel)| over this thread's escaped packages
+    s_drift[threadIdx.x] = 0.0f;
     s_tot[0][threadIdx.x] = 0.0; s_tot[1][threadIdx.x] = 0.0; s_tot[2][threadIdx.x] = 0.0;
     s_cnt[0][threadIdx.x] = 0u; s_cnt[1][threadIdx.x] = 0u;
     extern __shared__ float s_hot[];             // hot-cell partial sums, see photon_fast_kernel
@@ -1077,6 +1025,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                 const int src = v_src(p.sd);
                 const double e0 = package_e0(P, src);
                 const double esc = escaped_rel(p.w, p.absrel) * e0;
+                if (p.w != 0.0f) s_drift[threadIdx.x] = fmaxf(s_drift[threadIdx.x], fabsf(p.w - (1.0f - p.absrel)));
                 s_tot[1][threadIdx.x] += esc;
                 s_tot[2][threadIdx.x] += (double)p.absrel * e0;
                 s_cnt[0][threadIdx.x] += p.scat;
@@ -1126,28 +1075,9 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                 p.fx = __saturatef(fmaf(t_u, p.dx, p.fx));
                 p.fy = __saturatef(fmaf(t_u, p.dy, p.fy));
                 p.fz = __saturatef(fmaf(t_u, p.dz, p.fz));
-                const float g = P.g;
                 uint32_t s0, w_hg, w_az, s3;     // words 1, 2 of the block of the segment that ends here
                 philox_block(P.seed, P.ifreq, P.pkg_begin + (long long)p.idx, 2u + p.scat, s0, w_hg, w_az, s3);
-                const float mu0 = 2.0f * uniform01<float>(w_hg) - 1.0f;
-                const float num = mu0 + g * (3.0f + mu0 * mu0) * 0.5f + g * g * mu0 + g * g * g * (mu0 * mu0 - 1.0f) * 0.5f;
-                const float den = (1.0f + g * mu0) * (1.0f + g * mu0);
-                float ct = num / den;
-                ct = fminf(1.0f, fmaxf(-1.0f, ct));
-                const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
-                float sp, cp;
-                sincospif(2.0f * uniform01<float>(w_az), &sp, &cp);
-                const float sg = copysignf(1.0f, p.dz);
-                const float a = -1.0f / (sg + p.dz);
-                const float b = p.dx * p.dy * a;
-                const float t1x = 1.0f + sg * p.dx * p.dx * a, t1y = sg * b, t1z = -sg * p.dx;
-                const float t2x = b, t2y = sg + p.dy * p.dy * a, t2z = -p.dy;
-                const float c1 = st * cp, c2 = st * sp;
-                const float qx = c1 * t1x + c2 * t2x + ct * p.dx;
-                const float qy = c1 * t1y + c2 * t2y + ct * p.dy;
-                const float qz = c1 * t1z + c2 * t2z + ct * p.dz;
-                const float inv = rsqrtf(qx * qx + qy * qy + qz * qz);
-                ndx = qx * inv; ndy = qy * inv; ndz = qz * inv;
+                scatter_direction<float>(P.g, w_hg, w_az, p.dx, p.dy, p.dz, ndx, ndy, ndz);
                 p.scat += 1;
             }
             if (need == NEWID || need == SCAT) {
@@ -1274,6 +1204,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
     double acc_emit = s_tot[0][threadIdx.x], acc_esc = s_tot[1][threadIdx.x], acc_abs = s_tot[2][threadIdx.x];
     unsigned long long acc_steps = n_steps;
     unsigned acc_scat = s_cnt[0][threadIdx.x], acc_term = s_cnt[1][threadIdx.x];
+    float acc_drift = s_drift[threadIdx.x];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         acc_emit += __shfl_xor_sync(kFull, acc_emit, o);
@@ -1282,8 +1213,10 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
         acc_steps += __shfl_xor_sync(kFull, acc_steps, o);
         acc_scat += __shfl_xor_sync(kFull, acc_scat, o);
         acc_term += __shfl_xor_sync(kFull, acc_term, o);
+        acc_drift = fmaxf(acc_drift, __shfl_xor_sync(kFull, acc_drift, o));
     }
     if (lane == 0 && (acc_steps != 0 || acc_emit != 0.0)) {
+        atomicMax(&P.result->drift_bits, __float_as_uint(acc_drift));
         atomicAdd(&P.result->emitted, acc_emit);
         atomicAdd(&P.result->escaped, acc_esc);
         atomicAdd(&P.result->absorbed, acc_abs);
@@ -1708,7 +1641,6 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
                                                                : (P.ksca * G->rho_mean * nm >= 4.0 ? 16 : 8);
         }
         const int auto_threshold = G->opt_service_threshold > 0 ? G->opt_service_threshold : 8;     // photon_q_kernel: 8 throughout
-        F.debug = G->opt_debug;
         // hot-cell cache: R = 3 (343 cells per source) while it fits in 40 KB per block, else R = 2; regular grids
         F.hot_r = -1;
         if (!hier && P.n_point > 0 && !P.is_beam && G->opt_hot_cache)
@@ -1731,7 +1663,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         F.acc32 = G->acc_sel ? G->d_acc32_b : G->d_acc32;
         if (!acc32 && G->acc_sel && !G->d_acc_b) {           // fp64 fallback on the second stream: its own accumulator
             SOC_CUDA(cudaMalloc(&G->d_acc_b, sizeof(double) * (size_t)G->n_int));
-            SOC_CUDA(cudaMemset(G->d_acc_b, 0, sizeof(double) * (size_t)G->n_int));
+            SOC_CUDA(cudaMemsetAsync(G->d_acc_b, 0, sizeof(double) * (size_t)G->n_int, st));   // st = the stream that uses it
             F.acc = G->d_acc_b;
         }
         const double w_eff = acc32 ? weight * e_ref : weight;
@@ -1774,6 +1706,9 @@ int fetch_results(soc_grid *G, int n, soc_freq_result *out, cudaStream_t st)
         out[i].emitted = G->h_results[i].emitted; out[i].escaped = G->h_results[i].escaped;
         out[i].absorbed = G->h_results[i].absorbed; out[i].cell_steps = G->h_results[i].cell_steps;
         out[i].scatterings = G->h_results[i].scatterings; out[i].terminated = G->h_results[i].terminated;
+        float drift;
+        std::memcpy(&drift, &G->h_results[i].drift_bits, sizeof(float));
+        out[i].weight_drift = (double)drift;
     }
     return SOC_OK;
 }
@@ -1803,6 +1738,8 @@ void soc_grid_destroy(soc_grid *G)
     cudaFree(G->d_cellw); cudaFree(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
     cudaFree(G->d_table); cudaFree(G->d_cellw_int); cudaFree(G->d_parent_int); cudaFree(G->d_acc); cudaFree(G->d_acc32);
     if (G->h_results) cudaFreeHost(G->h_results);
+    if (G->h_table) cudaFreeHost(G->h_table);
+    if (G->ev_table) cudaEventDestroy(G->ev_table);
     cudaFree(G->d_acc32_b); cudaFree(G->d_acc_b);
     if (G->aux) cudaStreamDestroy(G->aux);
     if (G->ev_fork) cudaEventDestroy(G->ev_fork);
@@ -1952,6 +1889,9 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     }
     int rc = ensure_slots(G, d->n_freq > 8 ? d->n_freq : 8);
     if (rc != SOC_OK) return rc;
+    // the conversion kernels and memsets above ran on the legacy stream: a caller's non-blocking stream is not ordered
+    // after it, so the grid is complete before the call returns
+    SOC_CUDA(cudaDeviceSynchronize());
     guard.g = nullptr;
     *out = G;
     return SOC_OK;
@@ -1975,7 +1915,6 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     else if (k == "refill_threshold" && value >= 1 && value <= 32) G->opt_refill_threshold = (int)value;
     else if (k == "service_threshold" && value >= 0 && value <= 32) G->opt_service_threshold = (int)value;
     else if (k == "timing" && (value == 0 || value == 1)) G->opt_timing = (int)value;
-    else if (k == "debug" && value >= 0 && value <= 255) G->opt_debug = (int)value;
     else if (k == "hot_cache" && (value == 0 || value == 1)) G->opt_hot_cache = (int)value;
     else if (k == "kernel" && value >= 0 && value <= 2) G->opt_kernel = (int)value;
     else if (k == "overlap" && (value == 0 || value == 1)) G->opt_overlap = (int)value;
@@ -2046,7 +1985,7 @@ int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_package
             SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[0], cudaEventDisableTiming));
             SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[1], cudaEventDisableTiming));
             SOC_CUDA(cudaMalloc(&G->d_acc32_b, sizeof(float) * (size_t)G->n_int));
-            SOC_CUDA(cudaMemset(G->d_acc32_b, 0, sizeof(float) * (size_t)G->n_int));
+            SOC_CUDA(cudaMemsetAsync(G->d_acc32_b, 0, sizeof(float) * (size_t)G->n_int, st));   // ordered before the fork
         }
         SOC_CUDA(cudaEventRecord(G->ev_fork, st));
         SOC_CUDA(cudaStreamWaitEvent(G->aux, G->ev_fork, 0));
@@ -2080,7 +2019,17 @@ int soc_update_temperatures(soc_grid *G, const double *absorbed, double scale, c
     if ((reinterpret_cast<uintptr_t>(absorbed) & 15) || (reinterpret_cast<uintptr_t>(T_out) & 15))
         return fail(SOC_EINVAL, "absorbed and T_out must be 16-byte aligned");
     cudaStream_t st = (cudaStream_t)stream;
-    SOC_CUDA(cudaMemcpyAsync(G->d_table, table_T, sizeof(float) * n_table, cudaMemcpyHostToDevice, st));
+    // the caller's table is borrowed for the call only: stage it in pinned memory of our own, so that the asynchronous
+    // copy never reads the caller's buffer after the call has returned
+    if (!G->h_table) {
+        SOC_CUDA(cudaMallocHost(&G->h_table, sizeof(float) * 8192));
+        SOC_CUDA(cudaEventCreateWithFlags(&G->ev_table, cudaEventDisableTiming));
+    } else {
+        SOC_CUDA(cudaEventSynchronize(G->ev_table));     // the previous call's copy has left the staging buffer
+    }
+    std::memcpy(G->h_table, table_T, sizeof(float) * n_table);
+    SOC_CUDA(cudaMemcpyAsync(G->d_table, G->h_table, sizeof(float) * n_table, cudaMemcpyHostToDevice, st));
+    SOC_CUDA(cudaEventRecord(G->ev_table, st));
     TempParams P;
     std::memset(&P, 0, sizeof(P));
     P.cellw = G->d_cellw; P.absorbed = absorbed; P.table = G->d_table; P.T_out = T_out;
