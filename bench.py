@@ -1,15 +1,20 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the photon-package hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3|5|4p|4|2|1] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5|3|4p|4|2|1] [--scaling weak|strong]
+                    [--impl ours|reference]
 
 One STEP = one pass of the whole hot path over one batch of synthetic input: for every frequency of the
 config, emit / walk / deposit / scatter all packages (soc_simulate_spectrum: one persistent photon kernel per
-frequency queued back to back on one stream, rows a1-a10 of DESIGN.md), then the energy-balance temperature
-update (row a11).  Default workload: BASELINE.json configs[2] ("config 3": 128^3 lognormal cloud, 2 point
-sources + background, 64 frequencies, 4e6 packages per frequency, one temperature update) -- the smallest
-config that exercises every row except the octree walk and still reaches steady state; see DESIGN.md
-"Measurement" for why configs[1] (a single ~1 ms launch) is not the default.
+frequency, rows a1-a10 of DESIGN.md), then the energy-balance temperature update (row a11).  Default workload:
+BASELINE.json configs[4] ("config 5": 256^3 lognormal cloud, 10 point sources + background, 128 frequencies,
+1e7 packages per frequency, temperature update; one of its 3 iterations per step) -- the largest single-GPU
+configuration; see DESIGN.md "Measurement" for why configs[1] (a single ~1 ms launch) is not the default.
+
+--gpus N > 1: one process per GPU over NCCL.  Under torchrun (WORLD_SIZE set) the ranks are the launcher's; run
+directly, bench.py re-executes itself under `python -m torch.distributed.run --standalone --nproc-per-node N`.
+--scaling weak (default): every rank runs the full package count with seed + rank (independent realisations,
+mean by one all-reduce); strong: the package ids of ONE seed are split over the ranks.
 
 Prints ONE JSON line (rank 0).  `value` = cell-steps of all ranks per second of step time (device time, CUDA
 events on the launching stream, max over ranks), inputs resident in HBM.  `e2e` = the same through
@@ -178,15 +183,18 @@ def run_ours(args):
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    if local_rank >= torch.cuda.device_count():
+        raise SystemExit(f"bench.py: rank {rank} has no GPU (LOCAL_RANK {local_rank}, {torch.cuda.device_count()} visible)")
     torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    socdist.init("nccl", rank, world, local_rank)
     soc.load()
 
     P = inputs.make_config(args.config)
     if args.packages:
         P.n_packages = int(args.packages)
-    shard = socdist.plan("weak", rank, world, P.n_packages, P.seed)
+    shard = socdist.plan(args.scaling, rank, world, P.n_packages, P.seed)
     G = soc.Grid.from_problem(P)
     G.set_option("timing", 1)
     for kv in args.opt:
@@ -208,14 +216,20 @@ def run_ours(args):
             G.update_temperatures(Aint, P.t_scale, P.table_T, P.e_min, P.e_max, T, stream=stream)
         return res
 
-    # ---- warm-up (the first warm-up step also fetches the device counters: the walk is a deterministic
-    # function of (seed, ids), so the counts are those of every later step)
-    res = step(want_results=True)
+    # ---- warm-up (the first warm-up pass also fetches the device counters: the walk is a deterministic function of
+    # (seed, ids), so the counts are those of every later step), and conservation THROUGH THE CELLS: what the cells
+    # of this rank hold after the pass = sum_f w_f (emitted_f - escaped_f); the counters alone cannot show a lost
+    # scatter-add, and "escaped" is derived from the deposits for most packages (soc.h weight_drift)
+    Aint.zero_()
+    res = G.simulate_spectrum(srcs, P.n_packages, shard.seed, Aint, shard.pkg_begin, shard.pkg_count, stream=stream)
+    w_f = G.freq_weights()
+    budget = float(sum(w_f[f] * (res[f].emitted - res[f].escaped) for f in range(P.n_freq)))
+    cons_cells = abs(float(Aint.sum()) - budget) / budget
     steps_f = np.array([r.cell_steps for r in res], dtype=np.float64)
-    emitted = sum(r.emitted for r in res)
     cons = max(abs(r.emitted - r.absorbed - r.escaped) / r.emitted for r in res if r.emitted > 0)
+    drift = max(r.weight_drift for r in res)
     scat_total = sum(r.scatterings for r in res)
-    for _ in range(max(0, args.warmup - 1)):
+    for _ in range(max(1, args.warmup - 1)):
         step()
     torch.cuda.synchronize()
 
@@ -246,20 +260,16 @@ def run_ours(args):
     step_ms = float(sum(a.elapsed_time(b) for a, b in ev))
     kern_ms /= max(1, args.steps)
 
-    tot = torch.tensor([step_ms, float(steps_f.sum()), float(launches)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        mx = tot.clone()
-        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        step_ms = float(mx[0])
-    job_steps = float(tot[1])                    # cell-steps of all ranks in one step
-    job_launches = int(tot[2])
-    ms_per_step = step_ms / args.steps
+    job = socdist.job_totals(step_ms, float(steps_f.sum()), float(launches), world, device="cuda")
+    job_steps = job["cell_steps"]                # cell-steps of all ranks in one step
+    job_launches = job["launches"]
+    ms_per_step = job["step_ms"] / args.steps
     value = job_steps / (ms_per_step * 1e-3)
 
     # ---- end to end through the host-buffer entry (soc_run_host)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()        # noqa: E731
     Ph = dataclasses.replace(P, rho=pin(P.rho), child=None if P.child is None else pin(P.child), seed=shard.seed)
+    # (soc_run_host runs whole package counts: the e2e figure of a strong-scaling run is per-rank full work, not reported)
     a_out = torch.zeros(P.n_total, dtype=torch.float64).pin_memory().numpy()
     t_out = torch.zeros(P.n_total, dtype=torch.float32).pin_memory().numpy()
     h2d = Ph.rho.nbytes + (0 if P.child is None else Ph.child.nbytes) + 4 * 8 * P.n_freq + \
@@ -295,37 +305,41 @@ def run_ours(args):
             "kernel": "photon_q_kernel / photon_fast_kernel (production photon kernel, chosen per frequency)",
             "algorithmic_bytes_per_launch": algo_bytes, "mean_launch_ms": mean_launch_ms,
             "kernel_share_of_step": float(kern_ms.sum() / ms_per_step)}
-    roof.update(roofline_notes(args.config))
+    tr = ncu_traffic(args.config)
+    if tr:
+        roof["traffic"] = tr["bytes_per_cell_step"] * float(steps_f.mean())
+        roof["traffic_source"] = tr["source"]
+        roof["traffic_bytes_per_cell_step"] = tr["bytes_per_cell_step"]
+    roof["algorithmic_bytes_note"] = ("12 B per cell-step is SURVEY.md 8d.4's contract figure (4 B density + 8 B fp64 add); the path "
+                                      "as run adds into an fp32 per-launch accumulator: 4 B + 4 B = 8 B per cell-step")
+    roof["achieved_8B"] = achieved * 8.0 / ALGO_BYTES_PER_STEP
     if world == 1 and not args.no_probes:
-        # ceilings of the memory system for this footprint, measured in the same run:
-        # independent random accesses with no arithmetic, over 8 B per cell (cell words + fp32 accumulator)
-        fp = 8 * int(P.n_total)
-        n_ops = 1 << 31
-        rate = lambda kind: n_ops / (soc.probe_throughput(kind, fp, n_ops) * 1e-3)          # noqa: E731
-        g4, r4, cs = rate(0), rate(2), rate(5)
-        per_launch = float(steps_f.mean()) / (mean_launch_ms * 1e-3)
-        roof["probes"] = {"footprint_bytes": fp, "random_gather_4B_per_s": g4, "random_red_f32_per_s": r4,
-                          "gather_plus_red_per_s": cs, "cell_steps_per_s_mean_launch": per_launch,
-                          "frac_of_gather_plus_red": per_launch / cs,
-                          "note": "gather_plus_red = one 4-byte gather and one fp32 red.global.add per random cell: the memory "
-                                  "side of a cell-step with every access independent and no arithmetic"}
+        roof["components"] = roofline_components(G, P, srcs, shard, Aint, stream, steps_f, kern_ms, peak, roof.get("traffic"))
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": args.scaling,
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "dtype_note": "fp32 package state, weights and per-launch accumulator; fp64 frequency integral and totals",
             "config": {"workload": WORKLOADS[args.config], "cells": int(P.n_total), "n_freq": int(P.n_freq),
-                       "packages_per_frequency": int(P.n_packages), "parallelism": f"replicas x{world} (seed + rank), "
-                       "one fp64 all-reduce" if world > 1 else "single GPU",
+                       "packages_per_frequency": int(P.n_packages),
+                       "parallelism": "single GPU" if world == 1 else (
+                           f"{world} ranks, seed + rank each (independent realisations), one fp64 all-reduce" if args.scaling == "weak"
+                           else f"{world} ranks, package ids of one seed split evenly, one fp64 all-reduce"),
                        "l2": "flushed between timed steps (256 MB fill)"},
-            "packages_per_s": world * P.n_packages * P.n_freq / (ms_per_step * 1e-3),
+            "packages_per_s": (world if args.scaling == "weak" else 1) * P.n_packages * P.n_freq / (ms_per_step * 1e-3),
             "cell_steps_per_s_per_frequency": {"median": float(np.median(per_f)), "min": float(per_f.min()),
                                                "max": float(per_f.max())},
-            "cell_steps_per_step": job_steps, "scatterings_per_step": float(scat_total) * world,
-            "energy_conservation_rel": cons,
+            "cell_steps_per_step": job_steps, "scatterings_per_step_rank0": float(scat_total),
+            "energy_conservation_rel": cons_cells,
+            "energy_conservation": {"cells_vs_emitted_minus_escaped": cons_cells, "counters_emitted_absorbed_escaped": cons,
+                                    "weight_drift_max": drift,
+                                    "note": "cells: |sum_cells absorbed_int - sum_f w_f (emitted - escaped)| / sum; weight_drift: max "
+                                            "|w - (1 - deposits)| over escaped packages (fp32 running weight against the deposits made)"},
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "api": "soc_run_host (pinned host buffers)", "s_per_step": e2e_s},
+                    "api": "soc_run_host (pinned host buffers)", "s_per_step": e2e_s,
+                    **({"note": "soc_run_host runs whole package counts: under --scaling strong every rank runs the full "
+                                "problem end to end, so this is the single-GPU end-to-end figure"} if args.scaling == "strong" and world > 1 else {})},
             "gpu_launches": job_launches,
             "wall_s_timed_region": t_wall,
             "roofline": roof}
@@ -340,21 +354,86 @@ def run_ours(args):
     return 0
 
 
-# DRAM traffic of one photon-kernel launch from the committed `ncu --set full` capture of this command
-# (dram__bytes_read.sum + dram__bytes_write.sum, mean over the captured launches); None = not captured yet.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    "5": {"traffic": 54.81e9,
-          "traffic_source": "profiles/r01e_ncu_full_photon_q_config5.txt: dram__bytes_read.sum 40.46 GB + "
-                            "dram__bytes_write.sum 14.36 GB, mean of launches 65-67 (frequency indices 64-66)",
-          "binding_unit": "latency of dependent gathers at 62 % occupancy, not bytes: lts__t_tag_requests 60 %, l1tex2xbar 54 %, "
-                          "issue slots 64 %, DRAM 38 % busy (same capture); see DESIGN.md 6.1"},
-}
+def ncu_traffic(config):
+    """DRAM bytes per cell-step of the photon kernel from the NEWEST committed ncu capture: profiles/r*_ncu_dram_traffic.csv
+    (columns: config, kernel, cell_steps, dram_read_bytes, dram_write_bytes, source -- written from the `ncu --set full`
+    capture named in `source`).  Read at run time so that the figure cannot outlive the capture it came from; None when
+    no capture of this config is committed."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_ncu_dram_traffic.csv")))
+    for path in reversed(files):
+        try:
+            with open(path) as fh:
+                rows = [r for r in csv.DictReader(fh) if r.get("config") == str(config)]
+        except Exception:
+            continue
+        if rows:
+            steps = sum(float(r["cell_steps"]) for r in rows)
+            byts = sum(float(r["dram_read_bytes"]) + float(r["dram_write_bytes"]) for r in rows)
+            return {"bytes_per_cell_step": byts / steps,
+                    "source": f"{os.path.relpath(path, ROOT)} ({'; '.join(sorted({r['source'] for r in rows}))})"}
+    return None
 
 
-def roofline_notes(config):
-    """Static facts about the dominant kernel that go with the roofline object."""
-    d = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(str(config))
-    return dict(d) if d else {}
+def roofline_components(G, P, srcs, shard, Aint, stream, steps_f, kern_ms, hbm_peak, traffic):
+    """north_star's "achieved fraction of the gather and atomic roofline": request rates of the photon
+    kernels against ceilings measured in the same run.
+      requests  = what the lanes issued, counted on the device by the "stats" variant of the same kernels in one extra
+                  pass (the walk is a deterministic function of (seed, ids): the timed passes issue exactly these)
+      ceilings  = soc_probe_throughput, independent random accesses with no arithmetic, (a) over an L2-RESIDENT footprint
+                  (32 MB): the request rate the L1 -> L2 path sustains = the ceiling; (b) over the config's own footprint
+                  (8 B per cell): the NO-LOCALITY FLOOR -- every access its own sector, DRAM misses included; the walk
+                  beats it through the brick layout and L2 reuse along a path, so a ratio > 1 there is expected
+      dram      = ncu DRAM bytes per cell-step of the newest committed capture x cell-steps/s, against the measured HBM peak"""
+    from paper_1812_06632_b200 import soc
+    import torch
+    G.set_option("stats", 1)
+    Aint.zero_()
+    res = G.simulate_spectrum(srcs, P.n_packages, shard.seed, Aint, shard.pkg_begin, shard.pkg_count, stream=stream)
+    G.set_option("stats", 0)
+    torch.cuda.synchronize()
+    secs = float(kern_ms.sum()) * 1e-3
+    gathers, reds = float(sum(r.gather_requests for r in res)), float(sum(r.red_requests for r in res))
+    steps = float(steps_f.sum())
+    vec = P.child is None and 8 * int(P.n_total) > (64 << 20)      # photon_q_kernel (16-byte requests) carries such grids
+    n_ops = 1 << 30
+    rate = lambda kind, fp: n_ops / (soc.probe_throughput(kind, fp, n_ops) * 1e-3)          # noqa: E731
+    l2_fp, cfg_fp = 32 << 20, 8 * int(P.n_total)
+    kg, kr = (6, 4) if vec else (0, 2)
+    ceil_g, ceil_r = rate(kg, l2_fp), rate(kr, l2_fp)
+    floor_g, floor_r, floor_pair = rate(kg, cfg_fp), rate(kr, cfg_fp), rate(5, cfg_fp)
+    comp = {
+        "request_width": "16 B (ld.global.nc.v4 / red.global.add.v4.f32, photon_q_kernel)" if vec else "4 B (ld.global.nc / red.global.add.f32)",
+        "gather": {"requests_per_cell_step": gathers / steps, "per_s": gathers / secs, "ceiling_per_s": ceil_g,
+                   "frac": gathers / secs / ceil_g, "no_locality_floor_per_s": floor_g},
+        "red": {"requests_per_cell_step": reds / steps, "per_s": reds / secs, "ceiling_per_s": ceil_r,
+                "frac": reds / secs / ceil_r, "no_locality_floor_per_s": floor_r},
+        "gather_plus_red_no_locality_floor": {"pairs_per_s": floor_pair, "cell_steps_per_s": steps / secs,
+                                              "ratio": steps / secs / floor_pair,
+                                              "note": "a FLOOR, not a ceiling: one 4-byte gather + one fp32 add per uniformly random "
+                                                      "cell of the config's footprint; ratio > 1 = locality the walk exploits"},
+        "ceiling_footprint_bytes": l2_fp, "floor_footprint_bytes": cfg_fp,
+    }
+    fr = [comp["gather"]["frac"], comp["red"]["frac"]]
+    if traffic:
+        dram = traffic * len(steps_f) / secs / 1e9
+        comp["dram"] = {"GB_per_s": dram, "peak_GB_per_s": hbm_peak, "frac": dram / hbm_peak}
+        fr.append(dram / hbm_peak)
+    comp["frac_max"] = max(fr)
+    comp["binding"] = ["gather", "red", "dram"][int(np.argmax(fr))]
+    return comp
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: re-execute under torch.distributed.run, one rank per GPU."""
+    import subprocess
+    import torch
+    if torch.cuda.device_count() < args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but only {torch.cuda.device_count()} CUDA device(s) visible")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--local-addr", "127.0.0.1", os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -364,6 +443,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", choices=sorted(WORKLOADS), default="5")
+    ap.add_argument("--scaling", choices=["weak", "strong"], default="weak",
+                    help="weak: every rank the full package count with seed + rank; strong: ids of one seed split over ranks")
     ap.add_argument("--packages", type=int, default=0, help="override packages per frequency (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probes", action="store_true", help="skip the random gather / scatter-add ceiling probes")
@@ -373,7 +454,9 @@ def main():
         raise SystemExit("need --steps >= 1 and --warmup >= 0")
     if args.impl == "reference":
         return run_reference(args)
-    args.warmup = max(args.warmup, 1)
+    args.warmup = max(args.warmup, 2)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args)
     return run_ours(args)
 
 

@@ -95,6 +95,10 @@ typedef struct {
                                             the package's initial energy (escaped is taken from the deposits while less than
                                             half was absorbed, so emitted = absorbed + escaped does not see this drift);
                                             replay mode: 0 (fp64 weight, deposit = weight difference) */
+    uint64_t gather_requests, red_requests;   /* option "stats" = 1, production mode: global-memory gather instructions
+                                            (cell words, reverse links) and reduction instructions (red.global.add) the
+                                            lanes issued -- the request counts behind bench.py's roofline.components;
+                                            0 otherwise */
 } soc_freq_result;
 
 /* per-package replay record (DEVICE array written by soc_simulate_packages) */
@@ -159,7 +163,8 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
 
 /* Tuning knobs (all have defaults chosen for B200): "blocks_per_sm", "threads", "refill_threshold" (replay
  * kernel), "service_threshold" (parked lanes that trigger a service pass), "hot_cache" (0/1: shared partial sums
- * for the cells around point sources), "acc32" (0/1: fp32 per-launch accumulator), "overlap" (0/1: soc_simulate_spectrum overlaps consecutive frequencies on two streams), "kernel" (production kernel on
+ * for the cells around point sources), "stats" (0/1: the production kernels count their gather and reduction
+ * instructions into soc_freq_result; a slower kernel variant, for measurement runs), "acc32" (0/1: fp32 per-launch accumulator), "overlap" (0/1: soc_simulate_spectrum overlaps consecutive frequencies on two streams), "kernel" (production kernel on
  * regular grids: 0 = chosen by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel), "carveout"
  * (preferred shared-memory carve-out in %, -1 = driver default); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
@@ -175,8 +180,9 @@ int soc_get_timings(soc_grid *grid, int32_t n, float *ms);
 
 /* Roofline probes: random 4-byte gathers (kind 0), random fp64 red.global.add (kind 1),
  * random fp32 red.global.add (kind 2), random 32-byte gathers (kind 3: one sector = a 2x2x2 brick of fp32 cells),
- * random 16-byte red.global.add.v4.f32 (kind 4), and the memory side of one cell-step (kind 5: a 4-byte gather from
- * the first half of the footprint and an fp32 red.global.add at the same random cell of the second half) over a
+ * random 16-byte red.global.add.v4.f32 (kind 4), random 16-byte gathers (kind 6: half a brick), and the memory side of
+ * one cell-step (kind 5: a 4-byte gather from the first half of the footprint and an fp32 red.global.add at the same
+ * random cell of the second half) over a
  * footprint of `footprint_bytes`, n_ops operations in total, uniform addresses, no arithmetic, every access
  * independent of the others.  *ms receives the CUDA-event time of the probe kernel. */
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms);

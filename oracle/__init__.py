@@ -31,7 +31,9 @@ def build(force: bool = False) -> str:
 
 class _Sources(C.Structure):
     _fields_ = [("bg_intensity", C.c_double), ("n_point", C.c_int32), ("ps_pos", C.c_void_p),
-                ("ps_lum", C.c_void_p), ("n_bg", C.c_int64), ("beam", C.c_void_p)]
+                ("ps_lum", C.c_void_p), ("n_bg", C.c_int64), ("beam", C.c_void_p),
+                ("n_dust", C.c_int64), ("dust_T", C.c_void_p), ("dust_count", C.c_void_p),
+                ("dust_freq_hz", C.c_double), ("dust_self", C.c_void_p)]
 
 
 class _Result(C.Structure):
@@ -75,6 +77,17 @@ def lib():
         L.soc_oracle_trapezoid_weights.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
         L.soc_oracle_update_temperatures.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p,
                                                      C.c_int32, C.c_double, C.c_double, C.c_void_p]
+        L.soc_oracle_update_temperatures_ali.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
+                                                         C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_void_p]
+        L.soc_oracle_planck.argtypes = [C.c_double, C.c_double]
+        L.soc_oracle_planck.restype = C.c_double
+        L.soc_oracle_cell_luminosity.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
+        L.soc_oracle_emission_counts.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_int32, C.c_int64,
+                                                 C.c_int32, C.c_void_p]
+        L.soc_oracle_emission_counts.restype = C.c_int64
+        L.soc_oracle_emit_cell.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.soc_oracle_dust_stride.argtypes = [C.c_int64]
+        L.soc_oracle_dust_stride.restype = C.c_int64
         L.soc_oracle_sizeof_replay.restype = C.c_int64
         L.soc_oracle_sizeof_trace.restype = C.c_int64
         L.soc_oracle_grid_parent.argtypes = [C.c_void_p, C.c_int32]
@@ -202,6 +215,17 @@ def _sources_struct(src, keep):
         beam = np.ascontiguousarray(beam, dtype=np.float64).reshape(6)
         keep.append(beam)
         s.beam = beam.ctypes.data
+    if src.get("dust_count") is not None:             # f1: dust re-emission (the last n_dust package ids)
+        T = np.ascontiguousarray(src["dust_T"], dtype=np.float32)
+        cnt = np.ascontiguousarray(src["dust_count"], dtype=np.int32)
+        keep += [T, cnt]
+        s.dust_T, s.dust_count = T.ctypes.data, cnt.ctypes.data
+        s.n_dust = int(cnt.sum(dtype=np.int64))
+        s.dust_freq_hz = float(src["dust_freq_hz"])
+        if src.get("dust_self") is not None:          # f3: in-cell absorption of the cells' own packages, accumulated into
+            a = src["dust_self"]
+            assert a.dtype == np.float64 and a.flags.c_contiguous
+            s.dust_self = a.ctypes.data
     return s
 
 
@@ -210,7 +234,8 @@ def simulate(grid: Grid, kabs, ksca, g, ifreq, sources: dict, n_packages, seed, 
              f32state=False):
     """Run packages [pkg_begin, pkg_begin+pkg_count).  Returns (absorbed, Result, replay, trace).
 
-    sources: dict(bg_intensity=, ps_pos=, ps_lum=, n_bg=, beam=).  `absorbed` is accumulated into.
+    sources: dict(bg_intensity=, ps_pos=, ps_lum=, n_bg=, beam=, dust_T=, dust_count=, dust_freq_hz=, dust_self=).
+    `absorbed` (and `dust_self`, if given) are accumulated into.
     f32state=False: soc_oracle_simulate, THE oracle (fp64 throughout).  f32state=True: the named variant
     soc_oracle_simulate_f32state (state snapped to fp32 at every store; replay-parity tests only).
     """
@@ -226,10 +251,14 @@ def simulate(grid: Grid, kabs, ksca, g, ifreq, sources: dict, n_packages, seed, 
     keep = []
     s = _sources_struct(sources, keep)
 
-    def run(b, n, acc, rep, trc):
+    def run(b, n, acc, rep, trc, self_acc=None):
         r = _Result()
         nt = C.c_int64(0)
-        rc = entry(grid._h, float(kabs), float(ksca), float(g), int(ifreq), C.byref(s),
+        st = s
+        if self_acc is not None:                       # a thread's own in-cell accumulator
+            st = _Sources.from_buffer_copy(s)
+            st.dust_self = self_acc.ctypes.data
+        rc = entry(grid._h, float(kabs), float(ksca), float(g), int(ifreq), C.byref(st),
                    int(n_packages), int(seed), float(weight), int(b), int(n), _p(acc),
                    C.byref(r), _p(rep), _p(trc), 0 if trc is None else len(trc), C.byref(nt))
         if rc != 0:
@@ -244,19 +273,65 @@ def simulate(grid: Grid, kabs, ksca, g, ifreq, sources: dict, n_packages, seed, 
 
     bounds = np.linspace(0, pkg_count, threads + 1).astype(np.int64)
     accs = [np.zeros(grid.n_total, dtype=np.float64) for _ in range(threads)]
+    want_self = sources.get("dust_self") is not None and sources.get("dust_count") is not None
+    selfs = [np.zeros(grid.n_total, dtype=np.float64) for _ in range(threads)] if want_self else None
 
     def job(i):
         b, e = int(bounds[i]), int(bounds[i + 1])
         rep = None if replay is None else replay[b:e]
-        return run(pkg_begin + b, e - b, accs[i], rep, None)[0]
+        return run(pkg_begin + b, e - b, accs[i], rep, None, selfs[i] if want_self else None)[0]
 
     with ThreadPoolExecutor(threads) as ex:
         rs = list(ex.map(job, range(threads)))
     for a in accs:
         absorbed += a
+    if want_self:
+        for a in selfs:
+            sources["dust_self"] += a
     res = Result(sum(r.emitted for r in rs), sum(r.escaped for r in rs), sum(r.absorbed for r in rs),
                  sum(r.cell_steps for r in rs), sum(r.scatterings for r in rs), sum(r.terminated for r in rs))
     return absorbed, res, replay, None
+
+
+def planck(nu, T):
+    return lib().soc_oracle_planck(float(nu), float(T))
+
+
+def cell_luminosity(grid: Grid, kabs, freq_hz, T):
+    """L_c = 4 pi kabs rho_c h^3 B_nu(T_c) per cell (0 for parents, empty leaves, T <= 0)."""
+    T = np.ascontiguousarray(T, dtype=np.float32)
+    out = np.zeros(grid.n_total, dtype=np.float64)
+    lib().soc_oracle_cell_luminosity(grid._h, float(kabs), float(freq_hz), _p(T), _p(out))
+    return out
+
+
+def emission_counts(grid: Grid, kabs, freq_hz, T, mode, n_request, cap=10000):
+    """Packages per cell: mode 'uniform' (same number from every emitting cell) or 'weighted' (in proportion to the
+    cell's luminosity, capped).  Returns int32[n_total]."""
+    T = np.ascontiguousarray(T, dtype=np.float32)
+    out = np.zeros(grid.n_total, dtype=np.int32)
+    n = lib().soc_oracle_emission_counts(grid._h, float(kabs), float(freq_hz), _p(T), {"uniform": 0, "weighted": 1}[mode],
+                                         int(n_request), int(cap), _p(out))
+    if n < 0:
+        raise ValueError("soc_oracle_emission_counts: bad argument")
+    assert n == int(out.sum(dtype=np.int64))
+    return out
+
+
+def emit_cell(u):
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    f, d = np.zeros(3), np.zeros(3)
+    lib().soc_oracle_emit_cell(_p(u), _p(f), _p(d))
+    return f, d
+
+
+def update_temperatures_ali(grid: Grid, absorbed, self_abs, emitted, scale, table_T, E_min, E_max):
+    a, sa, em = (np.ascontiguousarray(x, dtype=np.float64) for x in (absorbed, self_abs, emitted))
+    table_T = np.ascontiguousarray(table_T, dtype=np.float32)
+    out = np.zeros(grid.n_total, dtype=np.float32)
+    lib().soc_oracle_update_temperatures_ali(grid._h, _p(a), _p(sa), _p(em), float(scale), _p(table_T), len(table_T),
+                                             float(E_min), float(E_max), _p(out))
+    return out
 
 
 def update_temperatures(grid: Grid, absorbed, scale, table_T, E_min, E_max):
@@ -265,4 +340,66 @@ def update_temperatures(grid: Grid, absorbed, scale, table_T, E_min, E_max):
     out = np.zeros(grid.n_total, dtype=np.float32)
     lib().soc_oracle_update_temperatures(grid._h, _p(absorbed), float(scale), _p(table_T), len(table_T),
                                          float(E_min), float(E_max), _p(out))
+    return out
+
+
+def dust_stride(n_dust):
+    return int(lib().soc_oracle_dust_stride(int(n_dust)))
+
+
+def iterate(grid: Grid, freq_hz, kabs, ksca, g, const_sources, n_const, n_request, seed, t_scale, table_T, E_min, E_max,
+            mode="weighted", cap=10000, reference_field=True, ali=False, update_T=True, T_start=None, threads=1,
+            f32state=False):
+    """Iterated run with dust re-emission (rows f1, f3; readings F4-F6 of DESIGN.md), step by step:
+
+      iteration 0   constant sources only (background, point sources), n_const packages per frequency, seed:
+                    A_const = sum_f w_f A_f;  T = table(A_const)   (T_start overrides it)
+      iteration i   i = 1 .. len(n_request): for every frequency the cells emit n_request[i-1] packages (counts by `mode`
+                    from the current T), seed + i:  D_i = sum_f w_f A_dust,f  (and the in-cell part S_i, emission Em_i)
+                    reference field: R_i = running mean of D_1..D_i weighted by n_request (else R_i = D_i)
+                    T = table(A_const + R_i)   -- with ALI from (A - S) / (1 - S / Em) (soc_oracle_update_temperatures_ali)
+    Returns dict(T=[T_0, T_1, ...], A_const, R, S, Em, emitted=[...], escaped=[...]) (frequency-integrated energies)."""
+    freq_hz = np.asarray(freq_hz, dtype=np.float64)
+    n_f = len(freq_hz)
+    w = trapezoid_weights(freq_hz)
+    A_const = np.zeros(grid.n_total)
+    esc0 = em0 = 0.0
+    for f in range(n_f):
+        _, r, _, _ = simulate(grid, kabs[f], ksca[f], g[f], f, const_sources[f], n_const, seed, w[f], absorbed=A_const,
+                              threads=threads, f32state=f32state)
+        esc0 += w[f] * r.escaped
+        em0 += w[f] * r.emitted
+    T = update_temperatures(grid, A_const, t_scale, table_T, E_min, E_max) if T_start is None else np.asarray(T_start, np.float32)
+    out = dict(T=[T.copy()], A_const=A_const, emitted=[em0], escaped=[esc0], D=[], n_dust=[])
+    R, S, Em, W = np.zeros(grid.n_total), np.zeros(grid.n_total), np.zeros(grid.n_total), 0.0
+    for i, n_req in enumerate(n_request, start=1):
+        D, Si, Emi = np.zeros(grid.n_total), np.zeros(grid.n_total), np.zeros(grid.n_total)
+        esc = em = 0.0
+        nd = 0
+        for f in range(n_f):
+            cnt = emission_counts(grid, kabs[f], freq_hz[f], T, mode, n_req, cap)
+            n_dust = int(cnt.sum(dtype=np.int64))
+            nd += n_dust
+            Emi += w[f] * cell_luminosity(grid, kabs[f], freq_hz[f], T)
+            if n_dust == 0:
+                continue
+            src = dict(dust_T=T, dust_count=cnt, dust_freq_hz=freq_hz[f], dust_self=Si, n_bg=0)
+            _, r, _, _ = simulate(grid, kabs[f], ksca[f], g[f], f, src, n_dust, seed + i, w[f], absorbed=D, threads=threads,
+                                  f32state=f32state)
+            esc += w[f] * r.escaped
+            em += w[f] * r.emitted
+        if reference_field:
+            R = (W * R + n_req * D) / (W + n_req)
+            S = (W * S + n_req * Si) / (W + n_req)
+            Em = (W * Em + n_req * Emi) / (W + n_req)
+            W += n_req
+        else:
+            R, S, Em = D, Si, Emi
+        A = A_const + R
+        if update_T:
+            T = (update_temperatures_ali(grid, A, S, Em, t_scale, table_T, E_min, E_max) if ali
+                 else update_temperatures(grid, A, t_scale, table_T, E_min, E_max))
+        out["T"].append(T.copy()); out["emitted"].append(em); out["escaped"].append(esc); out["D"].append(D)
+        out["n_dust"].append(nd)
+    out.update(R=R, S=S, Em=Em)
     return out

@@ -215,6 +215,14 @@ typedef struct {
     const double *ps_lum;  /* [n_point] */
     int64_t n_bg;          /* ids [0,n_bg) background, the rest point sources; -1 = default split */
     const double *beam;    /* test hook: [6] = position, direction; every package is this beam, E0 = 1 */
+    /* f1, dust re-emission: the LAST n_dust package ids are emitted by the cells themselves */
+    int64_t n_dust;            /* 0 = none; must equal the sum of dust_count */
+    const float *dust_T;       /* [n_total] dust temperature per cell (what soc_oracle_update_temperatures wrote) */
+    const int32_t *dust_count; /* [n_total] packages sent from each cell (soc_oracle_emission_counts) */
+    double dust_freq_hz;       /* frequency of this simulation, for B_nu(T) */
+    double *dust_self;         /* f3, may be NULL: [n_total] += weight * energy a dust package deposits in the cell that
+                                  emitted it before it first leaves that cell (the absorption-emission cycle inside a
+                                  cell that the diagonal ALI operator solves explicitly) */
 } soc_oracle_sources;
 
 typedef struct {
@@ -339,6 +347,89 @@ void soc_oracle_emit_point(const double pos[3], const double u[2],
     d[0] = st * cos(phi); d[1] = st * sin(phi); d[2] = mu;
 }
 
+/* ------------------------------------------------------------------ f1: dust re-emission
+ * "If grains are assumed to be in an equilibrium with the radiation field, the emission is calculated by SOC itself"
+ * (PAPER.md:67); the cells are then a third source of photon packages, needed when "dust is heated to such high
+ * temperatures that its emission no longer freely escapes the model volume".
+ * Luminosity of leaf c at frequency nu, in the energy unit of pi I S (lengths in root-cell edges):
+ *     L_c = 4 pi kabs rho_c h_l^3 B_nu(T_c)            (kabs rho = absorption optical depth per unit length)
+ * Package counts per cell are the host's policy (readings F1-F2 in DESIGN.md):
+ *   mode 0, uniform:  "the same number of photon packages is sent per each cell", the total "a multiple of the number
+ *                     of cells": m = ceil(n_request / n_emitting) packages from every cell with L_c > 0
+ *   mode 1, weighted: "the number of emitted photon packages is weighted according to the emission", "the maximum
+ *                     number of photon packages sent from any single cell was limited ... with a user-defined
+ *                     parameter": n_c = min(cap, ceil(n_request L_c / sum L)) for L_c > 0
+ * Each package of cell c carries L_c / n_c, so the emitted energy is exactly sum L_c whatever the counts. */
+#define SOC_O_H  6.62607015e-27
+#define SOC_O_KB 1.380649e-16
+#define SOC_O_C  2.99792458e10
+
+double soc_oracle_planck(double nu, double T)
+{
+    if (!(T > 0.0)) return 0.0;
+    return 2.0 * SOC_O_H * nu * nu * nu / (SOC_O_C * SOC_O_C) / expm1(SOC_O_H * nu / (SOC_O_KB * T));
+}
+
+/* L_c for every cell (0 for parents, empty leaves and T <= 0).  lum: [n_total]. */
+void soc_oracle_cell_luminosity(const soc_oracle_grid *G, double kabs, double freq_hz, const float *T, double *lum)
+{
+    for (int l = 1; l <= G->n_levels; ++l) {
+        const double h = ldexp(1.0, -(l - 1)), vol = h * h * h;
+        for (int64_t gid = G->level_off[l - 1]; gid < G->level_off[l]; ++gid) {
+            const double rho = (double)G->rho[gid];
+            lum[gid] = (G->child[gid] >= 0 || !(rho > 0.0)) ? 0.0
+                     : 4.0 * SOC_O_PI * kabs * rho * vol * soc_oracle_planck(freq_hz, (double)T[gid]);
+        }
+    }
+}
+
+/* Package counts per cell; returns their sum (n_dust), or -1 on a bad argument. */
+int64_t soc_oracle_emission_counts(const soc_oracle_grid *G, double kabs, double freq_hz, const float *T, int32_t mode,
+                                   int64_t n_request, int32_t cap, int32_t *count)
+{
+    if (!G || !T || !count || n_request < 0 || (mode != 0 && mode != 1) || (mode == 1 && cap < 1)) return -1;
+    double *lum = (double *)malloc(sizeof(double) * (size_t)G->n_total);
+    soc_oracle_cell_luminosity(G, kabs, freq_hz, T, lum);
+    double tot = 0.0;
+    int64_t n_emit = 0, n_dust = 0;
+    for (int64_t c = 0; c < G->n_total; ++c) { tot += lum[c]; n_emit += lum[c] > 0.0; }
+    const int64_t m = n_emit > 0 ? (n_request + n_emit - 1) / n_emit : 0;
+    for (int64_t c = 0; c < G->n_total; ++c) {
+        int64_t n = 0;
+        if (lum[c] > 0.0 && n_request > 0) {
+            if (mode == 0) n = m;
+            else { n = (int64_t)ceil((double)n_request * lum[c] / tot); if (n < 1) n = 1; if (n > cap) n = cap; }
+        }
+        count[c] = (int32_t)n;
+        n_dust += n;
+    }
+    free(lum);
+    return n_dust;
+}
+
+/* Stride that spreads consecutive dust package ids over the cells: the odd number nearest below n_dust / golden ratio
+ * that is coprime to n_dust (so that q -> q * stride mod n_dust is a permutation of [0, n_dust)). */
+int64_t soc_oracle_dust_stride(int64_t n_dust)
+{
+    if (n_dust <= 2) return 1;
+    int64_t s = (int64_t)floor((double)n_dust * 0.6180339887498949) | 1;
+    for (;;) {
+        int64_t a = s, b = n_dust;
+        while (b) { int64_t t = a % b; a = b; b = t; }
+        if (a == 1) return s;
+        s += 2;
+    }
+}
+
+/* A dust package (readings F3): uniform point in the cell, isotropic direction -- "random locations and directions
+ * within each cell".  u[0..2] -> position, u[3] -> cos(theta) = 2u - 1, u[4] -> azimuth. */
+void soc_oracle_emit_cell(const double u[5], double f[3], double d[3])
+{
+    for (int j = 0; j < 3; ++j) f[j] = u[j];
+    double mu = 2.0 * u[3] - 1.0, st = sqrt(fmax(0.0, 1.0 - mu * mu)), phi = 2.0 * SOC_O_PI * u[4];
+    d[0] = st * cos(phi); d[1] = st * sin(phi); d[2] = mu;
+}
+
 /* ------------------------------------------------------------------ a4-a9: the walk - */
 #define SOC_O_WMIN 1e-9   /* termination: weight below WMIN * E0, residual deposited (S7) */
 
@@ -355,14 +446,33 @@ static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g
     if (!G || !src || !absorbed || n_packages < 0 || pkg_begin < 0 || pkg_count < 0 ||
         pkg_begin + pkg_count > n_packages || !(kabs >= 0.0) || !(ksca >= 0.0) || !(fabs(g) < 1.0))
         return -1;
-    const int64_t n_bg = src->beam ? 0 : split_n_bg(src, n_packages);
-    if (n_bg > n_packages) return -1;
+    /* ids [0, n_bg) background, [n_bg, n_packages - n_dust) point sources, the last n_dust ids dust re-emission */
+    const int64_t n_dust = src->beam ? 0 : src->n_dust;
+    if (n_dust < 0 || n_dust > n_packages) return -1;
+    const int64_t n_const = n_packages - n_dust;
+    const int64_t n_bg = src->beam ? 0 : split_n_bg(src, n_const);
+    if (n_bg > n_const) return -1;
+    int64_t *dust_first = NULL;      /* [n_total + 1] first dust index of every cell: prefix sums of dust_count */
+    double *dust_lum = NULL;
+    if (n_dust > 0) {
+        if (!src->dust_T || !src->dust_count || !(src->dust_freq_hz > 0.0)) return -1;
+        dust_first = (int64_t *)malloc(sizeof(int64_t) * (size_t)(G->n_total + 1));
+        dust_lum = (double *)malloc(sizeof(double) * (size_t)G->n_total);
+        soc_oracle_cell_luminosity(G, kabs, src->dust_freq_hz, src->dust_T, dust_lum);
+        dust_first[0] = 0;
+        for (int64_t c = 0; c < G->n_total; ++c) {
+            if (src->dust_count[c] < 0 || (src->dust_count[c] > 0 && !(dust_lum[c] > 0.0))) { free(dust_first); free(dust_lum); return -1; }
+            dust_first[c + 1] = dust_first[c] + src->dust_count[c];
+        }
+        if (dust_first[G->n_total] != n_dust || n_dust >= ((int64_t)1 << 32)) { free(dust_first); free(dust_lum); return -1; }
+    }
+    const int64_t dust_stride = soc_oracle_dust_stride(n_dust);
     if (!src->beam) {
-        if (n_bg > 0 && !(src->bg_intensity > 0.0)) return -1;
-        if (n_packages - n_bg > 0 && src->n_point <= 0) return -1;
+        if (n_bg > 0 && !(src->bg_intensity > 0.0)) { free(dust_first); free(dust_lum); return -1; }
+        if (n_const - n_bg > 0 && src->n_point <= 0) { free(dust_first); free(dust_lum); return -1; }
         for (int k = 0; k < src->n_point; ++k) {
             const double *p = src->ps_pos + 3 * k;
-            if (!(p[0] > 0.0 && p[0] < G->nx && p[1] > 0.0 && p[1] < G->ny && p[2] > 0.0 && p[2] < G->nz)) return -1;
+            if (!(p[0] > 0.0 && p[0] < G->nx && p[1] > 0.0 && p[1] < G->ny && p[2] > 0.0 && p[2] < G->nz)) { free(dust_first); free(dust_lum); return -1; }
         }
     }
     const double surf = 2.0 * ((double)G->ny * G->nz + (double)G->nz * G->nx + (double)G->nx * G->ny);
@@ -373,6 +483,7 @@ static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g
         soc_oracle_state S;
         int32_t ijk[3];
         double E0, f0[3], d0[3];
+        int64_t origin_gid = -1;                   /* dust package: the cell that emitted it */
         uint32_t w0[4], w1[4];
         soc_oracle_stream_block(seed, ifreq, p, 0u, w0);
         soc_oracle_stream_block(seed, ifreq, p, 1u, w1);
@@ -390,8 +501,21 @@ static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g
                             soc_oracle_uniform(w0[3]), soc_oracle_uniform(w1[0]) };
             soc_oracle_emit_background(G->nx, G->ny, G->nz, u, ijk, f0, d0);
             E0 = SOC_O_PI * src->bg_intensity * surf / (double)n_bg;
+        } else if (p >= n_const) {
+            /* f1: dust package q belongs to the cell c with dust_first[c] <= q < dust_first[c + 1] */
+            /* (consecutive ids are spread over the cells -- q -> q * stride mod n_dust, stride coprime to n_dust --
+             * as point-source ids are interleaved over the sources (S3): simultaneous packages of one cell are what
+             * the paper blames for its GPU slow-down with emission weighting) */
+            const int64_t q = (int64_t)(((uint64_t)(p - n_const) * (uint64_t)dust_stride) % (uint64_t)n_dust);
+            int64_t lo = 0, hi = G->n_total;               /* invariant: dust_first[lo] <= q < dust_first[hi] */
+            while (hi - lo > 1) { int64_t mid = (lo + hi) / 2; if (dust_first[mid] <= q) lo = mid; else hi = mid; }
+            origin_gid = lo;
+            double u[5] = { soc_oracle_uniform(w0[0]), soc_oracle_uniform(w0[1]), soc_oracle_uniform(w0[2]),
+                            soc_oracle_uniform(w0[3]), soc_oracle_uniform(w1[0]) };
+            soc_oracle_emit_cell(u, f0, d0);
+            E0 = dust_lum[lo] / (double)src->dust_count[lo];
         } else {
-            int64_t q = p - n_bg, n_ps = n_packages - n_bg;
+            int64_t q = p - n_bg, n_ps = n_const - n_bg;
             int32_t k = (int32_t)(q % src->n_point);
             /* count_k = number of ids q in [0, n_ps) with q mod n_point == k */
             int64_t count_k = n_ps / src->n_point + ((n_ps % src->n_point) > k ? 1 : 0);
@@ -401,9 +525,17 @@ static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g
         }
         S.f32state = f32state;
         for (int j = 0; j < 3; ++j) { S.f[j] = keep(f0[j], f32state); S.d[j] = keep(d0[j], f32state); }
-        S.level = 1;
-        S.cell = ijk[0] + G->nx * (ijk[1] + G->ny * ijk[2]);
-        descend(G, &S);
+        if (origin_gid >= 0) {                         /* a dust package starts inside its (leaf) cell */
+            int32_t l = 1;
+            while (origin_gid >= G->level_off[l]) ++l;
+            S.level = l;
+            S.cell = (int32_t)(origin_gid - G->level_off[l - 1]);
+        } else {
+            S.level = 1;
+            S.cell = ijk[0] + G->nx * (ijk[1] + G->ny * ijk[2]);
+            descend(G, &S);
+        }
+        int in_origin = origin_gid >= 0;               /* f3: still inside the emitting cell, never left it */
 
         double E = E0;
         R.emitted += E0;
@@ -445,6 +577,7 @@ static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g
             /* a7: path-length estimator, continuous absorption */
             const double dep = E * (-expm1(-ds_used * rho * kabs));
             absorbed[gid] += weight * dep;
+            if (in_origin && src->dust_self) src->dust_self[gid] += weight * dep;
             R.absorbed += dep;
             E -= dep;
             steps += 1;
@@ -462,6 +595,7 @@ static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g
             /* a9: termination */
             if (E < SOC_O_WMIN * E0) {
                 absorbed[gid] += weight * E;
+                if (in_origin && src->dust_self) src->dust_self[gid] += weight * E;
                 R.absorbed += E;
                 E = 0.0;
                 R.terminated += 1;
@@ -492,6 +626,7 @@ static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g
                 tau_rem = tau_drawn;
             } else {
                 tau_rem = keep(tau_rem - dtau, f32state);
+                in_origin = 0;                           /* the package leaves the cell it is in */
                 if (!move_across(G, &S, a, S.d[a] > 0.0 ? 1 : -1)) {
                     e_esc = E;                           /* a9: escape */
                     R.escaped += E;
@@ -507,6 +642,7 @@ static int simulate(const soc_oracle_grid *G, double kabs, double ksca, double g
             rp->hash = hash; rp->steps = steps; rp->scatters = scat; rp->e_escaped = e_esc;
         }
     }
+    free(dust_first); free(dust_lum);
     if (res) *res = R;
     if (n_trace) *n_trace = nt;
     return 0;
@@ -576,6 +712,31 @@ void soc_oracle_update_temperatures(const soc_oracle_grid *G, const double *abso
             T_out[gid] = (float)T;
         }
     }
+}
+
+/* ------------------------------------------------------------------ f3: ALI ---------
+ * Accelerated lambda iteration "with a diagonal operator that solves explicitly for the cycle of photons that are
+ * absorbed within the emitting cell", at the cost of "one additional floating point number per cell, which is needed
+ * to keep track of the photon escape probabilities for each cell".  Reading F6:
+ *   self_c    = frequency-integrated energy that the cell's own packages deposited in it before first leaving it
+ *   emitted_c = frequency-integrated energy the cell emitted in that simulation (sum_f w_f L_c,f at the OLD temperature)
+ *   beta_c    = self_c / emitted_c                 (1 - beta_c = the cell's photon escape probability)
+ * Energy balance with the in-cell cycle taken out:  Lambda(T_new) rho V (1 - beta_c) = absorbed_c - self_c, i.e. the
+ * table is entered with  E_c = scale (absorbed_c - self_c) / (rho_c h^3 (1 - beta_c)).  beta_c = 0 gives a11 back. */
+void soc_oracle_update_temperatures_ali(const soc_oracle_grid *G, const double *absorbed, const double *self_abs,
+                                        const double *emitted, double scale, const float *table_T, int32_t n_table,
+                                        double E_min, double E_max, float *T_out)
+{
+    double *eff = (double *)malloc(sizeof(double) * (size_t)G->n_total);
+    for (int64_t c = 0; c < G->n_total; ++c) {
+        double beta = (emitted[c] > 0.0) ? self_abs[c] / emitted[c] : 0.0;
+        if (beta > 0.999) beta = 0.999;            /* a cell that keeps everything: bounded acceleration */
+        if (beta < 0.0) beta = 0.0;
+        eff[c] = (absorbed[c] - self_abs[c]) / (1.0 - beta);
+        if (eff[c] < 0.0) eff[c] = 0.0;
+    }
+    soc_oracle_update_temperatures(G, eff, scale, table_T, n_table, E_min, E_max, T_out);
+    free(eff);
 }
 
 int64_t soc_oracle_sizeof_replay(void) { return (int64_t)sizeof(soc_oracle_replay); }

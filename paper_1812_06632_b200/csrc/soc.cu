@@ -45,6 +45,7 @@ struct DevResult {                      // one slot per launch, accumulated with
     double emitted, escaped, absorbed;
     unsigned long long cell_steps, scatterings, terminated;
     unsigned int drift_bits, pad_;      // fp32 bits of max |w - (1 - sum of deposits)| over the packages that escaped
+    unsigned long long gathers, reds;   // option "stats": global-memory gather / reduction instructions issued by the lanes
 };
 
 struct SimParams {
@@ -112,6 +113,7 @@ struct soc_grid {
     int opt_refill_threshold = 1;
     int opt_service_threshold = 0;            // parked lanes that trigger a service pass; 0 = by scattering depth (8 or 16)
     int opt_hot_cache = 1;
+    int opt_stats = 0;                        // production kernels count their gather / reduction instructions (slower variant)
     int opt_carveout = -1;                    // preferred shared-memory carve-out of the photon kernels in %, -1 = driver default
     double rho_mean = 0.0;                    // mean density of the root-level leaves
     int opt_kernel = 0;                       // regular grids: 0 = by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel
@@ -550,6 +552,7 @@ __global__ void __launch_bounds__(256) photon_kernel(const __grid_constant__ Sim
 //     scatter-add is (double)(sum of deposits in the cell visit) * E0 into the fp64 accumulator
 // ------------------------------------------------------------------------------------------------
 constexpr uint32_t kSentinel = 0xffffffffu;       // cell word of a ghost cell
+
 enum : int { RUN = 0, SCAT = 1, DONE = 2, EMPTY = 3, NEWID = 4, DEAD = 5 };
 
 struct FastParams {
@@ -598,6 +601,7 @@ struct FPkg {
                             // source cell while the package is inside the cached cube, else -1
     long long id;
     unsigned long long hash;
+    uint32_t n_ld, n_red;   // REPLAY variants only (option "stats"): gathers / reductions issued for this package
 };
 
 // Distance to the exit face along axis a, in cell edges:  t_a = (d_a > 0 ? 1 - f_a : -f_a) / d_a
@@ -625,6 +629,7 @@ __device__ __forceinline__ float package_rel(const FastParams &P, int src)
 __device__ __forceinline__ bool fast_descend(const FastParams &P, FPkg &p)
 {
     uint32_t cw = __ldg(P.cellw + p.rel);
+    p.n_ld += 1;
     if (cw == kSentinel) { p.cw = cw; return false; }
     while ((int32_t)cw < 0) {
         int slot = 0;
@@ -635,6 +640,7 @@ __device__ __forceinline__ bool fast_descend(const FastParams &P, FPkg &p)
         p.rel = (int)(cw & 0x7fffffffu) + slot;
         p.h *= 0.5f;
         cw = __ldg(P.cellw + p.rel);
+        p.n_ld += 1;
     }
     p.cw = cw;
     return true;
@@ -671,8 +677,9 @@ __device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, long lon
     fast_emit_core(P, p, id, ix, iy, iz, dx, dy, dz);
     p.h = 1.0f;
     p.rel = root_id(P, ix, iy, iz);
+    p.n_ld = 0; p.n_red = 0;
     if (HIER) { p.anc1 = p.anc2 = p.anc3 = -1; fast_descend(P, p); }
-    else p.cw = __ldg(P.cellw + p.rel);
+    else { p.cw = __ldg(P.cellw + p.rel); p.n_ld = 1; }
     // hot-cell tracking starts at the centre of the cube of the package's own source (regular grids only)
     p.disp = (!HIER && p.src >= 0 && P.hot_r >= 0) ? P.hot_r * 0x010101 : -1;
     p.steps = 0; p.scat = 0;
@@ -713,7 +720,9 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
     unsigned long long acc_steps = 0;
     unsigned acc_scat = 0, acc_term = 0;
     float acc_drift = 0.0f;                      // max |w - (1 - absrel)|: the running weight against the sum of the deposits
+    unsigned long long acc_ld = 0, acc_red = 0;  // REPLAY variants: request counters (option "stats")
     FPkg p;
+    p.n_ld = 0; p.n_red = 0;
     p.src = -1; p.disp = -1; p.w = 0.0f; p.absrel = 0.0f; p.steps = 0; p.scat = 0; p.cw = 0; p.rel = 0; p.h = 1.0f;
     p.anc1 = p.anc2 = p.anc3 = -1;
     int need = EMPTY;
@@ -742,9 +751,12 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 acc_steps += p.steps;
                 acc_scat += p.scat;
                 if (REPLAY) {
-                    soc_replay_record r;
-                    r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = esc;
-                    P.replay[p.id - P.pkg_begin] = r;
+                    acc_ld += p.n_ld; acc_red += p.n_red;
+                    if (P.replay) {
+                        soc_replay_record r;
+                        r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = esc;
+                        P.replay[p.id - P.pkg_begin] = r;
+                    }
                 }
                 need = EMPTY;
             }
@@ -836,6 +848,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 } else if (p.pend > 0.0f) {
                     if (ACC32) atomicAdd(P.acc32 + p.rel, p.pend * package_rel(P, p.src));
                     else atomicAdd(P.acc + p.rel, (double)p.pend * package_e0(P, p.src));
+                    p.n_red += 1;
                 }
                 p.pend = 0.0f;
             }
@@ -864,6 +877,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                         p.fx = (p.fx + (float)(rel & 1)) * 0.5f;
                         p.fy = (p.fy + (float)((rel >> 1) & 1)) * 0.5f;
                         p.fz = (p.fz + (float)((rel >> 2) & 1)) * 0.5f;
+                        if (p.anc1 < 0) p.n_ld += 1;
                         rel = p.anc1 >= 0 ? p.anc1 : __ldg(P.parent + ((rel - P.nrp) >> 3));
                         p.anc1 = p.anc2; p.anc2 = p.anc3; p.anc3 = -1;
                         p.h *= 2.0f;
@@ -878,6 +892,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                     if (!fast_descend(P, p)) need = DONE;            // a9: escaped
                 } else {
                     p.cw = __ldg(P.cellw + rel);
+                    p.n_ld += 1;
                     if (p.cw == kSentinel) need = DONE;              // a9: escaped
                 }
             }
@@ -924,6 +939,14 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
         atomicAdd(&P.result->terminated, (unsigned long long)acc_term);
         atomicMax(&P.result->drift_bits, __float_as_uint(acc_drift));     // >= 0: fp32 order = integer order
     }
+    if (REPLAY) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            acc_ld += __shfl_xor_sync(kFull, acc_ld, o);
+            acc_red += __shfl_xor_sync(kFull, acc_red, o);
+        }
+        if (lane == 0) { atomicAdd(&P.result->gathers, acc_ld); atomicAdd(&P.result->reds, acc_red); }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -950,12 +973,14 @@ struct QPkg {
     float prel;             // package energy in units of the launch's reference energy (ACC32)
     int rel;                // internal cell id
     uint32_t q0, q1, q2, q3;    // cell words of the half brick rel & ~3
-    float a0, a1, a2, a3;       // deposits into those cells in units of the reference energy, not yet in the accumulator
+                            // (the deposits into those four cells, not yet in the accumulator, live in shared memory:
+                            //  s_acc[slot][thread] -- indexed by the slot, which registers cannot be)
     uint32_t scat;          // scatterings so far = index of the current flight segment
     uint32_t idx;           // package id - pkg_begin
     int sd;                 // < 0: background or beam; else source index << 16 | valid << 9 | hot-cube cell (3 bits per axis)
     uint32_t steps;         // REPLAY only
     unsigned long long hash;
+    uint32_t n_ld, n_red;   // REPLAY only (option "stats"): gathers / reductions issued for this package
 };
 
 __device__ __forceinline__ int v_src(int sd) { return sd < 0 ? -1 : (sd >> 16); }
@@ -971,18 +996,21 @@ __device__ __forceinline__ void q_load(const FastParams &P, QPkg &p)
 {
     const uint4 v = __ldg(reinterpret_cast<const uint4 *>(P.cellw + (p.rel & ~3)));
     p.q0 = v.x; p.q1 = v.y; p.q2 = v.z; p.q3 = v.w;
+    p.n_ld += 1;
 }
 
 // hand the deposits of the half brick (already in units of the launch's reference energy) to the accumulator:
 // one 16-byte reduction
-__device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p)
+__device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p, float (*s_acc)[256])
 {
+    const float a0 = s_acc[0][threadIdx.x], a1 = s_acc[1][threadIdx.x], a2 = s_acc[2][threadIdx.x], a3 = s_acc[3][threadIdx.x];
     // nothing to add: empty cells, or the cells around a point source, whose deposits went to the block's shared
     // partial sums -- a reduction of zeros there would bring back the very contention those sums avoid
-    if ((p.a0 + p.a1) + (p.a2 + p.a3) == 0.0f) return;
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(P.acc32 + (p.rel & ~3)), "f"(p.a0), "f"(p.a1),
-                 "f"(p.a2), "f"(p.a3) : "memory");
-    p.a0 = 0.0f; p.a1 = 0.0f; p.a2 = 0.0f; p.a3 = 0.0f;
+    if ((a0 + a1) + (a2 + a3) == 0.0f) return;
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(P.acc32 + (p.rel & ~3)), "f"(a0), "f"(a1),
+                 "f"(a2), "f"(a3) : "memory");
+    s_acc[0][threadIdx.x] = 0.0f; s_acc[1][threadIdx.x] = 0.0f; s_acc[2][threadIdx.x] = 0.0f; s_acc[3][threadIdx.x] = 0.0f;
+    p.n_red += 1;
 }
 
 template <bool REPLAY>
@@ -994,7 +1022,9 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
     __shared__ double s_tot[3][256];             // emitted, escaped, absorbed
     __shared__ unsigned s_cnt[2][256];           // scatterings, terminated
     __shared__ float s_drift[256];               // max |w - (1 - absrel)| over this thread's escaped packages
+    __shared__ float s_acc[4][256];              // this thread's deposits into the four cells of its half brick
     s_drift[threadIdx.x] = 0.0f;
+    s_acc[0][threadIdx.x] = 0.0f; s_acc[1][threadIdx.x] = 0.0f; s_acc[2][threadIdx.x] = 0.0f; s_acc[3][threadIdx.x] = 0.0f;
     s_tot[0][threadIdx.x] = 0.0; s_tot[1][threadIdx.x] = 0.0; s_tot[2][threadIdx.x] = 0.0;
     s_cnt[0][threadIdx.x] = 0u; s_cnt[1][threadIdx.x] = 0u;
     extern __shared__ float s_hot[];             // hot-cell partial sums, see photon_fast_kernel
@@ -1003,9 +1033,11 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
     for (int i = threadIdx.x; i < hot_cells * P.n_point; i += blockDim.x) s_hot[i] = 0.0f;
     __syncthreads();
 
+    unsigned long long acc_ld = 0, acc_red = 0;  // REPLAY variant: request counters (option "stats")
     QPkg p;
+    p.n_ld = 0; p.n_red = 0;
     p.sd = -1; p.w = 0.0f; p.absrel = 0.0f; p.scat = 0; p.rel = 0; p.idx = 0; p.steps = 0; p.hash = 0;
-    p.q0 = p.q1 = p.q2 = p.q3 = 0u; p.a0 = p.a1 = p.a2 = p.a3 = 0.0f; p.pend = 0.0f; p.prel = 0.0f;
+    p.q0 = p.q1 = p.q2 = p.q3 = 0u; p.pend = 0.0f; p.prel = 0.0f;
     p.fx = p.fy = p.fz = 0.5f; p.dx = p.dy = 0.0f; p.dz = 1.0f; p.rx = p.ry = p.rz = 1.0f; p.tau_rem = 0.0f;
     int need = EMPTY;
     unsigned n_steps = 0;                        // cell-steps of this lane (all its packages)
@@ -1021,7 +1053,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
         if (n_park > 0 && (n_park >= T || m_run == 0u)) {
             // ---------------------------------------------------------------- service, all parked lanes together
             if (need == DONE) {                  // retire the finished package
-                q_flush(P, p);
+                q_flush(P, p, s_acc);
                 const int src = v_src(p.sd);
                 const double e0 = package_e0(P, src);
                 const double esc = escaped_rel(p.w, p.absrel) * e0;
@@ -1030,9 +1062,12 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                 s_tot[2][threadIdx.x] += (double)p.absrel * e0;
                 s_cnt[0][threadIdx.x] += p.scat;
                 if (REPLAY) {
-                    soc_replay_record r;
-                    r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = esc;
-                    P.replay[p.idx] = r;
+                    acc_ld += p.n_ld; acc_red += p.n_red;
+                    if (P.replay) {
+                        soc_replay_record r;
+                        r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = esc;
+                        P.replay[p.idx] = r;
+                    }
                 }
                 need = EMPTY;
             }
@@ -1062,11 +1097,13 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                 FPkg q;
                 fast_emit<false>(P, q, P.pkg_begin + (long long)p.idx, ndx, ndy, ndz);
                 p.fx = q.fx; p.fy = q.fy; p.fz = q.fz; p.rel = q.rel;
+                p.n_ld = 0;
                 q_load(P, p);
                 p.sd = q.src < 0 ? -1 : ((q.src << 16) | (P.hot_r >= 0 ? (0x200 | (P.hot_r * 0x49)) : 0));
                 p.w = 1.0f; p.absrel = 0.0f; p.scat = 0; p.pend = 0.0f;
                 p.prel = package_rel(P, q.src);
                 p.steps = 0; p.hash = 0xcbf29ce484222325ull;
+                p.n_red = 0;                      // (n_ld = 1: the q_load above)
                 s_tot[0][threadIdx.x] += package_e0(P, q.src);
             } else if (need == SCAT) {
                 // finish the flight segment: advance to the scattering point (a4), then a8
@@ -1140,12 +1177,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                         const int j = (p.sd & 7) + hot_side * (((p.sd >> 3) & 7) + hot_side * ((p.sd >> 6) & 7));
                         atomicAdd(s_hot + (p.sd >> 16) * hot_cells + j, p.pend);
                     } else {
-                        const int s2 = p.rel & 3;
-                        const float v = p.pend * p.prel;
-                        p.a0 += s2 == 0 ? v : 0.0f;
-                        p.a1 += s2 == 1 ? v : 0.0f;
-                        p.a2 += s2 == 2 ? v : 0.0f;
-                        p.a3 += s2 == 3 ? v : 0.0f;
+                        s_acc[p.rel & 3][threadIdx.x] += p.pend * p.prel;
                     }
                     p.pend = 0.0f;
                 }
@@ -1168,7 +1200,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                     // neighbour inside the brick: flip the slot bit; otherwise the same bit flips and the brick changes
                     const bool inside = fwd == ((p.rel & abit) == 0);
                     if (!inside || abit == 4) {
-                        q_flush(P, p);    // leaving the half brick: its sums go out, the new half comes in
+                        q_flush(P, p, s_acc);    // leaving the half brick: its sums go out, the new half comes in
                         int rel = p.rel ^ abit;
                         if (!inside) rel += fwd ? bstride : -bstride;
                         p.rel = rel;
@@ -1217,6 +1249,16 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
     }
     if (lane == 0 && (acc_steps != 0 || acc_emit != 0.0)) {
         atomicMax(&P.result->drift_bits, __float_as_uint(acc_drift));
+    }
+    if (REPLAY) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            acc_ld += __shfl_xor_sync(kFull, acc_ld, o);
+            acc_red += __shfl_xor_sync(kFull, acc_red, o);
+        }
+        if (lane == 0) { atomicAdd(&P.result->gathers, acc_ld); atomicAdd(&P.result->reds, acc_red); }
+    }
+    if (lane == 0 && (acc_steps != 0 || acc_emit != 0.0)) {
         atomicAdd(&P.result->emitted, acc_emit);
         atomicAdd(&P.result->escaped, acc_esc);
         atomicAdd(&P.result->absorbed, acc_abs);
@@ -1414,13 +1456,16 @@ __global__ void __launch_bounds__(256) probe_kernel(void *buf, unsigned long lon
             } else if (KIND == 4) {              // 16-byte vector reduction (4 fp32 cells)
                 asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(reinterpret_cast<float *>(buf) + 4 * j),
                              "f"(1.0f), "f"(1.0f), "f"(1.0f), "f"(1.0f) : "memory");
+            } else if (KIND == 6) {              // 16-byte gather (half a brick: what photon_q_kernel loads)
+                const uint4 v = __ldg(reinterpret_cast<const uint4 *>(buf) + j);
+                acc[u] += __uint_as_float(v.x ^ v.y ^ v.z ^ v.w);
             } else {                             // the memory side of one cell-step: gather rho[cell], add to acc[cell]
                 acc[u] += __ldg(reinterpret_cast<const float *>(buf) + j);
                 atomicAdd(reinterpret_cast<float *>(buf) + n_elem + j, 1.0f);
             }
         }
     }
-    if ((KIND == 0 || KIND == 3 || KIND == 5) && acc[0] + acc[1] + acc[2] + acc[3] == 123.456f) *sink = acc[0];
+    if ((KIND == 0 || KIND == 3 || KIND == 5 || KIND == 6) && acc[0] + acc[1] + acc[2] + acc[3] == 123.456f) *sink = acc[0];
 }
 
 }  // namespace
@@ -1676,7 +1721,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         const bool big = 8ll * G->n_int > (64ll << 20) && P.ksca * G->rho_mean * n_max < 12.0;
         const bool v2 = !hier && acc32 && (G->opt_kernel == 2 || (G->opt_kernel == 0 && big)) && pkg_count < (1ll << 32);
         if (v2) F.service_threshold = auto_threshold;
-        const int sel = (v2 ? 8 : 0) | (hier ? 4 : 0) | (rep ? 2 : 0) | (acc32 ? 1 : 0);
+        const int sel = (v2 ? 8 : 0) | (hier ? 4 : 0) | ((rep || G->opt_stats) ? 2 : 0) | (acc32 ? 1 : 0);
         switch (sel) {
         case 9: rc = launch_fast<false, false, true, true>(G, F, w_eff, absorbed, st); break;
         case 11: rc = launch_fast<false, true, true, true>(G, F, w_eff, absorbed, st); break;
@@ -1709,6 +1754,7 @@ int fetch_results(soc_grid *G, int n, soc_freq_result *out, cudaStream_t st)
         float drift;
         std::memcpy(&drift, &G->h_results[i].drift_bits, sizeof(float));
         out[i].weight_drift = (double)drift;
+        out[i].gather_requests = G->h_results[i].gathers; out[i].red_requests = G->h_results[i].reds;
     }
     return SOC_OK;
 }
@@ -1916,6 +1962,7 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     else if (k == "service_threshold" && value >= 0 && value <= 32) G->opt_service_threshold = (int)value;
     else if (k == "timing" && (value == 0 || value == 1)) G->opt_timing = (int)value;
     else if (k == "hot_cache" && (value == 0 || value == 1)) G->opt_hot_cache = (int)value;
+    else if (k == "stats" && (value == 0 || value == 1)) G->opt_stats = (int)value;
     else if (k == "kernel" && value >= 0 && value <= 2) G->opt_kernel = (int)value;
     else if (k == "overlap" && (value == 0 || value == 1)) G->opt_overlap = (int)value;
     else if (k == "carveout" && value >= -1 && value <= 100) G->opt_carveout = (int)value;
@@ -2084,8 +2131,8 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
 
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms)
 {
-    if (kind < 0 || kind > 5 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
-    const size_t elem = (kind == 1 || kind == 5) ? 8 : (kind == 3 ? 32 : (kind == 4 ? 16 : 4));   // kind 5: 4 B rho + 4 B acc per cell
+    if (kind < 0 || kind > 6 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
+    const size_t elem = (kind == 1 || kind == 5) ? 8 : (kind == 3 ? 32 : ((kind == 4 || kind == 6) ? 16 : 4));   // kind 5: 4 B rho + 4 B acc per cell
     const unsigned long long n_elem = (unsigned long long)footprint_bytes / elem;
     void *buf = nullptr;
     float *sink = nullptr;
@@ -2108,6 +2155,7 @@ int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, f
         else if (kind == 2) probe_kernel<2><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else if (kind == 3) probe_kernel<3><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else if (kind == 4) probe_kernel<4><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else if (kind == 6) probe_kernel<6><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else probe_kernel<5><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         g_launches += 1;
         SOC_CUDA(cudaEventRecord(e1));

@@ -42,7 +42,7 @@ class Sources(C.Structure):
 class FreqResult(C.Structure):
     _fields_ = [("emitted", C.c_double), ("escaped", C.c_double), ("absorbed", C.c_double),
                 ("cell_steps", C.c_uint64), ("scatterings", C.c_uint64), ("terminated", C.c_uint64),
-                ("weight_drift", C.c_double)]
+                ("weight_drift", C.c_double), ("gather_requests", C.c_uint64), ("red_requests", C.c_uint64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

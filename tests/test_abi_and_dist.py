@@ -166,6 +166,87 @@ def test_world_size_2_gloo_all_reduce(mode, tmp_path):
         assert np.allclose(a0, 0.5 * (sim(3) + sim(4)), rtol=1e-12, atol=0)
 
 
+def _bench_worker(rank, world, port, mode, out_dir):
+    """The distributed bookkeeping of bench.py's run_ours (init -> plan -> per-rank pass -> combine -> job_totals) over
+    gloo, with the per-rank pass done by the oracle instead of the CUDA library (no GPU here)."""
+    sys.path.insert(0, ROOT)
+    import json
+    import torch
+    import torch.distributed as td
+    import oracle
+    from paper_1812_06632_b200 import dist, inputs
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init("gloo", rank, world)
+    P = inputs.make_config("3", n=8, n_packages=3000, n_freq=3)
+    og = oracle.Grid(P.nx, P.ny, P.nz, P.n_cells, P.rho, P.child)
+    sh = dist.plan(mode, rank, world, P.n_packages, P.seed)
+    w = oracle.trapezoid_weights(P.freq_hz)
+    A = np.zeros(P.n_total)
+    steps = 0
+    for f in range(P.n_freq):
+        _, res, _, _ = oracle.simulate(og, P.kabs[f], P.ksca[f], P.g[f], f, P.sources(f), P.n_packages, sh.seed, w[f],
+                                       sh.pkg_begin, sh.pkg_count, absorbed=A)
+        steps += res.cell_steps
+    t = torch.from_numpy(A)
+    dist.combine(t, sh)
+    job = dist.job_totals(step_ms=10.0 * (rank + 1), cell_steps=steps, launches=P.n_freq + 1, world=world)
+    with open(os.path.join(out_dir, f"job_{mode}_{rank}.json"), "w") as fh:
+        json.dump(dict(job=job, my_steps=steps, sum=float(t.sum())), fh)
+    td.destroy_process_group()
+
+
+@pytest.mark.parametrize("mode", ["strong", "weak"])
+def test_bench_job_bookkeeping_world_size_2_gloo(mode, tmp_path):
+    """time = MAX over ranks, cell-steps and launches = SUM over ranks, value = all cell-steps / that time; strong: the
+    ranks' steps add up to the single-process count, weak: each rank does the full count."""
+    import json
+    import torch.multiprocessing as mp
+    import oracle
+    from paper_1812_06632_b200 import inputs
+    mp.spawn(_bench_worker, args=(2, _free_port(), mode, str(tmp_path)), nprocs=2, join=True)
+    r = [json.load(open(tmp_path / f"job_{mode}_{k}.json")) for k in range(2)]
+    assert r[0]["job"] == r[1]["job"]                                  # every rank holds the job totals
+    job = r[0]["job"]
+    assert job["step_ms"] == 20.0 and job["launches"] == 8
+    assert job["cell_steps"] == r[0]["my_steps"] + r[1]["my_steps"]
+    assert job["value"] == pytest.approx(job["cell_steps"] / 20e-3, rel=1e-12)
+    assert r[0]["sum"] == pytest.approx(r[1]["sum"], rel=1e-14)
+    P = inputs.make_config("3", n=8, n_packages=3000, n_freq=3)
+    og = oracle.Grid(P.nx, P.ny, P.nz, P.n_cells, P.rho, P.child)
+    full = sum(oracle.simulate(og, P.kabs[f], P.ksca[f], P.g[f], f, P.sources(f), P.n_packages, P.seed)[1].cell_steps
+               for f in range(P.n_freq))
+    if mode == "strong":
+        assert job["cell_steps"] == full
+    else:
+        assert r[0]["my_steps"] == full and job["cell_steps"] > 1.9 * full
+
+
+def test_bench_refuses_a_rank_count_it_cannot_serve():
+    """`bench.py --gpus 2` with no launcher and fewer than 2 CUDA devices must fail loudly, not bench one GPU."""
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "1"],
+                         capture_output=True, text=True, timeout=600, env=env)
+    assert out.returncode != 0 and "CUDA device" in (out.stderr + out.stdout)
+    assert not [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+
+
+def test_bench_reads_dram_traffic_from_the_newest_capture(tmp_path, monkeypatch):
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(ROOT, "bench.py"))
+    b = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(b)
+    (tmp_path / "profiles").mkdir()
+    (tmp_path / "profiles" / "r01_ncu_dram_traffic.csv").write_text(
+        "config,kernel,cell_steps,dram_read_bytes,dram_write_bytes,source\n5,k,100,900,100,old.txt\n")
+    (tmp_path / "profiles" / "r02_ncu_dram_traffic.csv").write_text(
+        "config,kernel,cell_steps,dram_read_bytes,dram_write_bytes,source\n5,k,100,1500,500,new.txt\n5,k,100,500,500,new.txt\n")
+    monkeypatch.setattr(b, "ROOT", str(tmp_path))
+    t = b.ncu_traffic("5")
+    assert t["bytes_per_cell_step"] == 15.0 and "r02_ncu_dram_traffic.csv" in t["source"] and "new.txt" in t["source"]
+    assert b.ncu_traffic("3") is None
+
+
 def test_bench_reference_arm_prints_the_contract_line():
     """bench.py --impl reference runs the oracle on the host cores and prints ONE JSON line with the keys the
     driver reads (no GPU involved)."""
