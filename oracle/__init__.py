@@ -348,15 +348,16 @@ def dust_stride(n_dust):
 
 
 def iterate(grid: Grid, freq_hz, kabs, ksca, g, const_sources, n_const, n_request, seed, t_scale, table_T, E_min, E_max,
-            mode="weighted", cap=10000, reference_field=True, ali=False, update_T=True, T_start=None, threads=1,
-            f32state=False):
+            mode="weighted", cap=10000, reference_field=True, ref_start=1, ali=False, update_T=True, T_start=None,
+            threads=1, f32state=False):
     """Iterated run with dust re-emission (rows f1, f3; readings F4-F6 of DESIGN.md), step by step:
 
       iteration 0   constant sources only (background, point sources), n_const packages per frequency, seed:
                     A_const = sum_f w_f A_f;  T = table(A_const)   (T_start overrides it)
       iteration i   i = 1 .. len(n_request): for every frequency the cells emit n_request[i-1] packages (counts by `mode`
                     from the current T), seed + i:  D_i = sum_f w_f A_dust,f  (and the in-cell part S_i, emission Em_i)
-                    reference field: R_i = running mean of D_1..D_i weighted by n_request (else R_i = D_i)
+                    reference field: R_i = running mean of D_k, k = ref_start..i, weighted by n_request
+                    (R_i = D_i without it, and for i < ref_start)
                     T = table(A_const + R_i)   -- with ALI from (A - S) / (1 - S / Em) (soc_oracle_update_temperatures_ali)
     Returns dict(T=[T_0, T_1, ...], A_const, R, S, Em, emitted=[...], escaped=[...]) (frequency-integrated energies)."""
     freq_hz = np.asarray(freq_hz, dtype=np.float64)
@@ -388,7 +389,7 @@ def iterate(grid: Grid, freq_hz, kabs, ksca, g, const_sources, n_const, n_reques
                                   f32state=f32state)
             esc += w[f] * r.escaped
             em += w[f] * r.emitted
-        if reference_field:
+        if reference_field and i >= ref_start:
             R = (W * R + n_req * D) / (W + n_req)
             S = (W * S + n_req * Si) / (W + n_req)
             Em = (W * Em + n_req * Emi) / (W + n_req)
