@@ -85,6 +85,18 @@ typedef struct {
     int64_t n_bg;               /* -1 = default split: all packages to the only class present, n/2 each if both */
     const double *beam;         /* test hook, normally NULL: [6] = position, unit direction; every package is
                                    this beam with energy 1 and no random emission */
+    /* Dust re-emission (row f1; PAPER.md:67 "the emission is calculated by SOC itself", :79, :143): the LAST n_dust
+     * package ids are emitted by the cells -- uniform point in the cell, isotropic direction.  Cell c sends
+     * dust_count[c] packages of energy L_c / dust_count[c], L_c = 4 pi kabs rho_c h^3 B_nu(T_c) at the frequency of
+     * the call; consecutive ids are spread over the cells (id -> id * stride mod n_dust).  n_bg and the default split
+     * refer to the first n_packages - n_dust ids. */
+    int64_t n_dust;             /* 0 = none; must equal the sum of dust_count and be < 2^32 */
+    const float *dust_T;        /* DEVICE [n_total] dust temperature per cell (what soc_update_temperatures wrote) */
+    const int32_t *dust_count;  /* DEVICE [n_total] packages per cell (soc_emission_counts, or the caller's own policy);
+                                   0 wherever L_c = 0 */
+    double *dust_self;          /* DEVICE [n_total] or NULL (row f3): += weight * the energy a cell's own packages deposit
+                                   in it before they first leave it -- the absorption-emission cycle inside a cell that
+                                   the diagonal ALI operator takes out of the iteration */
 } soc_sources;
 
 typedef struct {
@@ -142,6 +154,58 @@ int soc_simulate_packages(soc_grid *grid, int32_t ifreq, const soc_sources *src,
 int soc_simulate_spectrum(soc_grid *grid, const soc_sources *src, int64_t n_packages, uint64_t seed,
                           int64_t pkg_begin, int64_t pkg_count, double *absorbed_int,
                           soc_freq_result *results, uint32_t flags, void *cuda_stream);
+
+/* Package counts of the dust re-emission (row f1).  mode 0 "the same number of photon packages is sent
+ * per each cell", the total a multiple of the number of emitting cells: m = ceil(n_request / n_emitting) from every
+ * cell with L_c > 0.  mode 1 "weighted according to the emission" with "the maximum number of photon packages sent
+ * from any single cell ... limited": n_c = min(cap, ceil(n_request L_c / sum L)), at least 1 where L_c > 0.
+ * T: DEVICE n_total floats.  count: DEVICE n_total int32, written.  *n_dust (HOST) receives the sum; *lum_total (HOST,
+ * may be NULL) the sum of the L_c.  Synchronises the stream. */
+int soc_emission_counts(soc_grid *grid, int32_t ifreq, const float *T, int32_t mode, int64_t n_request, int32_t cap,
+                        int32_t *count, int64_t *n_dust, double *lum_total, void *cuda_stream);
+
+/* Frequency-integrated emission of every cell, emitted[c] = sum_f w_f L_c,f(T_c) (w = soc_freq_weights): what the cell
+ * radiates in a dust simulation at these temperatures -- the denominator of the ALI escape probability.
+ * T: DEVICE n_total floats; emitted: DEVICE n_total doubles, written. */
+int soc_cell_emission(soc_grid *grid, const float *T, double *emitted, void *cuda_stream);
+
+/* Temperature update with the diagonal ALI operator (row f3; "solves explicitly for the cycle of photons
+ * that are absorbed within the emitting cell ... one additional floating point number per cell ... to keep track of
+ * the photon escape probabilities").  beta_c = self_abs[c] / emitted[c] (clamped to [0, 0.999]); the table is entered
+ * with E = scale (absorbed[c] - self_abs[c]) / (rho h^3 (1 - beta_c)); beta = 0 is soc_update_temperatures.
+ * absorbed, self_abs, emitted: DEVICE n_total doubles of the same simulation(s). */
+int soc_update_temperatures_ali(soc_grid *grid, const double *absorbed, const double *self_abs, const double *emitted,
+                                double scale, const float *table_T, int32_t n_table, double E_min, double E_max,
+                                float *T_out, void *cuda_stream);
+
+/* Iterated run with dust re-emission (rows f1, f3):
+ *   iteration 0   the constant sources src[f] (background, point sources), n_const packages per frequency, `seed`:
+ *                 A_const = sum_f w_f A_f;  T = table(A_const)
+ *   iteration i   1 .. n_iter: for every frequency the cells emit n_request[i-1] packages (counts by `mode`, `cap` from
+ *                 the current T), seed + i:  D_i = sum_f w_f A_dust,f
+ *                 reference field: R_i = mean of D_k, k = ref_start .. i, weighted by n_request[k-1]
+ *                 (R_i = D_i without it and for i < ref_start);  T = table(A_const + R_i), through the ALI update if ali
+ * n_request may change from iteration to iteration.  absorbed_out (DEVICE n_total doubles) receives
+ * A_const + R of the last iteration, T_out (DEVICE n_total floats) the temperatures; history (HOST, may be NULL):
+ * [n_iter + 1] records.  Synchronises. */
+typedef struct {
+    int32_t mode, cap;          /* package counts: soc_emission_counts */
+    int32_t reference_field;    /* 0 / 1 */
+    int32_t ref_start;          /* first iteration that enters the running mean (>= 1) */
+    int32_t ali;                /* 0 / 1 */
+    int32_t n_iter;
+    const int64_t *n_request;   /* HOST [n_iter] */
+} soc_iterate_opts;
+
+typedef struct {
+    double emitted, escaped, absorbed;   /* frequency-integrated (sum_f w_f ...) energies of the iteration's packages */
+    int64_t n_packages;                  /* packages simulated in the iteration, all frequencies */
+    uint64_t cell_steps;
+} soc_iterate_record;
+
+int soc_iterate(soc_grid *grid, const soc_sources *src, int64_t n_const, uint64_t seed, const soc_iterate_opts *opts,
+                double t_scale, const float *table_T, int32_t n_table, double E_min, double E_max,
+                double *absorbed_out, float *T_out, soc_iterate_record *history, uint32_t flags, void *cuda_stream);
 
 /* Energy balance by table lookup (row a11; reading S10).  For every leaf with rho > 0:
  *   E = scale * absorbed[cell] / (rho * h^3),  h = 2^-(level-1)

@@ -12,7 +12,7 @@ LIB = os.path.join(HERE, "libsoc_b200.so")
 INCLUDE = os.path.join(ROOT, "include")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-I", INCLUDE]
+              "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-fmad=false", "-I", INCLUDE]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

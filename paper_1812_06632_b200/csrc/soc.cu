@@ -48,6 +48,19 @@ struct DevResult {                      // one slot per launch, accumulated with
     unsigned long long gathers, reds;   // option "stats": global-memory gather / reduction instructions issued by the lanes
 };
 
+// f1: dust re-emission, the third package source.  Package ids [n_const, n_const + n_dust)
+struct DustParams {
+    long long n_const, n_dust;          // ids below n_const are background / point-source packages
+    unsigned long long stride;          // id -> (id * stride) mod n_dust spreads consecutive ids over the cells
+    const uint32_t *first;              // [n_total + 1] first dust index of every cell (prefix sums of count)
+    const int32_t *count;               // [n_total] packages per cell
+    const float *T;                     // [n_total] dust temperature
+    double *self_abs;                   // [n_total] or NULL: in-cell absorption of the cells' own packages (f3)
+    double kabs, freq_hz, weight;       // luminosity L_c = 4 pi kabs rho h^3 B_nu(T); weight of the self_abs adds
+    int n_levels;
+    int level_off[SOC_MAX_LEVELS + 1];  // ABI cell vector: first global id of every level
+};
+
 struct SimParams {
     // grid
     int nx, ny, nz, n_root;
@@ -62,6 +75,7 @@ struct SimParams {
     double beam[6];
     double ps_pos[SOC_MAX_POINT_SOURCES][3];
     double ps_e0[SOC_MAX_POINT_SOURCES];
+    DustParams dust;
     // run
     long long pkg_begin, pkg_end;
     unsigned long long seed;
@@ -87,6 +101,13 @@ struct soc_grid {
     unsigned long long *d_counters = nullptr; // n_slots
     DevResult *h_results = nullptr;           // pinned, n_slots
     float *d_table = nullptr;
+    // f1 / f3: dust re-emission
+    uint32_t *d_dust_first = nullptr;         // [n_total + 1] prefix sums of the package counts of the current launch
+    uint32_t *d_scan_blocks = nullptr;        // block sums of the scan
+    double *d_scalars = nullptr;              // [8] small reductions (sum of luminosities, emitting cells, packages)
+    double *h_scalars = nullptr;              // pinned mirror
+    double *d_freqtab = nullptr;              // [3][n_freq] freq_hz, kabs, quadrature weight
+    double *d_eff = nullptr;                  // [n_total] effective absorbed energy of the ALI update
     float *h_table = nullptr;                 // pinned staging copy of the caller's table (borrowed for the call only)
     cudaEvent_t ev_table = nullptr;           // the staging copy has been read
     // internal layout of the production kernel: root grid with one ghost layer, then the octet levels
@@ -196,6 +217,7 @@ template <typename A> struct Pkg {
     double E, e_min;       // weight and termination threshold 1e-9 E0
     double pend;           // energy absorbed in the current cell, not yet added to the accumulator
     long long id;
+    int origin;            // dust package that has not left the cell that emitted it: that cell's global id; else -1
 };
 
 template <typename A> __device__ __forceinline__ void set_direction(Pkg<A> &p, A dx, A dy, A dz)
@@ -220,14 +242,62 @@ template <typename A> __device__ __forceinline__ void descend(const SimParams &P
     p.cw = cw;
 }
 
+// f1: luminosity of leaf cell at (level, rho, T): L = 4 pi kabs rho h^3 B_nu(T), in the energy unit of pi I S
+__device__ __forceinline__ double planck_nu(double nu, double T)
+{
+    if (!(T > 0.0)) return 0.0;
+    const double h = 6.62607015e-27, kb = 1.380649e-16, c = 2.99792458e10;
+    return 2.0 * h * nu * nu * nu / (c * c) / expm1(h * nu / (kb * T));
+}
+
+__device__ __forceinline__ double cell_luminosity(double kabs, double freq_hz, uint32_t cw, int level0, float T)
+{
+    if ((int32_t)cw < 0) return 0.0;                                // parent cell
+    const double rho = (double)__uint_as_float(cw);
+    if (!(rho > 0.0)) return 0.0;
+    const double vol = 1.0 / (double)(1ull << (3 * level0));         // level0 = level - 1
+    return 4.0 * 3.14159265358979323846 * kabs * rho * vol * planck_nu(freq_hz, (double)T);
+}
+
+// f1: the cell that emits dust package `id` (global id of the ABI cell vector) and its level - 1
+__device__ __forceinline__ int dust_cell(const DustParams &D, long long id, int &level0)
+{
+    const unsigned long long q = ((unsigned long long)(id - D.n_const) * D.stride) % (unsigned long long)D.n_dust;
+    int lo = 0, hi = D.level_off[D.n_levels];                       // invariant: first[lo] <= q < first[hi]
+    while (hi - lo > 1) {
+        const int mid = (int)(((long long)lo + hi) >> 1);
+        if ((unsigned long long)__ldg(D.first + mid) <= q) lo = mid; else hi = mid;
+    }
+    level0 = 0;
+    while (level0 + 1 < D.n_levels && lo >= D.level_off[level0 + 1]) ++level0;
+    return lo;
+}
+
 // a1-a3: position, root cell, direction and source of package `id` (SURVEY.md 8c.3 / DESIGN.md readings S2, S3).
 // One definition for both kernels families: A = double in the replay kernel, float in the production kernels; PARAMS
 // is SimParams or FastParams (same field names).  src = point source index, -1 = background or beam.
+// Dust packages (f1): src = -2, ix = global id of the emitting cell, iy = its level - 1; uniform point in the cell,
+// isotropic direction (words 0..2 of block 0 -> position, word 3 -> cos theta, word 0 of block 1 -> azimuth).
 template <typename A, typename PARAMS>
 __device__ __forceinline__ void emit_core(const PARAMS &P, long long id, int &ix, int &iy, int &iz, float &fx, float &fy,
                                           float &fz, A &dx, A &dy, A &dz, int &src)
 {
     src = -1;
+    if (!P.is_beam && id >= P.dust.n_const) {
+        uint32_t w0, w1, w2, w3, v0, v1, v2, v3;
+        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
+        philox_block(P.seed, P.ifreq, id, 1u, v0, v1, v2, v3);
+        ix = dust_cell(P.dust, id, iy);
+        iz = 0;
+        fx = uniform01<float>(w0); fy = uniform01<float>(w1); fz = uniform01<float>(w2);       // exact in fp32
+        const A mu = (A)2 * uniform01<A>(w3) - (A)1;
+        const A st = RM<A>::sqrt_(fmax((A)0, fma(-mu, mu, (A)1)));
+        A sp, cp;
+        RM<A>::sincospi_((A)2 * uniform01<A>(v0), &sp, &cp);
+        dx = st * cp; dy = st * sp; dz = mu;
+        src = -2;
+        return;
+    }
     if (P.is_beam) {
         const int n[3] = {P.nx, P.ny, P.nz};
         int c[3];
@@ -282,8 +352,8 @@ __device__ __forceinline__ void emit_core(const PARAMS &P, long long id, int &ix
         const double px = P.ps_pos[k][0], py = P.ps_pos[k][1], pz = P.ps_pos[k][2];
         ix = (int)floor(px); iy = (int)floor(py); iz = (int)floor(pz);
         fx = (float)(px - (double)ix); fy = (float)(py - (double)iy); fz = (float)(pz - (double)iz);
-        const A mu = (A)2 * uniform01<A>(w0) - (A)1;
-        const A st = RM<A>::sqrt_(fmax((A)0, (A)1 - mu * mu));
+        const A mu = fma((A)2, uniform01<A>(w0), (A)-1);
+        const A st = RM<A>::sqrt_(fmax((A)0, fma(-mu, mu, (A)1)));
         A sp, cp;
         RM<A>::sincospi_((A)2 * uniform01<A>(w1), &sp, &cp);
         dx = st * cp; dy = st * sp; dz = mu;
@@ -296,24 +366,27 @@ __device__ __forceinline__ void emit_core(const PARAMS &P, long long id, int &ix
 template <typename A>
 __device__ __forceinline__ void scatter_direction(A g, uint32_t w_hg, uint32_t w_az, A odx, A ody, A odz, A &ndx, A &ndy, A &ndz)
 {
-    const A mu0 = (A)2 * uniform01<A>(w_hg) - (A)1;
-    const A num = mu0 + g * ((A)3 + mu0 * mu0) * (A)0.5 + g * g * mu0 + g * g * g * (mu0 * mu0 - (A)1) * (A)0.5;
-    const A den = ((A)1 + g * mu0) * ((A)1 + g * mu0);
-    A ct = num / den;
+    // every a * b + c below is written as an explicit fma: the two production kernels inline this function in different
+    // surroundings, and must not be left to contract it differently (they are tested to walk identical paths)
+    const A mu0 = fma((A)2, uniform01<A>(w_hg), (A)-1);
+    const A m2 = mu0 * mu0, g2 = g * g;
+    const A num = fma(g2 * g, (m2 - (A)1) * (A)0.5, fma(g2, mu0, fma(g, ((A)3 + m2) * (A)0.5, mu0)));
+    const A gm = fma(g, mu0, (A)1);
+    A ct = num / (gm * gm);
     ct = ct > (A)1 ? (A)1 : (ct < (A)-1 ? (A)-1 : ct);
-    const A st = RM<A>::sqrt_(fmax((A)0, (A)1 - ct * ct));
+    const A st = RM<A>::sqrt_(fmax((A)0, fma(-ct, ct, (A)1)));
     A sp, cp;
     RM<A>::sincospi_((A)2 * uniform01<A>(w_az), &sp, &cp);
     const A sg = RM<A>::copysign_((A)1, odz);
     const A a = (A)-1 / (sg + odz);
     const A b = odx * ody * a;
-    const A t1x = (A)1 + sg * odx * odx * a, t1y = sg * b, t1z = -sg * odx;
-    const A t2x = b, t2y = sg + ody * ody * a, t2z = -ody;
+    const A t1x = fma(sg * odx, odx * a, (A)1), t1y = sg * b, t1z = -sg * odx;
+    const A t2x = b, t2y = fma(ody, ody * a, sg), t2z = -ody;
     const A c1 = st * cp, c2 = st * sp;
-    const A nx = c1 * t1x + c2 * t2x + ct * odx;
-    const A ny = c1 * t1y + c2 * t2y + ct * ody;
-    const A nz = c1 * t1z + c2 * t2z + ct * odz;
-    const A inv = RM<A>::rsqrt_(nx * nx + ny * ny + nz * nz);
+    const A nx = fma(c1, t1x, fma(c2, t2x, ct * odx));
+    const A ny = fma(c1, t1y, fma(c2, t2y, ct * ody));
+    const A nz = fma(c1, t1z, fma(c2, t2z, ct * odz));
+    const A inv = RM<A>::rsqrt_(fma(nx, nx, fma(ny, ny, nz * nz)));
     ndx = nx * inv; ndy = ny * inv; ndz = nz * inv;
 }
 
@@ -325,16 +398,31 @@ __device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long 
     int src;
     p.id = id;
     emit_core<A>(P, id, p.ix, p.iy, p.iz, p.fx, p.fy, p.fz, dx, dy, dz, src);
-    const double e0 = P.is_beam ? 1.0 : (src >= 0 ? P.ps_e0[src] : P.bg_e0);
+    double e0 = P.is_beam ? 1.0 : (src >= 0 ? P.ps_e0[src] : P.bg_e0);
     set_direction(p, dx, dy, dz);
     p.h = 1.0f;
-    const int root = p.ix + P.nx * (p.iy + P.ny * p.iz);
-    if (HIER) {
-        p.rel = root - P.n_root;
-        descend(P, p);
+    p.origin = -1;
+    if (src == -2) {
+        // f1: the package starts inside the leaf that emitted it; its root cell is found by climbing the reverse links
+        const int gid = p.ix, level0 = p.iy;
+        p.origin = gid;
+        p.cw = __ldg(P.cellw + gid);
+        e0 = cell_luminosity(P.dust.kabs, P.dust.freq_hz, p.cw, level0, __ldg(P.dust.T + gid)) / (double)__ldg(P.dust.count + gid);
+        p.h = __int_as_float((127 - level0) << 23);              // 2^-(level - 1), exact
+        int r = HIER ? gid - P.n_root : gid;
+        p.rel = r;
+        if (HIER) while (r >= 0) r = __ldg(P.parent + (r >> 3));
+        const int root = HIER ? r + P.n_root : r;
+        p.ix = root % P.nx; p.iy = (root / P.nx) % P.ny; p.iz = root / (P.nx * P.ny);
     } else {
-        p.rel = root;
-        p.cw = __ldg(P.cellw + root);
+        const int root = p.ix + P.nx * (p.iy + P.ny * p.iz);
+        if (HIER) {
+            p.rel = root - P.n_root;
+            descend(P, p);
+        } else {
+            p.rel = root;
+            p.cw = __ldg(P.cellw + root);
+        }
     }
     p.seg = 0; p.steps = 0; p.scat = 0;
     p.hash = 0xcbf29ce484222325ull;
@@ -497,6 +585,10 @@ __global__ void __launch_bounds__(256) photon_kernel(const __grid_constant__ Sim
             // step (the hot-cell contention of PAPER.md:151, 279)
             if (flush) {
                 if (p.pend > 0.0) atomicAdd(P.absorbed + gid, P.weight * p.pend);
+                if (p.origin >= 0) {                 // f3: what a cell's own package left in it before first leaving it
+                    if (P.dust.self_abs && p.pend > 0.0) atomicAdd(P.dust.self_abs + gid, P.weight * p.pend);
+                    p.origin = -1;
+                }
                 p.pend = 0.0;
             }
             if (done) {
@@ -579,6 +671,8 @@ struct FastParams {
     float *acc32;                       // [n_int] internal accumulator in units of e_ref, ACC32 = true
     float bg_rel, beam_rel;             // package energy / e_ref of a background / beam package
     float ps_rel[SOC_MAX_POINT_SOURCES];  // ... of a package of point source k
+    DustParams dust;
+    double e_ref;                       // reference energy of the launch (unit of the fp32 accumulator)
     soc_replay_record *replay;
     unsigned long long *counter;
     DevResult *result;
@@ -670,16 +764,33 @@ __device__ __forceinline__ void fast_emit_core(const FastParams &P, FPkg &p, lon
     emit_core<float>(P, id, ix, iy, iz, p.fx, p.fy, p.fz, dx, dy, dz, p.src);
 }
 
+// prel receives the package energy in units of the launch's reference energy
 template <bool HIER>
-__device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, long long id, float &dx, float &dy, float &dz)
+__device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, long long id, float &dx, float &dy, float &dz, float &prel)
 {
     int ix, iy, iz;
     fast_emit_core(P, p, id, ix, iy, iz, dx, dy, dz);
     p.h = 1.0f;
-    p.rel = root_id(P, ix, iy, iz);
     p.n_ld = 0; p.n_red = 0;
-    if (HIER) { p.anc1 = p.anc2 = p.anc3 = -1; fast_descend(P, p); }
-    else { p.cw = __ldg(P.cellw + p.rel); p.n_ld = 1; }
+    if (HIER) p.anc1 = p.anc2 = p.anc3 = -1;
+    if (p.src == -2) {
+        // f1: a dust package starts inside the leaf that emitted it (ix = its global id, iy = its level - 1); the ids
+        // of its ancestors are not known (-1): a climb loads the reverse links
+        const int gid = ix, level0 = iy;
+        if (gid < P.n_root) p.rel = root_id(P, gid % P.nx, (gid / P.nx) % P.ny, gid / (P.nx * P.ny));
+        else p.rel = P.nrp + (gid - P.n_root);
+        p.cw = __ldg(P.cellw + p.rel);
+        p.n_ld = 1;
+        p.h = __int_as_float((127 - level0) << 23);
+        const double e0 = cell_luminosity(P.dust.kabs, P.dust.freq_hz, p.cw, level0, __ldg(P.dust.T + gid)) /
+                          (double)__ldg(P.dust.count + gid);
+        prel = (float)(e0 / P.e_ref);
+    } else {
+        p.rel = root_id(P, ix, iy, iz);
+        if (HIER) fast_descend(P, p);
+        else { p.cw = __ldg(P.cellw + p.rel); p.n_ld = 1; }
+        prel = package_rel(P, p.src);
+    }
     // hot-cell tracking starts at the centre of the cube of the package's own source (regular grids only)
     p.disp = (!HIER && p.src >= 0 && P.hot_r >= 0) ? P.hot_r * 0x010101 : -1;
     p.steps = 0; p.scat = 0;
@@ -711,7 +822,9 @@ __device__ __forceinline__ double escaped_rel(float w, float absrel)
     return absrel < 0.5f ? 1.0 - (double)absrel : (double)w;
 }
 
-template <bool HIER, bool REPLAY, bool ACC32>
+// DUST: the launch contains dust re-emission packages (f1): per-package energies, in-cell absorption (f3).  Compiled out of
+// the kernels that serve the constant sources, whose step loop it would lengthen (measured: -4 % ... -10 %).
+template <bool HIER, bool REPLAY, bool ACC32, bool DUST>
 __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __grid_constant__ FastParams P)
 {
     const int lane = threadIdx.x & 31;
@@ -729,6 +842,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
     // hot-cell cache (atomics to the cells around a point source serialise): fp32 partial sums
     // of the deposits (in units of the source's package energy) into the (2R+1)^3 root cells around each source
     extern __shared__ float s_hot[];
+    __shared__ float s_prel[256];                // dust packages: package energy / e_ref (one per package, not per class)
     const int hot_side = 2 * P.hot_r + 1;
     const int hot_cells = P.hot_r >= 0 ? hot_side * hot_side * hot_side : 0;
     for (int i = threadIdx.x; i < hot_cells * P.n_point; i += blockDim.x) s_hot[i] = 0.0f;
@@ -743,7 +857,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
         if (m_park && (__popc(m_park) >= T || m_run == 0u)) {
             // ---------------------------------------------------------------- service, all parked lanes together
             if (need == DONE) {                  // retire the finished package
-                const double e0 = package_e0(P, p.src);
+                const double e0 = (DUST && p.src <= -2) ? (double)s_prel[threadIdx.x] * P.e_ref : package_e0(P, p.src);
                 const double esc = escaped_rel(p.w, p.absrel) * e0;
                 if (p.w != 0.0f) acc_drift = fmaxf(acc_drift, fabsf(p.w - (1.0f - p.absrel)));
                 acc_esc += esc;
@@ -782,8 +896,10 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
             if (need == EMPTY && exhausted) need = DEAD;
             float ndx = 0.0f, ndy = 0.0f, ndz = 1.0f;
             if (need == NEWID) {
-                fast_emit<HIER>(P, p, p.id, ndx, ndy, ndz);
-                acc_emit += package_e0(P, p.src);
+                float prel;
+                fast_emit<HIER>(P, p, p.id, ndx, ndy, ndz, prel);
+                if (DUST && p.src <= -2) { s_prel[threadIdx.x] = prel; acc_emit += (double)prel * P.e_ref; }
+                else acc_emit += package_e0(P, p.src);
             } else if (need == SCAT) {
                 // finish the flight segment: advance to the scattering point (a4), then a8
                 const float rho = __uint_as_float(p.cw);
@@ -846,9 +962,15 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                     const int j = (p.disp & 255) + hot_side * (((p.disp >> 8) & 255) + hot_side * (p.disp >> 16));
                     atomicAdd(s_hot + p.src * hot_cells + j, p.pend);
                 } else if (p.pend > 0.0f) {
-                    if (ACC32) atomicAdd(P.acc32 + p.rel, p.pend * package_rel(P, p.src));
-                    else atomicAdd(P.acc + p.rel, (double)p.pend * package_e0(P, p.src));
+                    const bool dust = DUST && p.src <= -2;
+                    if (ACC32) atomicAdd(P.acc32 + p.rel, p.pend * (dust ? s_prel[threadIdx.x] : package_rel(P, p.src)));
+                    else atomicAdd(P.acc + p.rel, (double)p.pend * (dust ? (double)s_prel[threadIdx.x] * P.e_ref : package_e0(P, p.src)));
                     p.n_red += 1;
+                }
+                if (DUST && p.src == -2) {       // f3: what a cell's own package leaves in it before first leaving it
+                    if (P.dust.self_abs && p.pend > 0.0f)
+                        atomicAdd(P.dust.self_abs + global_id(P, p.rel), P.dust.weight * (double)p.pend * ((double)s_prel[threadIdx.x] * P.e_ref));
+                    p.src = -3;
                 }
                 p.pend = 0.0f;
             }
@@ -1013,7 +1135,7 @@ __device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p, float (*s_
     p.n_red += 1;
 }
 
-template <bool REPLAY>
+template <bool REPLAY, bool DUST>
 __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant__ FastParams P)
 {
     const int lane = threadIdx.x & 31;
@@ -1055,7 +1177,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
             if (need == DONE) {                  // retire the finished package
                 q_flush(P, p, s_acc);
                 const int src = v_src(p.sd);
-                const double e0 = package_e0(P, src);
+                const double e0 = (DUST && p.sd <= -2) ? (double)p.prel * P.e_ref : package_e0(P, src);
                 const double esc = escaped_rel(p.w, p.absrel) * e0;
                 if (p.w != 0.0f) s_drift[threadIdx.x] = fmaxf(s_drift[threadIdx.x], fabsf(p.w - (1.0f - p.absrel)));
                 s_tot[1][threadIdx.x] += esc;
@@ -1095,16 +1217,15 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
             float ndx = 0.0f, ndy = 0.0f, ndz = 1.0f;
             if (need == NEWID) {
                 FPkg q;
-                fast_emit<false>(P, q, P.pkg_begin + (long long)p.idx, ndx, ndy, ndz);
+                fast_emit<false>(P, q, P.pkg_begin + (long long)p.idx, ndx, ndy, ndz, p.prel);
                 p.fx = q.fx; p.fy = q.fy; p.fz = q.fz; p.rel = q.rel;
                 p.n_ld = 0;
                 q_load(P, p);
-                p.sd = q.src < 0 ? -1 : ((q.src << 16) | (P.hot_r >= 0 ? (0x200 | (P.hot_r * 0x49)) : 0));
+                p.sd = q.src < 0 ? q.src : ((q.src << 16) | (P.hot_r >= 0 ? (0x200 | (P.hot_r * 0x49)) : 0));   // -1 / -2 (dust)
                 p.w = 1.0f; p.absrel = 0.0f; p.scat = 0; p.pend = 0.0f;
-                p.prel = package_rel(P, q.src);
                 p.steps = 0; p.hash = 0xcbf29ce484222325ull;
                 p.n_red = 0;                      // (n_ld = 1: the q_load above)
-                s_tot[0][threadIdx.x] += package_e0(P, q.src);
+                s_tot[0][threadIdx.x] += (DUST && q.src <= -2) ? (double)p.prel * P.e_ref : package_e0(P, q.src);
             } else if (need == SCAT) {
                 // finish the flight segment: advance to the scattering point (a4), then a8
                 const float rho = __uint_as_float(q_word(p));
@@ -1178,6 +1299,11 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                         atomicAdd(s_hot + (p.sd >> 16) * hot_cells + j, p.pend);
                     } else {
                         s_acc[p.rel & 3][threadIdx.x] += p.pend * p.prel;
+                    }
+                    if (DUST && p.sd == -2) {    // f3: what a cell's own package leaves in it before first leaving it
+                        if (P.dust.self_abs && p.pend > 0.0f)
+                            atomicAdd(P.dust.self_abs + global_id(P, p.rel), P.dust.weight * (double)p.pend * ((double)p.prel * P.e_ref));
+                        p.sd = -3;
                     }
                     p.pend = 0.0f;
                 }
@@ -1426,6 +1552,187 @@ __global__ void scale_kernel(double *a, long long n, double s)
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) a[i] *= s;
 }
 
+// ------------------------------------------------------------------------------------------------
+// f1: dust re-emission -- luminosities, package counts, prefix sums
+// ------------------------------------------------------------------------------------------------
+struct LumParams {
+    const uint32_t *cellw;              // ABI order
+    const float *T;
+    double kabs, freq_hz;
+    long long n_total;
+    int n_levels;
+    long long level_off[SOC_MAX_LEVELS + 1];
+};
+
+__device__ __forceinline__ double lum_of(const LumParams &L, long long c)
+{
+    int l = 0;
+    while (l + 1 < L.n_levels && c >= L.level_off[l + 1]) ++l;
+    return cell_luminosity(L.kabs, L.freq_hz, L.cellw[c], l, L.T[c]);
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+
+// out[0] += sum of L_c over all cells (count == NULL) or over the cells that send packages; out[1] += number of cells
+// with L_c > 0
+__global__ void __launch_bounds__(256) lum_sum_kernel(const __grid_constant__ LumParams L, const int32_t *count, double *out)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double sum = 0.0, n_emit = 0.0;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < L.n_total; c += stride) {
+        const double l = lum_of(L, c);
+        if (l > 0.0 && (!count || count[c] > 0)) { sum += l; n_emit += 1.0; }
+    }
+    sum = warp_sum(sum); n_emit = warp_sum(n_emit);
+    if ((threadIdx.x & 31) == 0) { atomicAdd(out, sum); atomicAdd(out + 1, n_emit); }
+}
+
+// package counts per cell: mode 0 the same number m from every emitting cell, mode 1 in proportion to the
+// luminosity with a cap; out[2] += sum of the counts.  in[0] = sum L, in[1] = number of emitting cells
+__global__ void __launch_bounds__(256) dust_counts_kernel(const __grid_constant__ LumParams L, int mode, long long n_request,
+                                                          int cap, int32_t *count, double *scal)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const double tot = scal[0];
+    const long long n_emit = (long long)scal[1];
+    const long long m = n_emit > 0 ? (n_request + n_emit - 1) / n_emit : 0;
+    double n_sum = 0.0;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < L.n_total; c += stride) {
+        const double l = lum_of(L, c);
+        long long n = 0;
+        if (l > 0.0 && n_request > 0) {
+            if (mode == 0) n = m;
+            else {
+                n = (long long)ceil((double)n_request * l / tot);
+                n = n < 1 ? 1 : (n > cap ? cap : n);
+            }
+        }
+        count[c] = (int32_t)n;
+        n_sum += (double)n;
+    }
+    n_sum = warp_sum(n_sum);
+    if ((threadIdx.x & 31) == 0) atomicAdd(scal + 2, n_sum);
+}
+
+// exclusive prefix sums of count[n] -> first[n + 1], three passes over blocks of 2048 elements
+constexpr int kScanBlock = 2048;
+
+__global__ void __launch_bounds__(256) scan_block_sums_kernel(const int32_t *count, long long n, uint32_t *block_sums)
+{
+    __shared__ uint32_t s_w[8];
+    const long long base = (long long)blockIdx.x * kScanBlock;
+    uint32_t v = 0;
+    for (int i = threadIdx.x; i < kScanBlock; i += 256) {
+        const long long c = base + i;
+        if (c < n) v += (uint32_t)count[c];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t t = 0;
+        for (int w = 0; w < 8; ++w) t += s_w[w];
+        block_sums[blockIdx.x] = t;
+    }
+}
+
+__global__ void __launch_bounds__(1024) scan_offsets_kernel(uint32_t *block_sums, int n_blocks)      // one block, in place
+{
+    __shared__ uint32_t s_part[1024];
+    const int per = (n_blocks + 1023) / 1024;
+    const int b0 = threadIdx.x * per, b1 = b0 + per < n_blocks ? b0 + per : n_blocks;
+    uint32_t t = 0;
+    for (int b = b0; b < b1; ++b) t += block_sums[b];
+    s_part[threadIdx.x] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t run = 0;
+        for (int i = 0; i < 1024; ++i) { const uint32_t v = s_part[i]; s_part[i] = run; run += v; }
+    }
+    __syncthreads();
+    uint32_t run = s_part[threadIdx.x];
+    for (int b = b0; b < b1; ++b) { const uint32_t v = block_sums[b]; block_sums[b] = run; run += v; }
+}
+
+__global__ void __launch_bounds__(256) scan_write_kernel(const int32_t *count, long long n, const uint32_t *block_offsets,
+                                                         uint32_t *first)
+{
+    // thread t owns the 8 consecutive elements base + 8 t ..; warp and block scans of the per-thread sums
+    __shared__ uint32_t s_w[8];
+    const long long base = (long long)blockIdx.x * kScanBlock + 8ll * threadIdx.x;
+    uint32_t v[8], sum = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { v[j] = base + j < n ? (uint32_t)count[base + j] : 0u; sum += v[j]; }
+    uint32_t incl = sum;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(kFull, incl, o); if (lane >= o) incl += y; }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    uint32_t off = block_offsets[blockIdx.x];
+    for (int w = 0; w < warp; ++w) off += s_w[w];
+    uint32_t run = off + incl - sum;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { if (base + j < n) first[base + j] = run; run += v[j]; }
+    if (base <= n - 1 && n - 1 < base + 8) first[n] = run;          // the thread that owns the last element closes the array
+}
+
+// f3: emitted[c] = sum_f w_f L_c,f(T_c)
+__global__ void __launch_bounds__(256) cell_emission_kernel(const __grid_constant__ LumParams L, const double *freqtab,
+                                                            int n_freq, double *emitted)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < L.n_total; c += stride) {
+        int l = 0;
+        while (l + 1 < L.n_levels && c >= L.level_off[l + 1]) ++l;
+        const uint32_t cw = L.cellw[c];
+        const float T = L.T[c];
+        double sum = 0.0;
+        if ((int32_t)cw >= 0 && __uint_as_float(cw) > 0.0f && T > 0.0f)
+            for (int f = 0; f < n_freq; ++f)
+                sum += freqtab[2 * n_freq + f] * cell_luminosity(freqtab[n_freq + f], freqtab[f], cw, l, T);
+        emitted[c] = sum;
+    }
+}
+
+// f3: effective absorbed energy of the diagonal ALI update: (A - S) / (1 - beta), beta = S / emitted in [0, 0.999]
+__global__ void __launch_bounds__(256) ali_effective_kernel(const double *absorbed, const double *self_abs, const double *emitted,
+                                                            long long n, double *eff)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += stride) {
+        double beta = emitted[c] > 0.0 ? self_abs[c] / emitted[c] : 0.0;
+        beta = beta > 0.999 ? 0.999 : (beta < 0.0 ? 0.0 : beta);
+        const double e = (absorbed[c] - self_abs[c]) / (1.0 - beta);
+        eff[c] = e < 0.0 ? 0.0 : e;
+    }
+}
+
+// running mean of the reference field: r = (W r + n d) / (W + n) for up to three arrays at once
+__global__ void __launch_bounds__(256) running_mean_kernel(double *r0, const double *d0, double *r1, const double *d1, double *r2,
+                                                           const double *d2, long long n, double w_old, double w_new)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const double inv = 1.0 / (w_old + w_new);
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += stride) {
+        r0[c] = (w_old * r0[c] + w_new * d0[c]) * inv;
+        if (r1) r1[c] = (w_old * r1[c] + w_new * d1[c]) * inv;
+        if (r2) r2[c] = (w_old * r2[c] + w_new * d2[c]) * inv;
+    }
+}
+
+__global__ void __launch_bounds__(256) add_kernel(double *out, const double *a, const double *b, long long n)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += stride) out[c] = a[c] + b[c];
+}
+
 // roofline probes: random gathers / random reductions over a footprint
 __device__ __forceinline__ uint32_t mix32(uint32_t x)
 {
@@ -1547,7 +1854,7 @@ int launch_unpad(soc_grid *G, bool acc32, double weight, double *absorbed, cudaS
     return SOC_OK;
 }
 
-template <bool HIER, bool REPLAY, bool ACC32, bool QK = false>
+template <bool HIER, bool REPLAY, bool ACC32, bool QK, bool DUST>
 int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
 {
     static_assert(!(HIER && QK) && (ACC32 || !QK), "photon_q_kernel walks regular grids with the fp32 accumulator only");
@@ -1556,8 +1863,8 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
     const int side = 2 * P.hot_r + 1;
     const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
     int per_sm = 0;
-    if (QK) SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<REPLAY>, threads, smem));
-    else SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY, ACC32>, threads, smem));
+    if (QK) SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<REPLAY, DUST>, threads, smem));
+    else SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY, ACC32, DUST>, threads, smem));
     if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
     if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
     blocks = per_sm * G->n_sm;                   // persistent: a whole number of CTAs per SM
@@ -1565,11 +1872,11 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
     const long long need = (n_pkg + threads - 1) / threads;
     if (need < blocks) blocks = (int)(need > 0 ? need : 1);
     if (G->opt_carveout >= 0) {
-        if (QK) SOC_CUDA(cudaFuncSetAttribute(photon_q_kernel<REPLAY>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
-        else SOC_CUDA(cudaFuncSetAttribute(photon_fast_kernel<HIER, REPLAY, ACC32>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
+        if (QK) SOC_CUDA(cudaFuncSetAttribute(photon_q_kernel<REPLAY, DUST>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
+        else SOC_CUDA(cudaFuncSetAttribute(photon_fast_kernel<HIER, REPLAY, ACC32, DUST>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
     }
-    if (QK) photon_q_kernel<REPLAY><<<blocks, threads, smem, st>>>(P);
-    else photon_fast_kernel<HIER, REPLAY, ACC32><<<blocks, threads, smem, st>>>(P);
+    if (QK) photon_q_kernel<REPLAY, DUST><<<blocks, threads, smem, st>>>(P);
+    else photon_fast_kernel<HIER, REPLAY, ACC32, DUST><<<blocks, threads, smem, st>>>(P);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     if (G->ev_after_photon) {                    // "timing": the pair brackets the photon kernel alone
@@ -1577,6 +1884,73 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
         G->ev_after_photon = nullptr;
     }
     return launch_unpad(G, ACC32, weight, absorbed, st);
+}
+
+// ---- f1 host helpers
+void fill_lum_params(const soc_grid *G, int ifreq, const float *T, LumParams *L)
+{
+    std::memset(L, 0, sizeof(*L));
+    L->cellw = G->d_cellw; L->T = T; L->kabs = G->kabs[ifreq]; L->freq_hz = G->freq[ifreq];
+    L->n_total = G->n_total; L->n_levels = G->n_levels;
+    for (int l = 0; l <= G->n_levels; ++l) L->level_off[l] = G->level_off[l];
+}
+
+int ensure_dust_buffers(soc_grid *G)
+{
+    if (G->d_dust_first) return SOC_OK;
+    const long long n_blocks = (G->n_total + kScanBlock - 1) / kScanBlock;
+    SOC_CUDA(cudaMalloc(&G->d_dust_first, sizeof(uint32_t) * (size_t)(G->n_total + 1)));
+    SOC_CUDA(cudaMalloc(&G->d_scan_blocks, sizeof(uint32_t) * (size_t)n_blocks));
+    SOC_CUDA(cudaMalloc(&G->d_scalars, sizeof(double) * 8));
+    SOC_CUDA(cudaMallocHost(&G->h_scalars, sizeof(double) * 8));
+    return SOC_OK;
+}
+
+// stride that spreads consecutive dust package ids over the cells: the odd number nearest below n / golden ratio that
+// is coprime to n, so that q -> q * stride mod n is a permutation of [0, n)
+unsigned long long dust_stride(long long n)
+{
+    if (n <= 2) return 1;
+    long long s = (long long)std::floor((double)n * 0.6180339887498949) | 1;
+    for (;;) {
+        long long a = s, b = n;
+        while (b) { const long long t = a % b; a = b; b = t; }
+        if (a == 1) return (unsigned long long)s;
+        s += 2;
+    }
+}
+
+// prefix sums of the caller's package counts, sum of the luminosities of the sending cells; fills D.  Synchronises `st`.
+int dust_prepare(soc_grid *G, int ifreq, const soc_sources *src, long long n_const, double weight, DustParams *D,
+                 double *lum_total, cudaStream_t st)
+{
+    if (!src->dust_T || !src->dust_count) return fail(SOC_EINVAL, "dust packages requested but dust_T / dust_count is NULL");
+    if (src->n_dust >= (1ll << 32)) return fail(SOC_EINVAL, "n_dust must be < 2^32");
+    int rc = ensure_dust_buffers(G);
+    if (rc != SOC_OK) return rc;
+    LumParams L;
+    fill_lum_params(G, ifreq, src->dust_T, &L);
+    const int n_blocks = (int)((G->n_total + kScanBlock - 1) / kScanBlock);
+    SOC_CUDA(cudaMemsetAsync(G->d_scalars, 0, sizeof(double) * 8, st));
+    lum_sum_kernel<<<G->n_sm * 8, 256, 0, st>>>(L, src->dust_count, G->d_scalars);
+    scan_block_sums_kernel<<<n_blocks, 256, 0, st>>>(src->dust_count, G->n_total, G->d_scan_blocks);
+    scan_offsets_kernel<<<1, 1024, 0, st>>>(G->d_scan_blocks, n_blocks);
+    scan_write_kernel<<<n_blocks, 256, 0, st>>>(src->dust_count, G->n_total, G->d_scan_blocks, G->d_dust_first);
+    g_launches += 4;
+    SOC_CUDA(cudaGetLastError());
+    uint32_t total = 0;
+    SOC_CUDA(cudaMemcpyAsync(G->h_scalars, G->d_scalars, sizeof(double) * 2, cudaMemcpyDeviceToHost, st));
+    SOC_CUDA(cudaMemcpyAsync(&total, G->d_dust_first + G->n_total, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    SOC_CUDA(cudaStreamSynchronize(st));
+    if ((long long)total != src->n_dust) return fail(SOC_EINVAL, "n_dust is not the sum of dust_count");
+    *lum_total = G->h_scalars[0];
+    if (!(*lum_total > 0.0) || !std::isfinite(*lum_total)) return fail(SOC_EINVAL, "dust packages requested from cells that emit nothing");
+    D->n_const = n_const; D->n_dust = src->n_dust; D->stride = dust_stride(src->n_dust);
+    D->first = G->d_dust_first; D->count = src->dust_count; D->T = src->dust_T; D->self_abs = src->dust_self;
+    D->kabs = G->kabs[ifreq]; D->freq_hz = G->freq[ifreq]; D->weight = weight;
+    D->n_levels = G->n_levels;
+    for (int l = 0; l <= G->n_levels; ++l) D->level_off[l] = (int)G->level_off[l];
+    return SOC_OK;
 }
 
 int check_sources(const soc_grid *G, const soc_sources *src, long long n_packages, long long *n_bg_out)
@@ -1594,12 +1968,14 @@ int check_sources(const soc_grid *G, const soc_sources *src, long long n_package
     if (src->n_point < 0 || src->n_point > SOC_MAX_POINT_SOURCES) return fail(SOC_EINVAL, "n_point out of range");
     if (src->n_point > 0 && (!src->ps_pos || !src->ps_lum)) return fail(SOC_EINVAL, "point source arrays are NULL");
     const bool has_bg = src->bg_intensity > 0.0, has_ps = src->n_point > 0;
+    if (src->n_dust < 0 || src->n_dust > n_packages) return fail(SOC_EINVAL, "n_dust out of range");
+    const long long n_const = n_packages - src->n_dust;      // the dust packages are the last n_dust ids
     long long n_bg = src->n_bg;
-    if (n_bg < 0) n_bg = (has_bg && has_ps) ? n_packages / 2 : (has_bg ? n_packages : 0);
-    if (n_bg > n_packages) return fail(SOC_EINVAL, "n_bg > n_packages");
+    if (n_bg < 0) n_bg = (has_bg && has_ps) ? n_const / 2 : (has_bg ? n_const : 0);
+    if (n_bg > n_const) return fail(SOC_EINVAL, "n_bg > n_packages - n_dust");
     if (n_bg > 0 && !(has_bg && std::isfinite(src->bg_intensity)))
         return fail(SOC_EINVAL, "background packages requested but bg_intensity <= 0");
-    if (n_packages - n_bg > 0 && !has_ps) return fail(SOC_EINVAL, "point-source packages requested but n_point == 0");
+    if (n_const - n_bg > 0 && !has_ps) return fail(SOC_EINVAL, "point-source packages requested but n_point == 0");
     for (int k = 0; k < src->n_point; ++k) {
         const double *q = src->ps_pos + 3 * k;
         if (!(q[0] > 0.0 && q[0] < G->nx && q[1] > 0.0 && q[1] < G->ny && q[2] > 0.0 && q[2] < G->nz))
@@ -1639,12 +2015,19 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
     } else {
         P.n_point = src->n_point;
         if (n_bg > 0) P.bg_e0 = kPi * src->bg_intensity * P.surf / (double)n_bg;
-        const long long n_ps = n_packages - n_bg;
+        const long long n_ps = n_packages - src->n_dust - n_bg;
         for (int k = 0; k < src->n_point; ++k) {
             for (int j = 0; j < 3; ++j) P.ps_pos[k][j] = src->ps_pos[3 * k + j];
             const long long count_k = n_ps / src->n_point + ((n_ps % src->n_point) > k ? 1 : 0);
             P.ps_e0[k] = count_k > 0 ? src->ps_lum[k] / (double)count_k : 0.0;
         }
+    }
+    // f1: dust re-emission -- the last n_dust ids; prefix sums of the counts, sum of the luminosities (synchronises)
+    P.dust.n_const = n_packages;                 // no dust: every id is below n_const
+    double dust_lum_total = 0.0;
+    if (!src->beam && src->n_dust > 0 && pkg_count > 0) {
+        rc = dust_prepare(G, ifreq, src, n_packages - src->n_dust, weight, &P.dust, &dust_lum_total, st);
+        if (rc != SOC_OK) return rc;
     }
     P.pkg_begin = pkg_begin; P.pkg_end = pkg_begin + pkg_count;
     P.seed = seed; P.ifreq = ifreq; P.weight = weight;
@@ -1695,6 +2078,11 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         // this launch; falls back to the fp64 accumulator when a source class would underflow in those units
         double e_ref = P.is_beam ? 1.0 : P.bg_e0;
         for (int k = 0; k < P.n_point; ++k) e_ref = std::fmax(e_ref, P.ps_e0[k]);
+        // dust packages carry L_c / n_c each: the mean package energy is the unit (the sums are fp32: any unit within
+        // range will do; with weighted counts most packages carry about this much, capped cells more)
+        F.dust = P.dust;
+        if (P.dust.n_dust > 0) e_ref = std::fmax(e_ref, dust_lum_total / (double)P.dust.n_dust);
+        F.e_ref = e_ref;
         bool acc32 = G->opt_acc32 != 0 && e_ref > 0.0 && std::isfinite(e_ref);
         if (acc32) {
             F.beam_rel = (float)(1.0 / e_ref);
@@ -1722,18 +2110,21 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         const bool v2 = !hier && acc32 && (G->opt_kernel == 2 || (G->opt_kernel == 0 && big)) && pkg_count < (1ll << 32);
         if (v2) F.service_threshold = auto_threshold;
         const int sel = (v2 ? 8 : 0) | (hier ? 4 : 0) | ((rep || G->opt_stats) ? 2 : 0) | (acc32 ? 1 : 0);
+#define SOC_LF(H, R, A, Q) (F.dust.n_dust > 0 ? launch_fast<H, R, A, Q, true>(G, F, w_eff, absorbed, st) \
+                                              : launch_fast<H, R, A, Q, false>(G, F, w_eff, absorbed, st))
         switch (sel) {
-        case 9: rc = launch_fast<false, false, true, true>(G, F, w_eff, absorbed, st); break;
-        case 11: rc = launch_fast<false, true, true, true>(G, F, w_eff, absorbed, st); break;
-        case 0: rc = launch_fast<false, false, false>(G, F, w_eff, absorbed, st); break;
-        case 1: rc = launch_fast<false, false, true>(G, F, w_eff, absorbed, st); break;
-        case 2: rc = launch_fast<false, true, false>(G, F, w_eff, absorbed, st); break;
-        case 3: rc = launch_fast<false, true, true>(G, F, w_eff, absorbed, st); break;
-        case 4: rc = launch_fast<true, false, false>(G, F, w_eff, absorbed, st); break;
-        case 5: rc = launch_fast<true, false, true>(G, F, w_eff, absorbed, st); break;
-        case 6: rc = launch_fast<true, true, false>(G, F, w_eff, absorbed, st); break;
-        default: rc = launch_fast<true, true, true>(G, F, w_eff, absorbed, st); break;
+        case 9: rc = SOC_LF(false, false, true, true); break;
+        case 11: rc = SOC_LF(false, true, true, true); break;
+        case 0: rc = SOC_LF(false, false, false, false); break;
+        case 1: rc = SOC_LF(false, false, true, false); break;
+        case 2: rc = SOC_LF(false, true, false, false); break;
+        case 3: rc = SOC_LF(false, true, true, false); break;
+        case 4: rc = SOC_LF(true, false, false, false); break;
+        case 5: rc = SOC_LF(true, false, true, false); break;
+        case 6: rc = SOC_LF(true, true, false, false); break;
+        default: rc = SOC_LF(true, true, true, false); break;
         }
+#undef SOC_LF
     }
     if (rc == SOC_OK && G->opt_timing) {
         if (G->ev_after_photon) SOC_CUDA(cudaEventRecord(G->ev1[slot], st));
@@ -1785,6 +2176,8 @@ void soc_grid_destroy(soc_grid *G)
     cudaFree(G->d_table); cudaFree(G->d_cellw_int); cudaFree(G->d_parent_int); cudaFree(G->d_acc); cudaFree(G->d_acc32);
     if (G->h_results) cudaFreeHost(G->h_results);
     if (G->h_table) cudaFreeHost(G->h_table);
+    if (G->h_scalars) cudaFreeHost(G->h_scalars);
+    cudaFree(G->d_dust_first); cudaFree(G->d_scan_blocks); cudaFree(G->d_scalars); cudaFree(G->d_freqtab); cudaFree(G->d_eff);
     if (G->ev_table) cudaEventDestroy(G->ev_table);
     cudaFree(G->d_acc32_b); cudaFree(G->d_acc_b);
     if (G->aux) cudaStreamDestroy(G->aux);
@@ -2092,6 +2485,148 @@ int soc_update_temperatures(soc_grid *G, const double *absorbed, double scale, c
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     return SOC_OK;
+}
+
+int soc_emission_counts(soc_grid *G, int32_t ifreq, const float *T, int32_t mode, int64_t n_request, int32_t cap,
+                        int32_t *count, int64_t *n_dust, double *lum_total, void *stream)
+{
+    if (!G || !T || !count || !n_dust) return fail(SOC_EINVAL, "NULL argument");
+    if (ifreq < 0 || ifreq >= G->n_freq) return fail(SOC_EINVAL, "ifreq out of range");
+    if (n_request < 0 || (mode != 0 && mode != 1) || (mode == 1 && cap < 1)) return fail(SOC_EINVAL, "bad mode / n_request / cap");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ensure_dust_buffers(G);
+    if (rc != SOC_OK) return rc;
+    LumParams L;
+    fill_lum_params(G, ifreq, T, &L);
+    SOC_CUDA(cudaMemsetAsync(G->d_scalars, 0, sizeof(double) * 8, st));
+    lum_sum_kernel<<<G->n_sm * 8, 256, 0, st>>>(L, nullptr, G->d_scalars);
+    dust_counts_kernel<<<G->n_sm * 8, 256, 0, st>>>(L, mode, n_request, cap, count, G->d_scalars);
+    g_launches += 2;
+    SOC_CUDA(cudaGetLastError());
+    SOC_CUDA(cudaMemcpyAsync(G->h_scalars, G->d_scalars, sizeof(double) * 3, cudaMemcpyDeviceToHost, st));
+    SOC_CUDA(cudaStreamSynchronize(st));
+    *n_dust = (int64_t)G->h_scalars[2];
+    if (lum_total) *lum_total = G->h_scalars[0];
+    return SOC_OK;
+}
+
+int soc_cell_emission(soc_grid *G, const float *T, double *emitted, void *stream)
+{
+    if (!G || !T || !emitted) return fail(SOC_EINVAL, "NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!G->d_freqtab) {
+        std::vector<double> tab((size_t)3 * G->n_freq), w;
+        trapezoid(G->freq, w);
+        for (int f = 0; f < G->n_freq; ++f) { tab[f] = G->freq[f]; tab[G->n_freq + f] = G->kabs[f]; tab[2 * G->n_freq + f] = w[f]; }
+        SOC_CUDA(cudaMalloc(&G->d_freqtab, sizeof(double) * tab.size()));
+        SOC_CUDA(cudaMemcpy(G->d_freqtab, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice));
+    }
+    LumParams L;
+    fill_lum_params(G, 0, T, &L);
+    cell_emission_kernel<<<G->n_sm * 8, 256, 0, st>>>(L, G->d_freqtab, G->n_freq, emitted);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    return SOC_OK;
+}
+
+int soc_update_temperatures_ali(soc_grid *G, const double *absorbed, const double *self_abs, const double *emitted,
+                                double scale, const float *table_T, int32_t n_table, double E_min, double E_max,
+                                float *T_out, void *stream)
+{
+    if (!G || !absorbed || !self_abs || !emitted) return fail(SOC_EINVAL, "NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!G->d_eff) SOC_CUDA(cudaMalloc(&G->d_eff, sizeof(double) * (size_t)G->n_total));
+    ali_effective_kernel<<<G->n_sm * 8, 256, 0, st>>>(absorbed, self_abs, emitted, G->n_total, G->d_eff);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    return soc_update_temperatures(G, G->d_eff, scale, table_T, n_table, E_min, E_max, T_out, stream);
+}
+
+int soc_iterate(soc_grid *G, const soc_sources *src, int64_t n_const, uint64_t seed, const soc_iterate_opts *opts,
+                double t_scale, const float *table_T, int32_t n_table, double E_min, double E_max,
+                double *absorbed_out, float *T_out, soc_iterate_record *history, uint32_t flags, void *stream)
+{
+    if (!G || !src || !opts || !absorbed_out || !T_out || !table_T) return fail(SOC_EINVAL, "NULL argument");
+    if (opts->n_iter < 0 || (opts->n_iter > 0 && !opts->n_request) || opts->ref_start < 1)
+        return fail(SOC_EINVAL, "bad iteration options");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nb = sizeof(double) * (size_t)G->n_total;
+    const int nf = G->n_freq;
+    std::vector<double> w;
+    trapezoid(G->freq, w);
+    // work arrays: A_const, D (this iteration), R (reference field); with ALI also S_i, S_ref, Em_i, Em_ref
+    double *buf[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    int32_t *count = nullptr;
+    const int n_buf = opts->ali ? 7 : 3;
+    auto cleanup = [&]() { for (double *b : buf) cudaFree(b); cudaFree(count); };
+    for (int i = 0; i < n_buf; ++i)
+        if (cudaMalloc(&buf[i], nb) != cudaSuccess || cudaMemsetAsync(buf[i], 0, nb, st) != cudaSuccess) {
+            cleanup();
+            return fail(SOC_ENOMEM, "soc_iterate: device allocation failed");
+        }
+    if (cudaMalloc(&count, sizeof(int32_t) * (size_t)G->n_total) != cudaSuccess) { cleanup(); return fail(SOC_ENOMEM, "soc_iterate: device allocation failed"); }
+    double *A_const = buf[0], *D = buf[1], *R = buf[2], *Si = buf[3], *Sref = buf[4], *Emi = buf[5], *Emref = buf[6];
+    std::vector<soc_freq_result> res((size_t)nf);
+    int rc = SOC_OK;
+    auto record = [&](int it, int64_t n_pk) {
+        if (!history) return;
+        soc_iterate_record r{0.0, 0.0, 0.0, n_pk, 0};
+        for (int f = 0; f < nf; ++f) {
+            r.emitted += w[f] * res[f].emitted; r.escaped += w[f] * res[f].escaped; r.absorbed += w[f] * res[f].absorbed;
+            r.cell_steps += res[f].cell_steps;
+        }
+        history[it] = r;
+    };
+    // iteration 0: the constant sources
+    rc = soc_simulate_spectrum(G, src, n_const, seed, 0, n_const, A_const, res.data(), flags, stream);
+    if (rc == SOC_OK) record(0, n_const * nf);
+    if (rc == SOC_OK) rc = soc_update_temperatures(G, A_const, t_scale, table_T, n_table, E_min, E_max, T_out, stream);
+    double w_ref = 0.0;
+    const int blocks = G->n_sm * 8;
+    for (int it = 1; it <= opts->n_iter && rc == SOC_OK; ++it) {
+        const int64_t n_req = opts->n_request[it - 1];
+        if (cudaMemsetAsync(D, 0, nb, st) != cudaSuccess || (opts->ali && cudaMemsetAsync(Si, 0, nb, st) != cudaSuccess)) {
+            rc = fail(SOC_ECUDA, "soc_iterate: memset failed");
+            break;
+        }
+        int64_t n_pk = 0;
+        for (int f = 0; f < nf && rc == SOC_OK; ++f) {
+            std::memset(&res[f], 0, sizeof(res[f]));
+            int64_t n_dust = 0;
+            rc = soc_emission_counts(G, f, T_out, opts->mode, n_req, opts->cap, count, &n_dust, nullptr, stream);
+            if (rc != SOC_OK || n_dust == 0) continue;
+            soc_sources ds;
+            std::memset(&ds, 0, sizeof(ds));
+            ds.n_bg = 0; ds.n_dust = n_dust; ds.dust_T = T_out; ds.dust_count = count; ds.dust_self = opts->ali ? Si : nullptr;
+            rc = soc_simulate_frequency(G, f, &ds, n_dust, seed + (uint64_t)it, w[f], D, &res[f], flags, stream);
+            n_pk += n_dust;
+        }
+        if (rc != SOC_OK) break;
+        record(it, n_pk);
+        if (opts->ali) rc = soc_cell_emission(G, T_out, Emi, stream);
+        if (rc != SOC_OK) break;
+        const double *A_dust = D, *S_use = Si, *Em_use = Emi;
+        if (opts->reference_field && it >= opts->ref_start) {
+            running_mean_kernel<<<blocks, 256, 0, st>>>(R, D, opts->ali ? Sref : nullptr, Si, opts->ali ? Emref : nullptr, Emi,
+                                                        G->n_total, w_ref, (double)n_req);
+            g_launches += 1;
+            w_ref += (double)n_req;
+            A_dust = R; S_use = Sref; Em_use = Emref;
+        }
+        add_kernel<<<blocks, 256, 0, st>>>(absorbed_out, A_const, A_dust, G->n_total);
+        g_launches += 1;
+        if (cudaGetLastError() != cudaSuccess) { rc = fail(SOC_ECUDA, "soc_iterate: kernel launch failed"); break; }
+        if (opts->ali) rc = soc_update_temperatures_ali(G, absorbed_out, S_use, Em_use, t_scale, table_T, n_table, E_min, E_max, T_out, stream);
+        else rc = soc_update_temperatures(G, absorbed_out, t_scale, table_T, n_table, E_min, E_max, T_out, stream);
+    }
+    if (rc == SOC_OK && opts->n_iter == 0) {
+        cudaError_t e = cudaMemcpyAsync(absorbed_out, A_const, nb, cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) rc = fail(SOC_ECUDA, cudaGetErrorString(e));
+    }
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess && rc == SOC_OK) rc = fail(SOC_ECUDA, cudaGetErrorString(e));
+    cleanup();
+    return rc;
 }
 
 int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_packages, uint64_t seed, int32_t n_iter,

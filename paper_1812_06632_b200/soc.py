@@ -20,7 +20,8 @@ MAX_POINT_SOURCES = 64
 
 EXPORTS = ["soc_grid_create", "soc_grid_destroy", "soc_grid_n_total", "soc_freq_weights", "soc_simulate_frequency",
            "soc_simulate_packages", "soc_simulate_spectrum", "soc_update_temperatures", "soc_run_host",
-           "soc_set_option", "soc_get_timings", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version"]
+           "soc_set_option", "soc_get_timings", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version",
+           "soc_emission_counts", "soc_cell_emission", "soc_update_temperatures_ali", "soc_iterate"]
 
 
 class SocError(RuntimeError):
@@ -36,7 +37,18 @@ class GridDesc(C.Structure):
 
 class Sources(C.Structure):
     _fields_ = [("bg_intensity", C.c_double), ("n_point", C.c_int32), ("ps_pos", C.c_void_p),
-                ("ps_lum", C.c_void_p), ("n_bg", C.c_int64), ("beam", C.c_void_p)]
+                ("ps_lum", C.c_void_p), ("n_bg", C.c_int64), ("beam", C.c_void_p),
+                ("n_dust", C.c_int64), ("dust_T", C.c_void_p), ("dust_count", C.c_void_p), ("dust_self", C.c_void_p)]
+
+
+class IterateOpts(C.Structure):
+    _fields_ = [("mode", C.c_int32), ("cap", C.c_int32), ("reference_field", C.c_int32), ("ref_start", C.c_int32),
+                ("ali", C.c_int32), ("n_iter", C.c_int32), ("n_request", C.c_void_p)]
+
+
+class IterateRecord(C.Structure):
+    _fields_ = [("emitted", C.c_double), ("escaped", C.c_double), ("absorbed", C.c_double),
+                ("n_packages", C.c_int64), ("cell_steps", C.c_uint64)]
 
 
 class FreqResult(C.Structure):
@@ -74,6 +86,11 @@ def load():
                                         C.POINTER(FreqResult), u32, vp]
     L.soc_simulate_spectrum.argtypes = [vp, C.POINTER(Sources), i64, u64, i64, i64, vp, C.POINTER(FreqResult), u32, vp]
     L.soc_update_temperatures.argtypes = [vp, vp, dbl, vp, i32, dbl, dbl, vp, vp]
+    L.soc_emission_counts.argtypes = [vp, i32, vp, i32, i64, i32, vp, C.POINTER(i64), C.POINTER(dbl), vp]
+    L.soc_cell_emission.argtypes = [vp, vp, vp, vp]
+    L.soc_update_temperatures_ali.argtypes = [vp, vp, vp, vp, dbl, vp, i32, dbl, dbl, vp, vp]
+    L.soc_iterate.argtypes = [vp, C.POINTER(Sources), i64, u64, C.POINTER(IterateOpts), dbl, vp, i32, dbl, dbl, vp, vp,
+                              C.POINTER(IterateRecord), u32, vp]
     L.soc_run_host.argtypes = [C.POINTER(GridDesc), C.POINTER(Sources), i64, u64, i32, dbl, vp, i32, dbl, dbl, vp, vp,
                                C.POINTER(FreqResult), u32]
     L.soc_set_option.argtypes = [vp, C.c_char_p, i64]
@@ -140,6 +157,10 @@ def make_sources(src: dict, keep: list):
         beam = np.ascontiguousarray(beam, dtype=np.float64).reshape(6)
         keep.append(beam)
         s.beam = beam.ctypes.data
+    if src.get("dust_count") is not None:             # f1: DEVICE tensors; n_dust = the sum of dust_count (host int)
+        s.n_dust = int(src["n_dust"])
+        s.dust_T, s.dust_count = _dev_ptr(src["dust_T"]), _dev_ptr(src["dust_count"])
+        s.dust_self = _dev_ptr(src.get("dust_self"))
     return s
 
 
@@ -223,6 +244,38 @@ class Grid:
         _check(load().soc_simulate_spectrum(self._h, arr, int(n_packages), int(seed), int(pkg_begin), int(pkg_count),
                                             _dev_ptr(absorbed_int), res, int(flags), _stream_ptr(stream)))
         return list(res) if want_results else None
+
+    def emission_counts(self, ifreq, T, mode, n_request, cap, count_out, stream=None):
+        """soc_emission_counts: writes count_out (DEVICE int32), returns (n_dust, sum of the luminosities)."""
+        n, tot = C.c_int64(0), C.c_double(0.0)
+        _check(load().soc_emission_counts(self._h, int(ifreq), _dev_ptr(T), {"uniform": 0, "weighted": 1}[mode], int(n_request),
+                                          int(cap), _dev_ptr(count_out), C.byref(n), C.byref(tot), _stream_ptr(stream)))
+        return n.value, tot.value
+
+    def cell_emission(self, T, emitted_out, stream=None):
+        _check(load().soc_cell_emission(self._h, _dev_ptr(T), _dev_ptr(emitted_out), _stream_ptr(stream)))
+
+    def update_temperatures_ali(self, absorbed, self_abs, emitted, scale, table_T, e_min, e_max, T_out, stream=None):
+        tab = _np(table_T, np.float32)
+        _check(load().soc_update_temperatures_ali(self._h, _dev_ptr(absorbed), _dev_ptr(self_abs), _dev_ptr(emitted), float(scale),
+                                                  _ptr(tab), len(tab), float(e_min), float(e_max), _dev_ptr(T_out),
+                                                  _stream_ptr(stream)))
+
+    def iterate(self, sources_list, n_const, seed, n_request, t_scale, table_T, e_min, e_max, absorbed_out, T_out,
+                mode="weighted", cap=10000, reference_field=True, ref_start=1, ali=False, flags=SOC_GEOM_FP32, stream=None):
+        """soc_iterate: constant sources once, then len(n_request) iterations of dust re-emission.  Returns the history."""
+        assert len(sources_list) == self.n_freq
+        arr, keep = make_sources_array(sources_list)
+        req = _np(n_request, np.int64)
+        opts = IterateOpts({"uniform": 0, "weighted": 1}[mode], int(cap), int(bool(reference_field)), int(ref_start),
+                           int(bool(ali)), len(req), _ptr(req) if len(req) else None)
+        hist = (IterateRecord * (len(req) + 1))()
+        tab = _np(table_T, np.float32)
+        _check(load().soc_iterate(self._h, arr, int(n_const), int(seed), C.byref(opts), float(t_scale), _ptr(tab), len(tab),
+                                  float(e_min), float(e_max), _dev_ptr(absorbed_out), _dev_ptr(T_out), hist, int(flags),
+                                  _stream_ptr(stream)))
+        return [dict(emitted=h.emitted, escaped=h.escaped, absorbed=h.absorbed, n_packages=h.n_packages,
+                     cell_steps=h.cell_steps) for h in hist]
 
     def update_temperatures(self, absorbed, scale, table_T, e_min, e_max, T_out, stream=None):
         tab = _np(table_T, np.float32)
