@@ -86,6 +86,9 @@ def lib():
                                                  C.c_int32, C.c_void_p]
         L.soc_oracle_emission_counts.restype = C.c_int64
         L.soc_oracle_emit_cell.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.soc_oracle_make_map.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
+                                          C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_void_p]
+        L.soc_oracle_make_map.restype = None
         L.soc_oracle_dust_stride.argtypes = [C.c_int64]
         L.soc_oracle_dust_stride.restype = C.c_int64
         L.soc_oracle_sizeof_replay.restype = C.c_int64
@@ -340,6 +343,16 @@ def update_temperatures(grid: Grid, absorbed, scale, table_T, E_min, E_max):
     out = np.zeros(grid.n_total, dtype=np.float32)
     lib().soc_oracle_update_temperatures(grid._h, _p(absorbed), float(scale), _p(table_T), len(table_T),
                                          float(E_min), float(E_max), _p(out))
+    return out
+
+
+def make_map(grid: Grid, kabs, ksca, freq_hz, T, ex, ey, direction, centre, npx, npy, pixel):
+    """Surface-brightness map (row f2): float64 [npy, npx]."""
+    T = np.ascontiguousarray(T, dtype=np.float32)
+    v = [np.ascontiguousarray(x, dtype=np.float64).reshape(3) for x in (ex, ey, direction, centre)]
+    out = np.zeros((int(npy), int(npx)), dtype=np.float64)
+    lib().soc_oracle_make_map(grid._h, float(kabs), float(ksca), float(freq_hz), _p(T), _p(v[0]), _p(v[1]), _p(v[2]), _p(v[3]),
+                              int(npx), int(npy), float(pixel), _p(out))
     return out
 
 

@@ -739,6 +739,85 @@ void soc_oracle_update_temperatures_ali(const soc_oracle_grid *G, const double *
     free(eff);
 }
 
+/* ------------------------------------------------------------------ f2: maps --------
+ * "As the final step, the host calls a mapping kernel to make surface brightness maps for the desired frequencies and
+ * directions" (K3 of PAPER.md:55; 1310 x 1310 pixels of the size of the smallest cells).
+ * The paper gives no formula; reading M1: thermal dust emission integrated along parallel lines of sight
+ * with extinction by absorption + scattering, no background behind the cloud, no scattered light (the paper makes
+ * those "with separate runs"):
+ *     I = sum over the cells k crossed, front to back, of  exp(-tau_k) S_k (1 - exp(-dtau_k)),
+ *     dtau_k = (kabs + ksca) rho_k ds_k,  S_k = kabs / (kabs + ksca) B_nu(T_k),  tau_k = sum of dtau in front of k.
+ * Geometry (reading M2): orthographic.  Pixel (i, j), i < npx fastest, looks along the unit vector dir from the point
+ *     o = centre + ((i + 1/2) - npx/2) pixel ex + ((j + 1/2) - npy/2) pixel ey          (ex, ey, dir orthonormal)
+ * The line enters the root grid where the slab test says; the cells are walked exactly as the packages walk them (a5/a6). */
+void soc_oracle_make_map(const soc_oracle_grid *G, double kabs, double ksca, double freq_hz, const float *T,
+                         const double ex[3], const double ey[3], const double dir[3], const double centre[3],
+                         int32_t npx, int32_t npy, double pixel, double *map)
+{
+    const double N[3] = { (double)G->nx, (double)G->ny, (double)G->nz };
+    const double kext = kabs + ksca;
+    for (int32_t j = 0; j < npy; ++j) for (int32_t i = 0; i < npx; ++i) {
+        const double a = ((double)i + 0.5 - 0.5 * (double)npx) * pixel, b = ((double)j + 0.5 - 0.5 * (double)npy) * pixel;
+        double o[3], t_in = -INFINITY, t_out = INFINITY;
+        for (int k = 0; k < 3; ++k) o[k] = centre[k] + a * ex[k] + b * ey[k];
+        for (int k = 0; k < 3; ++k) {                       /* slab test against [0, N_k] */
+            if (dir[k] != 0.0) {
+                double t0 = (0.0 - o[k]) / dir[k], t1 = (N[k] - o[k]) / dir[k];
+                if (t0 > t1) { double t = t0; t0 = t1; t1 = t; }
+                if (t0 > t_in) t_in = t0;
+                if (t1 < t_out) t_out = t1;
+            } else if (o[k] < 0.0 || o[k] > N[k]) { t_in = INFINITY; }
+        }
+        double I = 0.0, tau = 0.0;
+        if (t_in < t_out) {
+            soc_oracle_state S;
+            S.f32state = 0;
+            int32_t ijk[3];
+            for (int k = 0; k < 3; ++k) {
+                double x = o[k] + t_in * dir[k];
+                int32_t c = (int32_t)floor(x);
+                const int32_t nk = (k == 0) ? G->nx : (k == 1) ? G->ny : G->nz;
+                if (c < 0) c = 0;
+                if (c > nk - 1) c = nk - 1;
+                double f = x - (double)c;
+                if (f < 0.0) f = 0.0;
+                if (f > 1.0) f = 1.0;
+                ijk[k] = c; S.f[k] = f; S.d[k] = dir[k];
+            }
+            S.level = 1;
+            S.cell = ijk[0] + G->nx * (ijk[1] + G->ny * ijk[2]);
+            descend(G, &S);
+            for (;;) {
+                const int64_t gid = G->level_off[S.level - 1] + S.cell;
+                const double h = ldexp(1.0, -(S.level - 1));
+                double t[3];
+                for (int k = 0; k < 3; ++k) {
+                    if (S.d[k] > 0.0) t[k] = (1.0 - S.f[k]) / S.d[k];
+                    else if (S.d[k] < 0.0) t[k] = (-S.f[k]) / S.d[k];
+                    else t[k] = INFINITY;
+                    if (t[k] < 0.0) t[k] = 0.0;
+                }
+                int ax = 0;
+                if (t[1] < t[ax]) ax = 1;
+                if (t[2] < t[ax]) ax = 2;
+                const double ds = t[ax] * h, rho = (double)G->rho[gid];
+                const double dtau = kext * rho * ds;
+                if (dtau > 0.0 && (double)T[gid] > 0.0)
+                    I += exp(-tau) * (kabs / kext) * soc_oracle_planck(freq_hz, (double)T[gid]) * (-expm1(-dtau));
+                tau += dtau;
+                for (int k = 0; k < 3; ++k) {
+                    double fn = S.f[k] + t[ax] * S.d[k];
+                    if (fn < 0.0) fn = 0.0;
+                    if (fn > 1.0) fn = 1.0;
+                    S.f[k] = fn;
+                }
+                if (!move_across(G, &S, ax, S.d[ax] > 0.0 ? 1 : -1)) break;
+            }
+        }
+        map[(int64_t)j * npx + i] = I;
+    }
+}
+
 int64_t soc_oracle_sizeof_replay(void) { return (int64_t)sizeof(soc_oracle_replay); }
 int64_t soc_oracle_sizeof_trace(void) { return (int64_t)sizeof(soc_oracle_trace); }
 int64_t soc_oracle_grid_n_total(const soc_oracle_grid *G) { return G->n_total; }
