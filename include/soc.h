@@ -207,6 +207,22 @@ int soc_iterate(soc_grid *grid, const soc_sources *src, int64_t n_const, uint64_
                 double t_scale, const float *table_T, int32_t n_table, double E_min, double E_max,
                 double *absorbed_out, float *T_out, soc_iterate_record *history, uint32_t flags, void *cuda_stream);
 
+/* Surface-brightness map at frequency index ifreq (row f2; PAPER.md:55 K3, :67 "a mapping kernel to make surface brightness
+ * maps for the desired frequencies and directions", :137).  Thermal dust emission integrated along parallel lines of
+ * sight with extinction by absorption + scattering, no background, no scattered light (reading M1):
+ *     I = sum over the cells k crossed, front to back:  exp(-tau_k) kabs/(kabs+ksca) B_nu(T_k) (1 - exp(-dtau_k)),
+ *     dtau_k = (kabs + ksca) rho_k ds_k.
+ * Pixel (i, j), i fastest, looks along `dir` from  centre + ((i+1/2) - npx/2) pixel ex + ((j+1/2) - npy/2) pixel ey;
+ * ex, ey, dir orthonormal (checked to 1e-6), lengths in root-cell edges (reading M2).  T: DEVICE n_total floats.
+ * map: DEVICE npx*npy floats, written (intensity in the unit of B_nu, cgs). */
+typedef struct {
+    double ex[3], ey[3], dir[3], centre[3];
+    int32_t npx, npy;
+    double pixel;
+} soc_map_desc;
+
+int soc_make_map(soc_grid *grid, int32_t ifreq, const float *T, const soc_map_desc *desc, float *map, void *cuda_stream);
+
 /* Energy balance by table lookup (row a11; reading S10).  For every leaf with rho > 0:
  *   E = scale * absorbed[cell] / (rho * h^3),  h = 2^-(level-1)
  *   T = table_T interpolated linearly in the index x = (ln E - ln E_min)/(ln E_max - ln E_min)*(n_table-1);

@@ -1733,6 +1733,121 @@ __global__ void __launch_bounds__(256) add_kernel(double *out, const double *a, 
     for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += stride) out[c] = a[c] + b[c];
 }
 
+// ------------------------------------------------------------------------------------------------
+// f2: surface-brightness maps: one line of sight per thread, the cells walked as the packages walk
+// them (a5 / a6) in fp64 on the ABI-order arrays; emission with extinction, front to back
+// ------------------------------------------------------------------------------------------------
+struct MapParams {
+    int nx, ny, nz, n_root, hier;
+    const uint32_t *cellw;
+    const int32_t *parent;
+    const float *T;
+    double kabs, ksca, freq_hz;
+    double ex[3], ey[3], dir[3], centre[3];
+    int npx, npy;
+    double pixel;
+    float *map;
+};
+
+__global__ void __launch_bounds__(128) map_kernel(const __grid_constant__ MapParams M)
+{
+    const long long n_pix = (long long)M.npx * M.npy;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const double N[3] = {(double)M.nx, (double)M.ny, (double)M.nz};
+    const int n_i[3] = {M.nx, M.ny, M.nz};
+    const double kext = M.kabs + M.ksca;
+    const double inf = __longlong_as_double(0x7ff0000000000000ll);
+    for (long long pix = (long long)blockIdx.x * blockDim.x + threadIdx.x; pix < n_pix; pix += stride) {
+        const int i = (int)(pix % M.npx), j = (int)(pix / M.npx);
+        const double a = ((double)i + 0.5 - 0.5 * (double)M.npx) * M.pixel, b = ((double)j + 0.5 - 0.5 * (double)M.npy) * M.pixel;
+        double o[3], t_in = -inf, t_out = inf;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) o[k] = M.centre[k] + a * M.ex[k] + b * M.ey[k];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {                        // slab test against [0, N_k]
+            if (M.dir[k] != 0.0) {
+                double t0 = (0.0 - o[k]) / M.dir[k], t1 = (N[k] - o[k]) / M.dir[k];
+                if (t0 > t1) { const double t = t0; t0 = t1; t1 = t; }
+                t_in = t0 > t_in ? t0 : t_in;
+                t_out = t1 < t_out ? t1 : t_out;
+            } else if (o[k] < 0.0 || o[k] > N[k]) t_in = inf;
+        }
+        double I = 0.0, tau = 0.0;
+        if (t_in < t_out) {
+            int c3[3];
+            double f[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double x = o[k] + t_in * M.dir[k];
+                int c = (int)floor(x);
+                c = c < 0 ? 0 : (c > n_i[k] - 1 ? n_i[k] - 1 : c);
+                double fk = x - (double)c;
+                f[k] = fk < 0.0 ? 0.0 : (fk > 1.0 ? 1.0 : fk);
+                c3[k] = c;
+            }
+            int rel = c3[0] + M.nx * (c3[1] + M.ny * c3[2]);            // root cell id; octet cells: id of the ABI vector
+            int lev = 0;                                              // level - 1
+            bool inside = true;
+            while (inside) {
+                // a6: down to the leaf that holds the position
+                uint32_t cw = __ldg(M.cellw + rel);
+                while ((int32_t)cw < 0) {
+                    int slot = 0;
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        if (f[k] >= 0.5) { slot |= 1 << k; f[k] = 2.0 * f[k] - 1.0; } else f[k] = 2.0 * f[k];
+                    }
+                    rel = M.n_root + (int)(cw & 0x7fffffffu) + slot;
+                    lev += 1;
+                    cw = __ldg(M.cellw + rel);
+                }
+                double t[3];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double d = M.dir[k];
+                    double tk = d > 0.0 ? (1.0 - f[k]) / d : (d < 0.0 ? (-f[k]) / d : inf);
+                    t[k] = tk < 0.0 ? 0.0 : tk;
+                }
+                int ax = 0;                                  // lowest axis wins a tie (S4)
+                if (t[1] < t[ax]) ax = 1;
+                if (t[2] < t[ax]) ax = 2;
+                const double ts = t[ax];
+                const double ds = ts / (double)(1 << lev);
+                const double dtau = kext * (double)__uint_as_float(cw) * ds;
+                const double Tc = (double)__ldg(M.T + rel);
+                if (dtau > 0.0 && Tc > 0.0) I += exp(-tau) * (M.kabs / kext) * planck_nu(M.freq_hz, Tc) * (-expm1(-dtau));
+                tau += dtau;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double fn = f[k] + ts * M.dir[k];
+                    f[k] = fn < 0.0 ? 0.0 : (fn > 1.0 ? 1.0 : fn);
+                }
+                // a5 / a6: across the face of axis ax -- sibling flip, else up to the common parent
+                const int sg = M.dir[ax] > 0.0 ? 1 : -1;
+                bool found = false;
+                while (lev > 0) {
+                    const int oct = rel - M.n_root;
+                    const int bit = (oct >> ax) & 1;
+                    if ((sg > 0) != (bit != 0)) { rel ^= (1 << ax); found = true; break; }
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) f[k] = (f[k] + (double)((oct >> k) & 1)) * 0.5;
+                    const int par = __ldg(M.parent + (oct >> 3));             // parent id - n_root (negative: a root cell)
+                    rel = par + M.n_root;
+                    lev -= 1;
+                }
+                if (!found) {
+                    int ix = rel % M.nx, iy = (rel / M.nx) % M.ny, iz = rel / (M.nx * M.ny);
+                    if (ax == 0) ix += sg; else if (ax == 1) iy += sg; else iz += sg;
+                    if ((unsigned)ix >= (unsigned)M.nx || (unsigned)iy >= (unsigned)M.ny || (unsigned)iz >= (unsigned)M.nz) inside = false;
+                    rel = ix + M.nx * (iy + M.ny * iz);
+                }
+                f[ax] = sg > 0 ? 0.0 : 1.0;
+            }
+        }
+        M.map[pix] = (float)I;
+    }
+}
+
 // roofline probes: random gathers / random reductions over a footprint
 __device__ __forceinline__ uint32_t mix32(uint32_t x)
 {
@@ -2627,6 +2742,37 @@ int soc_iterate(soc_grid *G, const soc_sources *src, int64_t n_const, uint64_t s
     if (e != cudaSuccess && rc == SOC_OK) rc = fail(SOC_ECUDA, cudaGetErrorString(e));
     cleanup();
     return rc;
+}
+
+int soc_make_map(soc_grid *G, int32_t ifreq, const float *T, const soc_map_desc *d, float *map, void *stream)
+{
+    if (!G || !T || !d || !map) return fail(SOC_EINVAL, "NULL argument");
+    if (ifreq < 0 || ifreq >= G->n_freq) return fail(SOC_EINVAL, "ifreq out of range");
+    if (d->npx < 1 || d->npy < 1 || !(d->pixel > 0.0) || !std::isfinite(d->pixel)) return fail(SOC_EINVAL, "bad map size");
+    auto dot = [](const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; };
+    const double *v[3] = {d->ex, d->ey, d->dir};
+    for (int a = 0; a < 3; ++a)
+        for (int b = a; b < 3; ++b) {
+            const double x = dot(v[a], v[b]);
+            if (!(std::fabs(x - (a == b ? 1.0 : 0.0)) <= 1e-6)) return fail(SOC_EINVAL, "ex, ey, dir must be orthonormal");
+        }
+    for (int k = 0; k < 3; ++k)
+        if (!std::isfinite(d->centre[k])) return fail(SOC_EINVAL, "centre is not finite");
+    MapParams M;
+    std::memset(&M, 0, sizeof(M));
+    M.nx = G->nx; M.ny = G->ny; M.nz = G->nz; M.n_root = (int)G->n_root; M.hier = G->n_levels > 1;
+    M.cellw = G->d_cellw; M.parent = G->d_parent; M.T = T;
+    M.kabs = G->kabs[ifreq]; M.ksca = G->ksca[ifreq]; M.freq_hz = G->freq[ifreq];
+    for (int k = 0; k < 3; ++k) { M.ex[k] = d->ex[k]; M.ey[k] = d->ey[k]; M.dir[k] = d->dir[k]; M.centre[k] = d->centre[k]; }
+    M.npx = d->npx; M.npy = d->npy; M.pixel = d->pixel; M.map = map;
+    const long long n_pix = (long long)d->npx * d->npy;
+    long long blocks = (n_pix + 127) / 128;
+    const long long cap = (long long)G->n_sm * 16;
+    if (blocks > cap) blocks = cap;
+    map_kernel<<<(int)blocks, 128, 0, (cudaStream_t)stream>>>(M);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    return SOC_OK;
 }
 
 int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_packages, uint64_t seed, int32_t n_iter,

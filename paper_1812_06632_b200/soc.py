@@ -21,7 +21,7 @@ MAX_POINT_SOURCES = 64
 EXPORTS = ["soc_grid_create", "soc_grid_destroy", "soc_grid_n_total", "soc_freq_weights", "soc_simulate_frequency",
            "soc_simulate_packages", "soc_simulate_spectrum", "soc_update_temperatures", "soc_run_host",
            "soc_set_option", "soc_get_timings", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version",
-           "soc_emission_counts", "soc_cell_emission", "soc_update_temperatures_ali", "soc_iterate"]
+           "soc_emission_counts", "soc_cell_emission", "soc_update_temperatures_ali", "soc_iterate", "soc_make_map"]
 
 
 class SocError(RuntimeError):
@@ -39,6 +39,11 @@ class Sources(C.Structure):
     _fields_ = [("bg_intensity", C.c_double), ("n_point", C.c_int32), ("ps_pos", C.c_void_p),
                 ("ps_lum", C.c_void_p), ("n_bg", C.c_int64), ("beam", C.c_void_p),
                 ("n_dust", C.c_int64), ("dust_T", C.c_void_p), ("dust_count", C.c_void_p), ("dust_self", C.c_void_p)]
+
+
+class MapDesc(C.Structure):
+    _fields_ = [("ex", C.c_double * 3), ("ey", C.c_double * 3), ("dir", C.c_double * 3), ("centre", C.c_double * 3),
+                ("npx", C.c_int32), ("npy", C.c_int32), ("pixel", C.c_double)]
 
 
 class IterateOpts(C.Structure):
@@ -91,6 +96,7 @@ def load():
     L.soc_update_temperatures_ali.argtypes = [vp, vp, vp, vp, dbl, vp, i32, dbl, dbl, vp, vp]
     L.soc_iterate.argtypes = [vp, C.POINTER(Sources), i64, u64, C.POINTER(IterateOpts), dbl, vp, i32, dbl, dbl, vp, vp,
                               C.POINTER(IterateRecord), u32, vp]
+    L.soc_make_map.argtypes = [vp, i32, vp, C.POINTER(MapDesc), vp, vp]
     L.soc_run_host.argtypes = [C.POINTER(GridDesc), C.POINTER(Sources), i64, u64, i32, dbl, vp, i32, dbl, dbl, vp, vp,
                                C.POINTER(FreqResult), u32]
     L.soc_set_option.argtypes = [vp, C.c_char_p, i64]
@@ -244,6 +250,14 @@ class Grid:
         _check(load().soc_simulate_spectrum(self._h, arr, int(n_packages), int(seed), int(pkg_begin), int(pkg_count),
                                             _dev_ptr(absorbed_int), res, int(flags), _stream_ptr(stream)))
         return list(res) if want_results else None
+
+    def make_map(self, ifreq, T, ex, ey, direction, centre, npx, npy, pixel, map_out, stream=None):
+        """soc_make_map: map_out = DEVICE float32 tensor of npx * npy elements (pixel i fastest)."""
+        d = MapDesc()
+        for name, v in (("ex", ex), ("ey", ey), ("dir", direction), ("centre", centre)):
+            setattr(d, name, (C.c_double * 3)(*[float(x) for x in v]))
+        d.npx, d.npy, d.pixel = int(npx), int(npy), float(pixel)
+        _check(load().soc_make_map(self._h, int(ifreq), _dev_ptr(T), C.byref(d), _dev_ptr(map_out), _stream_ptr(stream)))
 
     def emission_counts(self, ifreq, T, mode, n_request, cap, count_out, stream=None):
         """soc_emission_counts: writes count_out (DEVICE int32), returns (n_dust, sum of the luminosities)."""
