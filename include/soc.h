@@ -267,6 +267,11 @@ int soc_get_timings(soc_grid *grid, int32_t n, float *ms);
  * independent of the others.  *ms receives the CUDA-event time of the probe kernel. */
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms);
 
+/* Bounds-checked build (libsoc_b200_checked.so, compiled with -DSOC_CHECKED): number of out-of-range indices the photon
+ * kernels produced so far in this process (each such access was redirected to element 0), after synchronising the device.
+ * -1 in the product library, where the checks are compiled out.  -2 on a CUDA error. */
+int64_t soc_checked_violations(void);
+
 /* Number of kernel launches issued by this library in the calling process (bench.py's "gpu_launches"). */
 uint64_t soc_launch_count(void);
 

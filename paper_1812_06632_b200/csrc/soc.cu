@@ -41,6 +41,22 @@ constexpr double kWMin = 1e-9;          // termination threshold relative to the
 constexpr int kChunk = 64;              // package ids a warp claims from the global counter at a time
 constexpr unsigned kFull = 0xffffffffu;
 
+// Bounds-checked build (-DSOC_CHECKED; paper_1812_06632_b200/build.py --checked -> libsoc_b200_checked.so): every index
+// into a global or shared array of the photon kernels is tested against the array's length; a violation is counted
+// (soc_checked_violations) and the access redirected to element 0.  The stand-in for compute-sanitizer memcheck on
+// boxes where the sanitizer cannot run; compiled out of the product library.
+#ifdef SOC_CHECKED
+__device__ unsigned int g_violations = 0;
+__device__ __forceinline__ long long ck_index(long long i, long long n)
+{
+    if (i < 0 || i >= n) { atomicAdd(&g_violations, 1u); return 0; }
+    return i;
+}
+#define CK(i, n) ck_index((long long)(i), (long long)(n))
+#else
+#define CK(i, n) (i)
+#endif
+
 struct DevResult {                      // one slot per launch, accumulated with atomics
     double emitted, escaped, absorbed;
     unsigned long long cell_steps, scatterings, terminated;
@@ -64,6 +80,7 @@ struct DustParams {
 struct SimParams {
     // grid
     int nx, ny, nz, n_root;
+    int n_total, n_oct;                 // lengths of cellw / parent (bounds-checked build)
     const uint32_t *cellw;              // [n_total] leaf: fp32 density bits; parent: 0x80000000 | (first child id - n_root)
     const int32_t *parent;              // [n_octets] (parent id - n_root) of octet (id - n_root) >> 3
     // dust at this frequency
@@ -229,7 +246,7 @@ template <typename A> __device__ __forceinline__ void set_direction(Pkg<A> &p, A
 // a6: descend to the leaf that holds the position; 2f and 2f-1 are exact in fp32
 template <typename A> __device__ __forceinline__ void descend(const SimParams &P, Pkg<A> &p)
 {
-    uint32_t cw = __ldg(P.cellw + (p.rel + P.n_root));
+    uint32_t cw = __ldg(P.cellw + CK(p.rel + P.n_root, P.n_total));
     while ((int32_t)cw < 0) {
         int slot = 0;
         if (p.fx >= 0.5f) { slot |= 1; p.fx = 2.0f * p.fx - 1.0f; } else p.fx = 2.0f * p.fx;
@@ -237,7 +254,7 @@ template <typename A> __device__ __forceinline__ void descend(const SimParams &P
         if (p.fz >= 0.5f) { slot |= 4; p.fz = 2.0f * p.fz - 1.0f; } else p.fz = 2.0f * p.fz;
         p.rel = (int)(cw & 0x7fffffffu) + slot;
         p.h *= 0.5f;
-        cw = __ldg(P.cellw + (p.rel + P.n_root));
+        cw = __ldg(P.cellw + CK(p.rel + P.n_root, P.n_total));
     }
     p.cw = cw;
 }
@@ -266,7 +283,7 @@ __device__ __forceinline__ int dust_cell(const DustParams &D, long long id, int 
     int lo = 0, hi = D.level_off[D.n_levels];                       // invariant: first[lo] <= q < first[hi]
     while (hi - lo > 1) {
         const int mid = (int)(((long long)lo + hi) >> 1);
-        if ((unsigned long long)__ldg(D.first + mid) <= q) lo = mid; else hi = mid;
+        if ((unsigned long long)__ldg(D.first + CK(mid, D.level_off[D.n_levels] + 1)) <= q) lo = mid; else hi = mid;
     }
     level0 = 0;
     while (level0 + 1 < D.n_levels && lo >= D.level_off[level0 + 1]) ++level0;
@@ -406,12 +423,13 @@ __device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long 
         // f1: the package starts inside the leaf that emitted it; its root cell is found by climbing the reverse links
         const int gid = p.ix, level0 = p.iy;
         p.origin = gid;
-        p.cw = __ldg(P.cellw + gid);
-        e0 = cell_luminosity(P.dust.kabs, P.dust.freq_hz, p.cw, level0, __ldg(P.dust.T + gid)) / (double)__ldg(P.dust.count + gid);
+        p.cw = __ldg(P.cellw + CK(gid, P.n_total));
+        e0 = cell_luminosity(P.dust.kabs, P.dust.freq_hz, p.cw, level0, __ldg(P.dust.T + CK(gid, P.n_total))) /
+             (double)__ldg(P.dust.count + CK(gid, P.n_total));
         p.h = __int_as_float((127 - level0) << 23);              // 2^-(level - 1), exact
         int r = HIER ? gid - P.n_root : gid;
         p.rel = r;
-        if (HIER) while (r >= 0) r = __ldg(P.parent + (r >> 3));
+        if (HIER) while (r >= 0) r = __ldg(P.parent + CK(r >> 3, P.n_oct));
         const int root = HIER ? r + P.n_root : r;
         p.ix = root % P.nx; p.iy = (root / P.nx) % P.ny; p.iz = root / (P.nx * P.ny);
     } else {
@@ -421,7 +439,7 @@ __device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long 
             descend(P, p);
         } else {
             p.rel = root;
-            p.cw = __ldg(P.cellw + root);
+            p.cw = __ldg(P.cellw + CK(root, P.n_total));
         }
     }
     p.seg = 0; p.steps = 0; p.scat = 0;
@@ -461,7 +479,7 @@ __device__ __forceinline__ bool move_across(const SimParams &P, Pkg<A> &p, int a
             p.fx = (p.fx + (float)(p.rel & 1)) * 0.5f;
             p.fy = (p.fy + (float)((p.rel >> 1) & 1)) * 0.5f;
             p.fz = (p.fz + (float)((p.rel >> 2) & 1)) * 0.5f;
-            p.rel = __ldg(P.parent + (p.rel >> 3));
+            p.rel = __ldg(P.parent + CK(p.rel >> 3, P.n_oct));
             p.h *= 2.0f;
         }
     }
@@ -480,7 +498,7 @@ found:
         if (a == 0) p.fx = face; else if (a == 1) p.fy = face; else p.fz = face;
     }
     if (HIER) descend(P, p);
-    else p.cw = __ldg(P.cellw + p.rel);
+    else p.cw = __ldg(P.cellw + CK(p.rel, P.n_total));
     return true;
 }
 
@@ -584,9 +602,9 @@ __global__ void __launch_bounds__(256) photon_kernel(const __grid_constant__ Sim
             // scatterings inside one cell are summed in a register: one atomic per cell visit, not per
             // step (the hot-cell contention of PAPER.md:151, 279)
             if (flush) {
-                if (p.pend > 0.0) atomicAdd(P.absorbed + gid, P.weight * p.pend);
+                if (p.pend > 0.0) atomicAdd(P.absorbed + CK(gid, P.n_total), P.weight * p.pend);
                 if (p.origin >= 0) {                 // f3: what a cell's own package left in it before first leaving it
-                    if (P.dust.self_abs && p.pend > 0.0) atomicAdd(P.dust.self_abs + gid, P.weight * p.pend);
+                    if (P.dust.self_abs && p.pend > 0.0) atomicAdd(P.dust.self_abs + CK(gid, P.n_total), P.weight * p.pend);
                     p.origin = -1;
                 }
                 p.pend = 0.0;
@@ -597,7 +615,7 @@ __global__ void __launch_bounds__(256) photon_kernel(const __grid_constant__ Sim
                 if (REPLAY) {
                     soc_replay_record r;
                     r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = e_esc;
-                    P.replay[p.id - P.pkg_begin] = r;
+                    P.replay[CK(p.id - P.pkg_begin, P.pkg_end - P.pkg_begin)] = r;
                 }
                 active = false;
             }
@@ -653,6 +671,7 @@ struct FastParams {
     int bsy, bsz;                       // id strides between bricks along y, z (along x: 8): 8 nbx, 8 nbx nby
     int nrp;                            // number of padded root cells = 8 nbx nby nbz
     int n_root;                         // nx*ny*nz
+    int n_int, n_oct, n_abi, n_replay;  // lengths of cellw / parent / the ABI cell vector / replay (bounds-checked build)
     const uint32_t *cellw;              // [n_int] leaf: fp32 density bits; parent: 0x80000000 | internal id of first child
     const int32_t *parent;              // [n_octets] internal id of the parent of octet (id - nrp) >> 3
     float kabs, ksca, kratio, g;        // kratio = kabs / ksca
@@ -722,7 +741,7 @@ __device__ __forceinline__ float package_rel(const FastParams &P, int src)
 // a6: descend to the leaf.  Returns false on the sentinel (outside the root grid).
 __device__ __forceinline__ bool fast_descend(const FastParams &P, FPkg &p)
 {
-    uint32_t cw = __ldg(P.cellw + p.rel);
+    uint32_t cw = __ldg(P.cellw + CK(p.rel, P.n_int));
     p.n_ld += 1;
     if (cw == kSentinel) { p.cw = cw; return false; }
     while ((int32_t)cw < 0) {
@@ -733,7 +752,7 @@ __device__ __forceinline__ bool fast_descend(const FastParams &P, FPkg &p)
         p.anc3 = p.anc2; p.anc2 = p.anc1; p.anc1 = p.rel;       // the cell being left becomes the parent
         p.rel = (int)(cw & 0x7fffffffu) + slot;
         p.h *= 0.5f;
-        cw = __ldg(P.cellw + p.rel);
+        cw = __ldg(P.cellw + CK(p.rel, P.n_int));
         p.n_ld += 1;
     }
     p.cw = cw;
@@ -779,16 +798,16 @@ __device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, long lon
         const int gid = ix, level0 = iy;
         if (gid < P.n_root) p.rel = root_id(P, gid % P.nx, (gid / P.nx) % P.ny, gid / (P.nx * P.ny));
         else p.rel = P.nrp + (gid - P.n_root);
-        p.cw = __ldg(P.cellw + p.rel);
+        p.cw = __ldg(P.cellw + CK(p.rel, P.n_int));
         p.n_ld = 1;
         p.h = __int_as_float((127 - level0) << 23);
-        const double e0 = cell_luminosity(P.dust.kabs, P.dust.freq_hz, p.cw, level0, __ldg(P.dust.T + gid)) /
-                          (double)__ldg(P.dust.count + gid);
+        const double e0 = cell_luminosity(P.dust.kabs, P.dust.freq_hz, p.cw, level0, __ldg(P.dust.T + CK(gid, P.n_abi))) /
+                          (double)__ldg(P.dust.count + CK(gid, P.n_abi));
         prel = (float)(e0 / P.e_ref);
     } else {
         p.rel = root_id(P, ix, iy, iz);
         if (HIER) fast_descend(P, p);
-        else { p.cw = __ldg(P.cellw + p.rel); p.n_ld = 1; }
+        else { p.cw = __ldg(P.cellw + CK(p.rel, P.n_int)); p.n_ld = 1; }
         prel = package_rel(P, p.src);
     }
     // hot-cell tracking starts at the centre of the cube of the package's own source (regular grids only)
@@ -869,7 +888,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                     if (P.replay) {
                         soc_replay_record r;
                         r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = esc;
-                        P.replay[p.id - P.pkg_begin] = r;
+                        P.replay[CK(p.id - P.pkg_begin, P.n_replay)] = r;
                     }
                 }
                 need = EMPTY;
@@ -960,16 +979,16 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 // source, with one fp64 reduction to L2 otherwise
                 if (p.disp >= 0) {
                     const int j = (p.disp & 255) + hot_side * (((p.disp >> 8) & 255) + hot_side * (p.disp >> 16));
-                    atomicAdd(s_hot + p.src * hot_cells + j, p.pend);
+                    atomicAdd(s_hot + CK(p.src * hot_cells + j, hot_cells * P.n_point), p.pend);
                 } else if (p.pend > 0.0f) {
                     const bool dust = DUST && p.src <= -2;
-                    if (ACC32) atomicAdd(P.acc32 + p.rel, p.pend * (dust ? s_prel[threadIdx.x] : package_rel(P, p.src)));
-                    else atomicAdd(P.acc + p.rel, (double)p.pend * (dust ? (double)s_prel[threadIdx.x] * P.e_ref : package_e0(P, p.src)));
+                    if (ACC32) atomicAdd(P.acc32 + CK(p.rel, P.n_int), p.pend * (dust ? s_prel[threadIdx.x] : package_rel(P, p.src)));
+                    else atomicAdd(P.acc + CK(p.rel, P.n_int), (double)p.pend * (dust ? (double)s_prel[threadIdx.x] * P.e_ref : package_e0(P, p.src)));
                     p.n_red += 1;
                 }
                 if (DUST && p.src == -2) {       // f3: what a cell's own package leaves in it before first leaving it
                     if (P.dust.self_abs && p.pend > 0.0f)
-                        atomicAdd(P.dust.self_abs + global_id(P, p.rel), P.dust.weight * (double)p.pend * ((double)s_prel[threadIdx.x] * P.e_ref));
+                        atomicAdd(P.dust.self_abs + CK(global_id(P, p.rel), P.n_abi), P.dust.weight * (double)p.pend * ((double)s_prel[threadIdx.x] * P.e_ref));
                     p.src = -3;
                 }
                 p.pend = 0.0f;
@@ -1000,7 +1019,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                         p.fy = (p.fy + (float)((rel >> 1) & 1)) * 0.5f;
                         p.fz = (p.fz + (float)((rel >> 2) & 1)) * 0.5f;
                         if (p.anc1 < 0) p.n_ld += 1;
-                        rel = p.anc1 >= 0 ? p.anc1 : __ldg(P.parent + ((rel - P.nrp) >> 3));
+                        rel = p.anc1 >= 0 ? p.anc1 : __ldg(P.parent + CK((rel - P.nrp) >> 3, P.n_oct));
                         p.anc1 = p.anc2; p.anc2 = p.anc3; p.anc3 = -1;
                         p.h *= 2.0f;
                         inside = fwd == ((rel & abit) == 0);
@@ -1013,7 +1032,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 if (HIER) {
                     if (!fast_descend(P, p)) need = DONE;            // a9: escaped
                 } else {
-                    p.cw = __ldg(P.cellw + rel);
+                    p.cw = __ldg(P.cellw + CK(rel, P.n_int));
                     p.n_ld += 1;
                     if (p.cw == kSentinel) need = DONE;              // a9: escaped
                 }
@@ -1035,8 +1054,8 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
                 const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
                           iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
-                if (ACC32) atomicAdd(P.acc32 + root_id(P, ix, iy, iz), v * P.ps_rel[k]);
-                else atomicAdd(P.acc + root_id(P, ix, iy, iz), (double)v * P.ps_e0[k]);
+                if (ACC32) atomicAdd(P.acc32 + CK(root_id(P, ix, iy, iz), P.n_int), v * P.ps_rel[k]);
+                else atomicAdd(P.acc + CK(root_id(P, ix, iy, iz), P.n_int), (double)v * P.ps_e0[k]);
             }
         }
     }
@@ -1116,7 +1135,7 @@ __device__ __forceinline__ uint32_t q_word(const QPkg &p)
 
 __device__ __forceinline__ void q_load(const FastParams &P, QPkg &p)
 {
-    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(P.cellw + (p.rel & ~3)));
+    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(P.cellw + CK(p.rel & ~3, P.n_int - 3)));
     p.q0 = v.x; p.q1 = v.y; p.q2 = v.z; p.q3 = v.w;
     p.n_ld += 1;
 }
@@ -1129,7 +1148,7 @@ __device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p, float (*s_
     // nothing to add: empty cells, or the cells around a point source, whose deposits went to the block's shared
     // partial sums -- a reduction of zeros there would bring back the very contention those sums avoid
     if ((a0 + a1) + (a2 + a3) == 0.0f) return;
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(P.acc32 + (p.rel & ~3)), "f"(a0), "f"(a1),
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(P.acc32 + CK(p.rel & ~3, P.n_int - 3)), "f"(a0), "f"(a1),
                  "f"(a2), "f"(a3) : "memory");
     s_acc[0][threadIdx.x] = 0.0f; s_acc[1][threadIdx.x] = 0.0f; s_acc[2][threadIdx.x] = 0.0f; s_acc[3][threadIdx.x] = 0.0f;
     p.n_red += 1;
@@ -1188,7 +1207,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                     if (P.replay) {
                         soc_replay_record r;
                         r.hash = p.hash; r.steps = p.steps; r.scatters = p.scat; r.e_escaped = esc;
-                        P.replay[p.idx] = r;
+                        P.replay[CK(p.idx, P.n_replay)] = r;
                     }
                 }
                 need = EMPTY;
@@ -1296,13 +1315,13 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                     //
                     if (hot) {
                         const int j = (p.sd & 7) + hot_side * (((p.sd >> 3) & 7) + hot_side * ((p.sd >> 6) & 7));
-                        atomicAdd(s_hot + (p.sd >> 16) * hot_cells + j, p.pend);
+                        atomicAdd(s_hot + CK((p.sd >> 16) * hot_cells + j, hot_cells * P.n_point), p.pend);
                     } else {
-                        s_acc[p.rel & 3][threadIdx.x] += p.pend * p.prel;
+                        s_acc[CK(p.rel & 3, 4)][CK(threadIdx.x, 256)] += p.pend * p.prel;
                     }
                     if (DUST && p.sd == -2) {    // f3: what a cell's own package leaves in it before first leaving it
                         if (P.dust.self_abs && p.pend > 0.0f)
-                            atomicAdd(P.dust.self_abs + global_id(P, p.rel), P.dust.weight * (double)p.pend * ((double)p.prel * P.e_ref));
+                            atomicAdd(P.dust.self_abs + CK(global_id(P, p.rel), P.n_abi), P.dust.weight * (double)p.pend * ((double)p.prel * P.e_ref));
                         p.sd = -3;
                     }
                     p.pend = 0.0f;
@@ -1353,7 +1372,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                 const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
                 const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
                           iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
-                atomicAdd(P.acc32 + root_id(P, ix, iy, iz), v * P.ps_rel[k]);
+                atomicAdd(P.acc32 + CK(root_id(P, ix, iy, iz), P.n_int), v * P.ps_rel[k]);
             }
         }
     }
@@ -2120,7 +2139,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
     SimParams P;
     std::memset(&P, 0, sizeof(P));
     P.nx = G->nx; P.ny = G->ny; P.nz = G->nz; P.n_root = (int)G->n_root;
-    P.cellw = G->d_cellw; P.parent = G->d_parent;
+    P.cellw = G->d_cellw; P.parent = G->d_parent; P.n_total = (int)G->n_total; P.n_oct = (int)(G->n_octets > 0 ? G->n_octets : 1);
     P.kabs = G->kabs[ifreq]; P.ksca = G->ksca[ifreq]; P.g = G->g[ifreq];
     P.surf = 2.0 * ((double)G->ny * G->nz + (double)G->nz * G->nx + (double)G->nx * G->ny);
     P.n_bg = n_bg;
@@ -2169,6 +2188,8 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         F.nx = G->nx; F.ny = G->ny; F.nz = G->nz; F.nbx = G->nbx; F.nby = G->nby;
         F.bsy = 8 * G->nbx; F.bsz = 8 * G->nbx * G->nby; F.nrp = G->nrp; F.n_root = (int)G->n_root;
         F.cellw = G->d_cellw_int; F.parent = G->d_parent_int;
+        F.n_int = (int)G->n_int; F.n_oct = (int)(G->n_octets > 0 ? G->n_octets : 1); F.n_abi = (int)G->n_total;
+        F.n_replay = (int)(pkg_count < (1ll << 31) ? pkg_count : (1ll << 31) - 1);
         F.kabs = (float)P.kabs; F.ksca = (float)P.ksca; F.g = (float)P.g;
         F.kratio = P.ksca > 0.0 ? (float)(P.kabs / P.ksca) : 0.0f;
         F.is_beam = P.is_beam; F.n_point = P.n_point; F.n_bg = P.n_bg; F.bg_e0 = P.bg_e0; F.surf = P.surf;
@@ -2283,6 +2304,18 @@ extern "C" {
 const char *soc_last_error(void) { return g_last_error.c_str(); }
 const char *soc_version(void) { return "soc_b200 0.1 (sm_100a)"; }
 uint64_t soc_launch_count(void) { return g_launches; }
+
+int64_t soc_checked_violations(void)
+{
+#ifdef SOC_CHECKED
+    unsigned int v = 0;
+    if (cudaDeviceSynchronize() != cudaSuccess) return -2;
+    if (cudaMemcpyFromSymbol(&v, g_violations, sizeof(v)) != cudaSuccess) return -2;
+    return (int64_t)v;
+#else
+    return -1;
+#endif
+}
 
 void soc_grid_destroy(soc_grid *G)
 {

@@ -13,6 +13,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsoc_b200.so")
+if os.environ.get("SOC_B200_LIB"):                      # e.g. the bounds-checked build, libsoc_b200_checked.so (tests)
+    LIB_PATH = os.environ["SOC_B200_LIB"]
 
 SOC_GEOM_FP32 = 0
 SOC_GEOM_FP64 = 1
@@ -21,7 +23,8 @@ MAX_POINT_SOURCES = 64
 EXPORTS = ["soc_grid_create", "soc_grid_destroy", "soc_grid_n_total", "soc_freq_weights", "soc_simulate_frequency",
            "soc_simulate_packages", "soc_simulate_spectrum", "soc_update_temperatures", "soc_run_host",
            "soc_set_option", "soc_get_timings", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version",
-           "soc_emission_counts", "soc_cell_emission", "soc_update_temperatures_ali", "soc_iterate", "soc_make_map"]
+           "soc_emission_counts", "soc_cell_emission", "soc_update_temperatures_ali", "soc_iterate", "soc_make_map",
+           "soc_checked_violations"]
 
 
 class SocError(RuntimeError):
@@ -103,6 +106,7 @@ def load():
     L.soc_get_timings.argtypes = [vp, i32, vp]
     L.soc_probe_throughput.argtypes = [i32, i64, i64, C.POINTER(C.c_float)]
     L.soc_launch_count.restype = u64
+    L.soc_checked_violations.restype = i64
     L.soc_last_error.restype = C.c_char_p
     L.soc_version.restype = C.c_char_p
     _lib = L
@@ -315,6 +319,11 @@ def run_host(P, n_packages=None, seed=None, n_iter=None, flags=SOC_GEOM_FP32, wa
                           n_iter, float(P.t_scale or 0.0), _ptr(tab), 0 if tab is None else len(tab), float(P.e_min),
                           float(P.e_max), _ptr(absorbed_out), _ptr(T_out) if has_T else None, res, int(flags)))
     return absorbed_out, (T_out if has_T else None), (list(res) if want_results else None)
+
+
+def checked_violations():
+    """Bounds-checked build: out-of-range kernel indices so far (-1: the product library, checks compiled out)."""
+    return int(load().soc_checked_violations())
 
 
 def probe_throughput(kind, footprint_bytes, n_ops):
