@@ -1517,6 +1517,13 @@ __global__ void __launch_bounds__(256) temperature_kernel(const __grid_constant_
     }
 }
 
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+
 // regular grid, every cell a leaf: density -> cell word in place (-0 -> +0, sign bit clear), validity flag and sum of
 // the densities (soc_grid_create of large regular grids; small and hierarchical grids are converted on the host)
 __global__ void __launch_bounds__(256) leafwords_kernel(uint32_t *cellw, long long n, double *sum_out, int *bad_out)
@@ -1538,6 +1545,75 @@ __global__ void __launch_bounds__(256) leafwords_kernel(uint32_t *cellw, long lo
     if ((threadIdx.x & 31) == 0) {
         atomicAdd(sum_out, sum);
         if (bad) atomicOr(bad_out, 1);
+    }
+}
+
+__global__ void __launch_bounds__(256) fill_i32_kernel(int32_t *a, long long n, int32_t v)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) a[i] = v;
+}
+
+// hierarchical grids of >= 2^20 cells: cell words, reverse links and validation on the GPU (soc_grid_create).  cellw holds
+// the uploaded fp32 densities on entry.  flags: 1 bad density, 2 bad child index, 4 octet with two parents
+struct HierParams {
+    uint32_t *cellw;
+    const int32_t *child;
+    int32_t *parent;                    // [n_octets], preset to INT32_MIN
+    long long n_total, n_root;
+    int n_levels;
+    long long level_off[SOC_MAX_LEVELS + 1];
+    double *sum_out;                    // [0] sum of the root-leaf densities, [1] their number
+    int *flags;
+};
+
+__global__ void __launch_bounds__(256) hierwords_kernel(const __grid_constant__ HierParams H)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double sum = 0.0, cnt = 0.0;
+    int bad = 0;
+    for (long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x; gid < H.n_total; gid += stride) {
+        int l = 0;
+        while (l + 1 < H.n_levels && gid >= H.level_off[l + 1]) ++l;
+        const int32_t ch = H.child[gid];
+        if (ch < 0) {
+            const float r = __uint_as_float(H.cellw[gid]);
+            if (!(r >= 0.0f) || isinf(r)) bad |= 1;
+            H.cellw[gid] = __float_as_uint(r + 0.0f) & 0x7fffffffu;
+            if (gid < H.n_root) { sum += (double)r; cnt += 1.0; }
+            continue;
+        }
+        if (l + 1 >= H.n_levels || (ch & 7) != 0 || (long long)ch + 8 > H.level_off[l + 2] - H.level_off[l + 1]) { bad |= 2; continue; }
+        const long long child_rel = H.level_off[l + 1] + ch - H.n_root;
+        if (atomicCAS(H.parent + (child_rel >> 3), INT32_MIN, (int32_t)(gid - H.n_root)) != INT32_MIN) bad |= 4;
+        H.cellw[gid] = 0x80000000u | (uint32_t)child_rel;
+    }
+    sum = warp_sum(sum); cnt = warp_sum(cnt);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bad |= __shfl_xor_sync(kFull, bad, o);
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(H.sum_out, sum); atomicAdd(H.sum_out + 1, cnt);
+        if (bad) atomicOr(H.flags, bad);
+    }
+}
+
+// reverse links in the internal layout; flags |= 8 for an octet without a parent
+__global__ void __launch_bounds__(256) parent_internal_kernel(const int32_t *parent, int32_t *pi, long long n_octets, int nx, int ny,
+                                                              long long nbx, long long nby, long long nrp, long long n_root, int *flags)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < n_octets; o += stride) {
+        const int32_t p = parent[o];
+        if (p == INT32_MIN) { atomicOr(flags, 8); pi[o] = 0; continue; }
+        const long long gid = (long long)p + n_root;
+        long long j;
+        if (gid >= n_root) j = nrp + (gid - n_root);
+        else {
+            const long long ix = gid % nx, r = gid / nx, iy = r % ny, iz = r / ny;
+            const long long X = ix + 2, Y = iy + 2, Z = iz + 2;
+            j = 8 * ((X >> 1) + nbx * ((Y >> 1) + nby * (Z >> 1))) + (X & 1) + 2 * (Y & 1) + 4 * (Z & 1);
+        }
+        pi[o] = (int32_t)j;
     }
 }
 
@@ -1588,13 +1664,6 @@ __device__ __forceinline__ double lum_of(const LumParams &L, long long c)
     int l = 0;
     while (l + 1 < L.n_levels && c >= L.level_off[l + 1]) ++l;
     return cell_luminosity(L.kabs, L.freq_hz, L.cellw[c], l, L.T[c]);
-}
-
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-    return v;
 }
 
 // out[0] += sum of L_c over all cells (count == NULL) or over the cells that send packages; out[1] += number of cells
@@ -2378,14 +2447,17 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     // link per octet)
     std::vector<uint32_t> cellw;
     std::vector<int32_t> parent;
+    // grids of >= 2^20 cells are converted and validated on the GPU: regular grids by leafwords_kernel, hierarchies by
+    // hierwords_kernel + parent_internal_kernel (the host loops below cost 40 ms for the 11 M cells of config 4')
+    const bool big = G->n_total >= (1ll << 20);
+    const bool words_done = big;
+    const bool hier_gpu = big && d->child != nullptr;
+    const size_t n_par = (size_t)(G->n_octets > 0 ? G->n_octets : 1);
     try {
-        if (d->child || G->n_total < (1ll << 20)) cellw.resize((size_t)G->n_total);
-        parent.assign((size_t)(G->n_octets > 0 ? G->n_octets : 1), INT32_MIN);
+        if (!big) { cellw.resize((size_t)G->n_total); parent.assign(n_par, INT32_MIN); }
     } catch (const std::bad_alloc &) {
         return fail(SOC_ENOMEM, "out of host memory");
     }
-    // large regular grids: every cell is a leaf, the words are converted and validated on the GPU (leafwords_kernel)
-    const bool words_done = !d->child && G->n_total >= (1ll << 20);
     for (int l = 0; l < d->n_levels && !words_done; ++l) {
         for (long long c = 0; c < d->n_cells[l]; ++c) {
             const long long gid = G->level_off[l] + c;
@@ -2407,7 +2479,7 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
             cellw[(size_t)gid] = 0x80000000u | (uint32_t)child_rel;
         }
     }
-    for (long long o = 0; o < G->n_octets; ++o)
+    for (long long o = 0; o < G->n_octets && !words_done; ++o)
         if (parent[(size_t)o] == INT32_MIN) return fail(SOC_EINVAL, "octet without a parent");
     if (!words_done) {
         double sum = 0.0;
@@ -2420,9 +2492,35 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     SOC_CUDA(cudaGetDevice(&G->device));
     SOC_CUDA(cudaDeviceGetAttribute(&G->n_sm, cudaDevAttrMultiProcessorCount, G->device));
     SOC_CUDA(cudaMalloc(&G->d_cellw, sizeof(uint32_t) * (size_t)G->n_total));
-    SOC_CUDA(cudaMalloc(&G->d_parent, sizeof(int32_t) * parent.size()));
+    SOC_CUDA(cudaMalloc(&G->d_parent, sizeof(int32_t) * n_par));
     SOC_CUDA(cudaMalloc(&G->d_table, sizeof(float) * 8192));
-    if (words_done) {
+    if (hier_gpu) {
+        double *d_sum = nullptr;
+        int32_t *d_child = nullptr;
+        struct Tmp { double *&a; int32_t *&b; ~Tmp() { cudaFree(a); cudaFree(b); } } tmp{d_sum, d_child};
+        SOC_CUDA(cudaMalloc(&d_sum, 32));
+        SOC_CUDA(cudaMemset(d_sum, 0, 32));
+        SOC_CUDA(cudaMalloc(&d_child, sizeof(int32_t) * (size_t)G->n_total));
+        SOC_CUDA(cudaMemcpy(G->d_cellw, d->density, sizeof(float) * (size_t)G->n_total, cudaMemcpyHostToDevice));
+        SOC_CUDA(cudaMemcpy(d_child, d->child, sizeof(int32_t) * (size_t)G->n_total, cudaMemcpyHostToDevice));
+        HierParams H;
+        std::memset(&H, 0, sizeof(H));
+        H.cellw = G->d_cellw; H.child = d_child; H.parent = G->d_parent; H.n_total = G->n_total; H.n_root = G->n_root;
+        H.n_levels = G->n_levels;
+        for (int l = 0; l <= G->n_levels; ++l) H.level_off[l] = G->level_off[l];
+        H.sum_out = d_sum; H.flags = reinterpret_cast<int *>(d_sum + 2);
+        fill_i32_kernel<<<G->n_sm * 4, 256>>>(G->d_parent, (long long)n_par, INT32_MIN);
+        hierwords_kernel<<<G->n_sm * 8, 256>>>(H);
+        g_launches += 2;
+        double h_sum[4] = {0.0, 0.0, 0.0, 0.0};
+        SOC_CUDA(cudaMemcpy(h_sum, d_sum, 32, cudaMemcpyDeviceToHost));
+        int bad = 0;
+        std::memcpy(&bad, &h_sum[2], sizeof(int));
+        if (bad & 1) return fail(SOC_EINVAL, "leaf density must be finite and >= 0");
+        if (bad & 2) return fail(SOC_EINVAL, "child index out of range or not a multiple of 8");
+        if (bad & 4) return fail(SOC_EINVAL, "octet has two parents");
+        G->rho_mean = h_sum[1] > 0.0 ? h_sum[0] / h_sum[1] : 0.0;
+    } else if (words_done) {
         double *d_sum = nullptr;
         SOC_CUDA(cudaMalloc(&d_sum, 16));
         SOC_CUDA(cudaMemset(d_sum, 0, 16));
@@ -2440,7 +2538,8 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
     } else {
         SOC_CUDA(cudaMemcpy(G->d_cellw, cellw.data(), sizeof(uint32_t) * (size_t)G->n_total, cudaMemcpyHostToDevice));
     }
-    SOC_CUDA(cudaMemcpy(G->d_parent, parent.data(), sizeof(int32_t) * parent.size(), cudaMemcpyHostToDevice));
+    if (!big) SOC_CUDA(cudaMemcpy(G->d_parent, parent.data(), sizeof(int32_t) * n_par, cudaMemcpyHostToDevice));
+    else if (!hier_gpu) SOC_CUDA(cudaMemset(G->d_parent, 0, sizeof(int32_t) * n_par));
     // internal layout: root grid in 2x2x2 bricks with ghost cells around it (they hold the sentinel; cell ix
     // sits at X = ix + 2, so the low side has a whole ghost brick and the high side at least one ghost cell),
     // octet levels shifted behind it
@@ -2452,7 +2551,7 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
         G->nbx = (int)nbx; G->nby = (int)nby; G->nbz = (int)nbz; G->nrp = (int)nrp; G->n_int = n_int;
         std::vector<int32_t> pi;
         try {
-            pi.assign(parent.size(), 0);
+            if (!big) pi.assign(n_par, 0);
         } catch (const std::bad_alloc &) {
             return fail(SOC_ENOMEM, "out of host memory");
         }
@@ -2462,14 +2561,26 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
             const long long X = ix + 2, Y = iy + 2, Z = iz + 2;
             return 8 * ((X >> 1) + nbx * ((Y >> 1) + nby * (Z >> 1))) + (X & 1) + 2 * (Y & 1) + 4 * (Z & 1);
         };
-        for (long long o = 0; o < G->n_octets; ++o) pi[(size_t)o] = (int32_t)internal((long long)parent[(size_t)o] + G->n_root);
+        for (long long o = 0; o < G->n_octets && !big; ++o) pi[(size_t)o] = (int32_t)internal((long long)parent[(size_t)o] + G->n_root);
         SOC_CUDA(cudaMalloc(&G->d_cellw_int, sizeof(uint32_t) * (size_t)n_int));
-        SOC_CUDA(cudaMalloc(&G->d_parent_int, sizeof(int32_t) * pi.size()));
+        SOC_CUDA(cudaMalloc(&G->d_parent_int, sizeof(int32_t) * n_par));
         SOC_CUDA(cudaMalloc(&G->d_acc, sizeof(double) * (size_t)n_int));
         repad_kernel<<<G->n_sm * 8, 256>>>(G->d_cellw, G->d_cellw_int, G->nx, G->ny, G->nz, (int)nbx, (int)nby, nrp, G->n_root, n_int);
         g_launches += 1;
         SOC_CUDA(cudaGetLastError());
-        SOC_CUDA(cudaMemcpy(G->d_parent_int, pi.data(), sizeof(int32_t) * pi.size(), cudaMemcpyHostToDevice));
+        if (!big) SOC_CUDA(cudaMemcpy(G->d_parent_int, pi.data(), sizeof(int32_t) * n_par, cudaMemcpyHostToDevice));
+        else if (hier_gpu) {
+            int *d_f = nullptr;
+            SOC_CUDA(cudaMalloc(&d_f, 4));
+            SOC_CUDA(cudaMemset(d_f, 0, 4));
+            parent_internal_kernel<<<G->n_sm * 4, 256>>>(G->d_parent, G->d_parent_int, G->n_octets, G->nx, G->ny, nbx, nby, nrp, G->n_root, d_f);
+            g_launches += 1;
+            int f = 0;
+            cudaError_t e = cudaMemcpy(&f, d_f, 4, cudaMemcpyDeviceToHost);
+            cudaFree(d_f);
+            if (e != cudaSuccess) return fail(SOC_ECUDA, cudaGetErrorString(e));
+            if (f & 8) return fail(SOC_EINVAL, "octet without a parent");
+        } else SOC_CUDA(cudaMemset(G->d_parent_int, 0, sizeof(int32_t) * n_par));
         SOC_CUDA(cudaMemset(G->d_acc, 0, sizeof(double) * (size_t)n_int));
         SOC_CUDA(cudaMalloc(&G->d_acc32, sizeof(float) * (size_t)n_int));
         SOC_CUDA(cudaMemset(G->d_acc32, 0, sizeof(float) * (size_t)n_int));

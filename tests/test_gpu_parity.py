@@ -732,6 +732,26 @@ def test_bad_arguments_are_rejected():
     big[777_777] = np.inf
     with pytest.raises(soc.SocError, match="density"):
         soc.Grid(104, 104, 104, [104 ** 3], big, None, P.freq_hz, P.kabs, P.ksca, P.g)
+    # hierarchies of >= 2^20 cells are converted and validated on the GPU (hierwords_kernel, parent_internal_kernel)
+    H = inputs.make_config("4p", n=32, n_packages=10, n_freq=2)
+    assert H.n_total >= 1 << 20 and H.n_levels == 4
+    args = (H.freq_hz, H.kabs, H.ksca, H.g)
+    soc.Grid(32, 32, 32, H.n_cells, H.rho, H.child, *args).close()
+    first_parent = int(np.argmax(H.child >= 0))
+    leaf = int(np.argmax((H.child < 0) & (np.arange(H.n_total) > H.n_cells[0])))
+    for what, match in (("nan", "density"), ("index", "child index"), ("two", "two parents"), ("orphan", "two parents|without a parent")):
+        rho_b, child_b = H.rho.copy(), H.child.copy()
+        if what == "nan":
+            rho_b[leaf] = np.nan
+        elif what == "index":
+            child_b[first_parent] += 4
+        elif what == "two":
+            child_b[leaf] = child_b[first_parent]                 # a second cell claims the same octet
+        else:
+            other = int(np.nonzero(H.child >= 0)[0][5])
+            child_b[other] = child_b[first_parent]                 # one octet claimed twice, another left without a parent
+        with pytest.raises(soc.SocError, match=match):
+            soc.Grid(32, 32, 32, H.n_cells, rho_b, child_b, *args)
     n_cells, rho, child = random_octree((2, 2, 2), 2, 0.5, seed=1)
     c2 = child.copy(); c2[np.argmax(child >= 0)] += 4
     with pytest.raises(soc.SocError):
