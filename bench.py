@@ -330,6 +330,8 @@ def run_ours(args):
             "cell_steps_per_s_per_frequency": {"median": float(np.median(per_f)), "min": float(per_f.min()),
                                                "max": float(per_f.max())},
             "cell_steps_per_step": job_steps, "scatterings_per_step_rank0": float(scat_total),
+            "cell_steps_per_frequency_rank0": [int(x) for x in steps_f],
+            "launch_ms_per_frequency_rank0": [round(float(x), 4) for x in kern_ms],
             "energy_conservation_rel": cons_cells,
             "energy_conservation": {"cells_vs_emitted_minus_escaped": cons_cells, "counters_emitted_absorbed_escaped": cons,
                                     "weight_drift_max": drift,
@@ -356,8 +358,9 @@ def run_ours(args):
 
 def ncu_traffic(config):
     """DRAM bytes per cell-step of the photon kernel from the NEWEST committed ncu capture: profiles/r*_ncu_dram_traffic.csv
-    (columns: config, kernel, cell_steps, dram_read_bytes, dram_write_bytes, source -- written from the `ncu --set full`
-    capture named in `source`).  Read at run time so that the figure cannot outlive the capture it came from; None when
+    (columns: config, kernel, cell_steps, dram_read_bytes, dram_write_bytes, weight, source -- one row per captured launch,
+    written from the `ncu --set full` capture named in `source`; weight = how many launches of a pass the row stands for,
+    so that a config whose frequencies run two different kernels is averaged in the right proportion).  Read at run time so that the figure cannot outlive the capture it came from; None when
     no capture of this config is committed."""
     import csv
     import glob
@@ -369,8 +372,9 @@ def ncu_traffic(config):
         except Exception:
             continue
         if rows:
-            steps = sum(float(r["cell_steps"]) for r in rows)
-            byts = sum(float(r["dram_read_bytes"]) + float(r["dram_write_bytes"]) for r in rows)
+            wt = [float(r.get("weight") or 1.0) for r in rows]
+            steps = sum(w * float(r["cell_steps"]) for w, r in zip(wt, rows))
+            byts = sum(w * (float(r["dram_read_bytes"]) + float(r["dram_write_bytes"])) for w, r in zip(wt, rows))
             return {"bytes_per_cell_step": byts / steps,
                     "source": f"{os.path.relpath(path, ROOT)} ({'; '.join(sorted({r['source'] for r in rows}))})"}
     return None

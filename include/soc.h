@@ -267,6 +267,33 @@ int soc_get_timings(soc_grid *grid, int32_t n, float *ms);
  * independent of the others.  *ms receives the CUDA-event time of the probe kernel. */
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms);
 
+/* Stochastically heated grains (row f4; Appendix A -- a companion solver, "not part of SOC" proper).
+ * Per cell and grain size the fraction p_i of grains in each enthalpy bin solves R p = 0, sum p = 1, where "the upward
+ * transitions (R_ji, i < j) are obtained by taking a vector product of the intensity with the integration weights", "the
+ * pre-calculated cooling rates occupy the elements R_(i-1,i)", the diagonal follows from detailed balance and all other
+ * elements are zero, so that "the linear equations can be solved efficiently with forward-substitutions" (:361).  The
+ * emission is emission[cell][f] = sum_s abundance[s] sum_i p[cell][s][i] emis[s][i][f].
+ * The integration weights are given in the sparse form they have in practice: a photon of frequency f takes a grain of bin
+ * i to ONE bin jup[s][i][f] (-1: none) at the rate wup[s][i][f] * intensity[f].
+ * All model arrays: HOST, copied by soc_stochastic_create.  n_e <= 128, n_freq <= 1024. */
+typedef struct soc_stochastic soc_stochastic;
+typedef struct {
+    int32_t n_size, n_e, n_freq;
+    const int32_t *jup;         /* [n_size][n_e][n_freq]  target bin, > i, or -1 */
+    const double *wup;          /* [n_size][n_e][n_freq]  weight of that transition */
+    const double *cool;         /* [n_size][n_e]          cooling rate i -> i - 1 (element 0 unused), > 0 */
+    const double *emis;         /* [n_size][n_e][n_freq]  emission of one grain in bin i */
+    const double *abundance;    /* [n_size] */
+} soc_stochastic_model;
+
+int soc_stochastic_create(const soc_stochastic_model *model, soc_stochastic **out);
+void soc_stochastic_destroy(soc_stochastic *model);
+
+/* intensity: DEVICE [n_cells][n_freq] doubles.  emission: DEVICE [n_cells][n_freq] doubles, written.  p_out: DEVICE
+ * [n_cells][n_size][n_e] doubles or NULL. */
+int soc_stochastic_emission(soc_stochastic *model, const double *intensity, int64_t n_cells, double *emission,
+                            double *p_out, void *cuda_stream);
+
 /* Bounds-checked build (libsoc_b200_checked.so, compiled with -DSOC_CHECKED): number of out-of-range indices the photon
  * kernels produced so far in this process (each such access was redirected to element 0), after synchronising the device.
  * -1 in the product library, where the checks are compiled out.  -2 on a CUDA error. */

@@ -417,3 +417,63 @@ def iterate(grid: Grid, freq_hz, kabs, ksca, g, const_sources, n_const, n_reques
         out["n_dust"].append(nd)
     out.update(R=R, S=S, Em=Em)
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# f4: stochastically heated grains (Appendix A) -- plain numpy, fp64, the definition written out.
+# "The calculation reduces to a linear set of equations where the unknowns are the fraction of dust in each enthalpy bin.
+#  ... In the transition matrix R, the upward transitions (R_ji, i < j) are obtained by taking a vector product of the
+#  intensity with the integration weights.  The pre-calculated cooling rates occupy the elements R_(i-1,i) above the main
+#  diagonal.  The diagonal elements R_ii are determined from detailed balance and are equal to the sum of the other column
+#  elements multiplied by minus one.  The matrix elements R_ji = 0, i > j + 1 are zeros".
+# The paper's programs solve R p = 0 by forward substitution or Gauss-Seidel; the oracle solves the same linear system with
+# a general dense solver (LAPACK through numpy), the normalisation sum p = 1 taking the place of the redundant last row.
+def stochastic_rate_matrix(W, cool, intensity):
+    """R [n_E, n_E] for one grain size and one cell.  W[j, i, f]: integration weights of the upward transition i -> j
+    (zero for j <= i); cool[i]: cooling rate i -> i - 1 (cool[0] unused); intensity[f]."""
+    W, cool, intensity = (np.asarray(x, dtype=np.float64) for x in (W, cool, intensity))
+    n = len(cool)
+    R = np.zeros((n, n))
+    for i in range(n):
+        for j in range(i + 1, n):
+            R[j, i] = float(np.dot(W[j, i], intensity))          # "vector product of the intensity with the weights"
+    for i in range(1, n):
+        R[i - 1, i] = cool[i]
+    for i in range(n):
+        R[i, i] = -(R[:, i].sum() - R[i, i])                     # detailed balance: every column sums to zero
+    return R
+
+
+def stochastic_solve(R):
+    """p >= 0 with R p = 0 and sum p = 1."""
+    n = R.shape[0]
+    # columns differ by many orders of magnitude (cooling of the hot bins against absorption in the cold ones): scale the
+    # unknowns by the cooling time of their bin so that LAPACK sees an O(1) matrix; q_i = p_i * scale_i
+    scale = np.array([max(-R[i, i], 1e-300) for i in range(n)])
+    A = R / scale[None, :]
+    A[-1, :] = 1.0 / scale                                       # sum_i q_i / scale_i = 1 replaces the redundant last row
+    rhs = np.zeros(n); rhs[-1] = 1.0
+    row = np.abs(A).max(axis=1)
+    q = np.linalg.solve(A / row[:, None], rhs / row)
+    p = q / scale
+    return p / p.sum()
+
+
+def stochastic_emission(p, emis, abundance):
+    """emission[f] = sum_s abundance[s] sum_i p[s, i] emis[s, i, f]."""
+    return np.einsum("s,si,sif->f", np.asarray(abundance, np.float64), np.asarray(p, np.float64), np.asarray(emis, np.float64))
+
+
+def stochastic_cells(model, intensity):
+    """All cells and sizes: p[cell, s, i], emission[cell, f].  model: inputs.stochastic_model(); intensity[cell, f]."""
+    n_s, n_e, n_f = model["jup"].shape
+    W = np.zeros((n_s, n_e, n_e, n_f))
+    s_idx, i_idx, f_idx = np.nonzero(model["jup"] >= 0)
+    W[s_idx, model["jup"][s_idx, i_idx, f_idx], i_idx, f_idx] = model["wup"][s_idx, i_idx, f_idx]
+    intensity = np.asarray(intensity, dtype=np.float64)
+    p = np.zeros((len(intensity), n_s, n_e))
+    for c in range(len(intensity)):
+        for s in range(n_s):
+            p[c, s] = stochastic_solve(stochastic_rate_matrix(W[s], model["cool"][s], intensity[c]))
+    em = np.stack([stochastic_emission(p[c], model["emis"], model["abundance"]) for c in range(len(intensity))])
+    return p, em

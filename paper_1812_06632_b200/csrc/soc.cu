@@ -1936,6 +1936,102 @@ __global__ void __launch_bounds__(128) map_kernel(const __grid_constant__ MapPar
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// f4: stochastically heated grains.  One CTA per cell, its warps take the grain sizes in turn; per
+// (cell, size) a warp builds the upward rates in a shared tile (a lane owns the columns lane, lane + 32, ...: no atomics),
+// turns every column into its suffix sums B_ji = sum_{k >= j} R_ki, and runs the forward substitution on the probability
+// flux across the bin boundaries,  p_j = (sum_{i < j} p_i B_ji) / R_(j-1,j)  -- all terms positive, the sums in fp64 (the
+// paper: "worked reliably but only when part of the operations were performed in double precision").
+// ------------------------------------------------------------------------------------------------
+struct StochParams {
+    int n_size, n_e, n_freq, warps;
+    const int32_t *jupT;                // [n_size][n_freq][n_e]
+    const float *wupT;                  // [n_size][n_freq][n_e]
+    const double *cool;                 // [n_size][n_e]
+    const float *emis;                  // [n_size][n_e][n_freq], scaled by emis_scale[s] to stay inside fp32
+    const double *emis_scale;           // [n_size] abundance[s] / scale of emis
+    const double *intensity;
+    long long n_cells;
+    double *emission, *p_out;
+};
+
+__global__ void __launch_bounds__(128) stochastic_kernel(const __grid_constant__ StochParams S)
+{
+    extern __shared__ double s_mem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int ne = S.n_e, nf = S.n_freq;
+    double *s_int = s_mem;                                         // [nf] intensities of this cell
+    double *s_em = s_int + nf + (size_t)warp * (nf + ne);          // [nf] this warp's emission sums
+    double *s_p = s_em + nf;                                       // [ne]
+    float *s_tile = reinterpret_cast<float *>(s_mem + nf + (size_t)S.warps * (nf + ne)) + (size_t)warp * ne * ne;   // [ne][ne]
+    for (long long cell = blockIdx.x; cell < S.n_cells; cell += gridDim.x) {
+        __syncthreads();
+        for (int f = threadIdx.x; f < nf; f += blockDim.x) s_int[f] = S.intensity[cell * nf + f];
+        for (int f = lane; f < nf; f += 32) s_em[f] = 0.0;
+        __syncthreads();
+        for (int sz = warp; sz < S.n_size; sz += S.warps) {
+            for (int k = lane; k < ne * ne; k += 32) s_tile[k] = 0.0f;
+            __syncwarp();
+            // upward rates: R_ji += w_jif I_f, column i owned by one lane
+            const int32_t *jt = S.jupT + (size_t)sz * nf * ne;
+            const float *wt = S.wupT + (size_t)sz * nf * ne;
+            for (int i = lane; i < ne; i += 32)
+                for (int f = 0; f < nf; ++f) {
+                    const int j = __ldg(jt + (size_t)f * ne + i);
+                    if (j >= 0) s_tile[j * ne + i] += (float)((double)__ldg(wt + (size_t)f * ne + i) * s_int[f]);
+                }
+            // suffix sums down every column: B_ji = sum_{k >= j} R_ki
+            for (int i = lane; i < ne; i += 32) {
+                float run = 0.0f;
+                for (int j = ne - 1; j > i; --j) { run += s_tile[j * ne + i]; s_tile[j * ne + i] = run; }
+            }
+            __syncwarp();
+            // forward substitution, p_0 = 1, rescaled when it grows out of range
+            const double *cool = S.cool + (size_t)sz * ne;
+            if (lane == 0) s_p[0] = 1.0;
+            __syncwarp();
+            for (int j = 1; j < ne; ++j) {
+                double acc = 0.0;
+                for (int i = lane; i < j; i += 32) acc += s_p[i] * (double)s_tile[j * ne + i];
+                acc = warp_sum(acc);
+                double pj = acc / cool[j];
+                if (pj > 1e200) {                                  // warp-uniform
+                    for (int i = lane; i < j; i += 32) s_p[i] *= 1e-200;
+                    pj *= 1e-200;
+                }
+                __syncwarp();
+                if (lane == 0) s_p[j] = pj;
+                __syncwarp();
+            }
+            double tot = 0.0;
+            for (int i = lane; i < ne; i += 32) tot += s_p[i];
+            tot = warp_sum(tot);
+            const double inv = 1.0 / tot;
+            for (int i = lane; i < ne; i += 32) {
+                const double p = s_p[i] * inv;
+                s_p[i] = p;
+                if (S.p_out) S.p_out[((size_t)cell * S.n_size + sz) * ne + i] = p;
+            }
+            __syncwarp();
+            // emission of this size: sum_i p_i emis_if
+            const float *em = S.emis + (size_t)sz * ne * nf;
+            const double sc = S.emis_scale[sz];
+            for (int f = lane; f < nf; f += 32) {
+                double e = 0.0;
+                for (int i = 0; i < ne; ++i) e += s_p[i] * (double)__ldg(em + (size_t)i * nf + f);
+                s_em[f] += sc * e;
+            }
+            __syncwarp();
+        }
+        __syncthreads();
+        for (int f = threadIdx.x; f < nf; f += blockDim.x) {
+            double e = 0.0;
+            for (int w = 0; w < S.warps; ++w) e += s_mem[nf + (size_t)w * (nf + ne) + f];
+            S.emission[cell * nf + f] = e;
+        }
+    }
+}
+
 // roofline probes: random gathers / random reductions over a footprint
 __device__ __forceinline__ uint32_t mix32(uint32_t x)
 {
@@ -2914,6 +3010,99 @@ int soc_make_map(soc_grid *G, int32_t ifreq, const float *T, const soc_map_desc 
     const long long cap = (long long)G->n_sm * 16;
     if (blocks > cap) blocks = cap;
     map_kernel<<<(int)blocks, 128, 0, (cudaStream_t)stream>>>(M);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    return SOC_OK;
+}
+
+struct soc_stochastic {
+    int n_size = 0, n_e = 0, n_freq = 0, n_sm = 0;
+    int32_t *d_jupT = nullptr;
+    float *d_wupT = nullptr, *d_emis = nullptr;
+    double *d_cool = nullptr, *d_scale = nullptr;
+};
+
+void soc_stochastic_destroy(soc_stochastic *M)
+{
+    if (!M) return;
+    cudaFree(M->d_jupT); cudaFree(M->d_wupT); cudaFree(M->d_emis); cudaFree(M->d_cool); cudaFree(M->d_scale);
+    delete M;
+}
+
+int soc_stochastic_create(const soc_stochastic_model *m, soc_stochastic **out)
+{
+    if (!m || !out) return fail(SOC_EINVAL, "NULL argument");
+    *out = nullptr;
+    if (m->n_size < 1 || m->n_e < 2 || m->n_e > 128 || m->n_freq < 1 || m->n_freq > 1024)
+        return fail(SOC_EINVAL, "stochastic model: need n_size >= 1, 2 <= n_e <= 128, 1 <= n_freq <= 1024");
+    if (!m->jup || !m->wup || !m->cool || !m->emis || !m->abundance) return fail(SOC_EINVAL, "stochastic model: NULL table");
+    const size_t ns = (size_t)m->n_size, ne = (size_t)m->n_e, nf = (size_t)m->n_freq;
+    std::vector<int32_t> jT(ns * nf * ne);
+    std::vector<float> wT(ns * nf * ne), em(ns * ne * nf);
+    std::vector<double> scale(ns);
+    for (size_t s = 0; s < ns; ++s) {
+        double emax = 0.0;
+        for (size_t i = 0; i < ne; ++i) {
+            if (i > 0 && !(m->cool[s * ne + i] > 0.0) ) return fail(SOC_EINVAL, "stochastic model: cooling rates must be > 0");
+            for (size_t f = 0; f < nf; ++f) {
+                const int32_t j = m->jup[(s * ne + i) * nf + f];
+                const double w = m->wup[(s * ne + i) * nf + f];
+                if (j >= (int32_t)ne || (j >= 0 && j <= (int32_t)i) || !(w >= 0.0) || !std::isfinite(w))
+                    return fail(SOC_EINVAL, "stochastic model: upward transition must go to a higher bin with a finite weight >= 0");
+                jT[(s * nf + f) * ne + i] = j;
+                wT[(s * nf + f) * ne + i] = (float)w;
+                const double e = m->emis[(s * ne + i) * nf + f];
+                if (!(e >= 0.0) || !std::isfinite(e)) return fail(SOC_EINVAL, "stochastic model: emission must be finite and >= 0");
+                emax = std::fmax(emax, e);
+            }
+        }
+        const double unit = emax > 0.0 ? emax : 1.0;            // the table is stored in fp32 relative to its largest entry
+        for (size_t k = 0; k < ne * nf; ++k) em[s * ne * nf + k] = (float)(m->emis[s * ne * nf + k] / unit);
+        scale[s] = m->abundance[s] * unit;
+    }
+    soc_stochastic *M = new (std::nothrow) soc_stochastic;
+    if (!M) return fail(SOC_ENOMEM, "out of host memory");
+    struct Guard { soc_stochastic *g; ~Guard() { if (g) soc_stochastic_destroy(g); } } guard{M};
+    M->n_size = m->n_size; M->n_e = m->n_e; M->n_freq = m->n_freq;
+    int dev = 0;
+    SOC_CUDA(cudaGetDevice(&dev));
+    SOC_CUDA(cudaDeviceGetAttribute(&M->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    SOC_CUDA(cudaMalloc(&M->d_jupT, sizeof(int32_t) * jT.size()));
+    SOC_CUDA(cudaMalloc(&M->d_wupT, sizeof(float) * wT.size()));
+    SOC_CUDA(cudaMalloc(&M->d_emis, sizeof(float) * em.size()));
+    SOC_CUDA(cudaMalloc(&M->d_cool, sizeof(double) * ns * ne));
+    SOC_CUDA(cudaMalloc(&M->d_scale, sizeof(double) * ns));
+    SOC_CUDA(cudaMemcpy(M->d_jupT, jT.data(), sizeof(int32_t) * jT.size(), cudaMemcpyHostToDevice));
+    SOC_CUDA(cudaMemcpy(M->d_wupT, wT.data(), sizeof(float) * wT.size(), cudaMemcpyHostToDevice));
+    SOC_CUDA(cudaMemcpy(M->d_emis, em.data(), sizeof(float) * em.size(), cudaMemcpyHostToDevice));
+    SOC_CUDA(cudaMemcpy(M->d_cool, m->cool, sizeof(double) * ns * ne, cudaMemcpyHostToDevice));
+    SOC_CUDA(cudaMemcpy(M->d_scale, scale.data(), sizeof(double) * ns, cudaMemcpyHostToDevice));
+    guard.g = nullptr;
+    *out = M;
+    return SOC_OK;
+}
+
+int soc_stochastic_emission(soc_stochastic *M, const double *intensity, int64_t n_cells, double *emission, double *p_out,
+                            void *stream)
+{
+    if (!M || !intensity || !emission || n_cells < 0) return fail(SOC_EINVAL, "bad argument");
+    if (n_cells == 0) return SOC_OK;
+    StochParams S;
+    std::memset(&S, 0, sizeof(S));
+    S.n_size = M->n_size; S.n_e = M->n_e; S.n_freq = M->n_freq;
+    S.jupT = M->d_jupT; S.wupT = M->d_wupT; S.cool = M->d_cool; S.emis = M->d_emis; S.emis_scale = M->d_scale;
+    S.intensity = intensity; S.n_cells = n_cells; S.emission = emission; S.p_out = p_out;
+    const size_t per_warp = sizeof(double) * (size_t)(S.n_freq + S.n_e) + sizeof(float) * (size_t)S.n_e * S.n_e;
+    int warps = 4;
+    while (warps > 1 && sizeof(double) * S.n_freq + warps * per_warp > 200 * 1024) warps >>= 1;
+    if (warps > S.n_size) warps = S.n_size > 2 ? 2 : 1;
+    S.warps = warps;
+    const size_t smem = sizeof(double) * S.n_freq + warps * per_warp;
+    SOC_CUDA(cudaFuncSetAttribute(stochastic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    long long blocks = n_cells;
+    const long long cap = (long long)M->n_sm * 8;
+    if (blocks > cap) blocks = cap;
+    stochastic_kernel<<<(int)blocks, 32 * warps, smem, (cudaStream_t)stream>>>(S);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     return SOC_OK;

@@ -145,6 +145,56 @@ def temperature_table(freq_hz, sigma_abs_cm2, n_table=2048, t_lo=3.0, t_hi=1500.
     return np.exp(ln_t).astype(np.float32), e_min, e_max
 
 
+# ----------------------------------------------------------------------------- stochastically heated grains (row f4)
+def stochastic_model(freq_hz, n_size=25, n_e=64, a_min_um=4e-4, a_max_um=1e-2, t_lo=2.7, t_hi=2500.0):
+    """Synthetic stand-in for the grain data of the paper's Appendix A test (DustEM enthalpy tables are not available;
+    PAPER.md:359-371: 25 size bins, 128 frequencies).  INPUTS of soc_stochastic_emission, given to both sides:
+
+      per size s (radius a_s, log-spaced) and enthalpy bin i (temperatures T_i log-spaced, enthalpy E = c_V a^3 T^4 / 4,
+      a Debye solid):
+        jup[s, i, f], wup[s, i, f]   a photon of frequency f takes a grain from bin i to the bin jup that holds E_i + h nu
+                                     (the last bin takes everything above); the transition rate is wup * intensity[f]
+                                     with wup = 4 pi C_abs(nu) w_f / (h nu), C_abs = pi a^2 Q_abs, Q_abs ~ min(1, 2 pi a /
+                                     lambda).  A photon too soft to lift the grain out of its bin heats it continuously:
+                                     jup = i + 1 with the rate scaled by h nu / (E_(i+1) - E_i), which conserves the
+                                     energy; -1 only in the last bin
+        cool[s, i]                   "thermal continuous" cooling to the next lower bin: radiated power / (E_i - E_(i-1))
+        emis[s, i, f]                4 pi C_abs(nu_f) B_nu(T_i): emission of one grain in bin i
+        abundance[s]                 grains per H, MRN dn/da ~ a^-3.5
+    """
+    nu = np.asarray(freq_hz, dtype=np.float64)
+    w = trapz_weights(nu)
+    a = np.geomspace(a_min_um, a_max_um, n_size) * 1e-4                        # cm
+    lam = C_LIGHT / nu
+    T = np.geomspace(t_lo, t_hi, n_e)
+    jup = np.full((n_size, n_e, len(nu)), -1, dtype=np.int32)
+    wup = np.zeros((n_size, n_e, len(nu)))
+    cool = np.zeros((n_size, n_e))
+    emis = np.zeros((n_size, n_e, len(nu)))
+    E_all = np.zeros((n_size, n_e))
+    for s in range(n_size):
+        c_abs = np.pi * a[s] ** 2 * np.minimum(1.0, 2 * np.pi * a[s] / lam)
+        E = 2.5e4 * a[s] ** 3 * T ** 4 / 4.0                                    # erg; c_V ~ 2.5e4 T^3 erg cm^-3 K^-1
+        E_all[s] = E
+        edges = np.concatenate([[0.0], np.sqrt(E[:-1] * E[1:]), [np.inf]])      # bin i = [edges[i], edges[i+1])
+        power = np.array([4 * np.pi * float((w * c_abs * planck_nu(nu, t)).sum()) for t in T])
+        cool[s, 1:] = power[1:] / (E[1:] - E[:-1])
+        emis[s] = 4 * np.pi * c_abs[None, :] * planck_nu(nu[None, :], T[:, None])
+        for i in range(n_e):
+            j = np.searchsorted(edges, E[i] + H_PLANCK * nu, side="right") - 1
+            j = np.minimum(j, n_e - 1)
+            rate = 4 * np.pi * c_abs * w / (H_PLANCK * nu)
+            up = j > i
+            jup[s, i, up] = j[up]
+            wup[s, i, up] = rate[up]
+            if i + 1 < n_e:
+                jup[s, i, ~up] = i + 1
+                wup[s, i, ~up] = (rate * H_PLANCK * nu / (E[i + 1] - E[i]))[~up]
+    abundance = a ** -3.5
+    abundance *= 1e-9 / abundance.sum()
+    return dict(jup=jup, wup=wup, cool=cool, emis=emis, abundance=abundance, T=T, E=E_all, a_cm=a, freq_hz=nu)
+
+
 # ----------------------------------------------------------------------------- hierarchy
 def block_average(a):
     n = a.shape[0] // 2

@@ -24,7 +24,7 @@ EXPORTS = ["soc_grid_create", "soc_grid_destroy", "soc_grid_n_total", "soc_freq_
            "soc_simulate_packages", "soc_simulate_spectrum", "soc_update_temperatures", "soc_run_host",
            "soc_set_option", "soc_get_timings", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version",
            "soc_emission_counts", "soc_cell_emission", "soc_update_temperatures_ali", "soc_iterate", "soc_make_map",
-           "soc_checked_violations"]
+           "soc_checked_violations", "soc_stochastic_create", "soc_stochastic_destroy", "soc_stochastic_emission"]
 
 
 class SocError(RuntimeError):
@@ -47,6 +47,11 @@ class Sources(C.Structure):
 class MapDesc(C.Structure):
     _fields_ = [("ex", C.c_double * 3), ("ey", C.c_double * 3), ("dir", C.c_double * 3), ("centre", C.c_double * 3),
                 ("npx", C.c_int32), ("npy", C.c_int32), ("pixel", C.c_double)]
+
+
+class StochasticModel(C.Structure):
+    _fields_ = [("n_size", C.c_int32), ("n_e", C.c_int32), ("n_freq", C.c_int32), ("jup", C.c_void_p), ("wup", C.c_void_p),
+                ("cool", C.c_void_p), ("emis", C.c_void_p), ("abundance", C.c_void_p)]
 
 
 class IterateOpts(C.Structure):
@@ -100,6 +105,10 @@ def load():
     L.soc_iterate.argtypes = [vp, C.POINTER(Sources), i64, u64, C.POINTER(IterateOpts), dbl, vp, i32, dbl, dbl, vp, vp,
                               C.POINTER(IterateRecord), u32, vp]
     L.soc_make_map.argtypes = [vp, i32, vp, C.POINTER(MapDesc), vp, vp]
+    L.soc_stochastic_create.argtypes = [C.POINTER(StochasticModel), C.POINTER(vp)]
+    L.soc_stochastic_destroy.argtypes = [vp]
+    L.soc_stochastic_destroy.restype = None
+    L.soc_stochastic_emission.argtypes = [vp, vp, i64, vp, vp, vp]
     L.soc_run_host.argtypes = [C.POINTER(GridDesc), C.POINTER(Sources), i64, u64, i32, dbl, vp, i32, dbl, dbl, vp, vp,
                                C.POINTER(FreqResult), u32]
     L.soc_set_option.argtypes = [vp, C.c_char_p, i64]
@@ -319,6 +328,35 @@ def run_host(P, n_packages=None, seed=None, n_iter=None, flags=SOC_GEOM_FP32, wa
                           n_iter, float(P.t_scale or 0.0), _ptr(tab), 0 if tab is None else len(tab), float(P.e_min),
                           float(P.e_max), _ptr(absorbed_out), _ptr(T_out) if has_T else None, res, int(flags)))
     return absorbed_out, (T_out if has_T else None), (list(res) if want_results else None)
+
+
+class Stochastic:
+    """soc_stochastic handle (row f4): tables of inputs.stochastic_model() on the device."""
+
+    def __init__(self, model):
+        jup, wup = _np(model["jup"], np.int32), _np(model["wup"], np.float64)
+        cool, emis, ab = _np(model["cool"], np.float64), _np(model["emis"], np.float64), _np(model["abundance"], np.float64)
+        self.n_size, self.n_e, self.n_freq = jup.shape
+        m = StochasticModel(self.n_size, self.n_e, self.n_freq, _ptr(jup), _ptr(wup), _ptr(cool), _ptr(emis), _ptr(ab))
+        h = C.c_void_p()
+        _check(load().soc_stochastic_create(C.byref(m), C.byref(h)))
+        self._h = h
+
+    def emission(self, intensity, emission_out, p_out=None, stream=None):
+        n_cells = intensity.shape[0]
+        _check(load().soc_stochastic_emission(self._h, _dev_ptr(intensity), int(n_cells), _dev_ptr(emission_out), _dev_ptr(p_out),
+                                              _stream_ptr(stream)))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load().soc_stochastic_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def checked_violations():

@@ -240,7 +240,7 @@ def test_bench_reads_dram_traffic_from_the_newest_capture(tmp_path, monkeypatch)
     (tmp_path / "profiles" / "r01_ncu_dram_traffic.csv").write_text(
         "config,kernel,cell_steps,dram_read_bytes,dram_write_bytes,source\n5,k,100,900,100,old.txt\n")
     (tmp_path / "profiles" / "r02_ncu_dram_traffic.csv").write_text(
-        "config,kernel,cell_steps,dram_read_bytes,dram_write_bytes,source\n5,k,100,1500,500,new.txt\n5,k,100,500,500,new.txt\n")
+        "config,kernel,cell_steps,dram_read_bytes,dram_write_bytes,weight,source\n5,k,100,1500,500,1,new.txt\n5,k,100,500,500,1,new.txt\n")
     monkeypatch.setattr(b, "ROOT", str(tmp_path))
     t = b.ncu_traffic("5")
     assert t["bytes_per_cell_step"] == 15.0 and "r02_ncu_dram_traffic.csv" in t["source"] and "new.txt" in t["source"]
