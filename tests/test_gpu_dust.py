@@ -259,3 +259,37 @@ def test_iterate_production_mode_energy_balance():
     assert ratio[0] < 0.6 and 0.93 < ratio[-1] < 1.04 and (np.diff(ratio) > -0.03).all()
     for h in hist:
         assert abs(h["emitted"] - h["absorbed"] - h["escaped"]) <= 1e-6 * h["emitted"]
+
+
+def test_iterate_at_full_size_is_measured(capsys):
+    """Config 3 at full size (128^3, 64 frequencies), made opaque and luminous like the paper's iteration tests
+    (PAPER.md:139), through soc_iterate with the production kernels: emission-weighted counts with the paper's cap of 10000,
+    reference field after a burn-in, ALI.  Properties that hold at any size (conservation per iteration, global balance
+    approached) and the throughput of the dust launches, printed."""
+    import time
+    torch = _torch()
+    P = _hot_problem("3", n=128, n_freq=64, tau_scale=30.0, lum_scale=3000.0, n_packages=4_000_000)
+    G = soc.Grid.from_problem(P)
+    A = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+    T = torch.zeros(P.n_total, dtype=torch.float32, device="cuda")
+    n_req = [1_000_000, 2_000_000, 4_000_000, 4_000_000]          # growing package numbers (PAPER.md:231)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    hist = G.iterate([P.sources(f) for f in range(P.n_freq)], P.n_packages, P.seed, n_req, P.t_scale, P.table_T, P.e_min,
+                     P.e_max, A, T, mode="weighted", cap=10000, reference_field=True, ref_start=3, ali=True)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    G.close()
+    for h in hist:
+        assert abs(h["emitted"] - h["absorbed"] - h["escaped"]) <= 1e-6 * h["emitted"]
+    a_const = hist[0]["absorbed"]
+    ratio = [h["escaped"] / a_const for h in hist[1:]]
+    assert ratio[-1] > ratio[0] and 0.5 < ratio[-1] < 1.05
+    Tn = T.cpu().numpy()
+    assert Tn.max() > 100.0 and np.median(Tn[Tn > 0]) > 5.0       # hot dust near the sources only (PAPER.md:143)
+    steps = sum(h["cell_steps"] for h in hist)
+    with capsys.disabled():
+        print(f"\n[soc_iterate, config 3 at 128^3 x 64 frequencies, 4 iterations with ALI + reference field] {dt:.2f} s wall, "
+              f"{steps:.3e} cell-steps = {steps / dt:.3e} cell-steps/s incl. counts, scans and temperature updates; packages per "
+              f"iteration {[h['n_packages'] for h in hist]}; escaped dust emission / A_const per iteration {[round(r, 3) for r in ratio]}; "
+              f"T max {Tn.max():.0f} K")
