@@ -155,6 +155,13 @@ struct soc_grid {
     int opt_carveout = -1;                    // preferred shared-memory carve-out of the photon kernels in %, -1 = driver default
     double rho_mean = 0.0;                    // mean density of the root-level leaves
     int opt_kernel = 0;                       // regular grids: 0 = by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel
+    // z-slab blocking (SlabParams): package queues of the two accumulator sets
+    int opt_slabs = 0;                        // 0 = by working-set size, 1 = off, n >= 2 = n slabs
+    int opt_slab_sweeps = 0;                  // sweeps over the slabs before the final whole-grid phase; 0 = by scattering depth
+    double *d_hot64[2] = {nullptr, nullptr};  // hot-cell sums of the two accumulator sets (FastParams::hot64)
+    uint4 *d_slab_q[2] = {nullptr, nullptr};  // 3 arrays of n_slabs * cap entries
+    unsigned *d_slab_cnt[2] = {nullptr, nullptr};
+    size_t slab_q_entries[2] = {0, 0};
     int opt_timing = 0;                       // record a CUDA-event pair around every photon launch
     std::vector<cudaEvent_t> ev0, ev1;        // n_slots each (created on demand)
     std::vector<char> ev_set;
@@ -663,7 +670,57 @@ __global__ void __launch_bounds__(256) photon_kernel(const __grid_constant__ Sim
 // ------------------------------------------------------------------------------------------------
 constexpr uint32_t kSentinel = 0xffffffffu;       // cell word of a ghost cell
 
-enum : int { RUN = 0, SCAT = 1, DONE = 2, EMPTY = 3, NEWID = 4, DEAD = 5 };
+enum : int { RUN = 0, SCAT = 1, DONE = 2, EMPTY = 3, NEWID = 4, DEAD = 5, SUSP = 6 };
+
+// z-slab blocking of regular grids whose working set exceeds L2.  The bricks of the padded root grid are
+// stored z-major, so a slab of brick layers is one contiguous id range of the cell words and of the accumulator.  A
+// frequency is a sequence of launches ("phases"), each of which serves one slab: it pops that slab's queue, walks the
+// packages while they stay inside their slab and SUSPENDS a package that crosses into the next slab -- its state (48
+// bytes) goes to that slab's queue and the walk resumes when the slab's turn comes.  The phases sweep the slabs up and
+// down; a last phase pops every queue and confines nothing.
+//   * A launch pops the entries [head, frozen) of a queue; `frozen` is the tail as it stood when the previous launch
+//     ended (written by that launch's last block), so entries pushed while a queue is being popped wait for its next turn
+//     and no slot is ever read before it is written.
+//   * No tail: a warp that finds its queue empty does not wait for its running lanes -- it DUMPS them (state to a
+//     "leftover" queue, popped first by the next phase) and exits, so a phase ends within one service pass of the moment
+//     its queue runs dry.  Two leftover queues alternate between consecutive phases.
+//   * A queue that is full refuses the package, which then walks on unconfined (sl = -1) in the launch that holds it.
+constexpr int kMaxSlabs = 62;          // + 2 leftover queues = 64 queues
+constexpr int kSlabChunk = 16;         // queue slots a warp claims at a time
+struct SlabParams {
+    uint4 *qa, *qb, *qc;                // all queues, queue q from slab_qbase(q): (fx, fy, fz, tau_rem), (dx, dy, dz, w),
+                                        // (absrel, idx | (src + 1) << 25, rel, scat)
+    unsigned *cnt;                      // [64][4]: head, tail, frozen, -; then the count of finished blocks
+    unsigned cap, cap_left;             // entries per slab queue / per leftover queue
+    int n_slabs, slab_ids;              // ids per slab = brick layers per slab * 8 nbx nby
+    int q_left;                         // the leftover queue this launch pops (n_slabs or n_slabs + 1); it dumps to the other
+    int s_first, s_last;                // slab queues this launch pops, in this order
+    int final_phase;                    // nothing is suspended or dumped
+};
+__device__ __forceinline__ size_t slab_qbase(const SlabParams &S, int q)
+{
+    return q < S.n_slabs ? (size_t)q * S.cap : (size_t)S.n_slabs * S.cap + (size_t)(q - S.n_slabs) * S.cap_left;
+}
+// the last block of a launch to finish: the popped queues were drained up to `frozen`; every queue's new `frozen` is its
+// tail now (all pushes of this launch are complete)
+__device__ __forceinline__ void slab_epilogue(const SlabParams &S, bool pops)
+{
+    __shared__ unsigned s_is_last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_is_last = atomicAdd(S.cnt + 4 * 64, 1u) == gridDim.x - 1 ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_is_last && (int)threadIdx.x < S.n_slabs + 2) {
+        const int q = threadIdx.x;
+        volatile unsigned *c = S.cnt + 4 * q;
+        if (pops && (q == S.q_left || (q >= S.s_first && q <= S.s_last))) c[0] = c[2];
+        const unsigned cap = q < S.n_slabs ? S.cap : S.cap_left, t = c[1];
+        c[1] = c[2] = t < cap ? t : cap;
+        if (q == 0) S.cnt[4 * 64] = 0u;
+    }
+}
 
 struct FastParams {
     int nx, ny, nz;                     // root grid
@@ -688,6 +745,9 @@ struct FastParams {
     int hot_r;                          // half-width R of the cached cube around every point source, -1 = no cache
     double *acc;                        // [n_int] internal accumulator (unweighted energies), ACC32 = false
     float *acc32;                       // [n_int] internal accumulator in units of e_ref, ACC32 = true
+    double *hot64;                      // [n_point][(2 hot_r + 1)^3] ACC32: the blocks' hot-cell partial sums, in units of e_ref.
+                                        // fp64: a cell next to a source collects ~1e5 partial sums per launch, and an fp32
+                                        // sum that large silently drops the small ones
     float bg_rel, beam_rel;             // package energy / e_ref of a background / beam package
     float ps_rel[SOC_MAX_POINT_SOURCES];  // ... of a package of point source k
     DustParams dust;
@@ -695,6 +755,7 @@ struct FastParams {
     soc_replay_record *replay;
     unsigned long long *counter;
     DevResult *result;
+    SlabParams slab;
 };
 
 struct FPkg {
@@ -1054,7 +1115,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
                 const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
                           iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
-                if (ACC32) atomicAdd(P.acc32 + CK(root_id(P, ix, iy, iz), P.n_int), v * P.ps_rel[k]);
+                if (ACC32) atomicAdd(P.hot64 + i, (double)v * (double)P.ps_rel[k]);
                 else atomicAdd(P.acc + CK(root_id(P, ix, iy, iz), P.n_int), (double)v * P.ps_e0[k]);
             }
         }
@@ -1122,6 +1183,7 @@ struct QPkg {
     uint32_t steps;         // REPLAY only
     unsigned long long hash;
     uint32_t n_ld, n_red;   // REPLAY only (option "stats"): gathers / reductions issued for this package
+    int sl;                 // SLAB only: the z-slab the package is confined to, -1 = not confined
 };
 
 __device__ __forceinline__ int v_src(int sd) { return sd < 0 ? -1 : (sd >> 16); }
@@ -1154,9 +1216,12 @@ __device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p, float (*s_
     p.n_red += 1;
 }
 
-template <bool REPLAY, bool DUST>
-__global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant__ FastParams P)
+// SLAB: the launch serves one z-slab of the grid (SlabParams): packages come from the slab's queue instead of the id
+// counter (they were created by slab_emit_kernel), and a package that crosses out of the slab's id range is suspended.
+template <bool REPLAY, bool DUST, bool SLAB>
+__global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __grid_constant__ FastParams P)
 {
+    static_assert(!(SLAB && DUST), "slab launches carry constant-source packages only");
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
     // per-launch totals of this thread (touched only in the service block)
@@ -1177,22 +1242,57 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
     unsigned long long acc_ld = 0, acc_red = 0;  // REPLAY variant: request counters (option "stats")
     QPkg p;
     p.n_ld = 0; p.n_red = 0;
-    p.sd = -1; p.w = 0.0f; p.absrel = 0.0f; p.scat = 0; p.rel = 0; p.idx = 0; p.steps = 0; p.hash = 0;
+    p.sd = -1; p.w = 0.0f; p.absrel = 0.0f; p.scat = 0; p.rel = 0; p.idx = 0; p.steps = 0; p.hash = 0; p.sl = -1;
     p.q0 = p.q1 = p.q2 = p.q3 = 0u; p.pend = 0.0f; p.prel = 0.0f;
     p.fx = p.fy = p.fz = 0.5f; p.dx = p.dy = 0.0f; p.dz = 1.0f; p.rx = p.ry = p.rz = 1.0f; p.tau_rem = 0.0f;
     int need = EMPTY;
     unsigned n_steps = 0;                        // cell-steps of this lane (all its packages)
-    unsigned pool_next = 0, pool_end = 0;        // warp-uniform pool of package offsets
+    unsigned pool_next = 0, pool_end = 0;        // warp-uniform pool of package offsets (SLAB: of queue slots)
+    int cur_q = SLAB ? P.slab.s_first - 1 : 0;   // SLAB: position in the list of queues to pop (s_first - 1 = the leftover queue)
+    int pool_q = 0;                              // SLAB: the queue the pool was claimed from
     bool exhausted = false;
     int n_dead = 0;                              // warp-uniform: lanes that will get no more packages
     const unsigned n_pkg = (unsigned)(P.pkg_end - P.pkg_begin);      // the launcher keeps this below 2^32
     const int T = P.service_threshold;
+
+    // SLAB: the lanes with `sel` hand their package to queue `dest` (one slot reservation per warp and queue) and become
+    // EMPTY; a full queue refuses the package, which then walks on, not confined to a slab any more
+    auto push = [&](bool sel, int dest) {
+        unsigned todo = __ballot_sync(kFull, sel);
+        while (todo) {
+            const int leader = __ffs(todo) - 1;
+            const int d = __shfl_sync(kFull, dest, leader);
+            const bool mine = sel && dest == d;
+            const unsigned m = __ballot_sync(kFull, mine);
+            unsigned b = 0;
+            if (lane == leader) b = atomicAdd(P.slab.cnt + 4 * d + 1, (unsigned)__popc(m));
+            b = __shfl_sync(kFull, b, leader);
+            if (mine) {
+                const unsigned slot = b + __popc(m & lt_mask);
+                if (slot < (d < P.slab.n_slabs ? P.slab.cap : P.slab.cap_left)) {
+                    const size_t e = slab_qbase(P.slab, d) + slot;
+                    const uint32_t tag = p.idx | ((uint32_t)(v_src(p.sd) + 1) << 25);
+                    P.slab.qa[e] = make_uint4(__float_as_uint(p.fx), __float_as_uint(p.fy), __float_as_uint(p.fz), __float_as_uint(p.tau_rem));
+                    P.slab.qb[e] = make_uint4(__float_as_uint(p.dx), __float_as_uint(p.dy), __float_as_uint(p.dz), __float_as_uint(p.w));
+                    P.slab.qc[e] = make_uint4(__float_as_uint(p.absrel), tag, (uint32_t)p.rel, p.scat);
+                    if (REPLAY) { acc_ld += p.n_ld; acc_red += p.n_red; }
+                    need = EMPTY;
+                } else {
+                    p.sl = -1;
+                    q_load(P, p);
+                    need = RUN;
+                }
+            }
+            todo &= ~m;
+        }
+    };
 
     for (;;) {
         const unsigned m_run = __ballot_sync(kFull, need == RUN);
         const int n_park = 32 - __popc(m_run) - n_dead;
         if (n_park > 0 && (n_park >= T || m_run == 0u)) {
             // ---------------------------------------------------------------- service, all parked lanes together
+            if (SLAB) push(need == SUSP, p.sl + (p.rel >= (p.sl + 1) * P.slab.slab_ids ? 1 : -1));
             if (need == DONE) {                  // retire the finished package
                 q_flush(P, p, s_acc);
                 const int src = v_src(p.sd);
@@ -1215,7 +1315,21 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
             unsigned want = __ballot_sync(kFull, need == EMPTY);
             if (want && !exhausted) {
                 do {
-                    if (pool_next >= pool_end) {
+                    if (SLAB) {
+                        // entries [head, frozen) of the leftover queue, then of the slab queues
+                        while (pool_next >= pool_end && cur_q <= P.slab.s_last) {
+                            const int q = cur_q < P.slab.s_first ? P.slab.q_left : cur_q;
+                            const unsigned frozen = P.slab.cnt[4 * q + 2];
+                            unsigned base = 0;
+                            if (lane == 0) base = atomicAdd(P.slab.cnt + 4 * q, (unsigned)kSlabChunk);
+                            base = __shfl_sync(kFull, base, 0);
+                            if (base >= frozen) { cur_q += 1; continue; }
+                            pool_next = base;
+                            pool_end = frozen - base > (unsigned)kSlabChunk ? base + kSlabChunk : frozen;
+                            pool_q = q;
+                        }
+                        if (pool_next >= pool_end) { exhausted = true; break; }
+                    } else if (pool_next >= pool_end) {
                         unsigned long long base = 0;
                         if (lane == 0) base = atomicAdd(P.counter, (unsigned long long)kChunk);
                         base = __shfl_sync(kFull, base, 0);
@@ -1225,16 +1339,52 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                     }
                     const unsigned avail = pool_end - pool_next;
                     const unsigned rank = __popc(want & lt_mask);
-                    if (need == EMPTY && rank < avail) { p.idx = pool_next + rank; need = NEWID; }
+                    if (need == EMPTY && rank < avail) { p.idx = pool_next + rank; p.sd = SLAB ? pool_q : p.sd; need = NEWID; }
                     const unsigned n_want = __popc(want);
                     pool_next += n_want < avail ? n_want : avail;
                     want = __ballot_sync(kFull, need == EMPTY);
                 } while (want);
             }
-            if (need == EMPTY && exhausted) need = DEAD;
-            n_dead = __popc(__ballot_sync(kFull, need == DEAD));
+            if (!SLAB) {
+                if (need == EMPTY && exhausted) need = DEAD;
+                n_dead = __popc(__ballot_sync(kFull, need == DEAD));
+            }
             float ndx = 0.0f, ndy = 0.0f, ndz = 1.0f;
-            if (need == NEWID) {
+            if (SLAB && need == NEWID) {
+                // resume a package: slot p.idx of queue p.sd (reciprocals and the half brick are not part of the state)
+                const size_t e = slab_qbase(P.slab, p.sd) + p.idx;
+                const uint4 a = P.slab.qa[e], b = P.slab.qb[e], c = P.slab.qc[e];
+                p.fx = __uint_as_float(a.x); p.fy = __uint_as_float(a.y); p.fz = __uint_as_float(a.z); p.tau_rem = __uint_as_float(a.w);
+                p.dx = __uint_as_float(b.x); p.dy = __uint_as_float(b.y); p.dz = __uint_as_float(b.z); p.w = __uint_as_float(b.w);
+                p.rx = 1.0f / p.dx; p.ry = 1.0f / p.dy; p.rz = 1.0f / p.dz;
+                p.absrel = __uint_as_float(c.x); p.rel = (int)c.z; p.scat = c.w;
+                p.idx = c.y & 0xffffffu;
+                const int src = (int)(c.y >> 25) - 1;
+                p.sd = -1;
+                if (src >= 0) {
+                    // hot-cube tracking (deposits near the package's own source go to the block's partial sums) is not part
+                    // of the queued state: the position in the cube follows from the cell
+                    p.sd = src << 16;
+                    if (P.hot_r >= 0) {
+                        const int B = p.rel >> 3, bz = B / (P.nbx * P.nby), r = B - bz * (P.nbx * P.nby), by = r / P.nbx, bx = r - by * P.nbx;
+                        const int hx = 2 * bx + (p.rel & 1) - 2 - (int)floor(P.ps_pos[src][0]) + P.hot_r;
+                        const int hy = 2 * by + ((p.rel >> 1) & 1) - 2 - (int)floor(P.ps_pos[src][1]) + P.hot_r;
+                        const int hz = 2 * bz + ((p.rel >> 2) & 1) - 2 - (int)floor(P.ps_pos[src][2]) + P.hot_r;
+                        if ((unsigned)hx < (unsigned)hot_side && (unsigned)hy < (unsigned)hot_side && (unsigned)hz < (unsigned)hot_side)
+                            p.sd |= 0x200 | hx | (hy << 3) | (hz << 6);
+                    }
+                }
+                p.prel = package_rel(P, src);
+                p.pend = 0.0f;
+                p.n_ld = 0; p.n_red = 0;
+                p.sl = -1;
+                if (!P.slab.final_phase) {
+                    const int sl = p.rel / P.slab.slab_ids;
+                    p.sl = sl < P.slab.n_slabs ? sl : P.slab.n_slabs - 1;
+                }
+                q_load(P, p);
+                need = RUN;
+            } else if (!SLAB && need == NEWID) {
                 FPkg q;
                 fast_emit<false>(P, q, P.pkg_begin + (long long)p.idx, ndx, ndy, ndz, p.prel);
                 p.fx = q.fx; p.fy = q.fy; p.fz = q.fz; p.rel = q.rel;
@@ -1264,6 +1414,26 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                 philox_block(P.seed, P.ifreq, P.pkg_begin + (long long)p.idx, 2u + p.scat, s0, s1, s2, s3);
                 p.tau_rem = -__logf(uniform01<float>(s0));                    // a4
                 need = RUN;
+            }
+            if (SLAB && exhausted && !P.slab.final_phase) {
+                // the queue has run dry: the phase ends here for this warp.  Its running packages (those still confined to
+                // a slab) are handed to the next phase in mid-cell: deposits so far to the sums, sums to the accumulator
+                const bool dump = need == RUN && p.sl >= 0;
+                if (dump) {
+                    if (p.sd >= 0 && (p.sd & 0x200)) {
+                        const int j = (p.sd & 7) + hot_side * (((p.sd >> 3) & 7) + hot_side * ((p.sd >> 6) & 7));
+                        atomicAdd(s_hot + CK((p.sd >> 16) * hot_cells + j, hot_cells * P.n_point), p.pend);
+                    } else {
+                        s_acc[CK(p.rel & 3, 4)][CK(threadIdx.x, 256)] += p.pend * p.prel;
+                    }
+                    p.pend = 0.0f;
+                    q_flush(P, p, s_acc);
+                }
+                push(dump, P.slab.q_left ^ P.slab.n_slabs ^ (P.slab.n_slabs + 1));
+            }
+            if (SLAB) {
+                if (need == EMPTY && exhausted) need = DEAD;
+                n_dead = __popc(__ballot_sync(kFull, need == DEAD));
             }
             continue;
         }
@@ -1349,7 +1519,9 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
                         int rel = p.rel ^ abit;
                         if (!inside) rel += fwd ? bstride : -bstride;
                         p.rel = rel;
-                        q_load(P, p);
+                        if (SLAB && p.sl >= 0 && (unsigned)(rel - p.sl * P.slab.slab_ids) >= (unsigned)P.slab.slab_ids)
+                            need = SUSP;         // into the next slab
+                        else q_load(P, p);
                     } else {
                         p.rel ^= abit;
                     }
@@ -1368,11 +1540,7 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
         for (int i = threadIdx.x; i < hot_cells * P.n_point; i += blockDim.x) {
             const float v = s_hot[i];
             if (v != 0.0f) {
-                const int k = i / hot_cells, j = i - k * hot_cells;
-                const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
-                const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
-                          iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
-                atomicAdd(P.acc32 + CK(root_id(P, ix, iy, iz), P.n_int), v * P.ps_rel[k]);
+                atomicAdd(P.hot64 + i, (double)v * (double)P.ps_rel[i / hot_cells]);
             }
         }
     }
@@ -1411,6 +1579,56 @@ __global__ void __launch_bounds__(256, 5) photon_q_kernel(const __grid_constant_
         atomicAdd(&P.result->scatterings, (unsigned long long)acc_scat);
         atomicAdd(&P.result->terminated, (unsigned long long)acc_term);
     }
+    if (SLAB) slab_epilogue(P.slab, true);
+}
+
+// a1-a4 for a slab-blocked launch: creates every package of the launch (position, direction, first free path) and puts
+// it into the queue of the z-slab it starts in.  One package per thread; a block counts its packages per slab in shared
+// memory and reserves the slots of a batch of 256 with one atomic per slab.
+__global__ void __launch_bounds__(256) slab_emit_kernel(const __grid_constant__ FastParams P)
+{
+    __shared__ unsigned s_n[kMaxSlabs], s_base[kMaxSlabs];
+    const int lane = threadIdx.x & 31;
+    const unsigned n_pkg = (unsigned)(P.pkg_end - P.pkg_begin);
+    double acc_emit = 0.0;
+    for (unsigned base = blockIdx.x * 256u; base < n_pkg; base += gridDim.x * 256u) {      // block-uniform trip count
+        if (threadIdx.x < kMaxSlabs) s_n[threadIdx.x] = 0u;
+        __syncthreads();
+        const unsigned idx = base + threadIdx.x;
+        const bool live = idx < n_pkg;
+        FPkg q;
+        float dx = 0.0f, dy = 0.0f, dz = 1.0f, tau = 0.0f;
+        int slab = 0, rel = 0;
+        unsigned rank = 0;
+        if (live) {
+            int ix, iy, iz;
+            const long long id = P.pkg_begin + (long long)idx;
+            fast_emit_core(P, q, id, ix, iy, iz, dx, dy, dz);
+            rel = root_id(P, ix, iy, iz);
+            uint32_t s0, s1, s2, s3;
+            philox_block(P.seed, P.ifreq, id, 2u, s0, s1, s2, s3);
+            tau = -__logf(uniform01<float>(s0));                              // a4
+            slab = rel / P.slab.slab_ids;
+            slab = slab < P.slab.n_slabs ? slab : P.slab.n_slabs - 1;
+            acc_emit += package_e0(P, q.src);
+            rank = atomicAdd(s_n + slab, 1u);
+        }
+        __syncthreads();
+        if ((int)threadIdx.x < P.slab.n_slabs && s_n[threadIdx.x] > 0u)
+            s_base[threadIdx.x] = atomicAdd(P.slab.cnt + 4 * threadIdx.x + 1, s_n[threadIdx.x]);
+        __syncthreads();
+        if (live) {
+            const size_t e = slab_qbase(P.slab, slab) + CK(s_base[slab] + rank, P.slab.cap);
+            const uint32_t tag = idx | ((uint32_t)(q.src + 1) << 25);
+            P.slab.qa[e] = make_uint4(__float_as_uint(q.fx), __float_as_uint(q.fy), __float_as_uint(q.fz), __float_as_uint(tau));
+            P.slab.qb[e] = make_uint4(__float_as_uint(dx), __float_as_uint(dy), __float_as_uint(dz), __float_as_uint(1.0f));
+            P.slab.qc[e] = make_uint4(0u, tag, (uint32_t)rel, 0u);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc_emit += __shfl_xor_sync(kFull, acc_emit, o);
+    if (lane == 0 && acc_emit != 0.0) atomicAdd(&P.result->emitted, acc_emit);
+    slab_epilogue(P.slab, false);
 }
 
 // internal accumulator -> caller's array: out[gid] += weight * acc[internal(gid)], acc reset to zero
@@ -1449,6 +1667,28 @@ __global__ void __launch_bounds__(256) unpad_add_kernel(const __grid_constant__ 
                 U.acc[j] = 0.0;
             }
         }
+    }
+}
+
+// the hot-cell sums of a launch (FastParams::hot64) -> caller's array, sums reset to zero
+struct HotFoldParams {
+    double *out, *hot64;
+    double weight;
+    int nx, ny, nz, n_point, hot_r;
+    int cell[SOC_MAX_POINT_SOURCES][3];          // root cell of every point source
+};
+__global__ void __launch_bounds__(256) hot_fold_kernel(const __grid_constant__ HotFoldParams H)
+{
+    const int side = 2 * H.hot_r + 1, cells = side * side * side;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < cells * H.n_point; i += gridDim.x * blockDim.x) {
+        const double v = H.hot64[i];
+        if (v == 0.0) continue;
+        H.hot64[i] = 0.0;
+        const int k = i / cells, j = i - k * cells;
+        const int jz = j / (side * side), jr = j - jz * side * side, jy = jr / side, jx = jr - jy * side;
+        const int ix = H.cell[k][0] + jx - H.hot_r, iy = H.cell[k][1] + jy - H.hot_r, iz = H.cell[k][2] + jz - H.hot_r;
+        if ((unsigned)ix < (unsigned)H.nx && (unsigned)iy < (unsigned)H.ny && (unsigned)iz < (unsigned)H.nz)
+            atomicAdd(H.out + (ix + (long long)H.nx * (iy + (long long)H.ny * iz)), H.weight * v);   // cubes of two sources may overlap
     }
 }
 
@@ -2132,6 +2372,24 @@ template <typename R, bool HIER, bool REPLAY> int launch_photon(soc_grid *G, con
     return SOC_OK;
 }
 
+// the hot-cell sums of the launch described by P follow the internal accumulator into the caller's array
+int launch_hot_fold(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
+{
+    if (P.hot_r < 0 || P.n_point <= 0 || !P.hot64) return SOC_OK;
+    HotFoldParams H;
+    std::memset(&H, 0, sizeof(H));
+    H.out = absorbed; H.hot64 = P.hot64; H.weight = weight;
+    H.nx = G->nx; H.ny = G->ny; H.nz = G->nz; H.n_point = P.n_point; H.hot_r = P.hot_r;
+    for (int k = 0; k < P.n_point; ++k)
+        for (int j = 0; j < 3; ++j) H.cell[k][j] = (int)std::floor(P.ps_pos[k][j]);
+    const int side = 2 * P.hot_r + 1, n = side * side * side * P.n_point;
+    hot_fold_kernel<<<(n + 255) / 256, 256, 0, st>>>(H);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    if (G->overlap_active) SOC_CUDA(cudaEventRecord(G->ev_unpad[G->acc_sel], st));    // the fold into the caller's array ends here
+    return SOC_OK;
+}
+
 int launch_unpad(soc_grid *G, bool acc32, double weight, double *absorbed, cudaStream_t st)
 {
     UnpadParams U;
@@ -2162,7 +2420,7 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
     const int side = 2 * P.hot_r + 1;
     const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
     int per_sm = 0;
-    if (QK) SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<REPLAY, DUST>, threads, smem));
+    if (QK) SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<REPLAY, DUST, false>, threads, smem));
     else SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY, ACC32, DUST>, threads, smem));
     if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
     if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
@@ -2171,10 +2429,10 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
     const long long need = (n_pkg + threads - 1) / threads;
     if (need < blocks) blocks = (int)(need > 0 ? need : 1);
     if (G->opt_carveout >= 0) {
-        if (QK) SOC_CUDA(cudaFuncSetAttribute(photon_q_kernel<REPLAY, DUST>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
+        if (QK) SOC_CUDA(cudaFuncSetAttribute(photon_q_kernel<REPLAY, DUST, false>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
         else SOC_CUDA(cudaFuncSetAttribute(photon_fast_kernel<HIER, REPLAY, ACC32, DUST>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
     }
-    if (QK) photon_q_kernel<REPLAY, DUST><<<blocks, threads, smem, st>>>(P);
+    if (QK) photon_q_kernel<REPLAY, DUST, false><<<blocks, threads, smem, st>>>(P);
     else photon_fast_kernel<HIER, REPLAY, ACC32, DUST><<<blocks, threads, smem, st>>>(P);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
@@ -2182,7 +2440,83 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
         SOC_CUDA(cudaEventRecord(G->ev_after_photon, st));
         G->ev_after_photon = nullptr;
     }
-    return launch_unpad(G, ACC32, weight, absorbed, st);
+    const int rc = launch_unpad(G, ACC32, weight, absorbed, st);
+    return rc == SOC_OK && ACC32 ? launch_hot_fold(G, P, weight, absorbed, st) : rc;
+}
+
+// Slab-blocked launch of one frequency on a regular grid (SlabParams): create the packages, sweep the z-slabs up and down
+// `sweeps` times with photon_q_kernel<., ., SLAB> confined to one slab per launch, then one whole-grid launch that takes
+// what is still queued (packages that scattered back across a slab boundary after the last sweep).
+template <bool STATS>
+int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weight, double *absorbed, cudaStream_t st)
+{
+    const int sel = G->acc_sel;
+    const int threads = 256;
+    const unsigned n_pkg = (unsigned)(P.pkg_end - P.pkg_begin);
+    const int side = 2 * P.hot_r + 1;
+    const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
+    int per_sm = 0;
+    SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<STATS, false, true>, threads, smem));
+    if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
+    if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
+    int blocks = per_sm * G->n_sm;
+    const long long need = ((long long)n_pkg + threads - 1) / threads;
+    if (need < blocks) blocks = (int)(need > 0 ? need : 1);
+    // the phases: sweeps up and down over the slabs (an upward sweep ends at the top slab, the next starts just below it)
+    std::vector<int> phase;
+    for (int sweep = 0, s = 0, dir = 1; sweep < sweeps; ++sweep) {
+        for (;; s += dir) {
+            phase.push_back(s);
+            if (s + dir < 0 || s + dir >= n_slabs) break;
+        }
+        dir = -dir;
+        s += dir;
+    }
+    // queues: one per slab (every package of the launch may wait in one slab), two leftover queues (each receives, every
+    // other phase, at most the packages the lanes hold)
+    const size_t lanes = (size_t)blocks * threads;
+    const size_t cap_left = (lanes < n_pkg ? lanes : n_pkg) * (phase.size() / 2 + 1);
+    const size_t entries = (size_t)n_slabs * n_pkg + 2 * cap_left;
+    if (cap_left >= (1ull << 32)) return fail(SOC_EINVAL, "too many phases");
+    if (G->slab_q_entries[sel] < entries) {
+        if (G->d_slab_q[sel]) { SOC_CUDA(cudaStreamSynchronize(st)); SOC_CUDA(cudaFree(G->d_slab_q[sel])); G->d_slab_q[sel] = nullptr; }
+        G->slab_q_entries[sel] = 0;
+        if (cudaMalloc(&G->d_slab_q[sel], 3 * entries * sizeof(uint4)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(SOC_ENOMEM, "package queues of the slab-blocked launch");
+        }
+        G->slab_q_entries[sel] = entries;
+    }
+    const size_t cnt_bytes = sizeof(unsigned) * (4 * 64 + 4);
+    if (!G->d_slab_cnt[sel]) SOC_CUDA(cudaMalloc(&G->d_slab_cnt[sel], cnt_bytes));
+    SlabParams &S = P.slab;
+    S.qa = G->d_slab_q[sel]; S.qb = S.qa + entries; S.qc = S.qb + entries;
+    S.cnt = G->d_slab_cnt[sel]; S.cap = n_pkg; S.cap_left = (unsigned)cap_left; S.n_slabs = n_slabs;
+    S.slab_ids = ((G->nbz + n_slabs - 1) / n_slabs) * 8 * G->nbx * G->nby;
+    SOC_CUDA(cudaMemsetAsync(S.cnt, 0, cnt_bytes, st));
+    {
+        long long eb = ((long long)n_pkg + 255) / 256;
+        const long long cap = (long long)G->n_sm * 16;
+        S.q_left = n_slabs; S.s_first = 0; S.s_last = -1; S.final_phase = 0;
+        slab_emit_kernel<<<(int)(eb < cap ? eb : cap), 256, 0, st>>>(P);
+        g_launches += 1;
+    }
+    for (size_t k = 0; k < phase.size(); ++k) {
+        S.s_first = S.s_last = phase[k];
+        S.q_left = n_slabs + (int)(k & 1);
+        photon_q_kernel<STATS, false, true><<<blocks, threads, smem, st>>>(P);
+        g_launches += 1;
+    }
+    S.s_first = 0; S.s_last = n_slabs - 1; S.q_left = n_slabs + (int)(phase.size() & 1); S.final_phase = 1;
+    photon_q_kernel<STATS, false, true><<<blocks, threads, smem, st>>>(P);
+    g_launches += 1;
+    SOC_CUDA(cudaGetLastError());
+    if (G->ev_after_photon) {
+        SOC_CUDA(cudaEventRecord(G->ev_after_photon, st));
+        G->ev_after_photon = nullptr;
+    }
+    const int rc = launch_unpad(G, true, weight, absorbed, st);
+    return rc == SOC_OK ? launch_hot_fold(G, P, weight, absorbed, st) : rc;
 }
 
 // ---- f1 host helpers
@@ -2395,6 +2729,15 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
             }
         }
         F.acc32 = G->acc_sel ? G->d_acc32_b : G->d_acc32;
+        if (acc32 && F.hot_r >= 0) {
+            double *&h = G->d_hot64[G->acc_sel];
+            if (!h) {
+                const size_t bytes = sizeof(double) * SOC_MAX_POINT_SOURCES * 343;
+                SOC_CUDA(cudaMalloc(&h, bytes));
+                SOC_CUDA(cudaMemsetAsync(h, 0, bytes, st));              // st = the stream that uses it
+            }
+            F.hot64 = h;
+        }
         if (!acc32 && G->acc_sel && !G->d_acc_b) {           // fp64 fallback on the second stream: its own accumulator
             SOC_CUDA(cudaMalloc(&G->d_acc_b, sizeof(double) * (size_t)G->n_int));
             SOC_CUDA(cudaMemsetAsync(G->d_acc_b, 0, sizeof(double) * (size_t)G->n_int, st));   // st = the stream that uses it
@@ -2410,6 +2753,20 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         const bool big = 8ll * G->n_int > (64ll << 20) && P.ksca * G->rho_mean * n_max < 12.0;
         const bool v2 = !hier && acc32 && (G->opt_kernel == 2 || (G->opt_kernel == 0 && big)) && pkg_count < (1ll << 32);
         if (v2) F.service_threshold = auto_threshold;
+        // z-slab blocking: working set per launch <= ~20 MB, so that gathers and reductions hit L2
+        int n_slabs = G->opt_slabs;
+        if (n_slabs == 0) n_slabs = 8ll * G->n_int > (64ll << 20) ? (int)((8ll * G->n_int + (20ll << 20) - 1) / (20ll << 20)) : 1;
+        if (n_slabs > G->nbz / 2) n_slabs = G->nbz / 2;
+        if (n_slabs > kMaxSlabs) n_slabs = kMaxSlabs;
+        const bool slab = !hier && acc32 && !rep && F.dust.n_dust == 0 && n_slabs >= 2 && G->opt_kernel != 1 &&
+                          pkg_count <= (1ll << 24);
+        if (slab) {
+            const double depth = P.ksca * G->rho_mean * n_max;
+            const int sweeps = G->opt_slab_sweeps > 0 ? G->opt_slab_sweeps : (depth < 0.3 ? 2 : (depth < 3.0 ? 4 : 6));
+            F.service_threshold = auto_threshold;
+            rc = G->opt_stats ? launch_slab<true>(G, F, n_slabs, sweeps, w_eff, absorbed, st)
+                              : launch_slab<false>(G, F, n_slabs, sweeps, w_eff, absorbed, st);
+        } else {
         const int sel = (v2 ? 8 : 0) | (hier ? 4 : 0) | ((rep || G->opt_stats) ? 2 : 0) | (acc32 ? 1 : 0);
 #define SOC_LF(H, R, A, Q) (F.dust.n_dust > 0 ? launch_fast<H, R, A, Q, true>(G, F, w_eff, absorbed, st) \
                                               : launch_fast<H, R, A, Q, false>(G, F, w_eff, absorbed, st))
@@ -2426,6 +2783,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         default: rc = SOC_LF(true, true, true, false); break;
         }
 #undef SOC_LF
+        }
     }
     if (rc == SOC_OK && G->opt_timing) {
         if (G->ev_after_photon) SOC_CUDA(cudaEventRecord(G->ev1[slot], st));
@@ -2493,6 +2851,7 @@ void soc_grid_destroy(soc_grid *G)
     cudaFree(G->d_dust_first); cudaFree(G->d_scan_blocks); cudaFree(G->d_scalars); cudaFree(G->d_freqtab); cudaFree(G->d_eff);
     if (G->ev_table) cudaEventDestroy(G->ev_table);
     cudaFree(G->d_acc32_b); cudaFree(G->d_acc_b);
+    for (int i = 0; i < 2; ++i) { cudaFree(G->d_slab_q[i]); cudaFree(G->d_slab_cnt[i]); cudaFree(G->d_hot64[i]); }
     if (G->aux) cudaStreamDestroy(G->aux);
     if (G->ev_fork) cudaEventDestroy(G->ev_fork);
     if (G->ev_join) cudaEventDestroy(G->ev_join);
@@ -2712,6 +3071,8 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     else if (k == "hot_cache" && (value == 0 || value == 1)) G->opt_hot_cache = (int)value;
     else if (k == "stats" && (value == 0 || value == 1)) G->opt_stats = (int)value;
     else if (k == "kernel" && value >= 0 && value <= 2) G->opt_kernel = (int)value;
+    else if (k == "slabs" && value >= 0 && value <= 62) G->opt_slabs = (int)value;
+    else if (k == "slab_sweeps" && value >= 0 && value <= 64) G->opt_slab_sweeps = (int)value;
     else if (k == "overlap" && (value == 0 || value == 1)) G->opt_overlap = (int)value;
     else if (k == "carveout" && value >= -1 && value <= 100) G->opt_carveout = (int)value;
     else if (k == "acc32" && (value == 0 || value == 1)) G->opt_acc32 = (int)value;

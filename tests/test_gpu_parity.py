@@ -344,6 +344,30 @@ def test_production_kernels_walk_the_same_paths():
     G.close()
 
 
+@pytest.mark.parametrize("n_slabs,sweeps", [(2, 0), (5, 0), (12, 1), (4, 6)])
+def test_slab_blocked_launch_walks_the_same_paths(n_slabs, sweeps):
+    """z-slab blocking (packages suspended at slab boundaries and resumed from queues) changes the order in which the
+    cell-steps are made, not the steps: identical cell-step, scattering and termination counts as photon_q_kernel in one
+    launch; per-cell energies equal up to the order of the fp32 additions.  sweeps = 1 leaves most packages to the final
+    whole-grid phase; frequencies 7 and 5 scatter back and forth across the slab boundaries."""
+    P = inputs.make_config("5", n=48, n_packages=300_000, n_freq=8)
+    G = soc.Grid.from_problem(P)
+    G.set_option("kernel", 2)
+    for f in (0, 5, 7):
+        G.set_option("slabs", 1)
+        A1, r1, _ = gpu_packages(G, P, f, P.sources(f), P.n_packages, 3, flags=PROD, want_replay=False)
+        G.set_option("slabs", n_slabs)
+        G.set_option("slab_sweeps", sweeps)
+        A2, r2, _ = gpu_packages(G, P, f, P.sources(f), P.n_packages, 3, flags=PROD, want_replay=False)
+        assert (r1["cell_steps"], r1["scatterings"], r1["terminated"]) == (r2["cell_steps"], r2["scatterings"], r2["terminated"])
+        assert r1["emitted"] == pytest.approx(r2["emitted"], rel=1e-12)
+        assert r1["escaped"] == pytest.approx(r2["escaped"], rel=1e-9)
+        assert r1["absorbed"] == pytest.approx(r2["absorbed"], rel=1e-9)
+        assert rel_l1(A2, A1) <= 2e-6
+        assert A2.sum() == pytest.approx(r2["absorbed"], rel=2e-6)
+    G.close()
+
+
 @pytest.mark.parametrize("which,n_sub", [("3", 60_000), ("5", 40_000)])
 def test_production_full_size_subset_against_oracle(which, n_sub):
     """Full-size grid and package count, production mode, the kernel bench.py times (chosen by working-set size):
