@@ -893,6 +893,21 @@ __device__ __forceinline__ void absorb(float w, float x, float &w_new, float &de
     dep = lo ? d_lo : w - w_hi;
 }
 
+// the same, bit for bit, with the exponential behind a warp-uniform branch: at most wavelengths no lane of a warp ever has
+// x >= 1/8, and expf is a fifth of the arithmetic of a cell-step
+__device__ __forceinline__ void absorb_v(float w, float x, float &w_new, float &dep)
+{
+    const float small = x * fmaf(x, fmaf(x, fmaf(x, fmaf(x, 1.0f / 120.0f, -1.0f / 24.0f), 1.0f / 6.0f), -0.5f), 1.0f);
+    const bool lo = x < 0.125f;
+    const float d_lo = w * small;
+    w_new = w - d_lo;
+    dep = d_lo;
+    if (__any_sync(__activemask(), !lo)) {
+        const float w_hi = w * expf(-x);
+        if (!lo) { w_new = w_hi; dep = w - w_hi; }
+    }
+}
+
 // a9: weight with which a package leaves the grid, relative to its initial energy.  The sum of the deposits
 // (`absrel`) resolves a small absorbed fraction, the running weight a small remainder: take the one that is accurate
 // (they differ by accumulated fp32 rounding only)
@@ -1183,7 +1198,8 @@ struct QPkg {
     uint32_t steps;         // REPLAY only
     unsigned long long hash;
     uint32_t n_ld, n_red;   // REPLAY only (option "stats"): gathers / reductions issued for this package
-    int sl;                 // SLAB only: the z-slab the package is confined to, -1 = not confined
+    int lo;                 // SLAB only: the package is confined to the ids [lo, lo + span) of its z-slab;
+    unsigned span;          // not confined: lo = 0, span = 2^32 - 1
 };
 
 __device__ __forceinline__ int v_src(int sd) { return sd < 0 ? -1 : (sd >> 16); }
@@ -1242,7 +1258,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
     unsigned long long acc_ld = 0, acc_red = 0;  // REPLAY variant: request counters (option "stats")
     QPkg p;
     p.n_ld = 0; p.n_red = 0;
-    p.sd = -1; p.w = 0.0f; p.absrel = 0.0f; p.scat = 0; p.rel = 0; p.idx = 0; p.steps = 0; p.hash = 0; p.sl = -1;
+    p.sd = -1; p.w = 0.0f; p.absrel = 0.0f; p.scat = 0; p.rel = 0; p.idx = 0; p.steps = 0; p.hash = 0; p.lo = 0; p.span = 0xffffffffu;
     p.q0 = p.q1 = p.q2 = p.q3 = 0u; p.pend = 0.0f; p.prel = 0.0f;
     p.fx = p.fy = p.fz = 0.5f; p.dx = p.dy = 0.0f; p.dz = 1.0f; p.rx = p.ry = p.rz = 1.0f; p.tau_rem = 0.0f;
     int need = EMPTY;
@@ -1278,7 +1294,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                     if (REPLAY) { acc_ld += p.n_ld; acc_red += p.n_red; }
                     need = EMPTY;
                 } else {
-                    p.sl = -1;
+                    p.lo = 0; p.span = 0xffffffffu;
                     q_load(P, p);
                     need = RUN;
                 }
@@ -1292,7 +1308,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
         const int n_park = 32 - __popc(m_run) - n_dead;
         if (n_park > 0 && (n_park >= T || m_run == 0u)) {
             // ---------------------------------------------------------------- service, all parked lanes together
-            if (SLAB) push(need == SUSP, p.sl + (p.rel >= (p.sl + 1) * P.slab.slab_ids ? 1 : -1));
+            if (SLAB) push(need == SUSP, p.lo / P.slab.slab_ids + (p.rel >= p.lo + P.slab.slab_ids ? 1 : -1));
             if (need == DONE) {                  // retire the finished package
                 q_flush(P, p, s_acc);
                 const int src = v_src(p.sd);
@@ -1302,6 +1318,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                 s_tot[1][threadIdx.x] += esc;
                 s_tot[2][threadIdx.x] += (double)p.absrel * e0;
                 s_cnt[0][threadIdx.x] += p.scat;
+                if (p.w == 0.0f) s_cnt[1][threadIdx.x] += 1u;            // terminated (a package that escapes has w >= 1e-9)
                 if (REPLAY) {
                     acc_ld += p.n_ld; acc_red += p.n_red;
                     if (P.replay) {
@@ -1377,10 +1394,11 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                 p.prel = package_rel(P, src);
                 p.pend = 0.0f;
                 p.n_ld = 0; p.n_red = 0;
-                p.sl = -1;
+                p.lo = 0; p.span = 0xffffffffu;
                 if (!P.slab.final_phase) {
                     const int sl = p.rel / P.slab.slab_ids;
-                    p.sl = sl < P.slab.n_slabs ? sl : P.slab.n_slabs - 1;
+                    p.lo = (sl < P.slab.n_slabs ? sl : P.slab.n_slabs - 1) * P.slab.slab_ids;
+                    p.span = (unsigned)P.slab.slab_ids;
                 }
                 q_load(P, p);
                 need = RUN;
@@ -1418,7 +1436,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
             if (SLAB && exhausted && !P.slab.final_phase) {
                 // the queue has run dry: the phase ends here for this warp.  Its running packages (those still confined to
                 // a slab) are handed to the next phase in mid-cell: deposits so far to the sums, sums to the accumulator
-                const bool dump = need == RUN && p.sl >= 0;
+                const bool dump = need == RUN && p.span != 0xffffffffu;
                 if (dump) {
                     if (p.sd >= 0 && (p.sd & 0x200)) {
                         const int j = (p.sd & 7) + hot_side * (((p.sd >> 3) & 7) + hot_side * ((p.sd >> 6) & 7));
@@ -1452,7 +1470,8 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
             const bool ax0 = tx == ts, ax1 = !ax0 && ty == ts;           // lowest axis wins a tie (reading S4)
             const float da = ax0 ? p.dx : (ax1 ? p.dy : p.dz);
             const bool fwd = da > 0.0f;
-            const int bstride = ax0 ? 8 : (ax1 ? P.bsy : P.bsz);          // to the same slot of the next brick
+            const int bstride = ax0 ? 8 : (ax1 ? P.bsy : P.bsz);          // to the same slot of the next brick (selected
+                                                                          // here, not where it is used: measured)
             const int abit = ax0 ? 1 : (ax1 ? 2 : 4);
             const float gx = __saturatef(fmaf(ts, p.dx, p.fx));           // position after a crossing
             const float gy = __saturatef(fmaf(ts, p.dy, p.fy));
@@ -1467,7 +1486,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                 const bool sc = dtau >= p.tau_rem && ksr > 0.0f;
                 const float x = sc ? p.tau_rem * P.kratio : ts * (rho * P.kabs);
                 float w_new, dep;
-                absorb(p.w, x, w_new, dep);
+                absorb_v(p.w, x, w_new, dep);
                 const bool term = w_new < (float)kWMin;                  // a9: residual stays in the cell
                 if (term) { dep = p.w; w_new = 0.0f; }
                 p.pend += dep;
@@ -1497,8 +1516,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                     p.pend = 0.0f;
                 }
                 if (term) {
-                    s_cnt[1][threadIdx.x] += 1u;
-                    need = DONE;                 // the service block flushes the half-brick sums
+                    need = DONE;                 // the service block flushes the half-brick sums and counts the termination
                 } else if (sc) {
                     need = SCAT;                 // the segment is finished in the service block
                 } else {
@@ -1519,8 +1537,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                         int rel = p.rel ^ abit;
                         if (!inside) rel += fwd ? bstride : -bstride;
                         p.rel = rel;
-                        if (SLAB && p.sl >= 0 && (unsigned)(rel - p.sl * P.slab.slab_ids) >= (unsigned)P.slab.slab_ids)
-                            need = SUSP;         // into the next slab
+                        if (SLAB && (unsigned)(rel - p.lo) >= p.span) need = SUSP;      // into the next slab
                         else q_load(P, p);
                     } else {
                         p.rel ^= abit;
@@ -2753,16 +2770,20 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         const bool big = 8ll * G->n_int > (64ll << 20) && P.ksca * G->rho_mean * n_max < 12.0;
         const bool v2 = !hier && acc32 && (G->opt_kernel == 2 || (G->opt_kernel == 0 && big)) && pkg_count < (1ll << 32);
         if (v2) F.service_threshold = auto_threshold;
-        // z-slab blocking: working set per launch <= ~20 MB, so that gathers and reductions hit L2
+        // z-slab blocking: the cell words and the accumulator of one slab stay in L2 while it is served.
+        // Two slabs of 70 MB serve config 5 on B200 (126 MB of L2) as well as four or eight do (same hit rate, 3 GB of DRAM
+        // traffic per frequency against 54 GB) with the fewest suspensions; where packages scatter so often that the walk
+        // is bound by the service passes (scattering depth of the box >= 12) photon_fast_kernel without slabs is faster
         int n_slabs = G->opt_slabs;
-        if (n_slabs == 0) n_slabs = 8ll * G->n_int > (64ll << 20) ? (int)((8ll * G->n_int + (20ll << 20) - 1) / (20ll << 20)) : 1;
+        if (n_slabs == 0) n_slabs = 8ll * G->n_int > (96ll << 20) ? (int)((8ll * G->n_int + (80ll << 20) - 1) / (80ll << 20)) : 1;
         if (n_slabs > G->nbz / 2) n_slabs = G->nbz / 2;
         if (n_slabs > kMaxSlabs) n_slabs = kMaxSlabs;
-        const bool slab = !hier && acc32 && !rep && F.dust.n_dust == 0 && n_slabs >= 2 && G->opt_kernel != 1 &&
-                          pkg_count <= (1ll << 24);
+        const bool slab = !hier && acc32 && !rep && F.dust.n_dust == 0 && n_slabs >= 2 && pkg_count <= (1ll << 24) &&
+                          (G->opt_kernel == 2 || (G->opt_kernel == 0 && P.ksca * G->rho_mean * n_max < 12.0));
         if (slab) {
-            const double depth = P.ksca * G->rho_mean * n_max;
-            const int sweeps = G->opt_slab_sweeps > 0 ? G->opt_slab_sweeps : (depth < 0.3 ? 2 : (depth < 3.0 ? 4 : 6));
+            // one sweep up, one down; what scatters back across a slab boundary after that is left to the last, whole-grid
+            // phase (more sweeps were slower at every scattering depth)
+            const int sweeps = G->opt_slab_sweeps > 0 ? G->opt_slab_sweeps : 2;
             F.service_threshold = auto_threshold;
             rc = G->opt_stats ? launch_slab<true>(G, F, n_slabs, sweeps, w_eff, absorbed, st)
                               : launch_slab<false>(G, F, n_slabs, sweeps, w_eff, absorbed, st);

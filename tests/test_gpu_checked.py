@@ -64,6 +64,15 @@ for k in (1, 2):
     G.iterate([C3.sources(f) for f in range(C3.n_freq)], C3.n_packages, 1, [30000], C3.t_scale, C3.table_T, C3.e_min, C3.e_max, A, T,
               mode="weighted", cap=300, ali=True)
 G.close()
+# slab-blocked launches (queues, suspension, dump at the end of a phase), with and without the "stats" counters
+C5 = inputs.make_config("5", n=20, n_packages=60000, n_freq=4)
+G = soc.Grid.from_problem(C5)
+G.set_option("kernel", 2)
+for n_slabs, sweeps, stats in ((2, 0, 0), (5, 3, 0), (3, 1, 1)):
+    G.set_option("slabs", n_slabs); G.set_option("slab_sweeps", sweeps); G.set_option("stats", stats)
+    for f in range(C5.n_freq):
+        gpu_packages(G, C5, f, C5.sources(f), C5.n_packages, 2, flags=PROD, want_replay=False)
+G.close()
 print("VIOLATIONS", soc.checked_violations(), "LAUNCHES", soc.launch_count())
 '''
 
