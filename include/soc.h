@@ -244,9 +244,14 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
 /* Tuning knobs (all have defaults chosen for B200): "blocks_per_sm", "threads", "refill_threshold" (replay
  * kernel), "service_threshold" (parked lanes that trigger a service pass), "hot_cache" (0/1: shared partial sums
  * for the cells around point sources), "stats" (0/1: the production kernels count their gather and reduction
- * instructions into soc_freq_result; a slower kernel variant, for measurement runs), "acc32" (0/1: fp32 per-launch accumulator), "overlap" (0/1: soc_simulate_spectrum overlaps consecutive frequencies on two streams), "kernel" (production kernel on
+ * instructions, and the 16-byte loads / stores of queued package states, into soc_freq_result; a slower kernel variant,
+ * for measurement runs), "acc32" (0/1: fp32 per-launch accumulator), "overlap" (0/1: soc_simulate_spectrum overlaps consecutive frequencies on two streams), "kernel" (production kernel on
  * regular grids: 0 = chosen by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel), "carveout"
- * (preferred shared-memory carve-out in %, -1 = driver default); and
+ * (preferred shared-memory carve-out in %, -1 = driver default), "slabs" (regular grids whose cell words + fp32
+ * accumulator exceed L2: number of z-slabs a frequency is served in -- a package that crosses a slab boundary waits in a
+ * device queue for that slab's turn; 0 = by working-set size, 1 = off; the queues take 48 bytes x packages of the launch
+ * x slabs of device memory per accumulator set), "slab_sweeps" (sweeps over the slabs before the last, whole-grid launch
+ * of a frequency; 0 = 2); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
  * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
 int soc_set_option(soc_grid *grid, const char *key, int64_t value);

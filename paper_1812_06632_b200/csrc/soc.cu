@@ -806,10 +806,12 @@ __device__ __forceinline__ bool fast_descend(const FastParams &P, FPkg &p)
     p.n_ld += 1;
     if (cw == kSentinel) { p.cw = cw; return false; }
     while ((int32_t)cw < 0) {
-        int slot = 0;
-        if (p.fx >= 0.5f) { slot |= 1; p.fx = 2.0f * p.fx - 1.0f; } else p.fx = 2.0f * p.fx;
-        if (p.fy >= 0.5f) { slot |= 2; p.fy = 2.0f * p.fy - 1.0f; } else p.fy = 2.0f * p.fy;
-        if (p.fz >= 0.5f) { slot |= 4; p.fz = 2.0f * p.fz - 1.0f; } else p.fz = 2.0f * p.fz;
+        // 2 f and 2 f - 1 are exact in fp32: one fused operation per axis gives the bits of the two-step form
+        const bool bx = p.fx >= 0.5f, by = p.fy >= 0.5f, bz = p.fz >= 0.5f;
+        p.fx = fmaf(p.fx, 2.0f, bx ? -1.0f : 0.0f);
+        p.fy = fmaf(p.fy, 2.0f, by ? -1.0f : 0.0f);
+        p.fz = fmaf(p.fz, 2.0f, bz ? -1.0f : 0.0f);
+        const int slot = (bx ? 1 : 0) | (by ? 2 : 0) | (bz ? 4 : 0);
         p.anc3 = p.anc2; p.anc2 = p.anc1; p.anc1 = p.rel;       // the cell being left becomes the parent
         p.rel = (int)(cw & 0x7fffffffu) + slot;
         p.h *= 0.5f;
@@ -1040,7 +1042,8 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
             const bool sc = dtau >= p.tau_rem && ksr > 0.0f;
             const float x = sc ? p.tau_rem * P.kratio : tsh * (rho * P.kabs);
             float w_new, dep;
-            absorb(p.w, x, w_new, dep);
+            if (HIER) absorb_v(p.w, x, w_new, dep);      // (measured: the branch pays on the octree, not on the regular grids)
+            else absorb(p.w, x, w_new, dep);
             const bool term = w_new < (float)kWMin;                  // a9: residual stays in the cell
             if (term) { dep = p.w; w_new = 0.0f; }
             p.pend += dep;
@@ -1091,11 +1094,16 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 bool inside = fwd == ((rel & abit) == 0);
                 if (HIER) {
                     while (!inside && rel >= P.nrp) {
-                        p.fx = (p.fx + (float)(rel & 1)) * 0.5f;
-                        p.fy = (p.fy + (float)((rel >> 1) & 1)) * 0.5f;
-                        p.fz = (p.fz + (float)((rel >> 2) & 1)) * 0.5f;
-                        if (p.anc1 < 0) p.n_ld += 1;
-                        rel = p.anc1 >= 0 ? p.anc1 : __ldg(P.parent + CK((rel - P.nrp) >> 3, P.n_oct));
+                        // (f + b) / 2 = fl(f / 2 + b / 2): halving is exact, so the fused form rounds the same sum once
+                        p.fx = fmaf(p.fx, 0.5f, (rel & 1) ? 0.5f : 0.0f);
+                        p.fy = fmaf(p.fy, 0.5f, (rel & 2) ? 0.5f : 0.0f);
+                        p.fz = fmaf(p.fz, 0.5f, (rel & 4) ? 0.5f : 0.0f);
+                        if (p.anc1 >= 0) {
+                            rel = p.anc1;
+                        } else {                 // the lane does not know this ancestor: reverse link of the octet
+                            rel = __ldg(P.parent + CK((rel - P.nrp) >> 3, P.n_oct));
+                            p.n_ld += 1;
+                        }
                         p.anc1 = p.anc2; p.anc2 = p.anc3; p.anc3 = -1;
                         p.h *= 2.0f;
                         inside = fwd == ((rel & abit) == 0);
@@ -1291,7 +1299,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                     P.slab.qa[e] = make_uint4(__float_as_uint(p.fx), __float_as_uint(p.fy), __float_as_uint(p.fz), __float_as_uint(p.tau_rem));
                     P.slab.qb[e] = make_uint4(__float_as_uint(p.dx), __float_as_uint(p.dy), __float_as_uint(p.dz), __float_as_uint(p.w));
                     P.slab.qc[e] = make_uint4(__float_as_uint(p.absrel), tag, (uint32_t)p.rel, p.scat);
-                    if (REPLAY) { acc_ld += p.n_ld; acc_red += p.n_red; }
+                    if (REPLAY) { acc_ld += p.n_ld; acc_red += p.n_red + 3; }        // + the three 16-byte stores of the state
                     need = EMPTY;
                 } else {
                     p.lo = 0; p.span = 0xffffffffu;
@@ -1393,7 +1401,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                 }
                 p.prel = package_rel(P, src);
                 p.pend = 0.0f;
-                p.n_ld = 0; p.n_red = 0;
+                p.n_ld = 3; p.n_red = 0;         // ("stats": the three 16-byte loads of the state count as gathers)
                 p.lo = 0; p.span = 0xffffffffu;
                 if (!P.slab.final_phase) {
                     const int sl = p.rel / P.slab.slab_ids;
