@@ -111,6 +111,9 @@ typedef struct {
                                             (cell words, reverse links) and reduction instructions (red.global.add) the
                                             lanes issued -- the request counts behind bench.py's roofline.components;
                                             0 otherwise */
+    uint64_t suspensions, queue_refusals;     /* slab-blocked launches (option "slabs"): package states written to a queue
+                                            (slab crossings and end-of-phase hand-overs), and packages a full queue
+                                            refused, which walked on unconfined; 0 otherwise */
 } soc_freq_result;
 
 /* per-package replay record (DEVICE array written by soc_simulate_packages) */
@@ -251,7 +254,9 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
  * accumulator exceed L2: number of z-slabs a frequency is served in -- a package that crosses a slab boundary waits in a
  * device queue for that slab's turn; 0 = by working-set size, 1 = off; the queues take 48 bytes x packages of the launch
  * x slabs of device memory per accumulator set), "slab_sweeps" (sweeps over the slabs before the last, whole-grid launch
- * of a frequency; 0 = 2); and
+ * of a frequency; 0 = 2), "slab_queue_limit" (test hook: entries a slab / leftover queue accepts from the walk before it
+ * refuses packages; 0 = its capacity), "slab_chunk" (test hook: packages per sequence of phases, 0 = 2^24: a frequency of
+ * more packages is served in several sequences); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
  * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
 int soc_set_option(soc_grid *grid, const char *key, int64_t value);
@@ -306,6 +311,12 @@ int64_t soc_checked_violations(void);
 
 /* Number of kernel launches issued by this library in the calling process (bench.py's "gpu_launches"). */
 uint64_t soc_launch_count(void);
+
+/* The package queues of slab-blocked launches (option "slabs": ~1 GB per accumulator set for 1e7 packages in two slabs)
+ * outlive the grid that allocated them: soc_grid_destroy hands them to a process-wide cache of at most two buffers, from
+ * which the next grid takes them (soc_run_host creates a grid per call; cudaMalloc / cudaFree of buffers this size cost
+ * 0.1-0.2 s each).  This call frees the cache (device synchronised).  Returns the number of bytes released. */
+int64_t soc_release_cached_memory(void);
 
 const char *soc_last_error(void);
 const char *soc_version(void);

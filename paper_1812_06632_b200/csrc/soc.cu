@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -22,6 +23,12 @@ namespace {
 
 thread_local std::string g_last_error;
 unsigned long long g_launches = 0;
+
+// process-wide cache of the package-queue buffers of slab-blocked launches (see soc_release_cached_memory in soc.h)
+struct CachedBuffer { void *ptr; size_t entries; int device; };
+std::vector<CachedBuffer> g_queue_cache;
+std::mutex g_queue_cache_mutex;
+constexpr size_t kQueueCacheMax = 2;
 
 int fail(int code, const std::string &msg)
 {
@@ -62,6 +69,7 @@ struct DevResult {                      // one slot per launch, accumulated with
     unsigned long long cell_steps, scatterings, terminated;
     unsigned int drift_bits, pad_;      // fp32 bits of max |w - (1 - sum of deposits)| over the packages that escaped
     unsigned long long gathers, reds;   // option "stats": global-memory gather / reduction instructions issued by the lanes
+    unsigned long long suspensions, refusals;   // slab-blocked launches: states queued by the walk / refused by a full queue
 };
 
 // f1: dust re-emission, the third package source.  Package ids [n_const, n_const + n_dust)
@@ -157,7 +165,9 @@ struct soc_grid {
     int opt_kernel = 0;                       // regular grids: 0 = by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel
     // z-slab blocking (SlabParams): package queues of the two accumulator sets
     int opt_slabs = 0;                        // 0 = by working-set size, 1 = off, n >= 2 = n slabs
-    int opt_slab_sweeps = 0;                  // sweeps over the slabs before the final whole-grid phase; 0 = by scattering depth
+    int opt_slab_sweeps = 0;                  // sweeps over the slabs before the final whole-grid phase; 0 = 2
+    long long opt_slab_queue_limit = 0;       // test hook: entries a queue accepts from the walk; 0 = its capacity
+    long long opt_slab_chunk = 0;             // test hook: packages per sequence of phases; 0 = 2^24
     double *d_hot64[2] = {nullptr, nullptr};  // hot-cell sums of the two accumulator sets (FastParams::hot64)
     uint4 *d_slab_q[2] = {nullptr, nullptr};  // 3 arrays of n_slabs * cap entries
     unsigned *d_slab_cnt[2] = {nullptr, nullptr};
@@ -690,8 +700,10 @@ constexpr int kSlabChunk = 16;         // queue slots a warp claims at a time
 struct SlabParams {
     uint4 *qa, *qb, *qc;                // all queues, queue q from slab_qbase(q): (fx, fy, fz, tau_rem), (dx, dy, dz, w),
                                         // (absrel, idx | (src + 1) << 25, rel, scat)
-    unsigned *cnt;                      // [64][4]: head, tail, frozen, -; then the count of finished blocks
+    unsigned *cnt;                      // [64][4]: head, tail, frozen, entries written by slab_emit_kernel; then the count of
+                                        // finished blocks
     unsigned cap, cap_left;             // entries per slab queue / per leftover queue
+    unsigned limit, limit_left;         // entries a queue accepts before it refuses a package (= cap, cap_left; less: test hook)
     int n_slabs, slab_ids;              // ids per slab = brick layers per slab * 8 nbx nby
     int q_left;                         // the leftover queue this launch pops (n_slabs or n_slabs + 1); it dumps to the other
     int s_first, s_last;                // slab queues this launch pops, in this order
@@ -716,7 +728,10 @@ __device__ __forceinline__ void slab_epilogue(const SlabParams &S, bool pops)
         const int q = threadIdx.x;
         volatile unsigned *c = S.cnt + 4 * q;
         if (pops && (q == S.q_left || (q >= S.s_first && q <= S.s_last))) c[0] = c[2];
-        const unsigned cap = q < S.n_slabs ? S.cap : S.cap_left, t = c[1];
+        const unsigned t = c[1];
+        if (!pops) c[3] = t;                     // slab_emit_kernel: its entries are all in (it never fills a queue)
+        unsigned cap = q < S.n_slabs ? S.limit : S.limit_left;
+        cap = cap > c[3] ? cap : c[3];
         c[1] = c[2] = t < cap ? t : cap;
         if (q == 0) S.cnt[4 * 64] = 0u;
     }
@@ -776,6 +791,8 @@ struct FPkg {
     long long id;
     unsigned long long hash;
     uint32_t n_ld, n_red;   // REPLAY variants only (option "stats"): gathers / reductions issued for this package
+    uint32_t w_hg, w_az;    // regular grids: words 1, 2 of the current segment's Philox block (the scattering that ends the
+                            // segment takes its angles from them: kept, so that the block is computed once)
 };
 
 // Distance to the exit face along axis a, in cell edges:  t_a = (d_a > 0 ? 1 - f_a : -f_a) / d_a
@@ -1006,7 +1023,8 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 p.fy = __saturatef(fmaf(t_u, p.dy, p.fy));
                 p.fz = __saturatef(fmaf(t_u, p.dz, p.fz));
                 uint32_t s0, w_hg, w_az, s3;     // words 1, 2 of the block of the segment that ends here
-                philox_block(P.seed, P.ifreq, p.id, 2u + p.scat, s0, w_hg, w_az, s3);
+                if (HIER) philox_block(P.seed, P.ifreq, p.id, 2u + p.scat, s0, w_hg, w_az, s3);
+                else { w_hg = p.w_hg; w_az = p.w_az; }
                 scatter_direction<float>(P.g, w_hg, w_az, p.dx, p.dy, p.dz, ndx, ndy, ndz);
                 p.scat += 1;
             }
@@ -1014,6 +1032,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 fast_set_direction(p, ndx, ndy, ndz);
                 uint32_t s0, s1, s2, s3;
                 philox_block(P.seed, P.ifreq, p.id, 2u + p.scat, s0, s1, s2, s3);
+                if (!HIER) { p.w_hg = s1; p.w_az = s2; }                      // (the octree kernel has no registers to spare)
                 p.tau_rem = -__logf(uniform01<float>(s0));                    // a4
                 need = RUN;
                 if (HIER && p.cw == kSentinel) need = DONE;                   // cannot happen for valid sources
@@ -1271,6 +1290,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
     p.fx = p.fy = p.fz = 0.5f; p.dx = p.dy = 0.0f; p.dz = 1.0f; p.rx = p.ry = p.rz = 1.0f; p.tau_rem = 0.0f;
     int need = EMPTY;
     unsigned n_steps = 0;                        // cell-steps of this lane (all its packages)
+    unsigned n_susp = 0, n_refused = 0;          // SLAB: states this lane queued / packages a full queue refused
     unsigned pool_next = 0, pool_end = 0;        // warp-uniform pool of package offsets (SLAB: of queue slots)
     int cur_q = SLAB ? P.slab.s_first - 1 : 0;   // SLAB: position in the list of queues to pop (s_first - 1 = the leftover queue)
     int pool_q = 0;                              // SLAB: the queue the pool was claimed from
@@ -1293,15 +1313,19 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
             b = __shfl_sync(kFull, b, leader);
             if (mine) {
                 const unsigned slot = b + __popc(m & lt_mask);
-                if (slot < (d < P.slab.n_slabs ? P.slab.cap : P.slab.cap_left)) {
+                unsigned room = d < P.slab.n_slabs ? P.slab.limit : P.slab.limit_left;
+                if (slot >= room) { const unsigned emitted = P.slab.cnt[4 * d + 3]; room = room > emitted ? room : emitted; }
+                if (slot < room) {
                     const size_t e = slab_qbase(P.slab, d) + slot;
                     const uint32_t tag = p.idx | ((uint32_t)(v_src(p.sd) + 1) << 25);
                     P.slab.qa[e] = make_uint4(__float_as_uint(p.fx), __float_as_uint(p.fy), __float_as_uint(p.fz), __float_as_uint(p.tau_rem));
                     P.slab.qb[e] = make_uint4(__float_as_uint(p.dx), __float_as_uint(p.dy), __float_as_uint(p.dz), __float_as_uint(p.w));
                     P.slab.qc[e] = make_uint4(__float_as_uint(p.absrel), tag, (uint32_t)p.rel, p.scat);
                     if (REPLAY) { acc_ld += p.n_ld; acc_red += p.n_red + 3; }        // + the three 16-byte stores of the state
+                    n_susp += 1;
                     need = EMPTY;
                 } else {
+                    n_refused += 1;
                     p.lo = 0; p.span = 0xffffffffu;
                     q_load(P, p);
                     need = RUN;
@@ -1604,7 +1628,16 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
         atomicAdd(&P.result->scatterings, (unsigned long long)acc_scat);
         atomicAdd(&P.result->terminated, (unsigned long long)acc_term);
     }
-    if (SLAB) slab_epilogue(P.slab, true);
+    if (SLAB) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            n_susp += __shfl_xor_sync(kFull, n_susp, o);
+            n_refused += __shfl_xor_sync(kFull, n_refused, o);
+        }
+        if (lane == 0 && n_susp) atomicAdd(&P.result->suspensions, (unsigned long long)n_susp);
+        if (lane == 0 && n_refused) atomicAdd(&P.result->refusals, (unsigned long long)n_refused);
+        slab_epilogue(P.slab, true);
+    }
 }
 
 // a1-a4 for a slab-blocked launch: creates every package of the launch (position, direction, first free path) and puts
@@ -2472,8 +2505,10 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
 // Slab-blocked launch of one frequency on a regular grid (SlabParams): create the packages, sweep the z-slabs up and down
 // `sweeps` times with photon_q_kernel<., ., SLAB> confined to one slab per launch, then one whole-grid launch that takes
 // what is still queued (packages that scattered back across a slab boundary after the last sweep).
+// `last`: the launch ends the frequency (a frequency of more than 2^24 packages is served in several such launches): the
+// internal accumulator is folded into the caller's array.
 template <bool STATS>
-int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weight, double *absorbed, cudaStream_t st)
+int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weight, double *absorbed, bool last, cudaStream_t st)
 {
     const int sel = G->acc_sel;
     const int threads = 256;
@@ -2506,17 +2541,35 @@ int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weigh
     if (G->slab_q_entries[sel] < entries) {
         if (G->d_slab_q[sel]) { SOC_CUDA(cudaStreamSynchronize(st)); SOC_CUDA(cudaFree(G->d_slab_q[sel])); G->d_slab_q[sel] = nullptr; }
         G->slab_q_entries[sel] = 0;
-        if (cudaMalloc(&G->d_slab_q[sel], 3 * entries * sizeof(uint4)) != cudaSuccess) {
-            cudaGetLastError();
-            return fail(SOC_ENOMEM, "package queues of the slab-blocked launch");
+        // a buffer left by an earlier grid of this process, if one is large enough (the smallest such)
+        std::lock_guard<std::mutex> lock(g_queue_cache_mutex);
+        int best = -1;
+        for (size_t i = 0; i < g_queue_cache.size(); ++i)
+            if (g_queue_cache[i].device == G->device && g_queue_cache[i].entries >= entries &&
+                (best < 0 || g_queue_cache[i].entries < g_queue_cache[best].entries)) best = (int)i;
+        if (best >= 0) {
+            G->d_slab_q[sel] = (uint4 *)g_queue_cache[best].ptr;
+            G->slab_q_entries[sel] = g_queue_cache[best].entries;
+            g_queue_cache.erase(g_queue_cache.begin() + best);
+        } else {
+            if (cudaMalloc(&G->d_slab_q[sel], 3 * entries * sizeof(uint4)) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(SOC_ENOMEM, "package queues of the slab-blocked launch");
+            }
+            G->slab_q_entries[sel] = entries;
         }
-        G->slab_q_entries[sel] = entries;
     }
+    const size_t stride = G->slab_q_entries[sel];    // the three arrays of the buffer are `stride` entries apart
     const size_t cnt_bytes = sizeof(unsigned) * (4 * 64 + 4);
     if (!G->d_slab_cnt[sel]) SOC_CUDA(cudaMalloc(&G->d_slab_cnt[sel], cnt_bytes));
     SlabParams &S = P.slab;
-    S.qa = G->d_slab_q[sel]; S.qb = S.qa + entries; S.qc = S.qb + entries;
+    S.qa = G->d_slab_q[sel]; S.qb = S.qa + stride; S.qc = S.qb + stride;
     S.cnt = G->d_slab_cnt[sel]; S.cap = n_pkg; S.cap_left = (unsigned)cap_left; S.n_slabs = n_slabs;
+    S.limit = S.cap; S.limit_left = S.cap_left;
+    if (G->opt_slab_queue_limit > 0) {
+        if ((unsigned long long)G->opt_slab_queue_limit < S.limit) S.limit = (unsigned)G->opt_slab_queue_limit;
+        if ((unsigned long long)G->opt_slab_queue_limit < S.limit_left) S.limit_left = (unsigned)G->opt_slab_queue_limit;
+    }
     S.slab_ids = ((G->nbz + n_slabs - 1) / n_slabs) * 8 * G->nbx * G->nby;
     SOC_CUDA(cudaMemsetAsync(S.cnt, 0, cnt_bytes, st));
     {
@@ -2536,6 +2589,7 @@ int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weigh
     photon_q_kernel<STATS, false, true><<<blocks, threads, smem, st>>>(P);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
+    if (!last) return SOC_OK;
     if (G->ev_after_photon) {
         SOC_CUDA(cudaEventRecord(G->ev_after_photon, st));
         G->ev_after_photon = nullptr;
@@ -2786,15 +2840,22 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         if (n_slabs == 0) n_slabs = 8ll * G->n_int > (96ll << 20) ? (int)((8ll * G->n_int + (80ll << 20) - 1) / (80ll << 20)) : 1;
         if (n_slabs > G->nbz / 2) n_slabs = G->nbz / 2;
         if (n_slabs > kMaxSlabs) n_slabs = kMaxSlabs;
-        const bool slab = !hier && acc32 && !rep && F.dust.n_dust == 0 && n_slabs >= 2 && pkg_count <= (1ll << 24) &&
+        const bool slab = !hier && acc32 && !rep && F.dust.n_dust == 0 && n_slabs >= 2 &&
                           (G->opt_kernel == 2 || (G->opt_kernel == 0 && P.ksca * G->rho_mean * n_max < 12.0));
         if (slab) {
             // one sweep up, one down; what scatters back across a slab boundary after that is left to the last, whole-grid
             // phase (more sweeps were slower at every scattering depth)
             const int sweeps = G->opt_slab_sweeps > 0 ? G->opt_slab_sweeps : 2;
             F.service_threshold = auto_threshold;
-            rc = G->opt_stats ? launch_slab<true>(G, F, n_slabs, sweeps, w_eff, absorbed, st)
-                              : launch_slab<false>(G, F, n_slabs, sweeps, w_eff, absorbed, st);
+            // a queued state carries its package index in 24 bits: at most 2^24 packages per sequence of phases
+            const long long chunk = G->opt_slab_chunk > 0 ? G->opt_slab_chunk : (1ll << 24);
+            rc = SOC_OK;
+            for (long long b = P.pkg_begin; b < P.pkg_end && rc == SOC_OK; b += chunk) {
+                F.pkg_begin = b; F.pkg_end = b + chunk < P.pkg_end ? b + chunk : P.pkg_end;
+                const bool last = F.pkg_end == P.pkg_end;
+                rc = G->opt_stats ? launch_slab<true>(G, F, n_slabs, sweeps, w_eff, absorbed, last, st)
+                                  : launch_slab<false>(G, F, n_slabs, sweeps, w_eff, absorbed, last, st);
+            }
         } else {
         const int sel = (v2 ? 8 : 0) | (hier ? 4 : 0) | ((rep || G->opt_stats) ? 2 : 0) | (acc32 ? 1 : 0);
 #define SOC_LF(H, R, A, Q) (F.dust.n_dust > 0 ? launch_fast<H, R, A, Q, true>(G, F, w_eff, absorbed, st) \
@@ -2834,6 +2895,7 @@ int fetch_results(soc_grid *G, int n, soc_freq_result *out, cudaStream_t st)
         std::memcpy(&drift, &G->h_results[i].drift_bits, sizeof(float));
         out[i].weight_drift = (double)drift;
         out[i].gather_requests = G->h_results[i].gathers; out[i].red_requests = G->h_results[i].reds;
+        out[i].suspensions = G->h_results[i].suspensions; out[i].queue_refusals = G->h_results[i].refusals;
     }
     return SOC_OK;
 }
@@ -2856,6 +2918,19 @@ extern "C" {
 const char *soc_last_error(void) { return g_last_error.c_str(); }
 const char *soc_version(void) { return "soc_b200 0.1 (sm_100a)"; }
 uint64_t soc_launch_count(void) { return g_launches; }
+
+int64_t soc_release_cached_memory(void)
+{
+    int64_t bytes = 0;
+    std::lock_guard<std::mutex> lock(g_queue_cache_mutex);
+    if (!g_queue_cache.empty()) cudaDeviceSynchronize();
+    for (const CachedBuffer &b : g_queue_cache) {
+        cudaFree(b.ptr);
+        bytes += (int64_t)(3 * b.entries * sizeof(uint4));
+    }
+    g_queue_cache.clear();
+    return bytes;
+}
 
 int64_t soc_checked_violations(void)
 {
@@ -2880,7 +2955,21 @@ void soc_grid_destroy(soc_grid *G)
     cudaFree(G->d_dust_first); cudaFree(G->d_scan_blocks); cudaFree(G->d_scalars); cudaFree(G->d_freqtab); cudaFree(G->d_eff);
     if (G->ev_table) cudaEventDestroy(G->ev_table);
     cudaFree(G->d_acc32_b); cudaFree(G->d_acc_b);
-    for (int i = 0; i < 2; ++i) { cudaFree(G->d_slab_q[i]); cudaFree(G->d_slab_cnt[i]); cudaFree(G->d_hot64[i]); }
+    for (int i = 0; i < 2; ++i) {
+        if (G->d_slab_q[i]) {                    // the queue buffers go to the process-wide cache (soc.h); the smallest is evicted
+            cudaDeviceSynchronize();
+            std::lock_guard<std::mutex> lock(g_queue_cache_mutex);
+            g_queue_cache.push_back({G->d_slab_q[i], G->slab_q_entries[i], G->device});
+            if (g_queue_cache.size() > kQueueCacheMax) {
+                size_t small = 0;
+                for (size_t k = 1; k < g_queue_cache.size(); ++k)
+                    if (g_queue_cache[k].entries < g_queue_cache[small].entries) small = k;
+                cudaFree(g_queue_cache[small].ptr);
+                g_queue_cache.erase(g_queue_cache.begin() + small);
+            }
+        }
+        cudaFree(G->d_slab_cnt[i]); cudaFree(G->d_hot64[i]);
+    }
     if (G->aux) cudaStreamDestroy(G->aux);
     if (G->ev_fork) cudaEventDestroy(G->ev_fork);
     if (G->ev_join) cudaEventDestroy(G->ev_join);
@@ -3102,6 +3191,8 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     else if (k == "kernel" && value >= 0 && value <= 2) G->opt_kernel = (int)value;
     else if (k == "slabs" && value >= 0 && value <= 62) G->opt_slabs = (int)value;
     else if (k == "slab_sweeps" && value >= 0 && value <= 64) G->opt_slab_sweeps = (int)value;
+    else if (k == "slab_queue_limit" && value >= 0 && value < (1ll << 32)) G->opt_slab_queue_limit = value;
+    else if (k == "slab_chunk" && value >= 0 && value <= (1ll << 24)) G->opt_slab_chunk = value;
     else if (k == "overlap" && (value == 0 || value == 1)) G->opt_overlap = (int)value;
     else if (k == "carveout" && value >= -1 && value <= 100) G->opt_carveout = (int)value;
     else if (k == "acc32" && (value == 0 || value == 1)) G->opt_acc32 = (int)value;

@@ -24,7 +24,8 @@ EXPORTS = ["soc_grid_create", "soc_grid_destroy", "soc_grid_n_total", "soc_freq_
            "soc_simulate_packages", "soc_simulate_spectrum", "soc_update_temperatures", "soc_run_host",
            "soc_set_option", "soc_get_timings", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version",
            "soc_emission_counts", "soc_cell_emission", "soc_update_temperatures_ali", "soc_iterate", "soc_make_map",
-           "soc_checked_violations", "soc_stochastic_create", "soc_stochastic_destroy", "soc_stochastic_emission"]
+           "soc_checked_violations", "soc_stochastic_create", "soc_stochastic_destroy", "soc_stochastic_emission",
+           "soc_release_cached_memory"]
 
 
 class SocError(RuntimeError):
@@ -67,7 +68,8 @@ class IterateRecord(C.Structure):
 class FreqResult(C.Structure):
     _fields_ = [("emitted", C.c_double), ("escaped", C.c_double), ("absorbed", C.c_double),
                 ("cell_steps", C.c_uint64), ("scatterings", C.c_uint64), ("terminated", C.c_uint64),
-                ("weight_drift", C.c_double), ("gather_requests", C.c_uint64), ("red_requests", C.c_uint64)]
+                ("weight_drift", C.c_double), ("gather_requests", C.c_uint64), ("red_requests", C.c_uint64),
+                ("suspensions", C.c_uint64), ("queue_refusals", C.c_uint64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -115,6 +117,7 @@ def load():
     L.soc_get_timings.argtypes = [vp, i32, vp]
     L.soc_probe_throughput.argtypes = [i32, i64, i64, C.POINTER(C.c_float)]
     L.soc_launch_count.restype = u64
+    L.soc_release_cached_memory.restype = i64
     L.soc_checked_violations.restype = i64
     L.soc_last_error.restype = C.c_char_p
     L.soc_version.restype = C.c_char_p
@@ -372,3 +375,7 @@ def probe_throughput(kind, footprint_bytes, n_ops):
 
 def launch_count():
     return int(load().soc_launch_count())
+
+
+def release_cached_memory():
+    return int(load().soc_release_cached_memory())

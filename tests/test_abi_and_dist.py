@@ -76,6 +76,7 @@ def test_argument_validation_without_a_device():
     assert L.soc_simulate_frequency(None, 0, None, 1, 1, 1.0, None, None, 0, None) == -1
     assert L.soc_update_temperatures(None, None, 1.0, None, 2, 1.0, 2.0, None, None) == -1
     assert L.soc_launch_count() == 0
+    assert L.soc_release_cached_memory() == 0                            # nothing cached, no device touched
     assert L.soc_version().startswith(b"soc_b200")
 
 

@@ -344,12 +344,14 @@ def test_production_kernels_walk_the_same_paths():
     G.close()
 
 
-@pytest.mark.parametrize("n_slabs,sweeps", [(2, 0), (5, 0), (12, 1), (4, 6)])
-def test_slab_blocked_launch_walks_the_same_paths(n_slabs, sweeps):
+@pytest.mark.parametrize("n_slabs,sweeps,limit,chunk", [(2, 0, 0, 0), (5, 0, 0, 0), (12, 1, 0, 0), (4, 6, 0, 0), (4, 2, 3000, 0),
+                                                       (3, 2, 0, 70_001)])
+def test_slab_blocked_launch_walks_the_same_paths(n_slabs, sweeps, limit, chunk):
     """z-slab blocking (packages suspended at slab boundaries and resumed from queues) changes the order in which the
     cell-steps are made, not the steps: identical cell-step, scattering and termination counts as photon_q_kernel in one
     launch; per-cell energies equal up to the order of the fp32 additions.  sweeps = 1 leaves most packages to the final
-    whole-grid phase; frequencies 7 and 5 scatter back and forth across the slab boundaries."""
+    whole-grid phase; frequencies 7 and 5 scatter back and forth across the slab boundaries; limit > 0 makes the queues
+    refuse packages (a refused package walks on, not confined to a slab), which must not change a count either."""
     P = inputs.make_config("5", n=48, n_packages=300_000, n_freq=8)
     G = soc.Grid.from_problem(P)
     G.set_option("kernel", 2)
@@ -358,7 +360,11 @@ def test_slab_blocked_launch_walks_the_same_paths(n_slabs, sweeps):
         A1, r1, _ = gpu_packages(G, P, f, P.sources(f), P.n_packages, 3, flags=PROD, want_replay=False)
         G.set_option("slabs", n_slabs)
         G.set_option("slab_sweeps", sweeps)
+        G.set_option("slab_queue_limit", limit)
+        G.set_option("slab_chunk", chunk)       # > 0: the 300 000 packages in five sequences of phases (a ragged last one)
         A2, r2, _ = gpu_packages(G, P, f, P.sources(f), P.n_packages, 3, flags=PROD, want_replay=False)
+        assert r1["suspensions"] == 0 and r2["suspensions"] > 0
+        assert (r2["queue_refusals"] > 0) == (limit > 0)
         assert (r1["cell_steps"], r1["scatterings"], r1["terminated"]) == (r2["cell_steps"], r2["scatterings"], r2["terminated"])
         assert r1["emitted"] == pytest.approx(r2["emitted"], rel=1e-12)
         assert r1["escaped"] == pytest.approx(r2["escaped"], rel=1e-9)
@@ -366,6 +372,26 @@ def test_slab_blocked_launch_walks_the_same_paths(n_slabs, sweeps):
         assert rel_l1(A2, A1) <= 2e-6
         assert A2.sum() == pytest.approx(r2["absorbed"], rel=2e-6)
     G.close()
+
+
+def test_queue_buffers_are_cached_across_grids():
+    """The package queues of a slab-blocked launch go to a process-wide cache when their grid is destroyed and are taken
+    from it by the next grid (soc_run_host creates a grid per call); soc_release_cached_memory frees them."""
+    soc.release_cached_memory()
+    P = inputs.make_config("5", n=32, n_packages=100_000, n_freq=2)
+    out = []
+    for _ in range(2):
+        G = soc.Grid.from_problem(P)
+        G.set_option("kernel", 2)
+        G.set_option("slabs", 2)
+        A, r, _ = gpu_packages(G, P, 1, P.sources(1), P.n_packages, 5, flags=PROD, want_replay=False)
+        G.close()
+        out.append((A, r))
+    assert out[0][1]["cell_steps"] == out[1][1]["cell_steps"]
+    assert out[0][1]["suspensions"] > 0 and out[1][1]["suspensions"] > 0      # (hand-overs at the end of a phase depend on timing)
+    assert rel_l1(out[1][0], out[0][0]) <= 2e-6
+    assert soc.release_cached_memory() >= 3 * 16 * 2 * 100_000      # at least the two slab queues of one accumulator set
+    assert soc.release_cached_memory() == 0
 
 
 @pytest.mark.parametrize("which,n_sub", [("3", 60_000), ("5", 40_000)])
