@@ -252,7 +252,7 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
  * regular grids: 0 = chosen by working-set size, 1 = photon_fast_kernel, 2 = photon_q_kernel), "carveout"
  * (preferred shared-memory carve-out in %, -1 = driver default), "slabs" (regular grids whose cell words + fp32
  * accumulator exceed L2: number of z-slabs a frequency is served in -- a package that crosses a slab boundary waits in a
- * device queue for that slab's turn; 0 = by working-set size, 1 = off; the queues take 48 bytes x packages of the launch
+ * device queue for that slab's turn; 0 = by working-set size, 1 = off; the queues take 52 bytes x packages of the launch
  * x slabs of device memory per accumulator set), "slab_sweeps" (sweeps over the slabs before the last, whole-grid launch
  * of a frequency; 0 = 2), "slab_queue_limit" (test hook: entries a slab / leftover queue accepts from the walk before it
  * refuses packages; 0 = its capacity), "slab_chunk" (test hook: packages per sequence of phases, 0 = 2^24: a frequency of

@@ -29,6 +29,7 @@ struct CachedBuffer { void *ptr; size_t entries; int device; };
 std::vector<CachedBuffer> g_queue_cache;
 std::mutex g_queue_cache_mutex;
 constexpr size_t kQueueCacheMax = 2;
+constexpr size_t kQueueEntryBytes = 3 * 16 + 4;    // three uint4 arrays and one float array (SlabParams)
 
 int fail(int code, const std::string &msg)
 {
@@ -699,7 +700,9 @@ constexpr int kMaxSlabs = 62;          // + 2 leftover queues = 64 queues
 constexpr int kSlabChunk = 16;         // queue slots a warp claims at a time
 struct SlabParams {
     uint4 *qa, *qb, *qc;                // all queues, queue q from slab_qbase(q): (fx, fy, fz, tau_rem), (dx, dy, dz, w),
-                                        // (absrel, idx | (src + 1) << 25, rel, scat)
+                                        // (absrel, idx | class << 25, rel, scat); class = 0 background or beam, 1 + k point
+                                        // source k, 126 / 127 dust package that has left / not yet left the cell that sent it
+    float *qp;                          // launches with dust packages (f1): energy of the package / e_ref
     unsigned *cnt;                      // [64][4]: head, tail, frozen, entries written by slab_emit_kernel; then the count of
                                         // finished blocks
     unsigned cap, cap_left;             // entries per slab queue / per leftover queue
@@ -1264,7 +1267,6 @@ __device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p, float (*s_
 template <bool REPLAY, bool DUST, bool SLAB>
 __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __grid_constant__ FastParams P)
 {
-    static_assert(!(SLAB && DUST), "slab launches carry constant-source packages only");
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
     // per-launch totals of this thread (touched only in the service block)
@@ -1317,7 +1319,9 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                 if (slot >= room) { const unsigned emitted = P.slab.cnt[4 * d + 3]; room = room > emitted ? room : emitted; }
                 if (slot < room) {
                     const size_t e = slab_qbase(P.slab, d) + slot;
-                    const uint32_t tag = p.idx | ((uint32_t)(v_src(p.sd) + 1) << 25);
+                    const uint32_t cls = (DUST && p.sd <= -2) ? (uint32_t)(129 + p.sd) : (uint32_t)(v_src(p.sd) + 1);
+                    const uint32_t tag = p.idx | (cls << 25);
+                    if (DUST) P.slab.qp[e] = p.prel;
                     P.slab.qa[e] = make_uint4(__float_as_uint(p.fx), __float_as_uint(p.fy), __float_as_uint(p.fz), __float_as_uint(p.tau_rem));
                     P.slab.qb[e] = make_uint4(__float_as_uint(p.dx), __float_as_uint(p.dy), __float_as_uint(p.dz), __float_as_uint(p.w));
                     P.slab.qc[e] = make_uint4(__float_as_uint(p.absrel), tag, (uint32_t)p.rel, p.scat);
@@ -1410,7 +1414,9 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                 p.idx = c.y & 0xffffffu;
                 const int src = (int)(c.y >> 25) - 1;
                 p.sd = -1;
-                if (src >= 0) {
+                if (DUST && src >= 125) {        // a dust package: -3 = has left its cell, -2 = not yet (f3 counts what it leaves there)
+                    p.sd = src - 128;
+                } else if (src >= 0) {
                     // hot-cube tracking (deposits near the package's own source go to the block's partial sums) is not part
                     // of the queued state: the position in the cube follows from the cell
                     p.sd = src << 16;
@@ -1423,7 +1429,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                             p.sd |= 0x200 | hx | (hy << 3) | (hz << 6);
                     }
                 }
-                p.prel = package_rel(P, src);
+                p.prel = (DUST && p.sd <= -2) ? P.slab.qp[e] : package_rel(P, src);
                 p.pend = 0.0f;
                 p.n_ld = 3; p.n_red = 0;         // ("stats": the three 16-byte loads of the state count as gathers)
                 p.lo = 0; p.span = 0xffffffffu;
@@ -1476,6 +1482,8 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                     } else {
                         s_acc[CK(p.rel & 3, 4)][CK(threadIdx.x, 256)] += p.pend * p.prel;
                     }
+                    if (DUST && p.sd == -2 && P.dust.self_abs && p.pend > 0.0f)      // f3: the part left in its own cell so far
+                        atomicAdd(P.dust.self_abs + CK(global_id(P, p.rel), P.n_abi), P.dust.weight * (double)p.pend * ((double)p.prel * P.e_ref));
                     p.pend = 0.0f;
                     q_flush(P, p, s_acc);
                 }
@@ -1655,20 +1663,31 @@ __global__ void __launch_bounds__(256) slab_emit_kernel(const __grid_constant__ 
         const unsigned idx = base + threadIdx.x;
         const bool live = idx < n_pkg;
         FPkg q;
-        float dx = 0.0f, dy = 0.0f, dz = 1.0f, tau = 0.0f;
+        float dx = 0.0f, dy = 0.0f, dz = 1.0f, tau = 0.0f, prel = 0.0f;
         int slab = 0, rel = 0;
         unsigned rank = 0;
         if (live) {
             int ix, iy, iz;
             const long long id = P.pkg_begin + (long long)idx;
             fast_emit_core(P, q, id, ix, iy, iz, dx, dy, dz);
-            rel = root_id(P, ix, iy, iz);
+            if (q.src == -2) {
+                // f1: a dust package starts in the cell that sends it (ix = its global id; regular grid); its energy is the
+                // cell's luminosity over its package count, in units of the launch's reference energy
+                const int gid = ix;
+                rel = root_id(P, gid % P.nx, (gid / P.nx) % P.ny, gid / (P.nx * P.ny));
+                const double e0 = cell_luminosity(P.dust.kabs, P.dust.freq_hz, __ldg(P.cellw + CK(rel, P.n_int)), 0,
+                                                  __ldg(P.dust.T + CK(gid, P.n_abi))) / (double)__ldg(P.dust.count + CK(gid, P.n_abi));
+                prel = (float)(e0 / P.e_ref);
+                acc_emit += (double)prel * P.e_ref;
+            } else {
+                rel = root_id(P, ix, iy, iz);
+                acc_emit += package_e0(P, q.src);
+            }
             uint32_t s0, s1, s2, s3;
             philox_block(P.seed, P.ifreq, id, 2u, s0, s1, s2, s3);
             tau = -__logf(uniform01<float>(s0));                              // a4
             slab = rel / P.slab.slab_ids;
             slab = slab < P.slab.n_slabs ? slab : P.slab.n_slabs - 1;
-            acc_emit += package_e0(P, q.src);
             rank = atomicAdd(s_n + slab, 1u);
         }
         __syncthreads();
@@ -1677,7 +1696,8 @@ __global__ void __launch_bounds__(256) slab_emit_kernel(const __grid_constant__ 
         __syncthreads();
         if (live) {
             const size_t e = slab_qbase(P.slab, slab) + CK(s_base[slab] + rank, P.slab.cap);
-            const uint32_t tag = idx | ((uint32_t)(q.src + 1) << 25);
+            const uint32_t tag = idx | ((q.src == -2 ? 127u : (uint32_t)(q.src + 1)) << 25);
+            if (q.src == -2) P.slab.qp[e] = prel;
             P.slab.qa[e] = make_uint4(__float_as_uint(q.fx), __float_as_uint(q.fy), __float_as_uint(q.fz), __float_as_uint(tau));
             P.slab.qb[e] = make_uint4(__float_as_uint(dx), __float_as_uint(dy), __float_as_uint(dz), __float_as_uint(1.0f));
             P.slab.qc[e] = make_uint4(0u, tag, (uint32_t)rel, 0u);
@@ -2507,7 +2527,7 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
 // what is still queued (packages that scattered back across a slab boundary after the last sweep).
 // `last`: the launch ends the frequency (a frequency of more than 2^24 packages is served in several such launches): the
 // internal accumulator is folded into the caller's array.
-template <bool STATS>
+template <bool STATS, bool DUST>
 int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weight, double *absorbed, bool last, cudaStream_t st)
 {
     const int sel = G->acc_sel;
@@ -2516,7 +2536,7 @@ int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weigh
     const int side = 2 * P.hot_r + 1;
     const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
     int per_sm = 0;
-    SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<STATS, false, true>, threads, smem));
+    SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<STATS, DUST, true>, threads, smem));
     if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
     if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
     int blocks = per_sm * G->n_sm;
@@ -2552,7 +2572,7 @@ int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weigh
             G->slab_q_entries[sel] = g_queue_cache[best].entries;
             g_queue_cache.erase(g_queue_cache.begin() + best);
         } else {
-            if (cudaMalloc(&G->d_slab_q[sel], 3 * entries * sizeof(uint4)) != cudaSuccess) {
+            if (cudaMalloc(&G->d_slab_q[sel], entries * kQueueEntryBytes) != cudaSuccess) {
                 cudaGetLastError();
                 return fail(SOC_ENOMEM, "package queues of the slab-blocked launch");
             }
@@ -2563,7 +2583,7 @@ int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weigh
     const size_t cnt_bytes = sizeof(unsigned) * (4 * 64 + 4);
     if (!G->d_slab_cnt[sel]) SOC_CUDA(cudaMalloc(&G->d_slab_cnt[sel], cnt_bytes));
     SlabParams &S = P.slab;
-    S.qa = G->d_slab_q[sel]; S.qb = S.qa + stride; S.qc = S.qb + stride;
+    S.qa = G->d_slab_q[sel]; S.qb = S.qa + stride; S.qc = S.qb + stride; S.qp = reinterpret_cast<float *>(S.qc + stride);
     S.cnt = G->d_slab_cnt[sel]; S.cap = n_pkg; S.cap_left = (unsigned)cap_left; S.n_slabs = n_slabs;
     S.limit = S.cap; S.limit_left = S.cap_left;
     if (G->opt_slab_queue_limit > 0) {
@@ -2582,11 +2602,11 @@ int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weigh
     for (size_t k = 0; k < phase.size(); ++k) {
         S.s_first = S.s_last = phase[k];
         S.q_left = n_slabs + (int)(k & 1);
-        photon_q_kernel<STATS, false, true><<<blocks, threads, smem, st>>>(P);
+        photon_q_kernel<STATS, DUST, true><<<blocks, threads, smem, st>>>(P);
         g_launches += 1;
     }
     S.s_first = 0; S.s_last = n_slabs - 1; S.q_left = n_slabs + (int)(phase.size() & 1); S.final_phase = 1;
-    photon_q_kernel<STATS, false, true><<<blocks, threads, smem, st>>>(P);
+    photon_q_kernel<STATS, DUST, true><<<blocks, threads, smem, st>>>(P);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     if (!last) return SOC_OK;
@@ -2840,7 +2860,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         if (n_slabs == 0) n_slabs = 8ll * G->n_int > (96ll << 20) ? (int)((8ll * G->n_int + (80ll << 20) - 1) / (80ll << 20)) : 1;
         if (n_slabs > G->nbz / 2) n_slabs = G->nbz / 2;
         if (n_slabs > kMaxSlabs) n_slabs = kMaxSlabs;
-        const bool slab = !hier && acc32 && !rep && F.dust.n_dust == 0 && n_slabs >= 2 &&
+        const bool slab = !hier && acc32 && !rep && n_slabs >= 2 &&
                           (G->opt_kernel == 2 || (G->opt_kernel == 0 && P.ksca * G->rho_mean * n_max < 12.0));
         if (slab) {
             // one sweep up, one down; what scatters back across a slab boundary after that is left to the last, whole-grid
@@ -2853,8 +2873,12 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
             for (long long b = P.pkg_begin; b < P.pkg_end && rc == SOC_OK; b += chunk) {
                 F.pkg_begin = b; F.pkg_end = b + chunk < P.pkg_end ? b + chunk : P.pkg_end;
                 const bool last = F.pkg_end == P.pkg_end;
-                rc = G->opt_stats ? launch_slab<true>(G, F, n_slabs, sweeps, w_eff, absorbed, last, st)
-                                  : launch_slab<false>(G, F, n_slabs, sweeps, w_eff, absorbed, last, st);
+                if (F.dust.n_dust > 0)
+                    rc = G->opt_stats ? launch_slab<true, true>(G, F, n_slabs, sweeps, w_eff, absorbed, last, st)
+                                      : launch_slab<false, true>(G, F, n_slabs, sweeps, w_eff, absorbed, last, st);
+                else
+                    rc = G->opt_stats ? launch_slab<true, false>(G, F, n_slabs, sweeps, w_eff, absorbed, last, st)
+                                      : launch_slab<false, false>(G, F, n_slabs, sweeps, w_eff, absorbed, last, st);
             }
         } else {
         const int sel = (v2 ? 8 : 0) | (hier ? 4 : 0) | ((rep || G->opt_stats) ? 2 : 0) | (acc32 ? 1 : 0);
@@ -2926,7 +2950,7 @@ int64_t soc_release_cached_memory(void)
     if (!g_queue_cache.empty()) cudaDeviceSynchronize();
     for (const CachedBuffer &b : g_queue_cache) {
         cudaFree(b.ptr);
-        bytes += (int64_t)(3 * b.entries * sizeof(uint4));
+        bytes += (int64_t)(b.entries * kQueueEntryBytes);
     }
     g_queue_cache.clear();
     return bytes;
