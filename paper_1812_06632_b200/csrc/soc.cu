@@ -1044,8 +1044,8 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
         }
         if (m_run == 0u) break;                  // nothing parked that can be serviced, nothing running
 
-        // two cell-steps per look at the warp's state: the ballots and the loop overhead are paid once; a lane
-        // that parks in the first step sits out the second
+        // four cell-steps per look at the warp's state: the ballots and the loop overhead are paid once; a lane
+        // that parks in one of them sits out the rest
         auto cell_step = [&]() {
             // ---------------------------------------------------------------- one cell-step (a5-a7, a9)
             const float rho = __uint_as_float(p.cw);
@@ -1262,8 +1262,11 @@ __device__ __forceinline__ void q_flush(const FastParams &P, QPkg &p, float (*s_
     p.n_red += 1;
 }
 
-// SLAB: the launch serves one z-slab of the grid (SlabParams): packages come from the slab's queue instead of the id
-// counter (they were created by slab_emit_kernel), and a package that crosses out of the slab's id range is suspended.
+// SLAB: the launch is one phase of a slab-blocked frequency (SlabParams): packages come from the queues instead of the id
+// counter (they were created by slab_emit_kernel), a package that crosses out of its slab's id range is suspended, and a
+// warp whose queue has run dry hands its running packages to the next phase.  64 registers at 4 CTAs per SM: at 48 the
+// compiler re-materialised the shared-memory addresses of the step (+45 instructions per cell-step), and with the working
+// set in L2 the fifth CTA is worth less than that.
 template <bool REPLAY, bool DUST, bool SLAB>
 __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __grid_constant__ FastParams P)
 {
@@ -1497,8 +1500,8 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
         }
         if (m_run == 0u) break;                  // nothing parked that can be serviced, nothing running
 
-        // two cell-steps per look at the warp's state: the ballots and the loop overhead are paid once; a lane
-        // that parks in the first step sits out the second
+        // four cell-steps per look at the warp's state: the ballots and the loop overhead are paid once; a lane
+        // that parks in one of them sits out the rest
         auto cell_step = [&]() {
             // ---------------------------------------------------------------- one cell-step (a5-a7, a9)
             // the geometry of the step does not need the cell word: it goes first, so that the gather issued by the last
