@@ -169,6 +169,8 @@ struct soc_grid {
     int opt_slab_sweeps = 0;                  // sweeps over the slabs before the final whole-grid phase; 0 = 2
     long long opt_slab_queue_limit = 0;       // test hook: entries a queue accepts from the walk; 0 = its capacity
     long long opt_slab_chunk = 0;             // test hook: packages per sequence of phases; 0 = 2^24
+    int opt_group = 0;                        // frequencies per launch of soc_simulate_spectrum: 0 = by package count, 1..4
+    std::vector<int> slot_group;              // [n_slots] size of the grouped launch that starts at this result slot, else 0
     double *d_hot64[2] = {nullptr, nullptr};  // hot-cell sums of the two accumulator sets (FastParams::hot64)
     uint4 *d_slab_q[2] = {nullptr, nullptr};  // 3 arrays of n_slabs * cap entries
     unsigned *d_slab_cnt[2] = {nullptr, nullptr};
@@ -314,14 +316,14 @@ __device__ __forceinline__ int dust_cell(const DustParams &D, long long id, int 
 // Dust packages (f1): src = -2, ix = global id of the emitting cell, iy = its level - 1; uniform point in the cell,
 // isotropic direction (words 0..2 of block 0 -> position, word 3 -> cos theta, word 0 of block 1 -> azimuth).
 template <typename A, typename PARAMS>
-__device__ __forceinline__ void emit_core(const PARAMS &P, long long id, int &ix, int &iy, int &iz, float &fx, float &fy,
+__device__ __forceinline__ void emit_core(const PARAMS &P, int ifreq, long long id, int &ix, int &iy, int &iz, float &fx, float &fy,
                                           float &fz, A &dx, A &dy, A &dz, int &src)
 {
     src = -1;
     if (!P.is_beam && id >= P.dust.n_const) {
         uint32_t w0, w1, w2, w3, v0, v1, v2, v3;
-        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
-        philox_block(P.seed, P.ifreq, id, 1u, v0, v1, v2, v3);
+        philox_block(P.seed, ifreq, id, 0u, w0, w1, w2, w3);
+        philox_block(P.seed, ifreq, id, 1u, v0, v1, v2, v3);
         ix = dust_cell(P.dust, id, iy);
         iz = 0;
         fx = uniform01<float>(w0); fy = uniform01<float>(w1); fz = uniform01<float>(w2);       // exact in fp32
@@ -349,8 +351,8 @@ __device__ __forceinline__ void emit_core(const PARAMS &P, long long id, int &ix
         dx = (A)P.beam[3]; dy = (A)P.beam[4]; dz = (A)P.beam[5];
     } else if (id < P.n_bg) {
         uint32_t w0, w1, w2, w3, v0, v1, v2, v3;
-        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
-        philox_block(P.seed, P.ifreq, id, 1u, v0, v1, v2, v3);
+        philox_block(P.seed, ifreq, id, 0u, w0, w1, w2, w3);
+        philox_block(P.seed, ifreq, id, 1u, v0, v1, v2, v3);
         // face in proportion to its area, order x-, x+, y-, y+, z-, z+ (exact in fp64 like the definition)
         const double ax = (double)P.ny * P.nz, ay = (double)P.nz * P.nx, az = (double)P.nx * P.ny;
         const double x = uniform01<double>(w0) * P.surf;
@@ -382,7 +384,7 @@ __device__ __forceinline__ void emit_core(const PARAMS &P, long long id, int &ix
         else             { iz = ia; ix = i1; iy = i2; fz = fa; fx = f1; fy = f2; dz = da; dx = d1; dy = d2; }
     } else {
         uint32_t w0, w1, w2, w3;
-        philox_block(P.seed, P.ifreq, id, 0u, w0, w1, w2, w3);
+        philox_block(P.seed, ifreq, id, 0u, w0, w1, w2, w3);
         const int k = (int)((id - P.n_bg) % P.n_point);
         const double px = P.ps_pos[k][0], py = P.ps_pos[k][1], pz = P.ps_pos[k][2];
         ix = (int)floor(px); iy = (int)floor(py); iz = (int)floor(pz);
@@ -432,7 +434,7 @@ __device__ __forceinline__ double emit(const SimParams &P, Pkg<A> &p, long long 
     A dx, dy, dz;
     int src;
     p.id = id;
-    emit_core<A>(P, id, p.ix, p.iy, p.iz, p.fx, p.fy, p.fz, dx, dy, dz, src);
+    emit_core<A>(P, P.ifreq, id, p.ix, p.iy, p.iz, p.fx, p.fy, p.fz, dx, dy, dz, src);
     double e0 = P.is_beam ? 1.0 : (src >= 0 ? P.ps_e0[src] : P.bg_e0);
     set_direction(p, dx, dy, dz);
     p.h = 1.0f;
@@ -740,6 +742,21 @@ __device__ __forceinline__ void slab_epilogue(const SlabParams &S, bool pops)
     }
 }
 
+// Grouped launch: a launch of fewer than ~4e6 packages ends with its blocks waiting for their last
+// long-lived packages (0.4 ms on B200, a quarter of an octree launch of 1e6 packages), so up to kMaxJobs consecutive
+// frequencies share one launch: package g of the launch belongs to job g / job_pkgs, and everything that differs between
+// the frequencies is read per lane from this table.  The jobs add into ONE accumulator in units of e_ref, each with its
+// quadrature weight folded into its package energies (rel = weight * energy / e_ref).
+constexpr int kMaxJobs = 4;
+struct JobParams {
+    float ksca, kabs, kratio, g;
+    float bg_rel, beam_rel;
+    int ifreq, pad_;
+    double bg_e0;
+    double ps_e0[SOC_MAX_POINT_SOURCES];
+    float ps_rel[SOC_MAX_POINT_SOURCES];
+};
+
 struct FastParams {
     int nx, ny, nz;                     // root grid
     int nbx, nby;                       // bricks along x, y of the padded root grid (cell ix sits at X = ix + 2)
@@ -774,6 +791,9 @@ struct FastParams {
     unsigned long long *counter;
     DevResult *result;
     SlabParams slab;
+    int n_jobs;                         // GROUP launches: jobs of the launch; result + j is the slot of job j
+    long long job_pkgs;                 // packages per job: ids [pkg_begin, pkg_begin + job_pkgs) of each frequency
+    JobParams job[kMaxJobs];
 };
 
 struct FPkg {
@@ -796,6 +816,7 @@ struct FPkg {
     uint32_t n_ld, n_red;   // REPLAY variants only (option "stats"): gathers / reductions issued for this package
     uint32_t w_hg, w_az;    // regular grids: words 1, 2 of the current segment's Philox block (the scattering that ends the
                             // segment takes its angles from them: kept, so that the block is computed once)
+    int job;                // GROUP launches: the frequency of the launch this package belongs to
 };
 
 // Distance to the exit face along axis a, in cell edges:  t_a = (d_a > 0 ? 1 - f_a : -f_a) / d_a
@@ -859,19 +880,19 @@ __device__ __forceinline__ long long global_id(const FastParams &P, int rel)
 }
 
 // a1-a3 in the production kernels: the direction is returned, not installed
-__device__ __forceinline__ void fast_emit_core(const FastParams &P, FPkg &p, long long id, int &ix, int &iy, int &iz,
+__device__ __forceinline__ void fast_emit_core(const FastParams &P, FPkg &p, int ifreq, long long id, int &ix, int &iy, int &iz,
                                                float &dx, float &dy, float &dz)
 {
     p.id = id;
-    emit_core<float>(P, id, ix, iy, iz, p.fx, p.fy, p.fz, dx, dy, dz, p.src);
+    emit_core<float>(P, ifreq, id, ix, iy, iz, p.fx, p.fy, p.fz, dx, dy, dz, p.src);
 }
 
 // prel receives the package energy in units of the launch's reference energy
 template <bool HIER>
-__device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, long long id, float &dx, float &dy, float &dz, float &prel)
+__device__ __forceinline__ void fast_emit(const FastParams &P, FPkg &p, int ifreq, long long id, float &dx, float &dy, float &dz, float &prel)
 {
     int ix, iy, iz;
-    fast_emit_core(P, p, id, ix, iy, iz, dx, dy, dz);
+    fast_emit_core(P, p, ifreq, id, ix, iy, iz, dx, dy, dz);
     p.h = 1.0f;
     p.n_ld = 0; p.n_red = 0;
     if (HIER) p.anc1 = p.anc2 = p.anc3 = -1;
@@ -941,9 +962,23 @@ __device__ __forceinline__ double escaped_rel(float w, float absrel)
 
 // DUST: the launch contains dust re-emission packages (f1): per-package energies, in-cell absorption (f3).  Compiled out of
 // the kernels that serve the constant sources, whose step loop it would lengthen (measured: -4 % ... -10 %).
-template <bool HIER, bool REPLAY, bool ACC32, bool DUST>
+// GROUP: the launch carries the packages of several frequencies (JobParams).
+template <bool HIER, bool REPLAY, bool ACC32, bool DUST, bool GROUP>
 __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __grid_constant__ FastParams P)
 {
+    static_assert(!GROUP || (ACC32 && !DUST), "grouped launches: constant sources, fp32 accumulator");
+    // GROUP: totals per warp and job (touched when a package starts or ends): emitted, escaped, absorbed; cell-steps,
+    // scatterings, terminations; weight drift
+    __shared__ double s_jd[GROUP ? 8 : 1][kMaxJobs][3];
+    __shared__ unsigned long long s_jn[GROUP ? 8 : 1][kMaxJobs][3];
+    __shared__ unsigned s_jdrift[GROUP ? 8 : 1][kMaxJobs];
+    const int wid = GROUP ? (threadIdx.x >> 5) : 0;
+    if (GROUP && threadIdx.x < 8 * kMaxJobs) {
+        const int w = threadIdx.x / kMaxJobs, j = threadIdx.x % kMaxJobs;
+        s_jd[w][j][0] = s_jd[w][j][1] = s_jd[w][j][2] = 0.0;
+        s_jn[w][j][0] = s_jn[w][j][1] = s_jn[w][j][2] = 0ull;
+        s_jdrift[w][j] = 0u;
+    }
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
     double acc_emit = 0.0, acc_esc = 0.0, acc_abs = 0.0;
@@ -954,7 +989,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
     FPkg p;
     p.n_ld = 0; p.n_red = 0;
     p.src = -1; p.disp = -1; p.w = 0.0f; p.absrel = 0.0f; p.steps = 0; p.scat = 0; p.cw = 0; p.rel = 0; p.h = 1.0f;
-    p.anc1 = p.anc2 = p.anc3 = -1;
+    p.anc1 = p.anc2 = p.anc3 = -1; p.job = 0;
     int need = EMPTY;
     // hot-cell cache (atomics to the cells around a point source serialise): fp32 partial sums
     // of the deposits (in units of the source's package energy) into the (2R+1)^3 root cells around each source
@@ -974,13 +1009,23 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
         if (m_park && (__popc(m_park) >= T || m_run == 0u)) {
             // ---------------------------------------------------------------- service, all parked lanes together
             if (need == DONE) {                  // retire the finished package
-                const double e0 = (DUST && p.src <= -2) ? (double)s_prel[threadIdx.x] * P.e_ref : package_e0(P, p.src);
+                const double e0 = GROUP ? (p.src >= 0 ? P.job[p.job].ps_e0[p.src] : P.job[p.job].bg_e0)
+                                        : ((DUST && p.src <= -2) ? (double)s_prel[threadIdx.x] * P.e_ref : package_e0(P, p.src));
                 const double esc = escaped_rel(p.w, p.absrel) * e0;
-                if (p.w != 0.0f) acc_drift = fmaxf(acc_drift, fabsf(p.w - (1.0f - p.absrel)));
-                acc_esc += esc;
-                acc_abs += (double)p.absrel * e0;
-                acc_steps += p.steps;
-                acc_scat += p.scat;
+                if (GROUP) {
+                    atomicAdd(&s_jd[wid][p.job][1], esc);
+                    atomicAdd(&s_jd[wid][p.job][2], (double)p.absrel * e0);
+                    atomicAdd(&s_jn[wid][p.job][0], (unsigned long long)p.steps);
+                    atomicAdd(&s_jn[wid][p.job][1], (unsigned long long)p.scat);
+                    if (p.w == 0.0f) atomicAdd(&s_jn[wid][p.job][2], 1ull);
+                    else atomicMax(&s_jdrift[wid][p.job], __float_as_uint(fabsf(p.w - (1.0f - p.absrel))));
+                } else {
+                    if (p.w != 0.0f) acc_drift = fmaxf(acc_drift, fabsf(p.w - (1.0f - p.absrel)));
+                    acc_esc += esc;
+                    acc_abs += (double)p.absrel * e0;
+                    acc_steps += p.steps;
+                    acc_scat += p.scat;
+                }
                 if (REPLAY) {
                     acc_ld += p.n_ld; acc_red += p.n_red;
                     if (P.replay) {
@@ -1014,27 +1059,35 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
             float ndx = 0.0f, ndy = 0.0f, ndz = 1.0f;
             if (need == NEWID) {
                 float prel;
-                fast_emit<HIER>(P, p, p.id, ndx, ndy, ndz, prel);
-                if (DUST && p.src <= -2) { s_prel[threadIdx.x] = prel; acc_emit += (double)prel * P.e_ref; }
+                if (GROUP) {                     // id of the launch -> job and package id of that frequency
+                    const long long g = p.id - P.pkg_begin;
+                    p.job = (int)(g / P.job_pkgs);
+                    p.id = P.pkg_begin + (g - (long long)p.job * P.job_pkgs);
+                }
+                fast_emit<HIER>(P, p, GROUP ? P.job[p.job].ifreq : P.ifreq, p.id, ndx, ndy, ndz, prel);
+                if (GROUP) {
+                    s_prel[threadIdx.x] = p.src >= 0 ? P.job[p.job].ps_rel[p.src] : P.job[p.job].bg_rel;
+                    atomicAdd(&s_jd[wid][p.job][0], p.src >= 0 ? P.job[p.job].ps_e0[p.src] : P.job[p.job].bg_e0);
+                } else if (DUST && p.src <= -2) { s_prel[threadIdx.x] = prel; acc_emit += (double)prel * P.e_ref; }
                 else acc_emit += package_e0(P, p.src);
             } else if (need == SCAT) {
                 // finish the flight segment: advance to the scattering point (a4), then a8
                 const float rho = __uint_as_float(p.cw);
-                float t_u = p.tau_rem / (rho * P.ksca);
+                float t_u = p.tau_rem / (rho * (GROUP ? P.job[p.job].ksca : P.ksca));
                 if (HIER) t_u /= p.h;
                 p.fx = __saturatef(fmaf(t_u, p.dx, p.fx));
                 p.fy = __saturatef(fmaf(t_u, p.dy, p.fy));
                 p.fz = __saturatef(fmaf(t_u, p.dz, p.fz));
                 uint32_t s0, w_hg, w_az, s3;     // words 1, 2 of the block of the segment that ends here
-                if (HIER) philox_block(P.seed, P.ifreq, p.id, 2u + p.scat, s0, w_hg, w_az, s3);
+                if (HIER) philox_block(P.seed, GROUP ? P.job[p.job].ifreq : P.ifreq, p.id, 2u + p.scat, s0, w_hg, w_az, s3);
                 else { w_hg = p.w_hg; w_az = p.w_az; }
-                scatter_direction<float>(P.g, w_hg, w_az, p.dx, p.dy, p.dz, ndx, ndy, ndz);
+                scatter_direction<float>(GROUP ? P.job[p.job].g : P.g, w_hg, w_az, p.dx, p.dy, p.dz, ndx, ndy, ndz);
                 p.scat += 1;
             }
             if (need == NEWID || need == SCAT) {
                 fast_set_direction(p, ndx, ndy, ndz);
                 uint32_t s0, s1, s2, s3;
-                philox_block(P.seed, P.ifreq, p.id, 2u + p.scat, s0, s1, s2, s3);
+                philox_block(P.seed, GROUP ? P.job[p.job].ifreq : P.ifreq, p.id, 2u + p.scat, s0, s1, s2, s3);
                 if (!HIER) { p.w_hg = s1; p.w_az = s2; }                      // (the octree kernel has no registers to spare)
                 p.tau_rem = -__logf(uniform01<float>(s0));                    // a4
                 need = RUN;
@@ -1059,10 +1112,10 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
             const int bstride = ax0 ? 8 : (ax1 ? P.bsy : P.bsz);      // to the same slot of the next brick
             const int abit = ax0 ? 1 : (ax1 ? 2 : 4);
             const float tsh = HIER ? ts * p.h : ts;
-            const float ksr = rho * P.ksca;
+            const float ksr = rho * (GROUP ? P.job[p.job].ksca : P.ksca);
             const float dtau = tsh * ksr;
             const bool sc = dtau >= p.tau_rem && ksr > 0.0f;
-            const float x = sc ? p.tau_rem * P.kratio : tsh * (rho * P.kabs);
+            const float x = sc ? p.tau_rem * (GROUP ? P.job[p.job].kratio : P.kratio) : tsh * (rho * (GROUP ? P.job[p.job].kabs : P.kabs));
             float w_new, dep;
             if (HIER) absorb_v(p.w, x, w_new, dep);      // (measured: the branch pays on the octree, not on the regular grids)
             else absorb(p.w, x, w_new, dep);
@@ -1082,7 +1135,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                     const int j = (p.disp & 255) + hot_side * (((p.disp >> 8) & 255) + hot_side * (p.disp >> 16));
                     atomicAdd(s_hot + CK(p.src * hot_cells + j, hot_cells * P.n_point), p.pend);
                 } else if (p.pend > 0.0f) {
-                    const bool dust = DUST && p.src <= -2;
+                    const bool dust = (DUST && p.src <= -2) || GROUP;    // the package's own unit, kept in shared memory
                     if (ACC32) atomicAdd(P.acc32 + CK(p.rel, P.n_int), p.pend * (dust ? s_prel[threadIdx.x] : package_rel(P, p.src)));
                     else atomicAdd(P.acc + CK(p.rel, P.n_int), (double)p.pend * (dust ? (double)s_prel[threadIdx.x] * P.e_ref : package_e0(P, p.src)));
                     p.n_red += 1;
@@ -1095,7 +1148,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 p.pend = 0.0f;
             }
             if (term) {
-                acc_term += 1;
+                if (!GROUP) acc_term += 1;       // (GROUP: counted per job at retirement)
                 need = DONE;
             } else if (sc) {
                 need = SCAT;                     // the segment is finished in the service block
@@ -1177,7 +1230,21 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
         acc_term += __shfl_xor_sync(kFull, acc_term, o);
         acc_drift = fmaxf(acc_drift, __shfl_xor_sync(kFull, acc_drift, o));
     }
-    if (lane == 0 && acc_steps != 0) {
+    if (GROUP) {
+        // per-job totals of this warp -> the result slots of the jobs
+        __syncwarp();
+        if (lane < P.n_jobs && (s_jn[wid][lane][0] != 0ull || s_jd[wid][lane][0] != 0.0)) {
+            DevResult *r = P.result + lane;
+            atomicAdd(&r->emitted, s_jd[wid][lane][0]);
+            atomicAdd(&r->escaped, s_jd[wid][lane][1]);
+            atomicAdd(&r->absorbed, s_jd[wid][lane][2]);
+            atomicAdd(&r->cell_steps, s_jn[wid][lane][0]);
+            atomicAdd(&r->scatterings, s_jn[wid][lane][1]);
+            atomicAdd(&r->terminated, s_jn[wid][lane][2]);
+            atomicMax(&r->drift_bits, s_jdrift[wid][lane]);
+        }
+    }
+    if (!GROUP && lane == 0 && acc_steps != 0) {
         atomicAdd(&P.result->emitted, acc_emit);
         atomicAdd(&P.result->escaped, acc_esc);
         atomicAdd(&P.result->absorbed, acc_abs);
@@ -1445,7 +1512,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                 need = RUN;
             } else if (!SLAB && need == NEWID) {
                 FPkg q;
-                fast_emit<false>(P, q, P.pkg_begin + (long long)p.idx, ndx, ndy, ndz, p.prel);
+                fast_emit<false>(P, q, P.ifreq, P.pkg_begin + (long long)p.idx, ndx, ndy, ndz, p.prel);
                 p.fx = q.fx; p.fy = q.fy; p.fz = q.fz; p.rel = q.rel;
                 p.n_ld = 0;
                 q_load(P, p);
@@ -1672,7 +1739,7 @@ __global__ void __launch_bounds__(256) slab_emit_kernel(const __grid_constant__ 
         if (live) {
             int ix, iy, iz;
             const long long id = P.pkg_begin + (long long)idx;
-            fast_emit_core(P, q, id, ix, iy, iz, dx, dy, dz);
+            fast_emit_core(P, q, P.ifreq, id, ix, iy, iz, dx, dy, dz);
             if (q.src == -2) {
                 // f1: a dust package starts in the cell that sends it (ix = its global id; regular grid); its energy is the
                 // cell's luminosity over its package count, in units of the launch's reference energy
@@ -2492,7 +2559,7 @@ int launch_unpad(soc_grid *G, bool acc32, double weight, double *absorbed, cudaS
     return SOC_OK;
 }
 
-template <bool HIER, bool REPLAY, bool ACC32, bool QK, bool DUST>
+template <bool HIER, bool REPLAY, bool ACC32, bool QK, bool DUST, bool GROUP = false>
 int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbed, cudaStream_t st)
 {
     static_assert(!(HIER && QK) && (ACC32 || !QK), "photon_q_kernel walks regular grids with the fp32 accumulator only");
@@ -2502,7 +2569,7 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
     const size_t smem = P.hot_r >= 0 ? sizeof(float) * (size_t)side * side * side * (size_t)P.n_point : 0;
     int per_sm = 0;
     if (QK) SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_q_kernel<REPLAY, DUST, false>, threads, smem));
-    else SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY, ACC32, DUST>, threads, smem));
+    else SOC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, photon_fast_kernel<HIER, REPLAY, ACC32, DUST, GROUP>, threads, smem));
     if (per_sm < 1) return fail(SOC_ECUDA, "photon kernel does not fit on an SM");
     if (G->opt_blocks_per_sm > 0 && G->opt_blocks_per_sm < per_sm) per_sm = G->opt_blocks_per_sm;
     blocks = per_sm * G->n_sm;                   // persistent: a whole number of CTAs per SM
@@ -2511,10 +2578,10 @@ int launch_fast(soc_grid *G, const FastParams &P, double weight, double *absorbe
     if (need < blocks) blocks = (int)(need > 0 ? need : 1);
     if (G->opt_carveout >= 0) {
         if (QK) SOC_CUDA(cudaFuncSetAttribute(photon_q_kernel<REPLAY, DUST, false>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
-        else SOC_CUDA(cudaFuncSetAttribute(photon_fast_kernel<HIER, REPLAY, ACC32, DUST>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
+        else SOC_CUDA(cudaFuncSetAttribute(photon_fast_kernel<HIER, REPLAY, ACC32, DUST, GROUP>, cudaFuncAttributePreferredSharedMemoryCarveout, G->opt_carveout));
     }
     if (QK) photon_q_kernel<REPLAY, DUST, false><<<blocks, threads, smem, st>>>(P);
-    else photon_fast_kernel<HIER, REPLAY, ACC32, DUST><<<blocks, threads, smem, st>>>(P);
+    else photon_fast_kernel<HIER, REPLAY, ACC32, DUST, GROUP><<<blocks, threads, smem, st>>>(P);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     if (G->ev_after_photon) {                    // "timing": the pair brackets the photon kernel alone
@@ -2772,6 +2839,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
 
     SOC_CUDA(cudaMemsetAsync(G->d_counters + slot, 0, sizeof(unsigned long long), st));
     SOC_CUDA(cudaMemsetAsync(G->d_results + slot, 0, sizeof(DevResult), st));
+    if (slot < (int)G->slot_group.size()) G->slot_group[slot] = 0;
     if (pkg_count == 0) return SOC_OK;
     const bool hier = G->n_levels > 1, f64 = (flags & SOC_GEOM_FP64) != 0, rep = replay != nullptr;
     if (G->opt_timing) {
@@ -2905,6 +2973,101 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
     if (rc == SOC_OK && G->opt_timing) {
         if (G->ev_after_photon) SOC_CUDA(cudaEventRecord(G->ev1[slot], st));
         G->ev_set[slot] = 1;
+    }
+    G->ev_after_photon = nullptr;
+    return rc;
+}
+
+// Frequencies [f0, f0 + J) in ONE launch (FastParams::job): returns SOC_OK, an error, or 1 = "not eligible, launch them
+// one by one" (sources that differ in more than their energies, dust or beam packages, a grid served by photon_q_kernel
+// or by the hot-cell cache, energies that would underflow the common fp32 unit).
+int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long n_packages, unsigned long long seed,
+                  const double *w, long long pkg_begin, long long pkg_count, double *absorbed, int slot0, cudaStream_t st)
+{
+    const bool hier = G->n_levels > 1;
+    if (J < 2 || J > kMaxJobs || !G->opt_acc32 || pkg_count <= 0 || !absorbed) return 1;
+    if (n_packages < 0 || pkg_begin < 0 || pkg_begin + pkg_count > n_packages) return 1;
+    if (!hier && (8ll * G->n_int > (64ll << 20) || G->opt_kernel == 2)) return 1;
+    long long n_bg0 = 0;
+    for (int j = 0; j < J; ++j) {
+        long long n_bg = 0;
+        const int rc = check_sources(G, src + j, n_packages, &n_bg);
+        if (rc != SOC_OK) return rc;
+        if (src[j].beam || src[j].n_dust > 0 || !std::isfinite(w[j])) return 1;
+        if (j == 0) { n_bg0 = n_bg; continue; }
+        if (n_bg != n_bg0 || src[j].n_point != src[0].n_point) return 1;
+        for (int k = 0; k < 3 * src[0].n_point; ++k)
+            if (src[j].ps_pos[k] != src[0].ps_pos[k]) return 1;
+    }
+    if (!hier && src[0].n_point > 0 && G->opt_hot_cache) return 1;      // the hot-cell sums are per source class of ONE frequency
+    FastParams F;
+    std::memset(&F, 0, sizeof(F));
+    F.nx = G->nx; F.ny = G->ny; F.nz = G->nz; F.nbx = G->nbx; F.nby = G->nby;
+    F.bsy = 8 * G->nbx; F.bsz = 8 * G->nbx * G->nby; F.nrp = G->nrp; F.n_root = (int)G->n_root;
+    F.cellw = G->d_cellw_int; F.parent = G->d_parent_int;
+    F.n_int = (int)G->n_int; F.n_oct = (int)(G->n_octets > 0 ? G->n_octets : 1); F.n_abi = (int)G->n_total; F.n_replay = 1;
+    F.surf = 2.0 * ((double)G->ny * G->nz + (double)G->nz * G->nx + (double)G->nx * G->ny);
+    F.n_point = src[0].n_point; F.n_bg = n_bg0;
+    for (int k = 0; k < F.n_point; ++k)
+        for (int a = 0; a < 3; ++a) F.ps_pos[k][a] = src[0].ps_pos[3 * k + a];
+    F.dust.n_const = n_packages;
+    F.seed = seed; F.ifreq = f0; F.hot_r = -1;
+    F.n_jobs = J; F.job_pkgs = pkg_count; F.pkg_begin = pkg_begin; F.pkg_end = pkg_begin + (long long)J * pkg_count;
+    const int nm = G->nx > G->ny ? (G->nx > G->nz ? G->nx : G->nz) : (G->ny > G->nz ? G->ny : G->nz);
+    const long long n_ps = n_packages - n_bg0;
+    double e_ref = 0.0, depth = 0.0;
+    std::vector<double> bg_e0((size_t)J, 0.0);
+    for (int j = 0; j < J; ++j) {
+        JobParams &Q = F.job[j];
+        const double kabs = G->kabs[f0 + j], ksca = G->ksca[f0 + j];
+        Q.kabs = (float)kabs; Q.ksca = (float)ksca; Q.g = (float)G->g[f0 + j];
+        Q.kratio = ksca > 0.0 ? (float)(kabs / ksca) : 0.0f;
+        Q.ifreq = f0 + j;
+        depth = std::fmax(depth, ksca * G->rho_mean * nm);
+        if (n_bg0 > 0) Q.bg_e0 = kPi * src[j].bg_intensity * F.surf / (double)n_bg0;
+        e_ref = std::fmax(e_ref, w[j] * Q.bg_e0);
+        for (int k = 0; k < F.n_point; ++k) {
+            const long long count_k = n_ps / F.n_point + ((n_ps % F.n_point) > k ? 1 : 0);
+            Q.ps_e0[k] = count_k > 0 ? src[j].ps_lum[k] / (double)count_k : 0.0;
+            e_ref = std::fmax(e_ref, w[j] * Q.ps_e0[k]);
+        }
+    }
+    if (!(e_ref > 0.0) || !std::isfinite(e_ref)) return 1;
+    for (int j = 0; j < J; ++j) {
+        JobParams &Q = F.job[j];
+        Q.bg_rel = (float)(w[j] * Q.bg_e0 / e_ref);
+        if (n_bg0 > 0 && Q.bg_e0 > 0.0 && !(Q.bg_rel >= 1e-20f)) return 1;
+        for (int k = 0; k < F.n_point; ++k) {
+            Q.ps_rel[k] = (float)(w[j] * Q.ps_e0[k] / e_ref);
+            if (Q.ps_e0[k] > 0.0 && !(Q.ps_rel[k] >= 1e-20f)) return 1;
+        }
+    }
+    F.e_ref = e_ref;
+    F.service_threshold = G->opt_service_threshold > 0 ? G->opt_service_threshold : (depth >= 4.0 ? 16 : 8);
+    F.acc = G->acc_sel ? G->d_acc_b : G->d_acc; F.acc32 = G->acc_sel ? G->d_acc32_b : G->d_acc32;
+    F.counter = G->d_counters + slot0; F.result = G->d_results + slot0;
+    SOC_CUDA(cudaMemsetAsync(G->d_counters + slot0, 0, sizeof(unsigned long long) * (size_t)J, st));
+    SOC_CUDA(cudaMemsetAsync(G->d_results + slot0, 0, sizeof(DevResult) * (size_t)J, st));
+    if ((int)G->slot_group.size() < slot0 + J) G->slot_group.resize((size_t)(slot0 + J), 0);
+    for (int j = 0; j < J; ++j) G->slot_group[slot0 + j] = j == 0 ? J : 0;
+    if (G->opt_timing) {
+        const int rc = ensure_events(G, slot0 + J);
+        if (rc != SOC_OK) return rc;
+        SOC_CUDA(cudaEventRecord(G->ev0[slot0], st));
+        G->ev_after_photon = G->ev1[slot0];
+    }
+    int rc;
+    if (hier) rc = G->opt_stats ? launch_fast<true, true, true, false, false, true>(G, F, e_ref, absorbed, st)
+                                : launch_fast<true, false, true, false, false, true>(G, F, e_ref, absorbed, st);
+    else rc = G->opt_stats ? launch_fast<false, true, true, false, false, true>(G, F, e_ref, absorbed, st)
+                           : launch_fast<false, false, true, false, false, true>(G, F, e_ref, absorbed, st);
+    if (rc == SOC_OK && G->opt_timing) {
+        // every member of the group carries the group's event pair: soc_get_timings divides the time among them
+        for (int j = 0; j < J; ++j) G->ev_set[slot0 + j] = 1;
+        for (int j = 1; j < J; ++j) {
+            SOC_CUDA(cudaEventRecord(G->ev0[slot0 + j], st));
+            SOC_CUDA(cudaEventRecord(G->ev1[slot0 + j], st));
+        }
     }
     G->ev_after_photon = nullptr;
     return rc;
@@ -3220,6 +3383,7 @@ int soc_set_option(soc_grid *G, const char *key, int64_t value)
     else if (k == "slab_sweeps" && value >= 0 && value <= 64) G->opt_slab_sweeps = (int)value;
     else if (k == "slab_queue_limit" && value >= 0 && value < (1ll << 32)) G->opt_slab_queue_limit = value;
     else if (k == "slab_chunk" && value >= 0 && value <= (1ll << 24)) G->opt_slab_chunk = value;
+    else if (k == "group" && value >= 0 && value <= kMaxJobs) G->opt_group = (int)value;
     else if (k == "overlap" && (value == 0 || value == 1)) G->opt_overlap = (int)value;
     else if (k == "carveout" && value >= -1 && value <= 100) G->opt_carveout = (int)value;
     else if (k == "acc32" && (value == 0 || value == 1)) G->opt_acc32 = (int)value;
@@ -3243,6 +3407,14 @@ int soc_get_timings(soc_grid *G, int32_t n, float *ms)
                 SOC_CUDA(cudaEventElapsedTime(&ms[i], G->ev0[i], G->ev1[i]));
             }
         }
+    }
+    // the frequencies of a grouped launch share its time equally
+    for (int i = 0; i < n && i < (int)G->slot_group.size(); ++i) {
+        const int J = G->slot_group[i];
+        if (J < 2 || i + J > n) continue;
+        float total = 0.0f;
+        for (int k = 0; k < J; ++k) total += ms[i + k] > 0.0f ? ms[i + k] : 0.0f;
+        for (int k = 0; k < J; ++k) ms[i + k] = total / (float)J;
     }
     return SOC_OK;
 }
@@ -3295,10 +3467,22 @@ int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_package
         G->unpad_wait = nullptr;
         G->overlap_active = 1;
     }
-    for (int f = 0; f < G->n_freq && rc == SOC_OK; ++f) {
-        G->acc_sel = overlap ? (f & 1) : 0;
-        rc = enqueue_frequency(G, f, src + f, n_packages, seed, w[f], pkg_begin, pkg_count, absorbed_int, nullptr,
-                               flags, f, G->acc_sel ? G->aux : st);
+    // launches of few packages carry several consecutive frequencies each (enqueue_group): up to ~4e6 packages per launch
+    int J = G->opt_group;
+    if (J == 0) J = pkg_count > 0 && pkg_count < 3000000 ? (int)((4000000 + pkg_count - 1) / pkg_count) : 1;
+    if (J > kMaxJobs) J = kMaxJobs;
+    if (flags & SOC_GEOM_FP64) J = 1;
+    for (int f = 0, launch = 0; f < G->n_freq && rc == SOC_OK; ++launch) {
+        G->acc_sel = overlap ? (launch & 1) : 0;
+        cudaStream_t sf = G->acc_sel ? G->aux : st;
+        int n = J < G->n_freq - f ? J : G->n_freq - f;
+        if (n > 1) {
+            rc = enqueue_group(G, f, n, src + f, n_packages, seed, w.data() + f, pkg_begin, pkg_count, absorbed_int, f, sf);
+            if (rc == 1) { n = 1; rc = SOC_OK; }
+            else { f += n; continue; }
+        }
+        rc = enqueue_frequency(G, f, src + f, n_packages, seed, w[f], pkg_begin, pkg_count, absorbed_int, nullptr, flags, f, sf);
+        f += 1;
     }
     G->acc_sel = 0; G->overlap_active = 0; G->unpad_wait = nullptr;
     G->last_overlap = overlap ? 1 : 0;

@@ -13,6 +13,7 @@ Tolerances (BASELINE.json:north_star):
   temperatures     within 0.01 K
   conservation     emitted = absorbed + escaped to 1e-6 (relative)
 """
+import dataclasses
 import math
 
 import numpy as np
@@ -625,6 +626,44 @@ def test_spectrum_and_temperatures_match_oracle():
     assert np.abs(Tg - To2).max() <= 2e-3
     assert Tg.min() >= 3.0 and 5.0 < np.median(Tg) < 200.0
     G.close()
+
+
+@pytest.mark.parametrize("which,kw,point", [("4p", dict(n=8, n_packages=50_000, n_freq=7), False),
+                                           ("4p", dict(n=8, n_packages=50_000, n_freq=6), True),
+                                           ("2", dict(n=24, n_packages=80_000), False)])
+def test_grouped_launches_equal_single_ones(which, kw, point):
+    """Launches of few packages carry up to four consecutive frequencies (per-lane opacities, one accumulator with the
+    quadrature weights folded into the package energies): the per-frequency counters of the one-frequency launches, the
+    same energies, the same frequency integral up to the order of the fp32 additions -- on the octree with and without
+    point sources and on a regular grid without (with the hot-cell cache a launch stays with one frequency)."""
+    torch = _torch()
+    P = inputs.make_config(which, **kw)
+    if which == "2":          # a spectrum for the single-frequency config: five frequencies with their own opacities
+        lam = np.array([300.0, 60.0, 5.0, 0.55, 0.2])
+        P = dataclasses.replace(P, freq_hz=2.998e14 / lam, kabs=P.kabs[0] * np.array([0.01, 0.1, 0.5, 1.0, 2.0]),
+                                ksca=P.ksca[0] * np.array([0.0, 0.01, 0.3, 1.0, 2.5]), g=np.array([0.0, 0.1, 0.3, 0.6, 0.7]),
+                                bg_intensity=np.array([3.0, 2.0, 1.0, 0.5, 0.1]), ps_lum=np.zeros((5, 0)))
+    if point:
+        P.ps_pos = np.array([[2.3, 4.6, 1.2], [6.5, 3.5, 5.5]])
+        P.ps_lum = (np.pi * P.bg_intensity * 6 * 64)[:, None] * np.array([0.5, 2.0])[None, :]
+    srcs = [P.sources(f) for f in range(P.n_freq)]
+    G = soc.Grid.from_problem(P)
+    out = []
+    for group in (1, 4, 3, 0):
+        G.set_option("group", group)
+        A = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+        res = G.simulate_spectrum(srcs, P.n_packages, P.seed, A)
+        torch.cuda.synchronize()
+        out.append((A.cpu().numpy(), res))
+    G.close()
+    A1, r1 = out[0]
+    assert sum(r.cell_steps for r in r1) > 0
+    for A, res in out[1:]:
+        assert [(r.cell_steps, r.scatterings, r.terminated) for r in res] == [(r.cell_steps, r.scatterings, r.terminated) for r in r1]
+        for a, b in zip(res, r1):
+            assert a.emitted == pytest.approx(b.emitted, rel=1e-12) and a.escaped == pytest.approx(b.escaped, rel=1e-9)
+            assert a.absorbed == pytest.approx(b.absorbed, rel=1e-9)
+        assert rel_l1(A, A1) <= 2e-6
 
 
 @pytest.mark.parametrize("mode", ["acc32", "acc64", "faint_source", "own_stream"])
