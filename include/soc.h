@@ -256,16 +256,22 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
  * x slabs of device memory per accumulator set), "slab_sweeps" (sweeps over the slabs before the last, whole-grid launch
  * of a frequency; 0 = 2), "slab_queue_limit" (test hook: entries a slab / leftover queue accepts from the walk before it
  * refuses packages; 0 = its capacity), "slab_chunk" (test hook: packages per sequence of phases, 0 = 2^24: a frequency of
- * more packages is served in several sequences); and
+ * more packages is served in several sequences), "group" (soc_simulate_spectrum: consecutive frequencies per launch where
+ * a frequency has few packages -- one launch then carries the packages of up to 4 frequencies, each lane reading the
+ * opacities of its package's frequency, into one internal accumulator with the quadrature weights folded into the package
+ * energies; 0 = by package count (up to ~4e6 packages per launch), 1 = off; applies to the octree and to regular grids
+ * without point sources, constant sources only); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
  * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
 int soc_set_option(soc_grid *grid, const char *key, int64_t value);
 
 /* With option "timing" = 1: ms[i] = device time of the photon kernel last launched into result slot i
  * (slot = frequency index for soc_simulate_spectrum, 0 for the single-frequency calls); -1 where no launch
- * was recorded.  soc_simulate_spectrum overlaps consecutive frequencies on two streams (option "overlap", default 1):
- * there ms[i], i > 0, is the advance of the completion front, end of launch i - end of launch i-1, so that the sum
- * is the span from the first start to the last end.  Waits for those launches to finish.  ms: HOST, n floats. */
+ * was recorded.  soc_simulate_spectrum overlaps consecutive launches on two streams (option "overlap", default 1)
+ * and gives a launch of few packages up to four consecutive frequencies (option "group"): there the time of a launch is
+ * the advance of the completion front (end of this launch - end of the one before, so that the sum is the span from the
+ * first start to the last end), and the frequencies of two consecutive launches share the time of both equally.  Waits
+ * for those launches to finish.  ms: HOST, n floats. */
 int soc_get_timings(soc_grid *grid, int32_t n, float *ms);
 
 /* Roofline probes: random 4-byte gathers (kind 0), random fp64 red.global.add (kind 1),
