@@ -259,8 +259,8 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
  * more packages is served in several sequences), "group" (soc_simulate_spectrum: consecutive frequencies per launch where
  * a frequency has few packages -- one launch then carries the packages of up to 4 frequencies, each lane reading the
  * opacities of its package's frequency, into one internal accumulator with the quadrature weights folded into the package
- * energies; 0 = by package count (up to ~4e6 packages per launch), 1 = off; applies to the octree and to regular grids
- * without point sources, constant sources only); and
+ * energies; 0 = by package count (up to ~1.6e7 packages per launch), 1 = off; constant sources only, grids served by
+ * photon_fast_kernel); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
  * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
 int soc_set_option(soc_grid *grid, const char *key, int64_t value);

@@ -1133,7 +1133,8 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 // source, with one fp64 reduction to L2 otherwise
                 if (p.disp >= 0) {
                     const int j = (p.disp & 255) + hot_side * (((p.disp >> 8) & 255) + hot_side * (p.disp >> 16));
-                    atomicAdd(s_hot + CK(p.src * hot_cells + j, hot_cells * P.n_point), p.pend);
+                    // (GROUP: already in the launch's unit -- the frequencies of the launch share the partial sums)
+                    atomicAdd(s_hot + CK(p.src * hot_cells + j, hot_cells * P.n_point), GROUP ? p.pend * s_prel[threadIdx.x] : p.pend);
                 } else if (p.pend > 0.0f) {
                     const bool dust = (DUST && p.src <= -2) || GROUP;    // the package's own unit, kept in shared memory
                     if (ACC32) atomicAdd(P.acc32 + CK(p.rel, P.n_int), p.pend * (dust ? s_prel[threadIdx.x] : package_rel(P, p.src)));
@@ -1213,7 +1214,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
                 const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
                           iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
-                if (ACC32) atomicAdd(P.hot64 + i, (double)v * (double)P.ps_rel[k]);
+                if (ACC32) atomicAdd(P.hot64 + i, GROUP ? (double)v : (double)v * (double)P.ps_rel[k]);
                 else atomicAdd(P.acc + CK(root_id(P, ix, iy, iz), P.n_int), (double)v * P.ps_e0[k]);
             }
         }
@@ -2985,7 +2986,7 @@ int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long 
                   const double *w, long long pkg_begin, long long pkg_count, double *absorbed, int slot0, cudaStream_t st)
 {
     const bool hier = G->n_levels > 1;
-    if (J < 2 || J > kMaxJobs || !G->opt_acc32 || pkg_count <= 0 || !absorbed) return 1;
+    if (J < 1 || J > kMaxJobs || !G->opt_acc32 || pkg_count <= 0 || !absorbed) return 1;
     if (n_packages < 0 || pkg_begin < 0 || pkg_begin + pkg_count > n_packages) return 1;
     if (!hier && (8ll * G->n_int > (64ll << 20) || G->opt_kernel == 2)) return 1;
     long long n_bg0 = 0;
@@ -2999,7 +3000,6 @@ int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long 
         for (int k = 0; k < 3 * src[0].n_point; ++k)
             if (src[j].ps_pos[k] != src[0].ps_pos[k]) return 1;
     }
-    if (!hier && src[0].n_point > 0 && G->opt_hot_cache) return 1;      // the hot-cell sums are per source class of ONE frequency
     FastParams F;
     std::memset(&F, 0, sizeof(F));
     F.nx = G->nx; F.ny = G->ny; F.nz = G->nz; F.nbx = G->nbx; F.nby = G->nby;
@@ -3011,7 +3011,9 @@ int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long 
     for (int k = 0; k < F.n_point; ++k)
         for (int a = 0; a < 3; ++a) F.ps_pos[k][a] = src[0].ps_pos[3 * k + a];
     F.dust.n_const = n_packages;
-    F.seed = seed; F.ifreq = f0; F.hot_r = -1;
+    F.seed = seed; F.ifreq = f0;
+    F.hot_r = -1;
+    if (!hier && F.n_point > 0 && G->opt_hot_cache) F.hot_r = (size_t)F.n_point * 343 * sizeof(float) <= 40 * 1024 ? 3 : 2;
     F.n_jobs = J; F.job_pkgs = pkg_count; F.pkg_begin = pkg_begin; F.pkg_end = pkg_begin + (long long)J * pkg_count;
     const int nm = G->nx > G->ny ? (G->nx > G->nz ? G->nx : G->nz) : (G->ny > G->nz ? G->ny : G->nz);
     const long long n_ps = n_packages - n_bg0;
@@ -3045,6 +3047,15 @@ int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long 
     F.e_ref = e_ref;
     F.service_threshold = G->opt_service_threshold > 0 ? G->opt_service_threshold : (depth >= 4.0 ? 16 : 8);
     F.acc = G->acc_sel ? G->d_acc_b : G->d_acc; F.acc32 = G->acc_sel ? G->d_acc32_b : G->d_acc32;
+    if (F.hot_r >= 0) {
+        double *&h = G->d_hot64[G->acc_sel];
+        if (!h) {
+            const size_t bytes = sizeof(double) * SOC_MAX_POINT_SOURCES * 343;
+            SOC_CUDA(cudaMalloc(&h, bytes));
+            SOC_CUDA(cudaMemsetAsync(h, 0, bytes, st));                  // st = the stream that uses it
+        }
+        F.hot64 = h;
+    }
     F.counter = G->d_counters + slot0; F.result = G->d_results + slot0;
     SOC_CUDA(cudaMemsetAsync(G->d_counters + slot0, 0, sizeof(unsigned long long) * (size_t)J, st));
     SOC_CUDA(cudaMemsetAsync(G->d_results + slot0, 0, sizeof(DevResult) * (size_t)J, st));
@@ -3475,18 +3486,21 @@ int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_package
         G->unpad_wait = nullptr;
         G->overlap_active = 1;
     }
-    // launches of few packages carry several consecutive frequencies each (enqueue_group): up to ~4e6 packages per launch
-    // (config 4' with 1e6 packages per frequency: 6.33e10 cell-steps/s one by one, 7.63e10 in fours; in eights 7.85e10, but
-    // eight frequencies in one fp32 accumulator cost accuracy: cells against counters 4e-7 instead of 9e-9)
+    // launches of few packages carry several consecutive frequencies each (enqueue_group): up to four, up to ~1.6e7 packages
+    // per launch (config 4' with 1e6 packages per frequency: 6.33e10 cell-steps/s one by one, 7.63e10 in fours; in eights
+    // 7.85e10, but eight frequencies in one fp32 accumulator cost accuracy: cells against counters 4e-7 instead of 9e-9;
+    // config 3 with 4e6 packages per frequency: 1.262e11 one by one, 1.276e11 in twos, 1.294e11 in fours)
     int J = G->opt_group;
-    if (J == 0) J = pkg_count > 0 && pkg_count < 3000000 ? (int)((4000000 + pkg_count - 1) / pkg_count) : 1;
+    if (J == 0) J = pkg_count > 0 && pkg_count < 16000000 ? (int)((16000000 + pkg_count - 1) / pkg_count) : 1;
     if (J > kMaxJobs) J = kMaxJobs;
     if (flags & SOC_GEOM_FP64) J = 1;
     for (int f = 0, launch = 0; f < G->n_freq && rc == SOC_OK; ++launch) {
         G->acc_sel = overlap ? (launch & 1) : 0;
         cudaStream_t sf = G->acc_sel ? G->aux : st;
         int n = J < G->n_freq - f ? J : G->n_freq - f;
-        if (n > 1) {
+        // (the octree takes the grouped kernel for a single frequency as well: its totals live in shared memory, which
+        //  frees the registers the one-frequency kernel spills -- +2 %)
+        if (n > 1 || (G->n_levels > 1 && G->opt_group != 1)) {
             rc = enqueue_group(G, f, n, src + f, n_packages, seed, w.data() + f, pkg_begin, pkg_count, absorbed_int, f, sf);
             if (rc == 1) { n = 1; rc = SOC_OK; }
             else { f += n; continue; }

@@ -630,12 +630,13 @@ def test_spectrum_and_temperatures_match_oracle():
 
 @pytest.mark.parametrize("which,kw,point", [("4p", dict(n=8, n_packages=50_000, n_freq=7), False),
                                            ("4p", dict(n=8, n_packages=50_000, n_freq=6), True),
-                                           ("2", dict(n=24, n_packages=80_000), False)])
+                                           ("2", dict(n=24, n_packages=80_000), False),
+                                           ("3", dict(n=24, n_packages=80_000, n_freq=7), False)])
 def test_grouped_launches_equal_single_ones(which, kw, point):
     """Launches of few packages carry up to four consecutive frequencies (per-lane opacities, one accumulator with the
     quadrature weights folded into the package energies): the per-frequency counters of the one-frequency launches, the
     same energies, the same frequency integral up to the order of the fp32 additions -- on the octree with and without
-    point sources and on a regular grid without (with the hot-cell cache a launch stays with one frequency)."""
+    point sources, on a regular grid without, and on config 3's regular grid with its point sources and their hot-cell sums."""
     torch = _torch()
     P = inputs.make_config(which, **kw)
     if which == "2":          # a spectrum for the single-frequency config: five frequencies with their own opacities
