@@ -748,6 +748,10 @@ __device__ __forceinline__ void slab_epilogue(const SlabParams &S, bool pops)
 // the frequencies is read per lane from this table.  The jobs add into ONE accumulator in units of e_ref, each with its
 // quadrature weight folded into its package energies (rel = weight * energy / e_ref).
 constexpr int kMaxJobs = 4;
+#ifndef SOC_GROUP_MIN_REL
+#define SOC_GROUP_MIN_REL 1e-3f
+#endif
+constexpr float kGroupMinRel = SOC_GROUP_MIN_REL;   // a job's brightest source class, in units of the launch's (enqueue_group)
 struct JobParams {
     float ksca, kabs, kratio, g;
     float bg_rel, beam_rel;
@@ -3044,6 +3048,19 @@ int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long 
             if (Q.ps_e0[k] > 0.0 && !(Q.ps_rel[k] >= 1e-20f)) return 1;
         }
     }
+    // the jobs share one fp32 accumulator: a frequency whose packages carry much less than the launch's unit loses its
+    // deposits wherever a brighter one dominates the sum (they fall below half the last bit), one-sidedly: measured on the
+    // smoke problem (three frequencies decades apart, point sources in an octree) as 1e-6 of the absorbed energy.  Such a
+    // frequency is launched on its own (the caller retries the group from the next frequency): below 1e-3 of the unit, or
+    // 1e-2 where point sources make cells that collect 1e4 and more deposits per launch
+    for (int j = 0; j < J; ++j) {
+        float top = F.job[j].bg_rel;
+        for (int k = 0; k < F.n_point; ++k) top = std::fmax(top, F.job[j].ps_rel[k]);
+        if (!(top >= (F.n_point > 0 ? 10.0f * kGroupMinRel : kGroupMinRel))) return 1;
+        // (and with the group size chosen by the library, point sources keep one frequency per launch altogether: config 3
+        //  in fours gains 3 % and holds its cells to 6e-7 of the counters instead of 3e-8)
+        if (J > 1 && F.n_point > 0 && G->opt_group == 0) return 1;
+    }
     F.e_ref = e_ref;
     F.service_threshold = G->opt_service_threshold > 0 ? G->opt_service_threshold : (depth >= 4.0 ? 16 : 8);
     F.acc = G->acc_sel ? G->d_acc_b : G->d_acc; F.acc32 = G->acc_sel ? G->d_acc32_b : G->d_acc32;
@@ -3500,7 +3517,7 @@ int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_package
         int n = J < G->n_freq - f ? J : G->n_freq - f;
         // (the octree takes the grouped kernel for a single frequency as well: its totals live in shared memory, which
         //  frees the registers the one-frequency kernel spills -- +2 %)
-        if (n > 1 || (G->n_levels > 1 && G->opt_group != 1)) {
+        if (!(flags & SOC_GEOM_FP64) && (n > 1 || (G->n_levels > 1 && G->opt_group != 1))) {
             rc = enqueue_group(G, f, n, src + f, n_packages, seed, w.data() + f, pkg_begin, pkg_count, absorbed_int, f, sf);
             if (rc == 1) { n = 1; rc = SOC_OK; }
             else { f += n; continue; }

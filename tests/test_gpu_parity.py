@@ -656,6 +656,10 @@ def test_grouped_launches_equal_single_ones(which, kw, point):
         res = G.simulate_spectrum(srcs, P.n_packages, P.seed, A)
         torch.cuda.synchronize()
         out.append((A.cpu().numpy(), res))
+    # SOC_GEOM_FP64 stays with the replay kernel, one frequency per launch (its fp64 weight knows no drift)
+    Ar = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+    rr = G.simulate_spectrum(srcs, P.n_packages, P.seed, Ar, flags=soc.SOC_GEOM_FP64)
+    assert all(r.weight_drift == 0.0 for r in rr) and any(r.weight_drift > 0.0 for r in out[-1][1])
     G.close()
     A1, r1 = out[0]
     assert sum(r.cell_steps for r in r1) > 0
