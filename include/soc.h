@@ -321,9 +321,11 @@ int64_t soc_checked_violations(void);
 uint64_t soc_launch_count(void);
 
 /* The package queues of slab-blocked launches (option "slabs": ~1 GB per accumulator set for 1e7 packages in two slabs)
- * outlive the grid that allocated them: soc_grid_destroy hands them to a process-wide cache of at most two buffers, from
- * which the next grid takes them (soc_run_host creates a grid per call; cudaMalloc / cudaFree of buffers this size cost
- * 0.1-0.2 s each).  This call frees the cache (device synchronised).  Returns the number of bytes released. */
+ * and the large per-grid device arrays (cell words, links, accumulators) outlive the grid that allocated them:
+ * soc_grid_destroy hands them to a process-wide cache (two queue buffers; per-grid arrays up to 8 GB in total), from which
+ * the next grid takes buffers of the same size (soc_run_host creates a grid per call; cudaMalloc / cudaFree of buffers
+ * this size cost it tens to hundreds of milliseconds, differently every time).  This call frees the cache (device
+ * synchronised).  Returns the number of bytes released. */
 int64_t soc_release_cached_memory(void);
 
 const char *soc_last_error(void);

@@ -29,6 +29,51 @@ struct CachedBuffer { void *ptr; size_t entries; int device; };
 std::vector<CachedBuffer> g_queue_cache;
 std::mutex g_queue_cache_mutex;
 constexpr size_t kQueueCacheMax = 2;
+
+// ... and of the large per-grid arrays (cell words, links, accumulators): soc_run_host creates and destroys a grid per call,
+// and cudaMalloc / cudaFree of a dozen buffers of 45-140 MB cost it 10-80 ms, differently every time.  big_malloc takes a
+// cached buffer of exactly the size asked for if there is one; big_free hands buffers of >= 1 MB to the cache (at most
+// kBigCacheBytes in total), the others to cudaFree.  Contents are undefined, as after cudaMalloc.
+struct BigBuffer { void *ptr; size_t bytes; int device; };
+std::vector<BigBuffer> g_big_cache, g_big_live;
+std::mutex g_big_mutex;
+constexpr size_t kBigCacheBytes = 8ull << 30;
+
+cudaError_t big_malloc_impl(void **out, size_t bytes)
+{
+    int device = 0;
+    cudaGetDevice(&device);
+    std::lock_guard<std::mutex> lock(g_big_mutex);
+    for (size_t i = 0; i < g_big_cache.size(); ++i)
+        if (g_big_cache[i].bytes == bytes && g_big_cache[i].device == device) {
+            *out = g_big_cache[i].ptr;
+            g_big_live.push_back(g_big_cache[i]);
+            g_big_cache.erase(g_big_cache.begin() + i);
+            return cudaSuccess;
+        }
+    const cudaError_t e = cudaMalloc(out, bytes);
+    if (e == cudaSuccess && bytes >= (1u << 20)) g_big_live.push_back({*out, bytes, device});
+    return e;
+}
+template <typename T> cudaError_t big_malloc(T **out, size_t bytes) { return big_malloc_impl(reinterpret_cast<void **>(out), bytes); }
+
+void big_free(void *p)
+{
+    if (!p) return;
+    {
+        std::lock_guard<std::mutex> lock(g_big_mutex);
+        for (size_t i = 0; i < g_big_live.size(); ++i)
+            if (g_big_live[i].ptr == p) {
+                const BigBuffer b = g_big_live[i];
+                g_big_live.erase(g_big_live.begin() + i);
+                size_t total = b.bytes;
+                for (const BigBuffer &c : g_big_cache) total += c.bytes;
+                if (total <= kBigCacheBytes) { g_big_cache.push_back(b); return; }
+                break;
+            }
+    }
+    cudaFree(p);
+}
 constexpr size_t kQueueEntryBytes = 3 * 16 + 4;    // three uint4 arrays and one float array (SlabParams)
 
 int fail(int code, const std::string &msg)
@@ -2914,7 +2959,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
             F.hot64 = h;
         }
         if (!acc32 && G->acc_sel && !G->d_acc_b) {           // fp64 fallback on the second stream: its own accumulator
-            SOC_CUDA(cudaMalloc(&G->d_acc_b, sizeof(double) * (size_t)G->n_int));
+            SOC_CUDA(big_malloc(&G->d_acc_b, sizeof(double) * (size_t)G->n_int));
             SOC_CUDA(cudaMemsetAsync(G->d_acc_b, 0, sizeof(double) * (size_t)G->n_int, st));   // st = the stream that uses it
             F.acc = G->d_acc_b;
         }
@@ -3147,6 +3192,10 @@ int64_t soc_release_cached_memory(void)
         bytes += (int64_t)(b.entries * kQueueEntryBytes);
     }
     g_queue_cache.clear();
+    std::lock_guard<std::mutex> lock2(g_big_mutex);
+    if (!g_big_cache.empty()) cudaDeviceSynchronize();
+    for (const BigBuffer &b : g_big_cache) { cudaFree(b.ptr); bytes += (int64_t)b.bytes; }
+    g_big_cache.clear();
     return bytes;
 }
 
@@ -3165,14 +3214,15 @@ int64_t soc_checked_violations(void)
 void soc_grid_destroy(soc_grid *G)
 {
     if (!G) return;
-    cudaFree(G->d_cellw); cudaFree(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
-    cudaFree(G->d_table); cudaFree(G->d_cellw_int); cudaFree(G->d_parent_int); cudaFree(G->d_acc); cudaFree(G->d_acc32);
+    cudaDeviceSynchronize();                     // (the cached buffers may be handed to another grid at once)
+    big_free(G->d_cellw); big_free(G->d_parent); cudaFree(G->d_results); cudaFree(G->d_counters);
+    cudaFree(G->d_table); big_free(G->d_cellw_int); big_free(G->d_parent_int); big_free(G->d_acc); big_free(G->d_acc32);
     if (G->h_results) cudaFreeHost(G->h_results);
     if (G->h_table) cudaFreeHost(G->h_table);
     if (G->h_scalars) cudaFreeHost(G->h_scalars);
-    cudaFree(G->d_dust_first); cudaFree(G->d_scan_blocks); cudaFree(G->d_scalars); cudaFree(G->d_freqtab); cudaFree(G->d_eff);
+    cudaFree(G->d_dust_first); cudaFree(G->d_scan_blocks); cudaFree(G->d_scalars); cudaFree(G->d_freqtab); big_free(G->d_eff);
     if (G->ev_table) cudaEventDestroy(G->ev_table);
-    cudaFree(G->d_acc32_b); cudaFree(G->d_acc_b);
+    big_free(G->d_acc32_b); big_free(G->d_acc_b);
     for (int i = 0; i < 2; ++i) {
         if (G->d_slab_q[i]) {                    // the queue buffers go to the process-wide cache (soc.h); the smallest is evicted
             cudaDeviceSynchronize();
@@ -3282,16 +3332,16 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
 
     SOC_CUDA(cudaGetDevice(&G->device));
     SOC_CUDA(cudaDeviceGetAttribute(&G->n_sm, cudaDevAttrMultiProcessorCount, G->device));
-    SOC_CUDA(cudaMalloc(&G->d_cellw, sizeof(uint32_t) * (size_t)G->n_total));
-    SOC_CUDA(cudaMalloc(&G->d_parent, sizeof(int32_t) * n_par));
+    SOC_CUDA(big_malloc(&G->d_cellw, sizeof(uint32_t) * (size_t)G->n_total));
+    SOC_CUDA(big_malloc(&G->d_parent, sizeof(int32_t) * n_par));
     SOC_CUDA(cudaMalloc(&G->d_table, sizeof(float) * 8192));
     if (hier_gpu) {
         double *d_sum = nullptr;
         int32_t *d_child = nullptr;
-        struct Tmp { double *&a; int32_t *&b; ~Tmp() { cudaFree(a); cudaFree(b); } } tmp{d_sum, d_child};
+        struct Tmp { double *&a; int32_t *&b; ~Tmp() { cudaFree(a); big_free(b); } } tmp{d_sum, d_child};
         SOC_CUDA(cudaMalloc(&d_sum, 32));
         SOC_CUDA(cudaMemset(d_sum, 0, 32));
-        SOC_CUDA(cudaMalloc(&d_child, sizeof(int32_t) * (size_t)G->n_total));
+        SOC_CUDA(big_malloc(&d_child, sizeof(int32_t) * (size_t)G->n_total));
         SOC_CUDA(cudaMemcpy(G->d_cellw, d->density, sizeof(float) * (size_t)G->n_total, cudaMemcpyHostToDevice));
         SOC_CUDA(cudaMemcpy(d_child, d->child, sizeof(int32_t) * (size_t)G->n_total, cudaMemcpyHostToDevice));
         HierParams H;
@@ -3353,9 +3403,9 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
             return 8 * ((X >> 1) + nbx * ((Y >> 1) + nby * (Z >> 1))) + (X & 1) + 2 * (Y & 1) + 4 * (Z & 1);
         };
         for (long long o = 0; o < G->n_octets && !big; ++o) pi[(size_t)o] = (int32_t)internal((long long)parent[(size_t)o] + G->n_root);
-        SOC_CUDA(cudaMalloc(&G->d_cellw_int, sizeof(uint32_t) * (size_t)n_int));
-        SOC_CUDA(cudaMalloc(&G->d_parent_int, sizeof(int32_t) * n_par));
-        SOC_CUDA(cudaMalloc(&G->d_acc, sizeof(double) * (size_t)n_int));
+        SOC_CUDA(big_malloc(&G->d_cellw_int, sizeof(uint32_t) * (size_t)n_int));
+        SOC_CUDA(big_malloc(&G->d_parent_int, sizeof(int32_t) * n_par));
+        SOC_CUDA(big_malloc(&G->d_acc, sizeof(double) * (size_t)n_int));
         repad_kernel<<<G->n_sm * 8, 256>>>(G->d_cellw, G->d_cellw_int, G->nx, G->ny, G->nz, (int)nbx, (int)nby, nrp, G->n_root, n_int);
         g_launches += 1;
         SOC_CUDA(cudaGetLastError());
@@ -3373,7 +3423,7 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
             if (f & 8) return fail(SOC_EINVAL, "octet without a parent");
         } else SOC_CUDA(cudaMemset(G->d_parent_int, 0, sizeof(int32_t) * n_par));
         SOC_CUDA(cudaMemset(G->d_acc, 0, sizeof(double) * (size_t)n_int));
-        SOC_CUDA(cudaMalloc(&G->d_acc32, sizeof(float) * (size_t)n_int));
+        SOC_CUDA(big_malloc(&G->d_acc32, sizeof(float) * (size_t)n_int));
         SOC_CUDA(cudaMemset(G->d_acc32, 0, sizeof(float) * (size_t)n_int));
     }
     int rc = ensure_slots(G, d->n_freq > 8 ? d->n_freq : 8);
@@ -3495,7 +3545,7 @@ int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_package
             SOC_CUDA(cudaEventCreateWithFlags(&G->ev_join, cudaEventDisableTiming));
             SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[0], cudaEventDisableTiming));
             SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[1], cudaEventDisableTiming));
-            SOC_CUDA(cudaMalloc(&G->d_acc32_b, sizeof(float) * (size_t)G->n_int));
+            SOC_CUDA(big_malloc(&G->d_acc32_b, sizeof(float) * (size_t)G->n_int));
             SOC_CUDA(cudaMemsetAsync(G->d_acc32_b, 0, sizeof(float) * (size_t)G->n_int, st));   // ordered before the fork
         }
         SOC_CUDA(cudaEventRecord(G->ev_fork, st));
@@ -3519,6 +3569,10 @@ int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_package
         //  frees the registers the one-frequency kernel spills -- +2 %)
         if (!(flags & SOC_GEOM_FP64) && (n > 1 || (G->n_levels > 1 && G->opt_group != 1))) {
             rc = enqueue_group(G, f, n, src + f, n_packages, seed, w.data() + f, pkg_begin, pkg_count, absorbed_int, f, sf);
+            if (rc == 1 && n > 1 && G->n_levels > 1) {       // the group is not eligible: this frequency alone (octree: grouped kernel)
+                n = 1;
+                rc = enqueue_group(G, f, 1, src + f, n_packages, seed, w.data() + f, pkg_begin, pkg_count, absorbed_int, f, sf);
+            }
             if (rc == 1) { n = 1; rc = SOC_OK; }
             else { f += n; continue; }
         }
@@ -3623,7 +3677,7 @@ int soc_update_temperatures_ali(soc_grid *G, const double *absorbed, const doubl
 {
     if (!G || !absorbed || !self_abs || !emitted) return fail(SOC_EINVAL, "NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
-    if (!G->d_eff) SOC_CUDA(cudaMalloc(&G->d_eff, sizeof(double) * (size_t)G->n_total));
+    if (!G->d_eff) SOC_CUDA(big_malloc(&G->d_eff, sizeof(double) * (size_t)G->n_total));
     ali_effective_kernel<<<G->n_sm * 8, 256, 0, st>>>(absorbed, self_abs, emitted, G->n_total, G->d_eff);
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
@@ -3852,9 +3906,9 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
     double *d_abs = nullptr;
     float *d_T = nullptr;
     cudaStream_t st = nullptr;
-    auto cleanup = [&]() { cudaFree(d_abs); cudaFree(d_T); soc_grid_destroy(G); };
-    cudaError_t e = cudaMalloc(&d_abs, sizeof(double) * (size_t)G->n_total);
-    if (e == cudaSuccess) e = cudaMalloc(&d_T, sizeof(float) * (size_t)G->n_total);
+    auto cleanup = [&]() { big_free(d_abs); big_free(d_T); soc_grid_destroy(G); };
+    cudaError_t e = big_malloc(&d_abs, sizeof(double) * (size_t)G->n_total);
+    if (e == cudaSuccess) e = big_malloc(&d_T, sizeof(float) * (size_t)G->n_total);
     if (e == cudaSuccess) e = cudaMemsetAsync(d_abs, 0, sizeof(double) * (size_t)G->n_total, st);
     if (e != cudaSuccess) { cleanup(); return fail(SOC_ECUDA, cudaGetErrorString(e)); }
     for (int it = 0; it < n_iter && rc == SOC_OK; ++it)

@@ -393,6 +393,12 @@ def test_queue_buffers_are_cached_across_grids():
     assert rel_l1(out[1][0], out[0][0]) <= 2e-6
     assert soc.release_cached_memory() >= 3 * 16 * 2 * 100_000      # at least the two slab queues of one accumulator set
     assert soc.release_cached_memory() == 0
+    # the large per-grid arrays are cached the same way: a second soc_run_host finds the first one's buffers
+    Q = inputs.make_config("3", n=64, n_packages=50_000, n_freq=3)
+    a1, t1, _ = soc.run_host(Q, n_iter=1)
+    a2, t2, _ = soc.run_host(Q, n_iter=1)
+    assert rel_l1(a2, a1) <= 2e-6 and np.abs(t2 - t1).max() <= 1e-3
+    assert soc.release_cached_memory() >= 8 * 64 ** 3 and soc.release_cached_memory() == 0
 
 
 @pytest.mark.parametrize("which,n_sub", [("3", 60_000), ("5", 40_000)])
