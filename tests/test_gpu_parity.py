@@ -375,6 +375,45 @@ def test_slab_blocked_launch_walks_the_same_paths(n_slabs, sweeps, limit, chunk)
     G.close()
 
 
+def test_slab_blocked_and_grouped_edge_cases():
+    """Ragged and degenerate launches through the queues and the job table: a package-id subset that starts in the middle,
+    seven packages, a beam (every package starts in one cell of one slab), a slab count the brick layers do not divide;
+    frequencies of odd package counts in one grouped launch, on a subset of the ids."""
+    torch = _torch()
+    P = inputs.make_config("5", n=40, n_packages=123_457, n_freq=6)
+    G = soc.Grid.from_problem(P)
+    G.set_option("kernel", 2)
+    cases = [(P.sources(2), 123_457, 50_001, 61_003), (P.sources(4), 123_457, 0, 7), (P.sources(5), 123_457, 123_450, 7),
+             (dict(beam=[0.0, 17.3, 22.9, 0.6, 0.48, 0.64]), 5_000, 0, 5_000)]
+    for src, n, begin, count in cases:
+        out = []
+        for n_slabs in (1, 7):
+            G.set_option("slabs", n_slabs)
+            A = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+            r = G.simulate_packages(2, src, n, 11, 1.0, begin, count, A, None, flags=PROD)
+            torch.cuda.synchronize()
+            out.append((A.cpu().numpy(), r))
+        (A1, r1), (A2, r2) = out
+        assert (r1.cell_steps, r1.scatterings, r1.terminated) == (r2.cell_steps, r2.scatterings, r2.terminated) and r1.cell_steps > 0
+        assert r2.emitted == pytest.approx(r1.emitted, rel=1e-12) and r2.escaped == pytest.approx(r1.escaped, rel=1e-9)
+        assert rel_l1(A2, A1) <= 2e-6
+    G.close()
+    Q = inputs.make_config("4p", n=8, n_packages=33_331, n_freq=5)
+    srcs = [Q.sources(f) for f in range(Q.n_freq)]
+    G = soc.Grid.from_problem(Q)
+    out = []
+    for group in (1, 4):
+        G.set_option("group", group)
+        A = torch.zeros(Q.n_total, dtype=torch.float64, device="cuda")
+        res = G.simulate_spectrum(srcs, Q.n_packages, Q.seed, A, pkg_begin=10_007, pkg_count=20_011)
+        torch.cuda.synchronize()
+        out.append((A.cpu().numpy(), res))
+    G.close()
+    assert [(r.cell_steps, r.scatterings, r.terminated) for r in out[1][1]] == [(r.cell_steps, r.scatterings, r.terminated) for r in out[0][1]]
+    assert all(a.emitted == pytest.approx(b.emitted, rel=1e-12) for a, b in zip(out[1][1], out[0][1]))
+    assert rel_l1(out[1][0], out[0][0]) <= 2e-6
+
+
 def test_queue_buffers_are_cached_across_grids():
     """The package queues of a slab-blocked launch go to a process-wide cache when their grid is destroyed and are taken
     from it by the next grid (soc_run_host creates a grid per call); soc_release_cached_memory frees them."""
