@@ -262,7 +262,7 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
  * energies; 0 = by package count (up to ~1.6e7 packages per launch) for background-only sources, 1 = off, 2-4 = that
  * many also with point sources, where the shared fp32 accumulator costs accuracy near the sources: cells against counters
  * 6e-7 instead of 3e-8 on config 3; constant sources only, grids served by photon_fast_kernel, frequencies whose package
- * energies lie within 1e-3 (1e-2 with point sources) of the brightest of the launch); and
+ * energies lie within 1e-7 (1e-2 with point sources) of the brightest of the launch); and
  * "timing" (0/1): record a CUDA-event pair on the launching stream around every photon-kernel launch.
  * Returns SOC_EINVAL for an unknown key or an out-of-range value. */
 int soc_set_option(soc_grid *grid, const char *key, int64_t value);

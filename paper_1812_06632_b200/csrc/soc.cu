@@ -794,7 +794,7 @@ __device__ __forceinline__ void slab_epilogue(const SlabParams &S, bool pops)
 // quadrature weight folded into its package energies (rel = weight * energy / e_ref).
 constexpr int kMaxJobs = 4;
 #ifndef SOC_GROUP_MIN_REL
-#define SOC_GROUP_MIN_REL 1e-3f
+#define SOC_GROUP_MIN_REL 1e-7f
 #endif
 constexpr float kGroupMinRel = SOC_GROUP_MIN_REL;   // a job's brightest source class, in units of the launch's (enqueue_group)
 struct JobParams {
@@ -3096,12 +3096,14 @@ int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long 
     // the jobs share one fp32 accumulator: a frequency whose packages carry much less than the launch's unit loses its
     // deposits wherever a brighter one dominates the sum (they fall below half the last bit), one-sidedly: measured on the
     // smoke problem (three frequencies decades apart, point sources in an octree) as 1e-6 of the absorbed energy.  Such a
-    // frequency is launched on its own (the caller retries the group from the next frequency): below 1e-3 of the unit, or
-    // 1e-2 where point sources make cells that collect 1e4 and more deposits per launch
+    // frequency is launched on its own (the caller retries the group from the next frequency): below 1e-2 of the unit where
+    // point sources make cells that collect 1e4 and more deposits per launch; below 1e-7 with the background alone, where a
+    // cell collects some tens per launch and what such a frequency can lose is 1e-7 of the launch's energy at most
+    // (config 4' with its faintest UV frequencies grouped: cells against counters 9e-9)
     for (int j = 0; j < J; ++j) {
         float top = F.job[j].bg_rel;
         for (int k = 0; k < F.n_point; ++k) top = std::fmax(top, F.job[j].ps_rel[k]);
-        if (!(top >= (F.n_point > 0 ? 10.0f * kGroupMinRel : kGroupMinRel))) return 1;
+        if (!(top >= (F.n_point > 0 ? 1e-2f : kGroupMinRel))) return 1;
         // (and with the group size chosen by the library, point sources keep one frequency per launch altogether: config 3
         //  in fours gains 3 % and holds its cells to 6e-7 of the counters instead of 3e-8)
         if (J > 1 && F.n_point > 0 && G->opt_group == 0) return 1;
