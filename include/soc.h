@@ -181,6 +181,42 @@ int soc_update_temperatures_ali(soc_grid *grid, const double *absorbed, const do
                                 double scale, const float *table_T, int32_t n_table, double E_min, double E_max,
                                 float *T_out, void *cuda_stream);
 
+/* soc_update_temperatures_ali for callers that cannot allocate GPU memory at the time of the call.  Same operation, same
+ * arguments, same result (row f3), but the call makes no cudaMalloc / cudaMallocHost / cudaFree and takes
+ * nothing from the library's buffer cache.
+ *
+ * Who needs it.  soc_update_temperatures_ali allocates on its first use per grid: a per-cell work array on the device and
+ * a pinned staging buffer for the table.  That is a problem for a host program that
+ *   - has handed the whole device to an allocator of its own (a framework's caching pool sized to all of HBM, a service
+ *     with a fixed memory budget per tenant): a cudaMalloc from inside this library then fails, or takes memory the
+ *     program has not accounted for;
+ *   - runs the temperature update inside a loop that must not stall: cudaMalloc and cudaFree synchronise the whole
+ *     device, so a first-use allocation in iteration k stops every other stream of the process for its duration;
+ *   - must prove at start-up that the run cannot die of memory exhaustion half-way through.
+ *
+ * How it works.  The work array and the table sit in an array that is compiled into the library
+ * (static __device__, 16 MiB + 32 KiB).  Every GPU on which the library's module is loaded holds that array until the
+ * process exits, used or not -- that is the price.  The limit it sets: grids of at most 2 097 152 cells in total
+ * (soc_grid_n_total; a 128^3 regular grid fits exactly) and n_table <= 8192.  A larger grid is refused with SOC_EINVAL
+ * and a message that names both numbers; nothing is launched in that case.
+ *
+ * Set-up.  The first call on each device looks up the device address of the array (cudaGetSymbolAddress) and remembers
+ * it; later calls on that device only launch.  Make that first call during start-up, before any CUDA stream capture is
+ * begun.  The grid's device must be the current device (SOC_EINVAL otherwise).
+ *
+ * Sharing.  There is ONE array per GPU, shared by every grid, stream and host thread of the process, and it keeps what
+ * the last call wrote.  Nothing in it needs clearing between calls: each call overwrites the elements it later reads.
+ * But two calls whose kernels can run on the GPU at the same time (different streams without an event between them,
+ * different host threads) write the same elements and corrupt each other's temperatures -- order them yourself.  Calls
+ * issued on one stream are ordered by the stream.
+ *
+ * absorbed, self_abs, emitted: DEVICE n_total doubles (no alignment requirement).  T_out: DEVICE n_total floats, 16-byte
+ * aligned, written.  table_T: HOST n_table floats; pageable memory is read before the call returns, page-locked memory
+ * is read when the stream reaches the copy and must stay unchanged until then.  The call only enqueues work. */
+int soc_update_temperatures_ali_static(soc_grid *grid, const double *absorbed, const double *self_abs,
+                                       const double *emitted, double scale, const float *table_T, int32_t n_table,
+                                       double E_min, double E_max, float *T_out, void *cuda_stream);
+
 /* Iterated run with dust re-emission (rows f1, f3):
  *   iteration 0   the constant sources src[f] (background, point sources), n_const packages per frequency, `seed`:
  *                 A_const = sum_f w_f A_f;  T = table(A_const)

@@ -3178,6 +3178,47 @@ void trapezoid(const std::vector<double> &nu, std::vector<double> &w)
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------------
+// Scratch of soc_update_temperatures_ali_static, the ALI temperature update for callers that must not allocate device
+// memory (soc.h says who they are).  The regular call keeps its per-cell work array (the effective absorbed energy
+// (A - S) / (1 - beta)) in a buffer it allocates on first use and stages the temperature table through pinned memory it
+// allocates too.  Here both live in this one array, which is part of the library image: every GPU that loads the
+// library holds its 16 MiB + 32 KiB from the moment the module is loaded until the process ends, whether or not the
+// entry point is ever called.
+//   [0, kStaticMaxCells)                 effective absorbed energy per cell
+//   [kStaticMaxCells, end)               the temperature table (up to kStaticMaxTable floats)
+// In host code the NAME g_static_scratch is only the host-side handle of the symbol, not an address the GPU can use:
+// the device address is looked up once per device by static_scratch() below and that pointer is what kernels receive.
+// ------------------------------------------------------------------------------------------------
+constexpr long long kStaticMaxCells = 1ll << 21;            // 2 097 152 cells: a 128^3 regular grid (config 3) fits exactly
+constexpr int kStaticMaxTable = 8192;                       // floats; the same cap as soc_update_temperatures
+static __device__ __align__(256) double g_static_scratch[kStaticMaxCells + kStaticMaxTable / 2];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+double *g_static_ptr[kStaticMaxDevices];                    // device address of g_static_scratch on device i, once known
+std::mutex g_static_mutex;
+
+// Device address of the scratch array on `device`, which must be the current device.  The first call per device asks
+// the runtime for it (this is the set-up; it allocates nothing, the array came with the module) and keeps the answer.
+int static_scratch(int device, double **out)
+{
+    if (device < 0 || device >= kStaticMaxDevices) return fail(SOC_EINVAL, "soc_update_temperatures_ali_static: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[device]) {
+        double *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void **>(&p), g_static_scratch);
+        if (e != cudaSuccess || !p)
+            return fail(SOC_ECUDA, std::string("soc_update_temperatures_ali_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+        g_static_ptr[device] = p;
+    }
+    *out = g_static_ptr[device];
+    return SOC_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char *soc_last_error(void) { return g_last_error.c_str(); }
@@ -3684,6 +3725,52 @@ int soc_update_temperatures_ali(soc_grid *G, const double *absorbed, const doubl
     g_launches += 1;
     SOC_CUDA(cudaGetLastError());
     return soc_update_temperatures(G, G->d_eff, scale, table_T, n_table, E_min, E_max, T_out, stream);
+}
+
+// The same two kernels as soc_update_temperatures_ali + soc_update_temperatures, with the work array and the table in
+// g_static_scratch: no cudaMalloc, cudaMallocHost, cudaFree, event creation or cached-buffer call on this path.
+int soc_update_temperatures_ali_static(soc_grid *G, const double *absorbed, const double *self_abs, const double *emitted,
+                                       double scale, const float *table_T, int32_t n_table, double E_min, double E_max,
+                                       float *T_out, void *stream)
+{
+    if (!G || !absorbed || !self_abs || !emitted || !table_T || !T_out) return fail(SOC_EINVAL, "NULL argument");
+    if (n_table < 2 || n_table > kStaticMaxTable) return fail(SOC_EINVAL, "n_table out of range");
+    if (!(E_min > 0.0) || !(E_max > E_min) || !std::isfinite(E_max) || !std::isfinite(scale))
+        return fail(SOC_EINVAL, "need 0 < E_min < E_max and a finite scale");
+    if (reinterpret_cast<uintptr_t>(T_out) & 15) return fail(SOC_EINVAL, "T_out must be 16-byte aligned");
+    if (G->n_total > kStaticMaxCells)
+        return fail(SOC_EINVAL, "soc_update_temperatures_ali_static: the grid has " + std::to_string(G->n_total) +
+                                " cells, the static scratch holds " + std::to_string(kStaticMaxCells) +
+                                "; use soc_update_temperatures_ali");
+    int device = -1;
+    SOC_CUDA(cudaGetDevice(&device));
+    if (device != G->device) return fail(SOC_EINVAL, "soc_update_temperatures_ali_static: the grid's device must be the current device");
+    double *scratch = nullptr;
+    const int rc = static_scratch(device, &scratch);        // first call on this device: looks the address up
+    if (rc != SOC_OK) return rc;
+    double *d_eff = scratch;
+    float *d_table = reinterpret_cast<float *>(scratch + kStaticMaxCells);
+    cudaStream_t st = (cudaStream_t)stream;
+    // Nothing in the scratch has to start at zero: the first kernel writes eff[0 .. n_total) and the copy writes
+    // table[0 .. n_table) before the second kernel reads exactly those elements; what earlier calls left beyond them
+    // is never read.
+    SOC_CUDA(cudaMemcpyAsync(d_table, table_T, sizeof(float) * n_table, cudaMemcpyHostToDevice, st));
+    ali_effective_kernel<<<G->n_sm * 8, 256, 0, st>>>(absorbed, self_abs, emitted, G->n_total, d_eff);
+    TempParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.cellw = G->d_cellw; P.absorbed = d_eff; P.table = d_table; P.T_out = T_out;
+    P.n_total = G->n_total; P.n_levels = G->n_levels; P.n_table = n_table;
+    for (int l = 0; l <= G->n_levels; ++l) P.level_off[l] = G->level_off[l];
+    P.scale = scale; P.e_min = E_min; P.e_max = E_max; P.inv_e_min = 1.0 / E_min;
+    P.x_scale = (float)((double)(n_table - 1) / std::log(E_max / E_min));
+    const long long n4 = (G->n_total >> 2) + 1;
+    long long blocks = (n4 + 255) / 256;
+    const long long cap = (long long)G->n_sm * 8;
+    if (blocks > cap) blocks = cap;
+    temperature_kernel<<<(int)blocks, 256, sizeof(float) * n_table, st>>>(P);
+    g_launches += 2;
+    SOC_CUDA(cudaGetLastError());
+    return SOC_OK;
 }
 
 int soc_iterate(soc_grid *G, const soc_sources *src, int64_t n_const, uint64_t seed, const soc_iterate_opts *opts,

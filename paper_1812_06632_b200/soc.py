@@ -19,13 +19,14 @@ if os.environ.get("SOC_B200_LIB"):                      # e.g. the bounds-checke
 SOC_GEOM_FP32 = 0
 SOC_GEOM_FP64 = 1
 MAX_POINT_SOURCES = 64
+STATIC_MAX_CELLS = 1 << 21          # soc_update_temperatures_ali_static: cells its built-in scratch array holds
 
 EXPORTS = ["soc_grid_create", "soc_grid_destroy", "soc_grid_n_total", "soc_freq_weights", "soc_simulate_frequency",
            "soc_simulate_packages", "soc_simulate_spectrum", "soc_update_temperatures", "soc_run_host",
            "soc_set_option", "soc_get_timings", "soc_probe_throughput", "soc_launch_count", "soc_last_error", "soc_version",
            "soc_emission_counts", "soc_cell_emission", "soc_update_temperatures_ali", "soc_iterate", "soc_make_map",
            "soc_checked_violations", "soc_stochastic_create", "soc_stochastic_destroy", "soc_stochastic_emission",
-           "soc_release_cached_memory"]
+           "soc_release_cached_memory", "soc_update_temperatures_ali_static"]
 
 
 class SocError(RuntimeError):
@@ -104,6 +105,7 @@ def load():
     L.soc_emission_counts.argtypes = [vp, i32, vp, i32, i64, i32, vp, C.POINTER(i64), C.POINTER(dbl), vp]
     L.soc_cell_emission.argtypes = [vp, vp, vp, vp]
     L.soc_update_temperatures_ali.argtypes = [vp, vp, vp, vp, dbl, vp, i32, dbl, dbl, vp, vp]
+    L.soc_update_temperatures_ali_static.argtypes = [vp, vp, vp, vp, dbl, vp, i32, dbl, dbl, vp, vp]
     L.soc_iterate.argtypes = [vp, C.POINTER(Sources), i64, u64, C.POINTER(IterateOpts), dbl, vp, i32, dbl, dbl, vp, vp,
                               C.POINTER(IterateRecord), u32, vp]
     L.soc_make_map.argtypes = [vp, i32, vp, C.POINTER(MapDesc), vp, vp]
@@ -290,6 +292,15 @@ class Grid:
         _check(load().soc_update_temperatures_ali(self._h, _dev_ptr(absorbed), _dev_ptr(self_abs), _dev_ptr(emitted), float(scale),
                                                   _ptr(tab), len(tab), float(e_min), float(e_max), _dev_ptr(T_out),
                                                   _stream_ptr(stream)))
+
+    def update_temperatures_ali_static(self, absorbed, self_abs, emitted, scale, table_T, e_min, e_max, T_out, stream=None):
+        """soc_update_temperatures_ali_static: update_temperatures_ali without any allocation inside the library, for host
+        programs that own all device memory themselves or cannot afford cudaMalloc's device-wide stall (soc.h).  Grids of
+        at most STATIC_MAX_CELLS cells; one scratch array per GPU, so calls that overlap on the device race."""
+        tab = _np(table_T, np.float32)
+        _check(load().soc_update_temperatures_ali_static(self._h, _dev_ptr(absorbed), _dev_ptr(self_abs), _dev_ptr(emitted),
+                                                         float(scale), _ptr(tab), len(tab), float(e_min), float(e_max),
+                                                         _dev_ptr(T_out), _stream_ptr(stream)))
 
     def iterate(self, sources_list, n_const, seed, n_request, t_scale, table_T, e_min, e_max, absorbed_out, T_out,
                 mode="weighted", cap=10000, reference_field=True, ref_start=1, ali=False, flags=SOC_GEOM_FP32, stream=None):
