@@ -153,7 +153,9 @@ int soc_simulate_packages(soc_grid *grid, int32_t ifreq, const soc_sources *src,
  * [pkg_begin, pkg_begin + pkg_count) of n_packages with sources src[f], accumulated as
  *   absorbed_int[cell] += w_f * A_f[cell]            (w = soc_freq_weights)
  * All launches are queued back to back on the stream; results[n_freq] (may be NULL) are fetched once at
- * the end (the call then synchronises). */
+ * the end (the call then synchronises).  Sources with dust packages (n_dust > 0 at any frequency) are accepted; such a
+ * spectrum is served one frequency at a time whatever option "overlap" says (the offsets of the dust packages exist once
+ * per grid) and synchronises the stream once per frequency. */
 int soc_simulate_spectrum(soc_grid *grid, const soc_sources *src, int64_t n_packages, uint64_t seed,
                           int64_t pkg_begin, int64_t pkg_count, double *absorbed_int,
                           soc_freq_result *results, uint32_t flags, void *cuda_stream);
@@ -361,7 +363,10 @@ uint64_t soc_launch_count(void);
  * soc_grid_destroy hands them to a process-wide cache (two queue buffers; per-grid arrays up to 8 GB in total), from which
  * the next grid takes buffers of the same size (soc_run_host creates a grid per call; cudaMalloc / cudaFree of buffers
  * this size cost it tens to hundreds of milliseconds, differently every time).  This call frees the cache (device
- * synchronised).  Returns the number of bytes released. */
+ * synchronised).  Returns the number of bytes released.  The library makes the same call itself when one of its device
+ * allocations fails, and then tries that allocation once more, so idle cached buffers never cause SOC_ENOMEM.  The 8 GB
+ * limit of the per-grid array cache can be set in the environment: SOC_B200_CACHE_MB (megabytes, read once; 0 = cache
+ * nothing). */
 int64_t soc_release_cached_memory(void);
 
 const char *soc_last_error(void);

@@ -33,26 +33,47 @@ constexpr size_t kQueueCacheMax = 2;
 // ... and of the large per-grid arrays (cell words, links, accumulators): soc_run_host creates and destroys a grid per call,
 // and cudaMalloc / cudaFree of a dozen buffers of 45-140 MB cost it 10-80 ms, differently every time.  big_malloc takes a
 // cached buffer of exactly the size asked for if there is one; big_free hands buffers of >= 1 MB to the cache (at most
-// kBigCacheBytes in total), the others to cudaFree.  Contents are undefined, as after cudaMalloc.
+// big_cache_limit() in total), the others to cudaFree.  A cudaMalloc that fails empties both caches and is tried again.  Contents are undefined, as after cudaMalloc.
 struct BigBuffer { void *ptr; size_t bytes; int device; };
 std::vector<BigBuffer> g_big_cache, g_big_live;
 std::mutex g_big_mutex;
-constexpr size_t kBigCacheBytes = 8ull << 30;
+// most the big cache keeps, in bytes: 8 GB, or SOC_B200_CACHE_MB megabytes from the environment (0 = keep nothing)
+size_t big_cache_limit()
+{
+    static const size_t limit = [] {
+        const char *v = std::getenv("SOC_B200_CACHE_MB");
+        char *end = nullptr;
+        const unsigned long long mb = v ? std::strtoull(v, &end, 10) : 0;
+        return v && end != v ? (size_t)mb << 20 : (size_t)8 << 30;
+    }();
+    return limit;
+}
+
+int64_t release_caches();           // frees both caches (device synchronised); the caller holds neither mutex
 
 cudaError_t big_malloc_impl(void **out, size_t bytes)
 {
     int device = 0;
     cudaGetDevice(&device);
-    std::lock_guard<std::mutex> lock(g_big_mutex);
-    for (size_t i = 0; i < g_big_cache.size(); ++i)
-        if (g_big_cache[i].bytes == bytes && g_big_cache[i].device == device) {
-            *out = g_big_cache[i].ptr;
-            g_big_live.push_back(g_big_cache[i]);
-            g_big_cache.erase(g_big_cache.begin() + i);
-            return cudaSuccess;
-        }
-    const cudaError_t e = cudaMalloc(out, bytes);
-    if (e == cudaSuccess && bytes >= (1u << 20)) g_big_live.push_back({*out, bytes, device});
+    {
+        std::lock_guard<std::mutex> lock(g_big_mutex);
+        for (size_t i = 0; i < g_big_cache.size(); ++i)
+            if (g_big_cache[i].bytes == bytes && g_big_cache[i].device == device) {
+                *out = g_big_cache[i].ptr;
+                g_big_live.push_back(g_big_cache[i]);
+                g_big_cache.erase(g_big_cache.begin() + i);
+                return cudaSuccess;
+            }
+    }
+    cudaError_t e = cudaMalloc(out, bytes);
+    if (e == cudaErrorMemoryAllocation) {       // buffers of other sizes may be sitting idle in the caches: give them back, once
+        cudaGetLastError();
+        if (release_caches() > 0) e = cudaMalloc(out, bytes);
+    }
+    if (e == cudaSuccess && bytes >= (1u << 20)) {
+        std::lock_guard<std::mutex> lock(g_big_mutex);
+        g_big_live.push_back({*out, bytes, device});
+    }
     return e;
 }
 template <typename T> cudaError_t big_malloc(T **out, size_t bytes) { return big_malloc_impl(reinterpret_cast<void **>(out), bytes); }
@@ -68,7 +89,7 @@ void big_free(void *p)
                 g_big_live.erase(g_big_live.begin() + i);
                 size_t total = b.bytes;
                 for (const BigBuffer &c : g_big_cache) total += c.bytes;
-                if (total <= kBigCacheBytes) { g_big_cache.push_back(b); return; }
+                if (total <= big_cache_limit()) { g_big_cache.push_back(b); return; }
                 break;
             }
     }
@@ -2682,18 +2703,27 @@ int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weigh
         if (G->d_slab_q[sel]) { SOC_CUDA(cudaStreamSynchronize(st)); SOC_CUDA(cudaFree(G->d_slab_q[sel])); G->d_slab_q[sel] = nullptr; }
         G->slab_q_entries[sel] = 0;
         // a buffer left by an earlier grid of this process, if one is large enough (the smallest such)
-        std::lock_guard<std::mutex> lock(g_queue_cache_mutex);
         int best = -1;
-        for (size_t i = 0; i < g_queue_cache.size(); ++i)
-            if (g_queue_cache[i].device == G->device && g_queue_cache[i].entries >= entries &&
-                (best < 0 || g_queue_cache[i].entries < g_queue_cache[best].entries)) best = (int)i;
-        if (best >= 0) {
-            G->d_slab_q[sel] = (uint4 *)g_queue_cache[best].ptr;
-            G->slab_q_entries[sel] = g_queue_cache[best].entries;
-            g_queue_cache.erase(g_queue_cache.begin() + best);
-        } else {
-            if (cudaMalloc(&G->d_slab_q[sel], entries * kQueueEntryBytes) != cudaSuccess) {
+        {
+            std::lock_guard<std::mutex> lock(g_queue_cache_mutex);
+            for (size_t i = 0; i < g_queue_cache.size(); ++i)
+                if (g_queue_cache[i].device == G->device && g_queue_cache[i].entries >= entries &&
+                    (best < 0 || g_queue_cache[i].entries < g_queue_cache[best].entries)) best = (int)i;
+            if (best >= 0) {
+                G->d_slab_q[sel] = (uint4 *)g_queue_cache[best].ptr;
+                G->slab_q_entries[sel] = g_queue_cache[best].entries;
+                g_queue_cache.erase(g_queue_cache.begin() + best);
+            }
+        }
+        if (best < 0) {
+            cudaError_t e = cudaMalloc(&G->d_slab_q[sel], entries * kQueueEntryBytes);
+            if (e == cudaErrorMemoryAllocation) {           // idle buffers of the caches first, then once more
                 cudaGetLastError();
+                if (release_caches() > 0) e = cudaMalloc(&G->d_slab_q[sel], entries * kQueueEntryBytes);
+            }
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                G->d_slab_q[sel] = nullptr;
                 return fail(SOC_ENOMEM, "package queues of the slab-blocked launch");
             }
             G->slab_q_entries[sel] = entries;
@@ -3225,7 +3255,10 @@ const char *soc_last_error(void) { return g_last_error.c_str(); }
 const char *soc_version(void) { return "soc_b200 0.1 (sm_100a)"; }
 uint64_t soc_launch_count(void) { return g_launches; }
 
-int64_t soc_release_cached_memory(void)
+}  // extern "C"
+
+namespace {
+int64_t release_caches()
 {
     int64_t bytes = 0;
     std::lock_guard<std::mutex> lock(g_queue_cache_mutex);
@@ -3241,6 +3274,11 @@ int64_t soc_release_cached_memory(void)
     g_big_cache.clear();
     return bytes;
 }
+}  // namespace
+
+extern "C" {
+
+int64_t soc_release_cached_memory(void) { return release_caches(); }
 
 int64_t soc_checked_violations(void)
 {
@@ -3580,16 +3618,24 @@ int soc_simulate_spectrum(soc_grid *G, const soc_sources *src, int64_t n_package
     if (rc != SOC_OK) return rc;
     // production mode: odd frequencies go to a second stream with their own accumulators, so that the tail of one launch
     // (lanes that have run out of packages) is filled by the blocks of the next; the folds into absorbed_int stay ordered
-    const bool overlap = G->opt_overlap && G->n_freq > 1 && !(flags & SOC_GEOM_FP64);
+    // Dust packages keep the launches serial: the prefix sums of the package counts, the scan scratch and the luminosity
+    // scalars exist once per grid (dust_prepare), so the scan of frequency f + 1 on the other stream would rewrite the
+    // array the kernel of frequency f is still searching.
+    bool any_dust = false;
+    for (int f = 0; f < G->n_freq; ++f) any_dust = any_dust || src[f].n_dust > 0;
+    const bool overlap = G->opt_overlap && G->n_freq > 1 && !(flags & SOC_GEOM_FP64) && !any_dust;
     if (overlap) {
-        if (!G->aux) {
-            SOC_CUDA(cudaStreamCreateWithFlags(&G->aux, cudaStreamNonBlocking));
-            SOC_CUDA(cudaEventCreateWithFlags(&G->ev_fork, cudaEventDisableTiming));
-            SOC_CUDA(cudaEventCreateWithFlags(&G->ev_join, cudaEventDisableTiming));
-            SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[0], cudaEventDisableTiming));
-            SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[1], cudaEventDisableTiming));
+        // every piece is created on its own test, so that a call that failed half-way through (an event, the second
+        // accumulator) is completed by the next instead of launching on what is missing
+        if (!G->aux) SOC_CUDA(cudaStreamCreateWithFlags(&G->aux, cudaStreamNonBlocking));
+        if (!G->ev_fork) SOC_CUDA(cudaEventCreateWithFlags(&G->ev_fork, cudaEventDisableTiming));
+        if (!G->ev_join) SOC_CUDA(cudaEventCreateWithFlags(&G->ev_join, cudaEventDisableTiming));
+        if (!G->ev_unpad[0]) SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[0], cudaEventDisableTiming));
+        if (!G->ev_unpad[1]) SOC_CUDA(cudaEventCreateWithFlags(&G->ev_unpad[1], cudaEventDisableTiming));
+        if (!G->d_acc32_b) {
             SOC_CUDA(big_malloc(&G->d_acc32_b, sizeof(float) * (size_t)G->n_int));
-            SOC_CUDA(cudaMemsetAsync(G->d_acc32_b, 0, sizeof(float) * (size_t)G->n_int, st));   // ordered before the fork
+            const cudaError_t e = cudaMemsetAsync(G->d_acc32_b, 0, sizeof(float) * (size_t)G->n_int, st);   // ordered before the fork
+            if (e != cudaSuccess) { big_free(G->d_acc32_b); G->d_acc32_b = nullptr; return fail(SOC_ECUDA, cudaGetErrorString(e)); }
         }
         SOC_CUDA(cudaEventRecord(G->ev_fork, st));
         SOC_CUDA(cudaStreamWaitEvent(G->aux, G->ev_fork, 0));

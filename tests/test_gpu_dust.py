@@ -325,3 +325,51 @@ def test_iterate_at_full_size_is_measured(capsys):
               f"{steps:.3e} cell-steps = {steps / dt:.3e} cell-steps/s incl. counts, scans and temperature updates; packages per "
               f"iteration {[h['n_packages'] for h in hist]}; escaped dust emission / A_const per iteration {[round(r, 3) for r in ratio]}; "
               f"T max {Tn.max():.0f} K")
+
+
+def test_dust_spectrum_with_counts_per_frequency_does_not_depend_on_the_overlap_option():
+    """A dust spectrum passed straight to soc_simulate_spectrum, package counts differing from frequency to frequency
+    (emission-weighted).  The prefix sums of the counts and the scan scratch exist once per grid, so two frequencies in
+    flight on two streams would search each other's offsets: with dust sources the launches stay serial whatever the
+    option says.  overlap = 1 must give the counters of overlap = 0 exactly and the same integral up to the order of the
+    additions, every frequency must emit the luminosity of its sending cells, and nothing may turn inf / NaN."""
+    torch = _torch()
+    P = _hot_problem("3", n=16, n_freq=8, n_packages=60_000)
+    G = soc.Grid.from_problem(P)
+    Td = torch.from_numpy(_temperatures(P)).cuda()
+    srcs, lum = [], []
+    for f in range(P.n_freq):
+        cnt = torch.zeros(P.n_total, dtype=torch.int32, device="cuda")
+        n_dust, tot = G.emission_counts(f, Td, "weighted", 12_000 + 5_000 * f, 40, cnt)
+        assert 0 <= n_dust < P.n_packages
+        s = dict(P.sources(f))
+        if n_dust > 0:                  # (towards the UV no cell of 8-90 K emits: those frequencies carry constant sources only)
+            s.update(dust_T=Td, dust_count=cnt, n_dust=n_dust)
+        srcs.append(s)
+        lum.append(tot)
+    with_dust = [s["n_dust"] for s in srcs if s.get("n_dust", 0) > 0]
+    assert len(with_dust) >= 4 and len(set(with_dust)) == len(with_dust)      # every dust frequency has its own offsets
+    out = []
+    for overlap in (0, 1, 1):
+        G.set_option("overlap", overlap)
+        A = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+        res = G.simulate_spectrum(srcs, P.n_packages, 11, A)
+        torch.cuda.synchronize()
+        out.append((A.cpu().numpy(), res))
+    G.close()
+    for A, res in out:
+        assert np.isfinite(A).all() and all(np.isfinite(r.emitted) and r.emitted > 0 for r in res)
+        assert all(abs(r.emitted - r.absorbed - r.escaped) <= 1e-6 * r.emitted for r in res)
+    for A, res in out[1:]:
+        assert [(r.cell_steps, r.scatterings, r.terminated) for r in res] == [(r.cell_steps, r.scatterings, r.terminated) for r in out[0][1]]
+        assert all(a.emitted == pytest.approx(b.emitted, rel=1e-12) for a, b in zip(res, out[0][1]))
+        assert np.allclose(A, out[0][0], rtol=2e-5, atol=0)
+    # the dust part of what a frequency emits is the luminosity of all cells (weighted counts: every emitting cell sends)
+    Gc = soc.Grid.from_problem(P)
+    for f in (0, 2, P.n_freq - 1):
+        s = dict(P.sources(f))
+        n_const = P.n_packages - srcs[f].get("n_dust", 0)
+        A = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
+        rc = Gc.simulate_packages(f, s, n_const, 11, 1.0, 0, n_const, A, None, flags=PROD)
+        assert out[0][1][f].emitted - rc.emitted == pytest.approx(lum[f], rel=1e-5)
+    Gc.close()

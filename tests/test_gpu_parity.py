@@ -440,6 +440,33 @@ def test_queue_buffers_are_cached_across_grids():
     assert soc.release_cached_memory() >= 8 * 64 ** 3 and soc.release_cached_memory() == 0
 
 
+def test_a_failed_device_allocation_empties_the_caches_and_is_tried_again():
+    """Buffers in the process-wide cache are only reused at their exact size, so a grid of another size could run out of
+    device memory while the cache sits on what it needs: an allocation that fails gives the cached buffers back and is
+    tried once more.  Here the cache holds the arrays of a 160^3 grid, torch takes all free memory but 48 MB, and a
+    160 x 160 x 159 grid (about 150 MB of arrays of other sizes) must still come up."""
+    torch = _torch()
+    soc.release_cached_memory()
+    freq, one = np.array([1e14]), np.array([1.0])
+    n = 160
+    G = soc.Grid(n, n, n, [n ** 3], np.ones(n ** 3, dtype=np.float32), None, freq, one, one, 0.0 * one)
+    G.close()
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free = torch.cuda.mem_get_info()[0]
+    filler = torch.empty(free - (48 << 20), dtype=torch.uint8, device="cuda")
+    try:
+        m = n * n * (n - 1)
+        G = soc.Grid(n, n, n - 1, [m], np.ones(m, dtype=np.float32), None, freq, one, one, 0.0 * one)
+        assert G.n_total == m
+        assert soc.release_cached_memory() == 0          # the retry emptied the cache: the second attempt is what succeeded
+        G.close()
+    finally:
+        del filler
+        torch.cuda.empty_cache()
+    soc.release_cached_memory()
+
+
 @pytest.mark.parametrize("which,n_sub", [("3", 60_000), ("5", 40_000)])
 def test_production_full_size_subset_against_oracle(which, n_sub):
     """Full-size grid and package count, production mode, the kernel bench.py times (chosen by working-set size):
