@@ -779,7 +779,10 @@ struct SlabParams {
     int q_left;                         // the leftover queue this launch pops (n_slabs or n_slabs + 1); it dumps to the other
     int s_first, s_last;                // slab queues this launch pops, in this order
     int final_phase;                    // nothing is suspended or dumped
+    unsigned long long q_entries;       // entries of each of qa, qb, qc, qp (the bounds-checked build tests against it)
 };
+constexpr int kSlabCntLen = 4 * 64 + 4;                     // elements of SlabParams::cnt
+constexpr int kHot64Len = SOC_MAX_POINT_SOURCES * 343;      // elements of FastParams::hot64
 __device__ __forceinline__ size_t slab_qbase(const SlabParams &S, int q)
 {
     return q < S.n_slabs ? (size_t)q * S.cap : (size_t)S.n_slabs * S.cap + (size_t)(q - S.n_slabs) * S.cap_left;
@@ -792,12 +795,12 @@ __device__ __forceinline__ void slab_epilogue(const SlabParams &S, bool pops)
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
-        s_is_last = atomicAdd(S.cnt + 4 * 64, 1u) == gridDim.x - 1 ? 1u : 0u;
+        s_is_last = atomicAdd(S.cnt + CK(4 * 64, kSlabCntLen), 1u) == gridDim.x - 1 ? 1u : 0u;
     }
     __syncthreads();
     if (s_is_last && (int)threadIdx.x < S.n_slabs + 2) {
         const int q = threadIdx.x;
-        volatile unsigned *c = S.cnt + 4 * q;
+        volatile unsigned *c = S.cnt + CK(4 * q, kSlabCntLen - 3);
         if (pops && (q == S.q_left || (q >= S.s_first && q <= S.s_last))) c[0] = c[2];
         const unsigned t = c[1];
         if (!pops) c[3] = t;                     // slab_emit_kernel: its entries are all in (it never fills a queue)
@@ -1284,7 +1287,7 @@ __global__ void __launch_bounds__(256, HIER ? 5 : 4) photon_fast_kernel(const __
                 const int jz = j / (hot_side * hot_side), jr = j - jz * hot_side * hot_side, jy = jr / hot_side, jx = jr - jy * hot_side;
                 const int ix = (int)floor(P.ps_pos[k][0]) + jx - P.hot_r, iy = (int)floor(P.ps_pos[k][1]) + jy - P.hot_r,
                           iz = (int)floor(P.ps_pos[k][2]) + jz - P.hot_r;
-                if (ACC32) atomicAdd(P.hot64 + i, GROUP ? (double)v : (double)v * (double)P.ps_rel[k]);
+                if (ACC32) atomicAdd(P.hot64 + CK(i, kHot64Len), GROUP ? (double)v : (double)v * (double)P.ps_rel[k]);
                 else atomicAdd(P.acc + CK(root_id(P, ix, iy, iz), P.n_int), (double)v * P.ps_e0[k]);
             }
         }
@@ -1452,14 +1455,14 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
             const bool mine = sel && dest == d;
             const unsigned m = __ballot_sync(kFull, mine);
             unsigned b = 0;
-            if (lane == leader) b = atomicAdd(P.slab.cnt + 4 * d + 1, (unsigned)__popc(m));
+            if (lane == leader) b = atomicAdd(P.slab.cnt + CK(4 * d + 1, kSlabCntLen), (unsigned)__popc(m));
             b = __shfl_sync(kFull, b, leader);
             if (mine) {
                 const unsigned slot = b + __popc(m & lt_mask);
                 unsigned room = d < P.slab.n_slabs ? P.slab.limit : P.slab.limit_left;
-                if (slot >= room) { const unsigned emitted = P.slab.cnt[4 * d + 3]; room = room > emitted ? room : emitted; }
+                if (slot >= room) { const unsigned emitted = P.slab.cnt[CK(4 * d + 3, kSlabCntLen)]; room = room > emitted ? room : emitted; }
                 if (slot < room) {
-                    const size_t e = slab_qbase(P.slab, d) + slot;
+                    const size_t e = CK(slab_qbase(P.slab, d) + slot, P.slab.q_entries);
                     const uint32_t cls = (DUST && p.sd <= -2) ? (uint32_t)(129 + p.sd) : (uint32_t)(v_src(p.sd) + 1);
                     const uint32_t tag = p.idx | (cls << 25);
                     if (DUST) P.slab.qp[e] = p.prel;
@@ -1513,9 +1516,9 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
                         // entries [head, frozen) of the leftover queue, then of the slab queues
                         while (pool_next >= pool_end && cur_q <= P.slab.s_last) {
                             const int q = cur_q < P.slab.s_first ? P.slab.q_left : cur_q;
-                            const unsigned frozen = P.slab.cnt[4 * q + 2];
+                            const unsigned frozen = P.slab.cnt[CK(4 * q + 2, kSlabCntLen)];
                             unsigned base = 0;
-                            if (lane == 0) base = atomicAdd(P.slab.cnt + 4 * q, (unsigned)kSlabChunk);
+                            if (lane == 0) base = atomicAdd(P.slab.cnt + CK(4 * q, kSlabCntLen), (unsigned)kSlabChunk);
                             base = __shfl_sync(kFull, base, 0);
                             if (base >= frozen) { cur_q += 1; continue; }
                             pool_next = base;
@@ -1546,7 +1549,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
             float ndx = 0.0f, ndy = 0.0f, ndz = 1.0f;
             if (SLAB && need == NEWID) {
                 // resume a package: slot p.idx of queue p.sd (reciprocals and the half brick are not part of the state)
-                const size_t e = slab_qbase(P.slab, p.sd) + p.idx;
+                const size_t e = CK(slab_qbase(P.slab, p.sd) + p.idx, P.slab.q_entries);
                 const uint4 a = P.slab.qa[e], b = P.slab.qb[e], c = P.slab.qc[e];
                 p.fx = __uint_as_float(a.x); p.fy = __uint_as_float(a.y); p.fz = __uint_as_float(a.z); p.tau_rem = __uint_as_float(a.w);
                 p.dx = __uint_as_float(b.x); p.dy = __uint_as_float(b.y); p.dz = __uint_as_float(b.z); p.w = __uint_as_float(b.w);
@@ -1738,7 +1741,7 @@ __global__ void __launch_bounds__(256, SLAB ? 4 : 5) photon_q_kernel(const __gri
         for (int i = threadIdx.x; i < hot_cells * P.n_point; i += blockDim.x) {
             const float v = s_hot[i];
             if (v != 0.0f) {
-                atomicAdd(P.hot64 + i, (double)v * (double)P.ps_rel[i / hot_cells]);
+                atomicAdd(P.hot64 + CK(i, kHot64Len), (double)v * (double)P.ps_rel[i / hot_cells]);
             }
         }
     }
@@ -1833,10 +1836,10 @@ __global__ void __launch_bounds__(256) slab_emit_kernel(const __grid_constant__ 
         }
         __syncthreads();
         if ((int)threadIdx.x < P.slab.n_slabs && s_n[threadIdx.x] > 0u)
-            s_base[threadIdx.x] = atomicAdd(P.slab.cnt + 4 * threadIdx.x + 1, s_n[threadIdx.x]);
+            s_base[threadIdx.x] = atomicAdd(P.slab.cnt + CK(4 * threadIdx.x + 1, kSlabCntLen), s_n[threadIdx.x]);
         __syncthreads();
         if (live) {
-            const size_t e = slab_qbase(P.slab, slab) + CK(s_base[slab] + rank, P.slab.cap);
+            const size_t e = CK(slab_qbase(P.slab, slab) + CK(s_base[slab] + rank, P.slab.cap), P.slab.q_entries);
             const uint32_t tag = idx | ((q.src == -2 ? 127u : (uint32_t)(q.src + 1)) << 25);
             if (q.src == -2) P.slab.qp[e] = prel;
             P.slab.qa[e] = make_uint4(__float_as_uint(q.fx), __float_as_uint(q.fy), __float_as_uint(q.fz), __float_as_uint(tau));
@@ -2730,12 +2733,12 @@ int launch_slab(soc_grid *G, FastParams P, int n_slabs, int sweeps, double weigh
         }
     }
     const size_t stride = G->slab_q_entries[sel];    // the three arrays of the buffer are `stride` entries apart
-    const size_t cnt_bytes = sizeof(unsigned) * (4 * 64 + 4);
+    const size_t cnt_bytes = sizeof(unsigned) * kSlabCntLen;
     if (!G->d_slab_cnt[sel]) SOC_CUDA(cudaMalloc(&G->d_slab_cnt[sel], cnt_bytes));
     SlabParams &S = P.slab;
     S.qa = G->d_slab_q[sel]; S.qb = S.qa + stride; S.qc = S.qb + stride; S.qp = reinterpret_cast<float *>(S.qc + stride);
     S.cnt = G->d_slab_cnt[sel]; S.cap = n_pkg; S.cap_left = (unsigned)cap_left; S.n_slabs = n_slabs;
-    S.limit = S.cap; S.limit_left = S.cap_left;
+    S.limit = S.cap; S.limit_left = S.cap_left; S.q_entries = stride;
     if (G->opt_slab_queue_limit > 0) {
         if ((unsigned long long)G->opt_slab_queue_limit < S.limit) S.limit = (unsigned)G->opt_slab_queue_limit;
         if ((unsigned long long)G->opt_slab_queue_limit < S.limit_left) S.limit_left = (unsigned)G->opt_slab_queue_limit;
@@ -2982,7 +2985,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         if (acc32 && F.hot_r >= 0) {
             double *&h = G->d_hot64[G->acc_sel];
             if (!h) {
-                const size_t bytes = sizeof(double) * SOC_MAX_POINT_SOURCES * 343;
+                const size_t bytes = sizeof(double) * kHot64Len;
                 SOC_CUDA(cudaMalloc(&h, bytes));
                 SOC_CUDA(cudaMemsetAsync(h, 0, bytes, st));              // st = the stream that uses it
             }
@@ -3144,7 +3147,7 @@ int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long 
     if (F.hot_r >= 0) {
         double *&h = G->d_hot64[G->acc_sel];
         if (!h) {
-            const size_t bytes = sizeof(double) * SOC_MAX_POINT_SOURCES * 343;
+            const size_t bytes = sizeof(double) * kHot64Len;
             SOC_CUDA(cudaMalloc(&h, bytes));
             SOC_CUDA(cudaMemsetAsync(h, 0, bytes, st));                  // st = the stream that uses it
         }
