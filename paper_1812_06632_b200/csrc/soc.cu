@@ -3838,13 +3838,20 @@ int soc_iterate(soc_grid *G, const soc_sources *src, int64_t n_const, uint64_t s
     double *buf[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     int32_t *count = nullptr;
     const int n_buf = opts->ali ? 7 : 3;
-    auto cleanup = [&]() { for (double *b : buf) cudaFree(b); cudaFree(count); };
+    // (from the process-wide buffer cache: a second call on a grid of this size allocates nothing; every exit path below
+    //  synchronises the stream before the buffers go back)
+    auto cleanup = [&]() { cudaStreamSynchronize(st); for (double *b : buf) big_free(b); big_free(count); };
     for (int i = 0; i < n_buf; ++i)
-        if (cudaMalloc(&buf[i], nb) != cudaSuccess || cudaMemsetAsync(buf[i], 0, nb, st) != cudaSuccess) {
+        if (big_malloc(&buf[i], nb) != cudaSuccess || cudaMemsetAsync(buf[i], 0, nb, st) != cudaSuccess) {
+            cudaGetLastError();
             cleanup();
             return fail(SOC_ENOMEM, "soc_iterate: device allocation failed");
         }
-    if (cudaMalloc(&count, sizeof(int32_t) * (size_t)G->n_total) != cudaSuccess) { cleanup(); return fail(SOC_ENOMEM, "soc_iterate: device allocation failed"); }
+    if (big_malloc(&count, sizeof(int32_t) * (size_t)G->n_total) != cudaSuccess) {
+        cudaGetLastError();
+        cleanup();
+        return fail(SOC_ENOMEM, "soc_iterate: device allocation failed");
+    }
     double *A_const = buf[0], *D = buf[1], *R = buf[2], *Si = buf[3], *Sref = buf[4], *Emi = buf[5], *Emref = buf[6];
     std::vector<soc_freq_result> res((size_t)nf);
     int rc = SOC_OK;
