@@ -204,7 +204,8 @@ def run_ours(args):
     has_T = P.table_T is not None
     Aint = torch.zeros(P.n_total, dtype=torch.float64, device="cuda")
     T = torch.zeros(P.n_total, dtype=torch.float32, device="cuda")
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # 2 x L2 (126 MB)
+    l2_bytes = int(torch.cuda.get_device_properties(local_rank).L2_cache_size)
+    flush = torch.empty(max(256 << 20, 2 * l2_bytes), dtype=torch.uint8, device="cuda")      # 2 x L2 (B200: 126 MB)
     stream = torch.cuda.current_stream()
 
     def step(want_results=False):
@@ -326,6 +327,7 @@ def run_ours(args):
     if tr:
         roof["traffic"] = tr["bytes_per_cell_step"] * float(steps_f.mean())
         roof["traffic_source"] = tr["source"]
+        roof["traffic_measured_in_run"] = False        # carried from the committed ncu capture named in traffic_source
         roof["traffic_bytes_per_cell_step"] = tr["bytes_per_cell_step"]
     roof["algorithmic_bytes_note"] = ("12 B per cell-step is SURVEY.md 8d.4's contract figure (4 B density + 8 B fp64 add); the path "
                                       "as run adds into an fp32 per-launch accumulator: 4 B + 4 B = 8 B per cell-step")
@@ -342,7 +344,7 @@ def run_ours(args):
                        "parallelism": "single GPU" if world == 1 else (
                            f"{world} ranks, seed + rank each (independent realisations), one fp64 all-reduce" if args.scaling == "weak"
                            else f"{world} ranks, package ids of one seed split evenly, one fp64 all-reduce"),
-                       "l2": "flushed between timed steps (256 MB fill)"},
+                       "l2": f"flushed between timed steps ({flush.numel() >> 20} MB fill; L2 {l2_bytes} B)"},
             "packages_per_s": (world if args.scaling == "weak" else 1) * P.n_packages * P.n_freq / (ms_per_step * 1e-3),
             "cell_steps_per_s_per_frequency": {"median": float(np.median(per_f)), "min": float(per_f.min()),
                                                "max": float(per_f.max()), "note": "over pairs of consecutive frequencies"},
@@ -440,10 +442,12 @@ def roofline_components(G, P, srcs, shard, Aint, stream, steps_f, kern_ms, hbm_p
     secs = float(kern_ms.sum()) * 1e-3
     gathers, reds = float(sum(r.gather_requests for r in res)), float(sum(r.red_requests for r in res))
     steps = float(steps_f.sum())
-    vec = P.child is None and 8 * int(P.n_total) > (64 << 20)      # photon_q_kernel (16-byte requests) carries such grids
+    import torch
+    l2_bytes = int(torch.cuda.get_device_properties(torch.cuda.current_device()).L2_cache_size)
+    vec = P.child is None and 8 * int(P.n_total) > l2_bytes // 126 * 64      # photon_q_kernel (16-byte requests) carries such grids (soc.cu l2_share)
     n_ops = 1 << 30
     rate = lambda kind, fp: n_ops / (soc.probe_throughput(kind, fp, n_ops) * 1e-3)          # noqa: E731
-    l2_fp, cfg_fp = 32 << 20, 8 * int(P.n_total)
+    l2_fp, cfg_fp = min(32 << 20, l2_bytes // 4), 8 * int(P.n_total)
     kg, kr = (6, 4) if vec else (0, 2)
     ceil_g, ceil_r = rate(kg, l2_fp), rate(kr, l2_fp)
     floor_g, floor_r, floor_pair = rate(kg, cfg_fp), rate(kr, cfg_fp), rate(5, cfg_fp)

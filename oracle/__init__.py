@@ -1,10 +1,12 @@
 """ctypes access to oracle/soc_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
-import this package.  It holds no arithmetic of its own: every number comes out of the plain C
-file next to it (fp64, single-threaded per call).  `simulate(..., threads=k)` only splits the
-package-id range over k concurrent calls with private accumulators that are summed at the end
-(SURVEY.md 8d.5); the per-package arithmetic is untouched by it.
+import this package.  The package walk, the deposits, the temperature lookup and the maps (rows a1-a11,
+f2) are computed by the plain C file next to it (fp64, single-threaded per call); `simulate(...,
+threads=k)` only splits the package-id range over k concurrent calls with private accumulators that
+are summed at the end and leaves the per-package arithmetic untouched.  What is
+written here in numpy: the host loop of the iterated run (`iterate`: running-mean reference field,
+ALI update, rows f1 / f3) and the stochastic-heating solver (`stochastic_*`, row f4: dense fp64 solve).
 """
 from __future__ import annotations
 

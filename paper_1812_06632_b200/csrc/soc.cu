@@ -221,6 +221,7 @@ struct soc_grid {
     int opt_acc32 = 1;
     int n_slots = 0;
     int device = 0, n_sm = 0;
+    long long l2_bytes = 126ll << 20;   // cudaDevAttrL2CacheSize of the grid's device (B200: 126 MB), set by soc_grid_create
     int opt_blocks_per_sm = 0;                // 0 = from the occupancy calculator
     int opt_threads = 256;
     int opt_refill_threshold = 1;
@@ -246,6 +247,10 @@ struct soc_grid {
     std::vector<char> ev_set;
     cudaEvent_t ev_after_photon = nullptr;
 };
+
+// The working-set thresholds of the kernel choice were measured on B200's 126 MB of L2 (64 MB: photon_q_kernel instead of
+// photon_fast_kernel; 96 MB: slab blocking, in slabs of 80 MB); on another device they scale with its L2.
+static inline long long l2_share(const soc_grid *G, int mb_of_126) { return G->l2_bytes / 126 * mb_of_126; }
 
 // ------------------------------------------------------------------------------------------------
 // device code
@@ -3003,7 +3008,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         // and where packages do not scatter very often (every scattering parks the lane and reloads the half brick):
         // measured crossover on config 5, both kernels at their best occupancy, at a scattering depth of the box of 12-16
         const int n_max = G->nx > G->ny ? (G->nx > G->nz ? G->nx : G->nz) : (G->ny > G->nz ? G->ny : G->nz);
-        const bool big = 8ll * G->n_int > (64ll << 20) && P.ksca * G->rho_mean * n_max < 12.0;
+        const bool big = 8ll * G->n_int > l2_share(G, 64) && P.ksca * G->rho_mean * n_max < 12.0;
         const bool v2 = !hier && acc32 && (G->opt_kernel == 2 || (G->opt_kernel == 0 && big)) && pkg_count < (1ll << 32);
         if (v2) F.service_threshold = auto_threshold;
         // z-slab blocking: the cell words and the accumulator of one slab stay in L2 while it is served.
@@ -3011,7 +3016,7 @@ int enqueue_frequency(soc_grid *G, int ifreq, const soc_sources *src, long long 
         // traffic per frequency against 54 GB) with the fewest suspensions; where packages scatter so often that the walk
         // is bound by the service passes (scattering depth of the box >= 12) photon_fast_kernel without slabs is faster
         int n_slabs = G->opt_slabs;
-        if (n_slabs == 0) n_slabs = 8ll * G->n_int > (96ll << 20) ? (int)((8ll * G->n_int + (80ll << 20) - 1) / (80ll << 20)) : 1;
+        if (n_slabs == 0) n_slabs = 8ll * G->n_int > l2_share(G, 96) ? (int)((8ll * G->n_int + l2_share(G, 80) - 1) / l2_share(G, 80)) : 1;
         if (n_slabs > G->nbz / 2) n_slabs = G->nbz / 2;
         if (n_slabs > kMaxSlabs) n_slabs = kMaxSlabs;
         const bool slab = !hier && acc32 && !rep && n_slabs >= 2 &&
@@ -3070,7 +3075,7 @@ int enqueue_group(soc_grid *G, int f0, int J, const soc_sources *src, long long 
     const bool hier = G->n_levels > 1;
     if (J < 1 || J > kMaxJobs || !G->opt_acc32 || pkg_count <= 0 || !absorbed) return 1;
     if (n_packages < 0 || pkg_begin < 0 || pkg_begin + pkg_count > n_packages) return 1;
-    if (!hier && (8ll * G->n_int > (64ll << 20) || G->opt_kernel == 2)) return 1;
+    if (!hier && (8ll * G->n_int > l2_share(G, 64) || G->opt_kernel == 2)) return 1;
     long long n_bg0 = 0;
     for (int j = 0; j < J; ++j) {
         long long n_bg = 0;
@@ -3416,6 +3421,11 @@ int soc_grid_create(const soc_grid_desc *d, soc_grid **out)
 
     SOC_CUDA(cudaGetDevice(&G->device));
     SOC_CUDA(cudaDeviceGetAttribute(&G->n_sm, cudaDevAttrMultiProcessorCount, G->device));
+    {
+        int l2 = 0;
+        SOC_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, G->device));
+        if (l2 > 0) G->l2_bytes = l2;
+    }
     SOC_CUDA(big_malloc(&G->d_cellw, sizeof(uint32_t) * (size_t)G->n_total));
     SOC_CUDA(big_malloc(&G->d_parent, sizeof(int32_t) * n_par));
     SOC_CUDA(cudaMalloc(&G->d_table, sizeof(float) * 8192));
