@@ -463,6 +463,23 @@ def roofline_components(G, P, srcs, shard, Aint, stream, steps_f, kern_ms, hbm_p
                                                       "cell of the config's footprint; ratio > 1 = locality the walk exploits"},
         "ceiling_footprint_bytes": l2_fp, "floor_footprint_bytes": cfg_fp,
     }
+    # the ceilings over footprints from L1-sized to beyond L2, uniform addresses, and the hot-spot case
+    # -- every thread of the probe into the 343 cells of a hot_r = 3 cube around a source: contended
+    # global reductions in fp32 / fp64 against shared-memory partial sums with one fp64 reduction per cell and block
+    try:
+        n_small = 1 << 28
+        r2 = lambda kind, fp, n=n_small: n / (soc.probe_throughput(kind, fp, n) * 1e-3)          # noqa: E731
+        comp["ceilings_ops_per_s"] = {
+            "footprint_bytes": [128 << 10, 1 << 20, 8 << 20, 64 << 20, 256 << 20],
+            "gather_4B": [r2(0, fp) for fp in (128 << 10, 1 << 20, 8 << 20, 64 << 20, 256 << 20)],
+            "red_f32": [r2(2, fp) for fp in (128 << 10, 1 << 20, 8 << 20, 64 << 20, 256 << 20)],
+            "red_f64": [r2(1, fp) for fp in (128 << 10, 1 << 20, 8 << 20, 64 << 20, 256 << 20)],
+            "hot_spot_343_cells": {"red_f32": r2(2, 343 * 4, 1 << 26), "red_f64": r2(1, 343 * 8, 1 << 26),
+                                   "shared_f32_then_one_red_f64_per_cell_and_block": r2(7, 343 * 4, 1 << 28)},
+            "note": "uniformly random addresses within the footprint, no arithmetic; hot spot = all lanes into 343 cells",
+        }
+    except Exception as exc:                             # an older library without probe kind 7
+        comp["ceilings_ops_per_s"] = {"error": str(exc)[:200]}
     fr = [comp["gather"]["frac"], comp["red"]["frac"]]
     if traffic:
         dram = traffic * len(steps_f) / secs / 1e9

@@ -320,7 +320,11 @@ int soc_get_timings(soc_grid *grid, int32_t n, float *ms);
  * one cell-step (kind 5: a 4-byte gather from the first half of the footprint and an fp32 red.global.add at the same
  * random cell of the second half) over a
  * footprint of `footprint_bytes`, n_ops operations in total, uniform addresses, no arithmetic, every access
- * independent of the others.  *ms receives the CUDA-event time of the probe kernel. */
+ * independent of the others.  A footprint of a few hundred cells is the hot-spot case (many threads
+ * updating "a small number of cells close to the source"): kinds 1 and 2 over 343 cells give the rate of contended
+ * global reductions, and kind 7 the rate of the remedy the photon kernels use there -- fp32 atomic adds into a
+ * shared-memory copy of the cells (at most 8192 cells = 32 KB footprint), one fp64 red.global.add per touched cell and
+ * block at the end.  *ms receives the CUDA-event time of the probe kernel. */
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms);
 
 /* Stochastically heated grains (row f4; Appendix A -- a companion solver, "not part of SOC" proper).

@@ -2506,12 +2506,21 @@ __device__ __forceinline__ uint32_t mix32(uint32_t x)
     return x;
 }
 
+constexpr int kProbeHotMax = 8192;      // cells of the shared-memory hot-spot probe (kind 7)
+
 template <int KIND>
 __global__ void __launch_bounds__(256) probe_kernel(void *buf, unsigned long long n_elem, long long ops_per_thread, float *sink)
 {
     const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t s = mix32(tid * 2654435761u + 12345u);
     float acc[4] = {0.f, 0.f, 0.f, 0.f};          // four independent chains: four gathers in flight per thread
+    // KIND 7: the remedy the photon kernels use for the cells around a point source -- the block's partial sums in shared
+    // memory, one fp64 reduction per cell and block at the end (n_elem <= kProbeHotMax)
+    __shared__ float s_hot[KIND == 7 ? kProbeHotMax : 1];
+    if (KIND == 7) {
+        for (unsigned i = threadIdx.x; i < n_elem; i += blockDim.x) s_hot[i] = 0.0f;
+        __syncthreads();
+    }
     for (long long i = 0; i < ops_per_thread; i += 4) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -2529,6 +2538,8 @@ __global__ void __launch_bounds__(256) probe_kernel(void *buf, unsigned long lon
             } else if (KIND == 4) {              // 16-byte vector reduction (4 fp32 cells)
                 asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(reinterpret_cast<float *>(buf) + 4 * j),
                              "f"(1.0f), "f"(1.0f), "f"(1.0f), "f"(1.0f) : "memory");
+            } else if (KIND == 7) {
+                atomicAdd(s_hot + j, 1.0f);
             } else if (KIND == 6) {              // 16-byte gather (half a brick: what photon_q_kernel loads)
                 const uint4 v = __ldg(reinterpret_cast<const uint4 *>(buf) + j);
                 acc[u] += __uint_as_float(v.x ^ v.y ^ v.z ^ v.w);
@@ -2539,6 +2550,11 @@ __global__ void __launch_bounds__(256) probe_kernel(void *buf, unsigned long lon
         }
     }
     if ((KIND == 0 || KIND == 3 || KIND == 5 || KIND == 6) && acc[0] + acc[1] + acc[2] + acc[3] == 123.456f) *sink = acc[0];
+    if (KIND == 7) {
+        __syncthreads();
+        for (unsigned i = threadIdx.x; i < n_elem; i += blockDim.x)
+            if (s_hot[i] != 0.0f) atomicAdd(reinterpret_cast<double *>(buf) + i, (double)s_hot[i]);
+    }
 }
 
 }  // namespace
@@ -4087,9 +4103,12 @@ int soc_run_host(const soc_grid_desc *desc, const soc_sources *src, int64_t n_pa
 
 int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, float *ms)
 {
-    if (kind < 0 || kind > 6 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
-    const size_t elem = (kind == 1 || kind == 5) ? 8 : (kind == 3 ? 32 : ((kind == 4 || kind == 6) ? 16 : 4));   // kind 5: 4 B rho + 4 B acc per cell
-    const unsigned long long n_elem = (unsigned long long)footprint_bytes / elem;
+    if (kind < 0 || kind > 7 || footprint_bytes < 64 || n_ops < 1 || !ms) return fail(SOC_EINVAL, "bad probe argument");
+    // kind 5: 4 B rho + 4 B acc per cell; kind 7: footprint counted as fp32 cells (4 B), the sums behind them are fp64
+    const size_t cell = (kind == 1 || kind == 5) ? 8 : (kind == 3 ? 32 : ((kind == 4 || kind == 6) ? 16 : 4));
+    const unsigned long long n_elem = (unsigned long long)footprint_bytes / cell;
+    if (kind == 7 && n_elem > (unsigned long long)kProbeHotMax) return fail(SOC_EINVAL, "probe kind 7: at most 8192 cells (32 KB)");
+    const size_t elem = kind == 7 ? 8 : cell;
     void *buf = nullptr;
     float *sink = nullptr;
     int dev = 0, n_sm = 0;
@@ -4112,6 +4131,7 @@ int soc_probe_throughput(int32_t kind, int64_t footprint_bytes, int64_t n_ops, f
         else if (kind == 3) probe_kernel<3><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else if (kind == 4) probe_kernel<4><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else if (kind == 6) probe_kernel<6><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
+        else if (kind == 7) probe_kernel<7><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         else probe_kernel<5><<<blocks, threads>>>(buf, n_elem, per_thread, sink);
         g_launches += 1;
         SOC_CUDA(cudaEventRecord(e1));

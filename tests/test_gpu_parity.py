@@ -933,3 +933,20 @@ def test_bad_arguments_are_rejected():
     with pytest.raises(soc.SocError):
         G.simulate_packages(0, P.sources(0), 10, 1, 1.0, 5, 6, A)           # range beyond n_packages
     G.close()
+
+
+def test_roofline_probes_run_on_every_kind_and_refuse_bad_arguments():
+    """soc_probe_throughput (SURVEY.md 8d.3): every kind returns a positive device time over a small and a large footprint;
+    the hot-spot probe of the shared-memory remedy (kind 7) takes at most 8192 cells; unknown kinds are refused."""
+    for kind in range(7):
+        for fp in (343 * 8, 8 << 20):
+            assert soc.probe_throughput(kind, fp, 1 << 22) > 0.0
+    assert soc.probe_throughput(7, 343 * 4, 1 << 22) > 0.0
+    assert soc.probe_throughput(7, 8192 * 4, 1 << 22) > 0.0
+    with pytest.raises(soc.SocError, match="8192"):
+        soc.probe_throughput(7, 8193 * 4, 1 << 22)
+    with pytest.raises(soc.SocError):
+        soc.probe_throughput(8, 1 << 20, 1 << 22)
+    # contended global reductions into 343 cells are slower than the same adds into shared memory with one flush per block
+    n = 1 << 26
+    assert soc.probe_throughput(7, 343 * 4, n) < soc.probe_throughput(2, 343 * 4, n)
