@@ -75,6 +75,8 @@ def test_argument_validation_without_a_device():
     assert L.soc_probe_throughput(9, 1 << 20, 1000, C.byref(ms)) == -1
     assert L.soc_simulate_frequency(None, 0, None, 1, 1, 1.0, None, None, 0, None) == -1
     assert L.soc_update_temperatures(None, None, 1.0, None, 2, 1.0, 2.0, None, None) == -1
+    assert L.soc_update_temperatures_ali_static(None, None, None, None, 1.0, None, 2, 1.0, 2.0, None, None) == -1
+    assert b"NULL" in L.soc_last_error()                                 # refused before any device call
     assert L.soc_launch_count() == 0
     assert L.soc_release_cached_memory() == 0                            # nothing cached, no device touched
     assert L.soc_version().startswith(b"soc_b200")
